@@ -1,0 +1,244 @@
+"""Pins for the fp64 oracle (run with -m "not gpu").  Each test states which mistake it would catch.
+The oracle follows PAPER.md:112-119 §4.2 Eq. 7-8 + PAPER.md:149 + PAPER.md:66; see oracle/comb_oracle.c."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import comb_synth as cs
+import oracle
+from oracle import brute
+
+GOLD = {}
+with open(os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")) as f:
+    for line in f:
+        if line.strip() and not line.startswith("#"):
+            name, val = line.split()[:2]
+            GOLD[name] = float(val)
+
+
+def bits(x):
+    return cs.f32_to_bf16_bits(np.asarray(x, dtype=np.float32))
+
+
+def run(q, ks, vs, link, scale, lq=None):
+    """single request helper: q bits [lq][Hq][Dqk]"""
+    q_indptr = np.array([0, q.shape[0]], np.int32)
+    return oracle.attention(q, q_indptr, ks, vs, np.array([0, len(link)], np.int32), np.array(link, np.int32), scale)
+
+
+def rand_case(seed, lq, Hq, Hkv, Dqk, Dv, lens):
+    rng = np.random.default_rng(seed)
+    q = bits(rng.standard_normal((lq, Hq, Dqk)))
+    ks = [bits(rng.standard_normal((t, Hkv, Dqk))) for t in lens]
+    vs = [bits(rng.standard_normal((t, Hkv, Dv))) for t in lens]
+    return q, ks, vs
+
+
+# ---- P1: brute force, separately written, no max subtraction ------------------------------------
+@pytest.mark.parametrize("Hq,Hkv,Dqk,Dv,lens,link", [
+    (4, 2, 64, 64, [5, 17, 40], [2, 0, 1]),     # GQA 2, ragged chunk lengths, shuffled link order
+    (2, 2, 8, 4, [3], [0]),                       # Dqk != Dv, no GQA
+    (4, 1, 16, 8, [7, 9], [1, 0, 1]),            # a chunk linked twice (taken literally, reading I14)
+])
+def test_p1_brute_force(Hq, Hkv, Dqk, Dv, lens, link):
+    q, ks, vs = rand_case(1, 3, Hq, Hkv, Dqk, Dv, lens)
+    scale = 1.0 / math.sqrt(Dqk)
+    O, L = run(q, ks, vs, link, scale)
+    Ob, Lb = brute.attention_brute(q, ks, vs, link, scale)
+    assert np.max(np.abs(O - np.array(Ob))) <= 1e-12
+    assert np.max(np.abs(L - np.array(Lb))) <= 1e-12
+
+
+# ---- P2: library special case (one chunk): fp64 softmax(QK^T*scale)V with numpy matmul / torch SDPA -----
+@pytest.mark.parametrize("G", [1, 4])
+def test_p2_library_sdpa(G):
+    torch = pytest.importorskip("torch")
+    Hkv, Dqk, Dv, T, lq = 2, 64, 32, 48, 5
+    Hq = Hkv * G
+    q, ks, vs = rand_case(2, lq, Hq, Hkv, Dqk, Dv, [T])
+    scale = 0.2  # deliberately not 1/sqrt(d): a hard-wired scale fails here
+    O, L = run(q, ks, vs, [0], scale)
+    qf = torch.from_numpy(cs.bf16_bits_to_f64(q)).permute(1, 0, 2)                       # [Hq][lq][Dqk]
+    kf = torch.from_numpy(cs.bf16_bits_to_f64(ks[0])).permute(1, 0, 2).repeat_interleave(G, 0)   # consecutive grouping
+    vf = torch.from_numpy(cs.bf16_bits_to_f64(vs[0])).permute(1, 0, 2).repeat_interleave(G, 0)
+    ref = torch.nn.functional.scaled_dot_product_attention(qf, kf, vf, scale=scale).permute(1, 0, 2).numpy()
+    assert np.max(np.abs(O - ref)) <= 1e-12
+    s = np.einsum("hid,hjd->hij", qf.numpy(), kf.numpy()) * scale
+    lse_ref = np.log(np.exp(s).sum(-1)).T
+    assert np.max(np.abs(L - lse_ref)) <= 1e-12
+
+
+# ---- P3: single key returns its V exactly; LSE = its score -----------------------------------------
+def test_p3_single_key():
+    q, ks, vs = rand_case(3, 2, 4, 2, 64, 64, [1])
+    O, L = run(q, ks, vs, [0], 0.125)
+    v = cs.bf16_bits_to_f64(vs[0])[0]                    # [Hkv][Dv]
+    for h in range(4):
+        assert np.array_equal(O[:, h, :], np.broadcast_to(v[h // 2], (2, 64)))
+    s = 0.125 * np.einsum("ihd,hd->ih", cs.bf16_bits_to_f64(q), np.repeat(cs.bf16_bits_to_f64(ks[0])[0], 2, 0))
+    assert np.max(np.abs(L - s)) <= 1e-12
+
+
+# ---- P4: equal scores -> mean of V, LSE = ln(kv_len) ----------------------------------------------
+def test_p4_equal_scores():
+    _, ks, vs = rand_case(4, 1, 4, 2, 64, 64, [128, 128, 128, 128])
+    q = np.zeros((3, 4, 64), np.uint16)                   # Q = 0 => every score is 0
+    O, L = run(q, ks, vs, [3, 1, 0, 2], 0.125)
+    mean_v = np.concatenate([cs.bf16_bits_to_f64(v) for v in vs], 0).mean(0)   # [Hkv][Dv]
+    for h in range(4):
+        assert np.max(np.abs(O[:, h, :] - mean_v[h // 2])) <= 1e-13
+    assert np.max(np.abs(L - GOLD["ln_512"])) <= 1e-13
+
+
+# ---- P5: two-level closed form sigma(1), and the unbalanced 3:1 case ------------------------------
+@pytest.mark.parametrize("n1,n0,gold", [(8, 8, "sigmoid_1"), (3, 1, "two_level_3_to_1")])
+def test_p5_two_level(n1, n0, gold):
+    D = 16
+    q = np.zeros((1, 1, D), np.float32); q[0, 0, 0] = 1.0
+    k1 = np.zeros((n1, 1, D), np.float32); k1[:, 0, 0] = 1.0       # score 1, V = 1
+    k0 = np.zeros((n0, 1, D), np.float32)                           # score 0, V = 0
+    O, L = run(bits(q), [bits(k1), bits(k0)], [bits(np.ones((n1, 1, D))), bits(np.zeros((n0, 1, D)))], [1, 0], 1.0)
+    assert np.max(np.abs(O - GOLD[gold])) <= 1e-15
+    assert abs(L[0, 0] - math.log(n1 * math.e + n0)) <= 1e-14
+
+
+# ---- P6: permutation invariance ("in any order/position") ---------------------------
+def test_p6_permutation():
+    q, ks, vs = rand_case(6, 4, 8, 2, 64, 64, [33, 16, 50, 7])
+    base = run(q, ks, vs, [0, 1, 2, 3], 0.125)
+    for perm in ([3, 2, 1, 0], [2, 0, 3, 1]):
+        got = run(q, ks, vs, perm, 0.125)
+        assert np.max(np.abs(got[0] - base[0])) <= 1e-12 and np.max(np.abs(got[1] - base[1])) <= 1e-12
+
+
+# ---- P7: a chunk split in two == kept whole (l_doc = sum l_doc,i) -------------------
+def test_p7_split_equals_whole():
+    q, ks, vs = rand_case(7, 3, 4, 2, 64, 64, [53])
+    whole = run(q, ks, vs, [0], 0.125)
+    t1 = 21                                              # not a multiple of 16: interior partial page
+    split = run(q, [ks[0][:t1], ks[0][t1:]], [vs[0][:t1], vs[0][t1:]], [0, 1], 0.125)
+    assert np.max(np.abs(whole[0] - split[0])) <= 1e-12 and np.max(np.abs(whole[1] - split[1])) <= 1e-12
+
+
+# ---- P8: merge identity over a disjoint split of the keys ------------------------------------------
+def test_p8_merge_identity():
+    q, ks, vs = rand_case(8, 3, 4, 2, 64, 64, [40, 25])
+    OA, LA = run(q, ks, vs, [0], 0.125)
+    OB, LB = run(q, ks, vs, [1], 0.125)
+    O, L = run(q, ks, vs, [0, 1], 0.125)
+    wa, wb = np.exp(LA)[..., None], np.exp(LB)[..., None]
+    assert np.max(np.abs(O - (wa * OA + wb * OB) / (wa + wb))) <= 1e-12
+    assert np.max(np.abs(L - np.log(np.exp(LA) + np.exp(LB)))) <= 1e-12
+    # two identical halves: LSE shifts by exactly ln 2, O unchanged
+    O2, L2 = run(q, ks, vs, [0, 0], 0.125)
+    assert np.max(np.abs(O2 - OA)) <= 1e-12 and np.max(np.abs(L2 - LA - GOLD["ln_2"])) <= 1e-12
+
+
+# ---- P9: shift invariance: add a vector c to every key ---------------------------------------------
+def test_p9_shift_invariance():
+    rng = np.random.default_rng(9)
+    D, T = 8, 12
+    q = rng.integers(-3, 4, (2, 2, D)).astype(np.float32)       # small integers: sums stay exact in bf16
+    k = rng.integers(-3, 4, (T, 1, D)).astype(np.float32)
+    v = rng.standard_normal((T, 1, D)).astype(np.float32)
+    c = rng.integers(-2, 3, (D,)).astype(np.float32)
+    O1, L1 = run(bits(q), [bits(k)], [bits(v)], [0], 0.25)
+    O2, L2 = run(bits(q), [bits(k + c)], [bits(v)], [0], 0.25)
+    assert np.max(np.abs(O1 - O2)) <= 1e-12
+    assert np.max(np.abs((L2 - L1) - 0.25 * (q.astype(np.float64) @ c.astype(np.float64)))) <= 1e-12
+
+
+# ---- P10: V-affinity: constant V -> that constant; O linear in V ----------------------------------
+def test_p10_v_affinity():
+    q, ks, vs = rand_case(10, 2, 4, 2, 64, 64, [19, 30])
+    const = [bits(np.full(v.shape, 1.5)) for v in vs]
+    O, _ = run(q, ks, const, [1, 0], 0.125)
+    assert np.array_equal(O, np.full_like(O, 1.5)) or np.max(np.abs(O - 1.5)) <= 1e-15
+    # linearity: V scaled by 2 (exact in bf16) doubles O exactly
+    v2 = [bits(cs.bf16_bits_to_f32(v) * 2.0) for v in vs]
+    Oa, _ = run(q, ks, vs, [1, 0], 0.125)
+    Ob, _ = run(q, ks, v2, [1, 0], 0.125)
+    assert np.max(np.abs(Ob - 2.0 * Oa)) <= 1e-13
+
+
+# ---- P12: empty link -> O = 0, LSE = -inf (reading I13) ------------------------------------------------
+def test_p12_empty_link():
+    q, ks, vs = rand_case(12, 2, 4, 2, 64, 64, [16])
+    q2 = np.concatenate([q, q], 0)
+    O, L = oracle.attention(q2, np.array([0, 2, 4], np.int32), ks, vs, np.array([0, 0, 1], np.int32),
+                            np.array([0], np.int32), 0.125)
+    assert np.all(O[:2] == 0.0) and np.all(np.isneginf(L[:2]))
+    assert np.all(np.isfinite(L[2:])) and np.any(O[2:] != 0.0)
+
+
+# ---- multi-request bookkeeping: rows of request r only see request r's chunks ----------------------
+def test_requests_are_independent():
+    w = cs.custom("two", num_q_heads=4, num_kv_heads=2, head_dim_qk=64, head_dim_v=64,
+                  chunk_len=[20, 33, 16], links=[[2, 0], [1]], lq=[3, 2])
+    O, L = oracle.attention_for(w)
+    O0, L0 = oracle.attention_for(w, [0])
+    O1, L1 = oracle.attention_for(w, [1])
+    assert np.array_equal(O, np.concatenate([O0, O1])) and np.array_equal(L, np.concatenate([L0, L1]))
+    # sampled entry point agrees with the full one
+    ks, vs = zip(*[w.chunk_kv(c) for c in range(3)])
+    Os, Ls = oracle.attention_samples(1, w.all_q(), w.q_indptr, ks, vs, np.array([0, 2, 3], np.int32),
+                                      np.array([2, 0, 1], np.int32), w.scale, np.array([3, 4]), np.array([1, 3]))
+    assert np.array_equal(Os[0], O[3, 1]) and np.array_equal(Os[1], O[4, 3]) and Ls[1] == L[4, 3]
+
+
+# ---- O3: table model ---------------------------------------------------------------------------------
+def test_o3_tables_hand_example():
+    m = oracle.PoolModel(10, 0)
+    assert m.store(7, 20) == [0, 1]          # ceil(20/16) = 2 pages from the head
+    assert m.store(9, 16) == [2]
+    assert m.store(3, 33) == [3, 4, 5]
+    t = m.link([[3, 7], [], [9, 7]])
+    assert t["page_indptr"].tolist() == [0, 5, 5, 8]
+    assert t["page_ids"].tolist() == [3, 4, 5, 0, 1, 2, 0, 1]
+    assert t["page_ntok"].tolist() == [16, 16, 1, 16, 4, 16, 16, 4]   # interior partial pages keep their count
+    assert t["kv_len"].tolist() == [53, 0, 36]
+    m.release(7)                              # freed ids go to the TAIL
+    assert m.store(11, 80) == [6, 7, 8, 9, 0]
+    with pytest.raises(MemoryError):
+        m.store(12, 40)
+
+
+def test_o3_shuffled_free_list_is_a_permutation():
+    a = oracle.initial_free_list(1000, 12345)
+    assert sorted(a) == list(range(1000)) and a != list(range(1000))
+    assert a == oracle.initial_free_list(1000, 12345)
+    assert oracle.initial_free_list(5, 0) == [0, 1, 2, 3, 4]
+    # first splitmix64 output for seed 1 is a published constant of the generator
+    g = oracle._splitmix64_stream(1)
+    assert next(g) == 0x910A2DEC89025CC1
+
+
+# ---- O2: page image round trip -------------------------------------------------------------------------
+def test_o2_page_image_round_trip():
+    rng = np.random.default_rng(5)
+    x = rng.integers(0, 2**16, (37, 2, 8), dtype=np.uint16)
+    pages = [4, 1, 6]
+    img = oracle.page_image(8, 2, 8, [(x, pages)])
+    back = np.concatenate([np.transpose(img[p], (1, 0, 2)) for p in pages], 0)   # gather pages back
+    assert np.array_equal(back[:37], x) and np.all(back[37:] == 0)
+    assert np.all(img[[0, 2, 3, 5, 7]] == 0x7FC0)
+
+
+# ---- P16: layer-count sanity of the pool byte formula ("saves 75%") -------------------
+def test_p16_kv_saving():
+    per_layer = 1024 * 8 * (128 + 128) * 2
+    assert 1.0 - (8 * per_layer) / (32 * per_layer) == GOLD["kv_saving_llama"]
+
+
+# ---- bf16 helpers used by every generator ----------------------------------------------------------------
+def test_bf16_rounding_is_rne():
+    x = np.array([1.0, 1.00390625, 1.01171875, -2.5, 3.0e-5], np.float32)   # 1+2^-8 ties to even (1.0); 1+3*2^-8 ties up
+    b = cs.f32_to_bf16_bits(x)
+    assert b[0] == 0x3F80 and b[1] == 0x3F80 and b[2] == 0x3F82 and b[3] == 0xC020
+    assert np.array_equal(cs.f32_to_bf16_bits(cs.bf16_bits_to_f32(b)), b)
+    torch = pytest.importorskip("torch")
+    y = np.random.default_rng(0).standard_normal(4096).astype(np.float32)
+    ref = torch.from_numpy(y).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+    assert np.array_equal(cs.f32_to_bf16_bits(y), ref)
