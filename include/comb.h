@@ -1,0 +1,191 @@
+/*
+ * comb.h — C ABI of the COMB link-stage hot path on B200 (sm_100a).
+ *
+ * The calls follow the paper's compile/link statement of the problem (arxiv 2602.01519;
+ * PAPER.md = the text under /root/reference at authoring time):
+ *   lookup -> (miss) allocate -> compile -> store -> update table -> fetch/link -> attend with the
+ *   query tokens -> attend with every generated token   (§3 steps 1-8, §5.3,
+ *   PAPER.md:66 §4).
+ *
+ * Conventions
+ *   - Every function returns int32_t: COMB_OK (0) or a negative comb_status_t. No exception or abort
+ *     crosses the ABI.
+ *   - "device" pointers are CUDA device pointers on the current device; "host" pointers are ordinary
+ *     host memory. `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   - NO function synchronises the device. Kernels and copies are enqueued on `stream`. (A call may
+ *     block the host on an event only when its staging ring of 4 slots is full, i.e. the GPU is four
+ *     calls behind.)
+ *   - The library allocates NO device memory: arenas, scratch, link buffers, Q/O and workspace are
+ *     allocated by the caller (PyTorch) and stay caller-owned; they must outlive their use on the
+ *     stream. Host metadata (directory, free list, pinned staging) belongs to the pool and is freed by
+ *     comb_pool_destroy.
+ *   - A pool is not thread-safe; callers serialise. A store and a later attention call that reads the
+ *     chunk must be ordered by the caller (same stream, or an event) — the paper stores PICaches
+ *     "asynchronously".
+ *   - dtype: bf16 storage for Q, K, V and O (bit patterns, 2 bytes); fp32 statistics (lse).
+ *
+ * Layout of the chunk-KV pool (part of the bit-exact contract)
+ *   K arena  bf16 [num_layers][num_pages][num_kv_heads][16][head_dim_qk]
+ *   V arena  bf16 [num_layers][num_pages][num_kv_heads][16][head_dim_v]
+ *   One (page, kv-head) block is a contiguous 16 x D burst. Slots of a chunk's last page beyond its
+ *   length are zero-filled by the store. Pages owned by no chunk are never touched.
+ *
+ * Allocation policy (part of the contract, so block tables are reproducible)
+ *   FIFO free list, initially 0,1,...,num_pages-1 (or the seeded permutation below); a chunk of T
+ *   tokens takes ceil(T/16) ids from the head; comb_chunk_free appends a chunk's ids to the tail in
+ *   page-list order. Page ids are shared by all layers (a chunk has one page list).
+ */
+#ifndef COMB_H_
+#define COMB_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    COMB_OK = 0,
+    COMB_ERR_INVALID = -1,       /* null pointer, page_size != 16, head dims outside {64,128,192}x{64,128},
+                                    Hq % Hkv != 0 or an unsupported group size, num_tokens <= 0, layer out of
+                                    range, non-monotone indptr */
+    COMB_ERR_NO_SPACE = -2,      /* store/alloc needs more pages than are free; nothing allocated */
+    COMB_ERR_EXISTS = -3,        /* chunk id already present with a different length */
+    COMB_ERR_UNKNOWN_CHUNK = -4, /* link/free/query names an id that is not in the directory (the caller
+                                    must compile + store first, PAPER.md:62 step 2); nothing is written */
+    COMB_ERR_CAPACITY = -5,      /* link buffer, scratch or workspace too small */
+    COMB_ERR_CUDA = -6           /* a CUDA call failed; cudaGetLastError() is preserved for the caller */
+} comb_status_t;
+
+typedef struct comb_pool comb_pool_t; /* opaque */
+
+/* (a1) chunk-KV pool + chunk directory — PAPER.md:205 "reserves a portion ... of GPU memory, initializes
+ * the PIC allocator"; PAPER.md:62 step 1/4 the hash table context -> PICache. */
+typedef struct {
+    int32_t num_layers;    /* cross-attention layers sharing one page-id space (>= 1) */
+    int32_t num_kv_heads;  /* Hkv */
+    int32_t head_dim_qk;   /* Dqk in {64, 128, 192} */
+    int32_t head_dim_v;    /* Dv  in {64, 128} */
+    int32_t page_size;     /* must be 16 */
+    int32_t num_pages;     /* pages per layer */
+    void *k_arena;         /* device, bf16, comb_pool_bytes().k_bytes, 1024-byte aligned */
+    void *v_arena;         /* device, bf16, comb_pool_bytes().v_bytes, 1024-byte aligned */
+    void *scratch;         /* device, comb_pool_bytes().scratch_bytes: store page descriptors (ring of 4) */
+    uint64_t free_list_shuffle_seed; /* 0: ascending ids. Else: Fisher-Yates (i = n-1..1, j = next() mod
+                                        (i+1), swap) driven by splitmix64(seed) — scatters a chunk's pages
+                                        over the arena like a long-running server would */
+} comb_pool_config_t;
+
+/* Sizes the caller must allocate for a config (pointers in cfg are ignored). */
+int32_t comb_pool_bytes(const comb_pool_config_t *cfg, size_t *k_bytes, size_t *v_bytes, size_t *scratch_bytes);
+
+/* Validates cfg, builds the free list and an empty directory. Touches no device memory. */
+int32_t comb_pool_create(const comb_pool_config_t *cfg, comb_pool_t **out);
+int32_t comb_pool_destroy(comb_pool_t *pool);
+int32_t comb_pool_free_pages(const comb_pool_t *pool); /* pages currently on the free list (>= 0) */
+
+/* Directory-only half of a store: insert chunk_id with num_tokens and take ceil(T/16) pages from the head
+ * of the free list; no data moves (a fused producer may write the pages itself). Idempotent for an
+ * existing id with the same length; COMB_ERR_EXISTS for a different length. */
+int32_t comb_chunk_alloc(comb_pool_t *pool, uint64_t chunk_id, int32_t num_tokens);
+/* Remove the chunk; its pages go to the free-list tail in page-list order. */
+int32_t comb_chunk_free(comb_pool_t *pool, uint64_t chunk_id);
+/* Lookup (PAPER.md:62 step 1). Writes num_tokens and up to `cap` page ids (host); returns the number of
+ * pages (>= 0) or COMB_ERR_UNKNOWN_CHUNK. `pages` may be NULL when cap == 0. */
+int32_t comb_chunk_query(const comb_pool_t *pool, uint64_t chunk_id, int32_t *num_tokens, int32_t *pages,
+                         int32_t cap);
+
+/* (a2) paged store of one chunk's K/V — PAPER.md:62 step 3, "stored asynchronously",
+ * PAPER.md:119 (store K^cross and V^cross, not H^E; Eq. 5-6 produce them as [T][H][D]).
+ *   k  device bf16 [num_tokens][Hkv][Dqk] contiguous;  v  device bf16 [num_tokens][Hkv][Dv] contiguous
+ * For t < T, head h:  Kpage[layer][pages[t/16]][h][t%16][:] = k[t][h][:]  (same for V); slots T%16..15 of
+ * the last page are zero-filled. Allocates the page list on the first store of chunk_id (any layer);
+ * stores on other layers reuse it. Errors: INVALID, NO_SPACE, EXISTS, CUDA. */
+int32_t comb_store_chunk(comb_pool_t *pool, int32_t layer, uint64_t chunk_id, int32_t num_tokens, const void *k,
+                         const void *v, void *stream);
+/* Batched form, one kernel launch: chunk i has tokens tok_indptr[i]..tok_indptr[i+1] (host int32 [n+1]) of the
+ * packed device tensors k_packed [sum T][Hkv][Dqk], v_packed [sum T][Hkv][Dv]. All-or-nothing on error. */
+int32_t comb_store_chunks(comb_pool_t *pool, int32_t layer, int32_t n, const uint64_t *chunk_ids,
+                          const int32_t *tok_indptr, const void *k_packed, const void *v_packed, void *stream);
+
+/* (a3) link — PAPER.md:24 "loads and concatenates needed KV vectors (in any order/position)",
+ * PAPER.md:119, PAPER.md:62 step 5.  Zero-copy: builds the request's block table from an ORDERED
+ * chunk-id list; no kernel touches K/V.
+ *
+ * The caller provides device_buf (comb_link_bytes() bytes, 16-byte aligned). comb_link lays the tables
+ * out inside it, fills the pointers below and enqueues ONE host->device copy on `stream`.
+ *   page_indptr int32 [R+1]      page range of request r in page_ids / page_ntok
+ *   page_ids    int32 [total]    pages(c_0) || ... || pages(c_{m-1}) in the caller's order
+ *   page_ntok   int32 [total]    16, except the last page of each chunk = T - 16*(npages-1)
+ *   kv_len      int32 [R]        sum of the linked chunks' lengths
+ *   tile_indptr int32 [R+1]      tile range of request r in tile_ntok (a tile = 8 consecutive table
+ *                                entries of the request, i.e. 128 slots, counted from its first page)
+ *   tile_ntok   uint64 [tiles]   byte j = page_ntok of entry 8*t+j, 0 past the request's last page
+ *                                (derived from page_ntok; lets kernels skip the slot mask on full tiles)
+ * A request with zero chunks is legal (kv_len 0). Duplicate ids inside a request are taken literally.
+ * Errors: INVALID, UNKNOWN_CHUNK (nothing written), CAPACITY, CUDA. */
+typedef struct {
+    /* in: caller-owned device memory */
+    void *device_buf;
+    size_t device_bytes;
+    /* out: device pointers into device_buf */
+    int32_t *page_indptr;
+    int32_t *page_ids;
+    int32_t *page_ntok;
+    int32_t *kv_len;
+    int32_t *tile_indptr;
+    uint64_t *tile_ntok;
+    /* out: host-side summary */
+    int32_t num_requests;
+    int32_t max_pages_per_request;
+    int64_t total_pages;
+    int64_t total_tiles;
+    int64_t total_kv_tokens;
+    size_t bytes_used; /* bytes of device_buf written = size of the single H2D copy */
+} comb_link_t;
+
+/* Bytes of device_buf that suffice for num_requests requests naming total_pages table entries. */
+size_t comb_link_bytes(int32_t num_requests, int64_t total_pages);
+int32_t comb_link(comb_pool_t *pool, int32_t num_requests, const int32_t *chunk_indptr /* host [R+1] */,
+                  const uint64_t *chunk_ids /* host, link order */, comb_link_t *link, void *stream);
+/* Same tables written into HOST memory `host_buf` (link->device_bytes bytes available); the pointers in
+ * `link` are laid out as if host_buf were device_buf. No CUDA call — used by comb_link and by host tests. */
+int32_t comb_link_plan(const comb_pool_t *pool, int32_t num_requests, const int32_t *chunk_indptr,
+                       const uint64_t *chunk_ids, comb_link_t *link, void *host_buf);
+
+/* (a4) prefill cross-attention — PAPER.md:112-115 §4.2 Eq. 7-8 (softmax(QK^T/sqrt d) V, NO mask), over the
+ * concatenation of the linked chunks; cost O(l_query * l_doc) per layer (Eq. 12).
+ *   q         device bf16 [sum lq][Hq][Dqk];   q_indptr  HOST int32 [R+1] (rows of request r)
+ *   out       device bf16 [sum lq][Hq][Dv];    lse       device fp32 [sum lq][Hq] or NULL
+ *   scale     multiplies q.k before the softmax (the paper's 1/sqrt(d), per head: 1/sqrt(Dqk))
+ *   workspace device, comb_workspace_bytes() bytes, 16-byte aligned
+ * q-head h reads kv-head h / (Hq/Hkv). kv_len == 0 gives out = 0, lse = -inf. tcgen05/TMEM/TMA kernel.
+ * Errors: INVALID, CAPACITY, CUDA. */
+int32_t comb_cross_attn_prefill(comb_pool_t *pool, int32_t layer, const comb_link_t *link, int32_t num_requests,
+                                const void *q, const int32_t *q_indptr, int32_t num_q_heads, float scale, void *out,
+                                float *lse, void *workspace, size_t workspace_bytes, void *stream);
+
+/* (a5) decode cross-attention — the same function with exactly one query row per request (PAPER.md:66:
+ * generated tokens are "treated identically to the initial query tokens").
+ *   q device bf16 [R][Hq][Dqk];  out device bf16 [R][Hq][Dv];  lse device fp32 [R][Hq] or NULL
+ * Split-KV kernel (HBM-bound, CUDA cores) + LSE-merge kernel. Errors as above. */
+int32_t comb_cross_attn_decode(comb_pool_t *pool, int32_t layer, const comb_link_t *link, int32_t num_requests,
+                               const void *q, int32_t num_q_heads, float scale, void *out, float *lse,
+                               void *workspace, size_t workspace_bytes, void *stream);
+
+/* Workspace that suffices for either attention call: num_requests requests, num_q_heads heads, total_q
+ * query rows, max_pages_per_request table entries in the longest request. */
+size_t comb_workspace_bytes(const comb_pool_t *pool, int32_t num_requests, int32_t num_q_heads, int64_t total_q,
+                            int32_t max_pages_per_request);
+
+/* Kernels launched by this library since the pool was created (store/attention/reduce; copies excluded). */
+int64_t comb_pool_launch_count(const comb_pool_t *pool);
+
+const char *comb_strerror(int32_t status);
+const char *comb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* COMB_H_ */

@@ -1,0 +1,70 @@
+// kernels.h — host-side launch interface between the C-ABI runtime (comb_host.cu) and the sm_100a
+// kernels (store_kernel.cu, decode_kernel.cu, prefill_kernel.cu).  Internal; not part of the ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+namespace comb {
+
+constexpr int kPage = 16;            // tokens per page (BASELINE.json)
+constexpr int kTilePages = 8;        // pages per 128-slot KV tile
+constexpr int kTileSlots = kPage * kTilePages;
+
+// One destination page of a (batched) store.  16 bytes, read once per CTA.
+struct StorePageDesc {
+    int32_t dst_page;   // page id inside the layer
+    int32_t src_tok;    // first token row of this page in the packed source tensors
+    int32_t ntok;       // valid tokens in this page (1..16); slots beyond are zero-filled
+    int32_t pad;
+};
+
+struct PoolGeom {
+    int32_t num_layers, num_kv_heads, head_dim_qk, head_dim_v, num_pages;
+    void *k_arena, *v_arena;
+};
+
+// Device pointers of a link (see comb_link_t in include/comb.h).
+struct LinkView {
+    const int32_t *page_indptr, *page_ids, *page_ntok, *kv_len, *tile_indptr;
+    const uint64_t *tile_ntok;
+};
+
+// ---- (a2) store -------------------------------------------------------------------------------
+cudaError_t launch_store(const PoolGeom &g, int layer, const StorePageDesc *descs_dev, int num_descs,
+                         const void *k_src, const void *v_src, cudaStream_t stream);
+
+// ---- (a5) decode ------------------------------------------------------------------------------
+struct DecodePlan {
+    int chunk_pages;   // table entries per split (multiple of the warps per CTA)
+    int num_splits;    // splits of the longest request
+};
+DecodePlan make_decode_plan(int num_requests, int num_kv_heads, int max_pages_per_request, int num_sms);
+size_t decode_workspace_bytes(int num_requests, int num_q_heads, int head_dim_v, const DecodePlan &p);
+bool decode_supported(int group, int dqk, int dv);
+// launches the split kernel and (if num_splits > 1) the merge kernel; *launches += kernels launched
+cudaError_t launch_decode(const PoolGeom &g, int layer, const LinkView &lv, int num_requests, int num_q_heads,
+                          const void *q, float scale, void *out, float *lse, void *workspace, const DecodePlan &p,
+                          cudaStream_t stream, int *launches);
+
+// ---- (a4) prefill -----------------------------------------------------------------------------
+// One CTA work item: up to two consecutive 128-row Q tiles of one (request, kv-head).
+struct PrefillItem {
+    int32_t request;
+    int32_t kv_head;
+    int32_t q_row0;     // first query token row (absolute row in q) of tile 0
+    int32_t q_rows;     // valid query tokens in this item (1 .. 2*128/G)
+};
+bool prefill_supported(int group, int dqk, int dv);
+// CUtensorMap is 128 bytes, 64-byte aligned; kept opaque here so the runtime needs no cuda.h.
+struct alignas(64) TensorMapBlob { unsigned char bytes[128]; };
+struct PrefillMaps { TensorMapBlob q, k, v; };
+// Encodes the TMA maps (k/v depend on pool + layer-independent geometry; q on the call).
+cudaError_t prefill_encode_kv_maps(const PoolGeom &g, TensorMapBlob *k_map, TensorMapBlob *v_map);
+cudaError_t prefill_encode_q_map(const void *q, int64_t total_q, int num_q_heads, int group, int dqk,
+                                 TensorMapBlob *q_map);
+cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &maps,
+                           const PrefillItem *items_dev, int num_items, int num_q_heads, float scale, void *out,
+                           float *lse, cudaStream_t stream);
+
+}  // namespace comb
