@@ -158,7 +158,8 @@ int32_t comb_link_plan(const comb_pool_t *pool, int32_t num_requests, const int3
  * concatenation of the linked chunks; cost O(l_query * l_doc) per layer (Eq. 12).
  *   q         device bf16 [sum lq][Hq][Dqk];   q_indptr  HOST int32 [R+1] (rows of request r)
  *   out       device bf16 [sum lq][Hq][Dv];    lse       device fp32 [sum lq][Hq] or NULL
- *   scale     multiplies q.k before the softmax (the paper's 1/sqrt(d), per head: 1/sqrt(Dqk))
+ *   scale     multiplies q.k before the softmax (the paper's 1/sqrt(d), per head: 1/sqrt(Dqk)); must be a
+ *             finite positive number (INVALID otherwise)
  *   workspace device, comb_workspace_bytes() bytes, 16-byte aligned
  * q-head h reads kv-head h / (Hq/Hkv). kv_len == 0 gives out = 0, lse = -inf. tcgen05/TMEM/TMA kernel.
  * Errors: INVALID, CAPACITY, CUDA. */
@@ -181,6 +182,15 @@ size_t comb_workspace_bytes(const comb_pool_t *pool, int32_t num_requests, int32
 
 /* Kernels launched by this library since the pool was created (store/attention/reduce; copies excluded). */
 int64_t comb_pool_launch_count(const comb_pool_t *pool);
+
+/* Optional per-kernel device timing (bench.py uses it for the roofline of the dominant kernel). While enabled,
+ * every kernel this pool launches is bracketed by two CUDA events recorded on the launching stream.
+ * comb_profile_read synchronises on the recorded events (the one call here that waits for the device), adds up
+ * the elapsed times of kernel class `kernel` (COMB_KERNEL_*), reports them and forgets those records.
+ * Errors: INVALID, CUDA. */
+enum { COMB_KERNEL_STORE = 0, COMB_KERNEL_DECODE_SPLIT = 1, COMB_KERNEL_DECODE_MERGE = 2, COMB_KERNEL_PREFILL = 3 };
+int32_t comb_profile_enable(comb_pool_t *pool, int32_t on);
+int32_t comb_profile_read(comb_pool_t *pool, int32_t kernel, double *total_ms, int64_t *launches);
 
 const char *comb_strerror(int32_t status);
 const char *comb_version(void);

@@ -1,0 +1,291 @@
+"""Python binding of the C ABI in include/comb.h — same names, argument marshalling only.
+
+PyTorch is used here for device memory and streams (plumbing); every step of the path (store, link,
+prefill and decode cross-attention: §3 steps 1-8, §4.2 Eq. 7-8) runs inside
+libcomb.so.  ``Pool`` owns the torch allocations the library asks the caller to provide.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+import torch
+
+from . import _lib
+from ._lib import CombError, Link, PoolConfig, check, lib
+
+PAGE = 16
+
+
+def _ptr(t) -> Optional[int]:
+    if t is None:
+        return None
+    if isinstance(t, torch.Tensor):
+        return t.data_ptr()
+    if isinstance(t, np.ndarray):
+        return t.ctypes.data
+    return int(t)
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else None
+    if isinstance(stream, torch.cuda.Stream):
+        return stream.cuda_stream
+    return int(stream)
+
+
+# ------------------------------------------------------------------------------------------------
+# the C calls, one to one
+# ------------------------------------------------------------------------------------------------
+def comb_pool_bytes(num_layers: int, num_kv_heads: int, head_dim_qk: int, head_dim_v: int, num_pages: int,
+                    page_size: int = PAGE) -> Tuple[int, int, int]:
+    cfg = PoolConfig(num_layers, num_kv_heads, head_dim_qk, head_dim_v, page_size, num_pages, None, None, None, 0)
+    k, v, s = C.c_size_t(), C.c_size_t(), C.c_size_t()
+    check(lib.comb_pool_bytes(C.byref(cfg), C.byref(k), C.byref(v), C.byref(s)), "comb_pool_bytes")
+    return k.value, v.value, s.value
+
+
+def comb_pool_create(cfg: PoolConfig) -> int:
+    out = C.c_void_p()
+    check(lib.comb_pool_create(C.byref(cfg), C.byref(out)), "comb_pool_create")
+    return out.value
+
+
+def comb_pool_destroy(pool: int) -> None:
+    check(lib.comb_pool_destroy(pool), "comb_pool_destroy")
+
+
+def comb_chunk_alloc(pool: int, chunk_id: int, num_tokens: int) -> None:
+    check(lib.comb_chunk_alloc(pool, chunk_id, num_tokens), "comb_chunk_alloc")
+
+
+def comb_chunk_free(pool: int, chunk_id: int) -> None:
+    check(lib.comb_chunk_free(pool, chunk_id), "comb_chunk_free")
+
+
+def comb_chunk_query(pool: int, chunk_id: int) -> Tuple[int, np.ndarray]:
+    """(num_tokens, page ids) of a stored chunk."""
+    nt = C.c_int32()
+    n = check(lib.comb_chunk_query(pool, chunk_id, C.byref(nt), None, 0), "comb_chunk_query")
+    pages = np.zeros(max(n, 1), dtype=np.int32)
+    check(lib.comb_chunk_query(pool, chunk_id, C.byref(nt), pages.ctypes.data, n), "comb_chunk_query")
+    return nt.value, pages[:n]
+
+
+def comb_store_chunk(pool: int, layer: int, chunk_id: int, num_tokens: int, k, v, stream=None) -> None:
+    check(lib.comb_store_chunk(pool, layer, chunk_id, num_tokens, _ptr(k), _ptr(v), _stream_ptr(stream)),
+          "comb_store_chunk")
+
+
+def comb_store_chunks(pool: int, layer: int, chunk_ids: Sequence[int], tok_indptr, k_packed, v_packed,
+                      stream=None) -> None:
+    ids = np.ascontiguousarray(chunk_ids, dtype=np.uint64)
+    ind = np.ascontiguousarray(tok_indptr, dtype=np.int32)
+    check(lib.comb_store_chunks(pool, layer, int(ids.shape[0]), ids.ctypes.data, ind.ctypes.data, _ptr(k_packed),
+                                _ptr(v_packed), _stream_ptr(stream)), "comb_store_chunks")
+
+
+def comb_link_bytes(num_requests: int, total_pages: int) -> int:
+    return int(lib.comb_link_bytes(num_requests, total_pages))
+
+
+def comb_link(pool: int, chunk_indptr, chunk_ids, link: Link, stream=None) -> Link:
+    ind = np.ascontiguousarray(chunk_indptr, dtype=np.int32)
+    ids = np.ascontiguousarray(chunk_ids, dtype=np.uint64)
+    check(lib.comb_link(pool, int(ind.shape[0]) - 1, ind.ctypes.data, ids.ctypes.data if ids.size else None,
+                        C.byref(link), _stream_ptr(stream)), "comb_link")
+    return link
+
+
+def comb_link_plan(pool: int, chunk_indptr, chunk_ids, link: Link, host_buf: np.ndarray) -> Link:
+    """Host-only table build (no CUDA call); ``host_buf`` is a uint8 array of link.device_bytes bytes."""
+    ind = np.ascontiguousarray(chunk_indptr, dtype=np.int32)
+    ids = np.ascontiguousarray(chunk_ids, dtype=np.uint64)
+    check(lib.comb_link_plan(pool, int(ind.shape[0]) - 1, ind.ctypes.data, ids.ctypes.data if ids.size else None,
+                             C.byref(link), host_buf.ctypes.data), "comb_link_plan")
+    return link
+
+
+def comb_workspace_bytes(pool: int, num_requests: int, num_q_heads: int, total_q: int, max_pages: int) -> int:
+    return int(lib.comb_workspace_bytes(pool, num_requests, num_q_heads, total_q, max_pages))
+
+
+def comb_cross_attn_prefill(pool: int, layer: int, link: Link, q, q_indptr, num_q_heads: int, scale: float, out,
+                            lse=None, workspace=None, workspace_bytes: int = 0, stream=None) -> None:
+    ind = np.ascontiguousarray(q_indptr, dtype=np.int32)
+    check(lib.comb_cross_attn_prefill(pool, layer, C.byref(link), int(ind.shape[0]) - 1, _ptr(q), ind.ctypes.data,
+                                      num_q_heads, float(scale), _ptr(out), _ptr(lse), _ptr(workspace),
+                                      int(workspace_bytes), _stream_ptr(stream)), "comb_cross_attn_prefill")
+
+
+def comb_cross_attn_decode(pool: int, layer: int, link: Link, num_requests: int, q, num_q_heads: int, scale: float,
+                           out, lse=None, workspace=None, workspace_bytes: int = 0, stream=None) -> None:
+    check(lib.comb_cross_attn_decode(pool, layer, C.byref(link), num_requests, _ptr(q), num_q_heads, float(scale),
+                                     _ptr(out), _ptr(lse), _ptr(workspace), int(workspace_bytes),
+                                     _stream_ptr(stream)), "comb_cross_attn_decode")
+
+
+def comb_pool_launch_count(pool: int) -> int:
+    return int(lib.comb_pool_launch_count(pool))
+
+
+KERNEL_STORE, KERNEL_DECODE_SPLIT, KERNEL_DECODE_MERGE, KERNEL_PREFILL = 0, 1, 2, 3
+
+
+def comb_profile_enable(pool: int, on: bool) -> None:
+    check(lib.comb_profile_enable(pool, 1 if on else 0), "comb_profile_enable")
+
+
+def comb_profile_read(pool: int, kernel: int) -> Tuple[float, int]:
+    """(total device ms, launches) of one kernel class since the last read; waits for those launches."""
+    ms, n = C.c_double(), C.c_int64()
+    check(lib.comb_profile_read(pool, kernel, C.byref(ms), C.byref(n)), "comb_profile_read")
+    return ms.value, n.value
+
+
+def comb_version() -> str:
+    return lib.comb_version().decode()
+
+
+# ------------------------------------------------------------------------------------------------
+# convenience owner of the caller-side allocations (torch = memory + streams only)
+# ------------------------------------------------------------------------------------------------
+class LinkedBatch:
+    """A comb_link_t plus the torch buffer that backs it."""
+
+    def __init__(self, link: Link, buf: torch.Tensor):
+        self.link, self.buf = link, buf
+
+    def _view(self, ptr: int, n: int, dtype: torch.dtype) -> torch.Tensor:
+        off = ptr - self.buf.data_ptr()
+        return self.buf[off:off + n * torch.empty((), dtype=dtype).element_size()].view(dtype)
+
+    @property
+    def num_requests(self) -> int:
+        return self.link.num_requests
+
+    def tables(self) -> dict:
+        """Device tables copied to host numpy arrays (synchronises)."""
+        L = self.link
+        R, n, t = L.num_requests, int(L.total_pages), int(L.total_tiles)
+        return {
+            "page_indptr": self._view(L.page_indptr, R + 1, torch.int32).cpu().numpy(),
+            "page_ids": self._view(L.page_ids, n, torch.int32).cpu().numpy(),
+            "page_ntok": self._view(L.page_ntok, n, torch.int32).cpu().numpy(),
+            "kv_len": self._view(L.kv_len, R, torch.int32).cpu().numpy(),
+            "tile_indptr": self._view(L.tile_indptr, R + 1, torch.int32).cpu().numpy(),
+            "tile_ntok": self._view(L.tile_ntok, t, torch.int64).cpu().numpy().view(np.uint64),
+        }
+
+
+class Pool:
+    """Chunk-KV pool (a1): allocates the arenas with torch and forwards every call to libcomb.so."""
+
+    def __init__(self, num_kv_heads: int, head_dim_qk: int, head_dim_v: int, num_pages: int, num_layers: int = 1,
+                 shuffle_seed: int = 0, device: str = "cuda", sentinel: Optional[int] = None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2602_01519_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.device = torch.device(device)
+        self.num_layers, self.num_kv_heads = num_layers, num_kv_heads
+        self.head_dim_qk, self.head_dim_v, self.num_pages = head_dim_qk, head_dim_v, num_pages
+        kb, vb, sb = comb_pool_bytes(num_layers, num_kv_heads, head_dim_qk, head_dim_v, num_pages)
+        # arenas as int16 bit patterns [L][pages][Hkv][16][D]; optional sentinel (e.g. 0x7FC0 = bf16 NaN) for tests
+        self.k_arena = self._aligned_i16(kb)
+        self.v_arena = self._aligned_i16(vb)
+        if sentinel is not None:
+            s = int(np.array(sentinel, dtype=np.uint16).view(np.int16))
+            self.k_arena.fill_(s)
+            self.v_arena.fill_(s)
+        self.scratch = torch.empty(max(sb, 256), dtype=torch.uint8, device=self.device)
+        self.cfg = PoolConfig(num_layers, num_kv_heads, head_dim_qk, head_dim_v, PAGE, num_pages,
+                              self.k_arena.data_ptr(), self.v_arena.data_ptr(), self.scratch.data_ptr(), shuffle_seed)
+        self.handle = comb_pool_create(self.cfg)
+        self._ws: Optional[torch.Tensor] = None
+
+    def _aligned_i16(self, nbytes: int, align: int = 1024) -> torch.Tensor:
+        raw = torch.empty(nbytes // 2 + align // 2, dtype=torch.int16, device=self.device)
+        off = (-raw.data_ptr()) % align
+        return raw[off // 2: off // 2 + nbytes // 2]
+
+    def close(self) -> None:
+        if self.handle:
+            torch.cuda.synchronize()
+            comb_pool_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- (a2) store ----
+    def store_chunk(self, chunk_id: int, k: torch.Tensor, v: torch.Tensor, layer: int = 0, stream=None) -> None:
+        comb_store_chunk(self.handle, layer, chunk_id, int(k.shape[0]), k, v, stream)
+
+    def store_chunks(self, chunk_ids, tok_indptr, k_packed: torch.Tensor, v_packed: torch.Tensor, layer: int = 0,
+                     stream=None) -> None:
+        comb_store_chunks(self.handle, layer, chunk_ids, tok_indptr, k_packed, v_packed, stream)
+
+    # ---- (a3) link ----
+    def link(self, chunk_lists: Sequence[Sequence[int]], stream=None, into: Optional[LinkedBatch] = None) -> LinkedBatch:
+        indptr = np.zeros(len(chunk_lists) + 1, dtype=np.int32)
+        np.cumsum([len(c) for c in chunk_lists], out=indptr[1:])
+        ids = (np.concatenate([np.asarray(c, dtype=np.uint64) for c in chunk_lists])
+               if indptr[-1] else np.zeros(0, dtype=np.uint64))
+        return self.link_flat(indptr, ids, stream, into)
+
+    def link_flat(self, chunk_indptr: np.ndarray, chunk_ids: np.ndarray, stream=None,
+                  into: Optional[LinkedBatch] = None) -> LinkedBatch:
+        R = int(chunk_indptr.shape[0]) - 1
+        if into is None:
+            total_pages = 0
+            for c in np.asarray(chunk_ids).tolist():
+                nt = C.c_int32()
+                total_pages += check(lib.comb_chunk_query(self.handle, int(c), C.byref(nt), None, 0), "comb_link")
+            nbytes = comb_link_bytes(R, total_pages)
+            buf = torch.empty(max(nbytes, 16), dtype=torch.uint8, device=self.device)
+            into = LinkedBatch(Link(), buf)
+        into.link.device_buf = into.buf.data_ptr()
+        into.link.device_bytes = into.buf.numel()
+        comb_link(self.handle, chunk_indptr, chunk_ids, into.link, stream)
+        return into
+
+    # ---- (a4)/(a5) attention ----
+    def workspace(self, num_requests: int, num_q_heads: int, total_q: int, max_pages: int) -> torch.Tensor:
+        need = comb_workspace_bytes(self.handle, num_requests, num_q_heads, total_q, max_pages)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = torch.empty(max(need, 256), dtype=torch.uint8, device=self.device)
+        return self._ws
+
+    def prefill(self, lb: LinkedBatch, q: torch.Tensor, q_indptr, scale: float, out: Optional[torch.Tensor] = None,
+                lse: Optional[torch.Tensor] = None, layer: int = 0, want_lse: bool = True, stream=None):
+        total_q, Hq = int(q.shape[0]), int(q.shape[1])
+        if out is None:
+            out = torch.empty((total_q, Hq, self.head_dim_v), dtype=q.dtype, device=self.device)
+        if lse is None and want_lse:
+            lse = torch.empty((total_q, Hq), dtype=torch.float32, device=self.device)
+        ws = self.workspace(lb.num_requests, Hq, total_q, lb.link.max_pages_per_request)
+        comb_cross_attn_prefill(self.handle, layer, lb.link, q, q_indptr, Hq, scale, out, lse, ws, ws.numel(), stream)
+        return out, lse
+
+    def decode(self, lb: LinkedBatch, q: torch.Tensor, scale: float, out: Optional[torch.Tensor] = None,
+               lse: Optional[torch.Tensor] = None, layer: int = 0, want_lse: bool = True, stream=None):
+        R, Hq = int(q.shape[0]), int(q.shape[1])
+        if out is None:
+            out = torch.empty((R, Hq, self.head_dim_v), dtype=q.dtype, device=self.device)
+        if lse is None and want_lse:
+            lse = torch.empty((R, Hq), dtype=torch.float32, device=self.device)
+        ws = self.workspace(R, Hq, R, lb.link.max_pages_per_request)
+        comb_cross_attn_decode(self.handle, layer, lb.link, R, q, Hq, scale, out, lse, ws, ws.numel(), stream)
+        return out, lse
+
+    @property
+    def launches(self) -> int:
+        return comb_pool_launch_count(self.handle)
+
+    @property
+    def free_pages(self) -> int:
+        return int(lib.comb_pool_free_pages(self.handle))

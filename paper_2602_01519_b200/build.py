@@ -1,6 +1,6 @@
 """In-tree build of libcomb.so (C ABI of include/comb.h) with nvcc for sm_100a.
 
-    python -m paper_2602_01519_b200.build [--force]
+    python paper_2602_01519_b200/build.py [--force] [-v]      (run as a file: importing the package needs the library)
 
 One nvcc invocation per .cu (in parallel), then one link step.  cudart is linked statically and libcuda is
 reached through cudaGetDriverEntryPoint, so the library loads on a machine without a GPU driver (the

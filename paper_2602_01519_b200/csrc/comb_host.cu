@@ -49,6 +49,29 @@ struct comb_pool {
     bool kv_maps_ready = false;
     TensorMapBlob k_map, v_map;
     int64_t launches = 0;
+    // per-kernel timing (comb_profile_*)
+    struct ProfRec { int id; cudaEvent_t a, b; };
+    bool prof_on = false;
+    std::vector<ProfRec> prof_recs;
+    std::vector<cudaEvent_t> prof_free;
+    LaunchHook hook{};
+
+    cudaEvent_t prof_event() {
+        if (!prof_free.empty()) { cudaEvent_t e = prof_free.back(); prof_free.pop_back(); return e; }
+        cudaEvent_t e = nullptr;
+        if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+        return e;
+    }
+    static void hook_begin(void *ctx, int id, cudaStream_t st) {
+        comb_pool *p = (comb_pool *)ctx;
+        ProfRec r{id, p->prof_event(), p->prof_event()};
+        if (r.a && r.b) { cudaEventRecord(r.a, st); p->prof_recs.push_back(r); }
+    }
+    static void hook_end(void *ctx, cudaStream_t st) {
+        comb_pool *p = (comb_pool *)ctx;
+        if (!p->prof_recs.empty()) cudaEventRecord(p->prof_recs.back().b, st);
+    }
+    const LaunchHook *active_hook() { return prof_on ? &hook : nullptr; }
 
     size_t scratch_slot_bytes() const { return align_up((size_t)cfg.num_pages * sizeof(StorePageDesc), 256); }
 
@@ -230,6 +253,8 @@ int32_t comb_pool_create(const comb_pool_config_t *cfg, comb_pool_t **out) {
 
 int32_t comb_pool_destroy(comb_pool_t *p) {
     if (!p) return COMB_ERR_INVALID;
+    for (auto &r : p->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (auto &e : p->prof_free) cudaEventDestroy(e);
     for (auto &s : p->ring) {
         if (s.busy) cudaEventSynchronize(s.ev);
         if (s.ev) cudaEventDestroy(s.ev);
@@ -245,6 +270,34 @@ int32_t comb_pool_free_pages(const comb_pool_t *p) {
 }
 
 int64_t comb_pool_launch_count(const comb_pool_t *p) { return p ? p->launches : 0; }
+
+int32_t comb_profile_enable(comb_pool_t *p, int32_t on) {
+    if (!p) return COMB_ERR_INVALID;
+    p->hook = LaunchHook{&comb_pool::hook_begin, &comb_pool::hook_end, p};
+    p->prof_on = on != 0;
+    return COMB_OK;
+}
+
+int32_t comb_profile_read(comb_pool_t *p, int32_t kernel, double *total_ms, int64_t *launches) {
+    if (!p || kernel < 0 || kernel > 3) return COMB_ERR_INVALID;
+    double tot = 0.0;
+    int64_t n = 0;
+    std::vector<comb_pool::ProfRec> keep;
+    for (auto &r : p->prof_recs) {
+        if (r.id != kernel) { keep.push_back(r); continue; }
+        float ms = 0.f;
+        if (cudaEventSynchronize(r.b) != cudaSuccess || cudaEventElapsedTime(&ms, r.a, r.b) != cudaSuccess)
+            return COMB_ERR_CUDA;
+        tot += ms;
+        ++n;
+        p->prof_free.push_back(r.a);
+        p->prof_free.push_back(r.b);
+    }
+    p->prof_recs.swap(keep);
+    if (total_ms) *total_ms = tot;
+    if (launches) *launches = n;
+    return COMB_OK;
+}
 
 int32_t comb_chunk_alloc(comb_pool_t *p, uint64_t id, int32_t T) {
     if (!p) return COMB_ERR_INVALID;
@@ -323,7 +376,10 @@ int32_t comb_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, const uint64
     StorePageDesc *dev = (StorePageDesc *)((char *)p->cfg.scratch + (size_t)slot * p->scratch_slot_bytes());
     if (cudaMemcpyAsync(dev, h, at * sizeof(StorePageDesc), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return COMB_ERR_CUDA;
-    if (launch_store(p->geom, layer, dev, (int)at, k_packed, v_packed, st) != cudaSuccess) return COMB_ERR_CUDA;
+    if (p->prof_on) p->hook.begin(p, kKernelStore, st);
+    const cudaError_t se = launch_store(p->geom, layer, dev, (int)at, k_packed, v_packed, st);
+    if (p->prof_on) p->hook.end(p, st);
+    if (se != cudaSuccess) return COMB_ERR_CUDA;
     p->launches += 1;
     if (!p->release(slot, st)) return COMB_ERR_CUDA;
     return COMB_OK;
@@ -450,6 +506,7 @@ int32_t comb_cross_attn_decode(comb_pool_t *p, int32_t layer, const comb_link_t 
                                int32_t Hq, float scale, void *out, float *lse, void *ws, size_t ws_bytes,
                                void *stream) {
     if (!p || !link || R < 0 || Hq <= 0) return COMB_ERR_INVALID;
+    if (!(scale > 0.f) || scale > 3.0e38f) return COMB_ERR_INVALID;  // also rejects NaN
     if (layer < 0 || layer >= p->cfg.num_layers) return COMB_ERR_INVALID;
     if (Hq % p->cfg.num_kv_heads) return COMB_ERR_INVALID;
     if (R != link->num_requests) return COMB_ERR_INVALID;
@@ -463,7 +520,7 @@ int32_t comb_cross_attn_decode(comb_pool_t *p, int32_t layer, const comb_link_t 
     if (need > 0 && (!ws || ws_bytes < need)) return COMB_ERR_CAPACITY;
     int launches = 0;
     cudaError_t e = launch_decode(p->geom, layer, view_of(link), R, Hq, q, scale, out, lse, ws, plan,
-                                  (cudaStream_t)stream, &launches);
+                                  (cudaStream_t)stream, &launches, p->active_hook());
     p->launches += launches;
     return e == cudaSuccess ? COMB_OK : COMB_ERR_CUDA;
 }
@@ -472,6 +529,7 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
                                 const int32_t *q_indptr, int32_t Hq, float scale, void *out, float *lse, void *ws,
                                 size_t ws_bytes, void *stream) {
     if (!p || !link || R < 0 || Hq <= 0) return COMB_ERR_INVALID;
+    if (!(scale > 0.f) || scale > 3.0e38f) return COMB_ERR_INVALID;  // also rejects NaN
     if (layer < 0 || layer >= p->cfg.num_layers) return COMB_ERR_INVALID;
     if (Hq % p->cfg.num_kv_heads) return COMB_ERR_INVALID;
     if (R != link->num_requests) return COMB_ERR_INVALID;
@@ -523,8 +581,10 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
                 h[at++] = PrefillItem{x.r, g, row0 + (int32_t)t, (int32_t)std::min<int64_t>(tok_per_item, x.cost - t)};
     }
     if (cudaMemcpyAsync(ws, h, need, cudaMemcpyHostToDevice, st) != cudaSuccess) return COMB_ERR_CUDA;
+    if (p->prof_on) p->hook.begin(p, kKernelPrefill, st);
     cudaError_t e = launch_prefill(p->geom, layer, view_of(link), maps, (const PrefillItem *)ws, (int)num_items, Hq,
                                    scale, out, lse, st);
+    if (p->prof_on) p->hook.end(p, st);
     if (e != cudaSuccess) return COMB_ERR_CUDA;
     p->launches += 1;
     if (!p->release(slot, st)) return COMB_ERR_CUDA;

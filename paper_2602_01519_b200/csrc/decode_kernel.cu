@@ -369,17 +369,21 @@ __global__ void __launch_bounds__(DV) decode_merge_kernel(const DecodeArgs a) {
 }
 
 template <int G, int DQK, int DV>
-cudaError_t launch_t(const DecodeArgs &a, int R, bool merge, cudaStream_t st, int *launches) {
+cudaError_t launch_t(const DecodeArgs &a, int R, bool merge, cudaStream_t st, int *launches, const LaunchHook *hook) {
     using C = Cfg<G, DQK, DV>;
     auto kern = decode_split_kernel<G, DQK, DV>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     if (e != cudaSuccess) return e;
     dim3 grid(a.num_splits, a.num_kv_heads, R);
+    if (hook) hook->begin(hook->ctx, kKernelDecodeSplit, st);
     kern<<<grid, kThreads, C::SMEM, st>>>(a);
+    if (hook) hook->end(hook->ctx, st);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     *launches += 1;
     if (merge) {
+        if (hook) hook->begin(hook->ctx, kKernelDecodeMerge, st);
         decode_merge_kernel<DV><<<dim3(a.num_q_heads, R), DV, 0, st>>>(a);
+        if (hook) hook->end(hook->ctx, st);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         *launches += 1;
     }
@@ -419,7 +423,7 @@ size_t decode_workspace_bytes(int R, int Hq, int dv, const DecodePlan &p) {
 
 cudaError_t launch_decode(const PoolGeom &g, int layer, const LinkView &lv, int R, int Hq, const void *q, float scale,
                           void *out, float *lse, void *workspace, const DecodePlan &p, cudaStream_t stream,
-                          int *launches) {
+                          int *launches, const LaunchHook *hook) {
     DecodeArgs a;
     const size_t kb = (size_t)kPage * g.head_dim_qk * 2, vb = (size_t)kPage * g.head_dim_v * 2;
     a.k_layer = (const char *)g.k_arena + (size_t)layer * g.num_pages * g.num_kv_heads * kb;
@@ -440,7 +444,7 @@ cudaError_t launch_decode(const PoolGeom &g, int layer, const LinkView &lv, int 
     const bool merge = p.num_splits > 1;
     const int G = Hq / g.num_kv_heads;
 #define COMB_DECODE_CASE(GG, DQ, DVV) \
-    if (G == GG && g.head_dim_qk == DQ && g.head_dim_v == DVV) return launch_t<GG, DQ, DVV>(a, R, merge, stream, launches);
+    if (G == GG && g.head_dim_qk == DQ && g.head_dim_v == DVV) return launch_t<GG, DQ, DVV>(a, R, merge, stream, launches, hook);
     COMB_DECODE_CASE(4, 128, 128)
     COMB_DECODE_CASE(4, 64, 64)
     COMB_DECODE_CASE(1, 192, 128)

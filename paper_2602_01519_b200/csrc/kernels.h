@@ -19,6 +19,14 @@ struct StorePageDesc {
     int32_t pad;
 };
 
+// Optional bracket around a kernel launch (per-kernel CUDA-event timing, comb_profile_*).
+struct LaunchHook {
+    void (*begin)(void *ctx, int kernel_id, cudaStream_t st);
+    void (*end)(void *ctx, cudaStream_t st);
+    void *ctx;
+};
+enum { kKernelStore = 0, kKernelDecodeSplit = 1, kKernelDecodeMerge = 2, kKernelPrefill = 3 };
+
 struct PoolGeom {
     int32_t num_layers, num_kv_heads, head_dim_qk, head_dim_v, num_pages;
     void *k_arena, *v_arena;
@@ -45,7 +53,7 @@ bool decode_supported(int group, int dqk, int dv);
 // launches the split kernel and (if num_splits > 1) the merge kernel; *launches += kernels launched
 cudaError_t launch_decode(const PoolGeom &g, int layer, const LinkView &lv, int num_requests, int num_q_heads,
                           const void *q, float scale, void *out, float *lse, void *workspace, const DecodePlan &p,
-                          cudaStream_t stream, int *launches);
+                          cudaStream_t stream, int *launches, const LaunchHook *hook);
 
 // ---- (a4) prefill -----------------------------------------------------------------------------
 // One CTA work item: up to two consecutive 128-row Q tiles of one (request, kv-head).

@@ -1,0 +1,176 @@
+"""CPU-only tests of the C-ABI library: it loads without a GPU, exports every symbol include/comb.h declares,
+and its host logic (allocator, directory, block-table builder, error paths) agrees bit-exactly with the
+oracle's independent table model O3 (oracle.PoolModel).  No compute call is made here."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2602_01519_b200 as comb
+from paper_2602_01519_b200 import _lib
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+FAKE_K, FAKE_V, FAKE_S = 0x7000_0000_0000, 0x7100_0000_0000, 0x7200_0000_0000  # never dereferenced on the host
+
+
+def make_pool(num_pages=64, Hkv=2, Dqk=64, Dv=64, seed=0, layers=1):
+    cfg = comb.PoolConfig(layers, Hkv, Dqk, Dv, 16, num_pages, FAKE_K, FAKE_V, FAKE_S, seed)
+    return comb.comb_pool_create(cfg)
+
+
+def plan(pool, lists):
+    indptr = np.zeros(len(lists) + 1, np.int32)
+    np.cumsum([len(x) for x in lists], out=indptr[1:])
+    ids = np.array([c for l in lists for c in l], np.uint64)
+    total = sum(len(comb.comb_chunk_query(pool, int(c))[1]) for c in ids)
+    nbytes = comb.comb_link_bytes(len(lists), total)
+    host = np.zeros(nbytes, np.uint8)
+    link = comb.Link()
+    link.device_buf = 0x10000  # layout base only; comb_link_plan writes into host_buf
+    link.device_bytes = nbytes
+    comb.comb_link_plan(pool, indptr, ids, link, host)
+
+    def view(ptr, n, dt):
+        off = ptr - 0x10000
+        return host[off:off + n * np.dtype(dt).itemsize].view(dt).copy()
+    R = len(lists)
+    return link, {
+        "page_indptr": view(link.page_indptr, R + 1, np.int32),
+        "page_ids": view(link.page_ids, int(link.total_pages), np.int32),
+        "page_ntok": view(link.page_ntok, int(link.total_pages), np.int32),
+        "kv_len": view(link.kv_len, R, np.int32),
+        "tile_indptr": view(link.tile_indptr, R + 1, np.int32),
+        "tile_ntok": view(link.tile_ntok, int(link.total_tiles), np.uint64),
+    }
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "comb.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(comb_[a-z_]+)\s*\(", hdr))
+    assert {"comb_pool_create", "comb_store_chunk", "comb_link", "comb_cross_attn_prefill",
+            "comb_cross_attn_decode"} <= declared
+    lib = C.CDLL(_lib.LIB_PATH)
+    for name in sorted(declared):
+        assert hasattr(lib, name), "libcomb.so does not export %s" % name
+    assert declared == set(_lib.EXPORTS), "binding and header disagree: %s" % (declared ^ set(_lib.EXPORTS))
+    assert "sm_100a" in comb.comb_version()
+
+
+def test_pool_bytes_and_layer_saving():
+    k, v, s = comb.comb_pool_bytes(8, 8, 128, 128, 64)  # 8 cross layers, 1024 tokens
+    per_layer_tok = 8 * 128 * 2
+    assert k == 8 * 1024 * per_layer_tok and v == k and s > 0
+    # PAPER.md:277 (Fig. 9): 8 cross layers instead of 32 decoder layers of the same head shape => 75 % saved
+    k32, v32, _ = comb.comb_pool_bytes(32, 8, 128, 128, 64)
+    assert 1.0 - (k + v) / (k32 + v32) == 0.75
+    k, v, _ = comb.comb_pool_bytes(1, 16, 192, 128, 10)  # MLA-shaped: Dqk != Dv
+    assert (k, v) == (10 * 16 * 16 * 192 * 2, 10 * 16 * 16 * 128 * 2)
+
+
+def test_config_validation():
+    for bad in [dict(page=8), dict(Dqk=96), dict(Dv=192), dict(pages=0), dict(Hkv=0)]:
+        cfg = comb.PoolConfig(1, bad.get("Hkv", 2), bad.get("Dqk", 64), bad.get("Dv", 64), bad.get("page", 16),
+                              bad.get("pages", 8), FAKE_K, FAKE_V, FAKE_S, 0)
+        with pytest.raises(comb.CombError) as e:
+            comb.comb_pool_create(cfg)
+        assert e.value.status == comb.COMB_ERR_INVALID
+    cfg = comb.PoolConfig(1, 2, 64, 64, 16, 8, FAKE_K + 16, FAKE_V, FAKE_S, 0)  # misaligned arena
+    with pytest.raises(comb.CombError):
+        comb.comb_pool_create(cfg)
+
+
+@pytest.mark.parametrize("seed", [0, 12345])
+def test_allocator_and_tables_match_oracle_model(seed):
+    rng = np.random.default_rng(seed + 1)
+    pool, model = make_pool(200, seed=seed), oracle.PoolModel(200, seed)
+    lens = {}
+    for cid in range(20):
+        T = int(rng.integers(1, 100))
+        comb.comb_chunk_alloc(pool, cid, T)
+        model.store(cid, T)
+        lens[cid] = T
+    for cid in (3, 11, 7):  # freed pages go to the tail, in page-list order
+        comb.comb_chunk_free(pool, cid)
+        model.release(cid)
+        del lens[cid]
+    for cid in range(20, 30):
+        T = int(rng.integers(1, 60))
+        comb.comb_chunk_alloc(pool, cid, T)
+        model.store(cid, T)
+        lens[cid] = T
+    assert _lib.lib.comb_pool_free_pages(pool) == model.free_pages()
+    for cid, T in lens.items():
+        nt, pages = comb.comb_chunk_query(pool, cid)
+        assert nt == T and pages.tolist() == model.dir[cid][1]
+    ids = sorted(lens)
+    lists = [list(rng.choice(ids, size=int(rng.integers(0, 9)), replace=False)) for _ in range(7)]
+    lists[2] = []                     # a request with no contexts
+    lists[4] = [ids[0], ids[0]]       # duplicates are taken literally (reading I14)
+    link, got = plan(pool, lists)
+    exp = model.link(lists)
+    for key in ("page_indptr", "page_ids", "page_ntok", "kv_len"):
+        assert np.array_equal(got[key], exp[key]), key
+    # tile_ntok is page_ntok regrouped by 8 (derived; checked against its definition)
+    for r in range(len(lists)):
+        pn = exp["page_ntok"][exp["page_indptr"][r]:exp["page_indptr"][r + 1]]
+        tiles = got["tile_ntok"][got["tile_indptr"][r]:got["tile_indptr"][r + 1]]
+        assert len(tiles) == (len(pn) + 7) // 8
+        for t, packed in enumerate(tiles):
+            want = [int(x) for x in pn[8 * t:8 * t + 8]] + [0] * (8 - len(pn[8 * t:8 * t + 8]))
+            assert [(int(packed) >> (8 * j)) & 0xff for j in range(8)] == want
+    assert link.total_kv_tokens == int(exp["kv_len"].sum())
+    assert link.max_pages_per_request == int(np.diff(exp["page_indptr"]).max())
+    comb.comb_pool_destroy(pool)
+
+
+def test_error_paths():
+    pool = make_pool(4)
+    comb.comb_chunk_alloc(pool, 1, 33)                     # 3 pages
+    comb.comb_chunk_alloc(pool, 1, 33)                     # idempotent
+    with pytest.raises(comb.CombError) as e:
+        comb.comb_chunk_alloc(pool, 1, 34)
+    assert e.value.status == comb.COMB_ERR_EXISTS
+    with pytest.raises(comb.CombError) as e:
+        comb.comb_chunk_alloc(pool, 2, 17)                 # needs 2 pages, 1 free; nothing allocated
+    assert e.value.status == comb.COMB_ERR_NO_SPACE
+    assert _lib.lib.comb_pool_free_pages(pool) == 1
+    with pytest.raises(comb.CombError) as e:
+        comb.comb_chunk_alloc(pool, 3, 0)
+    assert e.value.status == comb.COMB_ERR_INVALID
+    with pytest.raises(comb.CombError) as e:
+        comb.comb_chunk_query(pool, 99)
+    assert e.value.status == comb.COMB_ERR_UNKNOWN_CHUNK
+    with pytest.raises(comb.CombError) as e:
+        comb.comb_chunk_free(pool, 99)
+    assert e.value.status == comb.COMB_ERR_UNKNOWN_CHUNK
+    # link before store: UNKNOWN_CHUNK, nothing written (PAPER.md:62 step 2: a miss must compile + store first)
+    link = comb.Link()
+    link.device_buf, link.device_bytes = 0x10000, 4096
+    host = np.full(4096, 0xAB, np.uint8)
+    with pytest.raises(comb.CombError) as e:
+        comb.comb_link_plan(pool, np.array([0, 2], np.int32), np.array([1, 42], np.uint64), link, host)
+    assert e.value.status == comb.COMB_ERR_UNKNOWN_CHUNK and np.all(host == 0xAB)
+    link.device_bytes = 16                                  # too small
+    with pytest.raises(comb.CombError) as e:
+        comb.comb_link_plan(pool, np.array([0, 1], np.int32), np.array([1], np.uint64), link, host)
+    assert e.value.status == comb.COMB_ERR_CAPACITY
+    with pytest.raises(comb.CombError) as e:                # non-monotone indptr
+        link.device_bytes = 4096
+        comb.comb_link_plan(pool, np.array([0, 1, 0], np.int32), np.array([1], np.uint64), link, host)
+    assert e.value.status == comb.COMB_ERR_INVALID
+    comb.comb_pool_destroy(pool)
+
+
+def test_product_does_not_import_oracle():
+    """The product path must not reach into oracle/ (or _work/)."""
+    pkg = os.path.join(ROOT, "paper_2602_01519_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", src, flags=re.M), f
+                assert "comb_oracle" not in src and "_work/" not in src, f
