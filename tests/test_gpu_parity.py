@@ -41,10 +41,13 @@ def check_attention(out_bits, lse, O, L, tag=""):
 
 
 def close_in_ulps(a, b, tag=""):
-    """Two GPU results for the same mathematical value (different tile partitions / kernels): they differ only by
-    fp32 reassociation and bf16 rounding of P and of the output, i.e. by about two bf16 ulps of the output."""
-    ratio = np.abs(a - b) / np.maximum(np.abs(a), 2.0 ** -6)
-    assert ratio.max() <= 2.0 ** -6, "%s: worst |a-b|/max(|a|,2^-6) = %.3e" % (tag, ratio.max())
+    """Two GPU results for the same mathematical value (other tile partition, other kernel). They differ by the
+    bf16 rounding of the output (<= 2^-8 relative each) and of the P weights fed to the PV contraction (each weight
+    2^-9 relative, so about 2^-9 * sum_j p_j |v_j| / l ~ 2e-3 absolute for N(0,1) values), and by fp32 reassociation."""
+    d = np.abs(a - b)
+    assert np.all(d <= 2.0 ** -7 * np.abs(a) + 2.5e-3), "%s: worst excess %.3e" % (
+        tag, (d - 2.0 ** -7 * np.abs(a)).max())
+    assert d.mean() <= 3e-4, "%s: mean |a-b| = %.3e" % (tag, d.mean())
 
 
 def run_prefill(w, **kw):
