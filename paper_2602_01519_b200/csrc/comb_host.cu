@@ -562,6 +562,7 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     const size_t need = num_items * sizeof(PrefillItem);
     if (!ws || ws_bytes < need) return COMB_ERR_CAPACITY;
     cudaStream_t st = (cudaStream_t)stream;
+    p->probe_device();
     if (!p->kv_maps_ready) {
         if (prefill_encode_kv_maps(p->geom, &p->k_map, &p->v_map) != cudaSuccess) return COMB_ERR_CUDA;
         p->kv_maps_ready = true;
@@ -583,7 +584,7 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     if (cudaMemcpyAsync(ws, h, need, cudaMemcpyHostToDevice, st) != cudaSuccess) return COMB_ERR_CUDA;
     if (p->prof_on) p->hook.begin(p, kKernelPrefill, st);
     cudaError_t e = launch_prefill(p->geom, layer, view_of(link), maps, (const PrefillItem *)ws, (int)num_items, Hq,
-                                   scale, out, lse, st);
+                                   scale, out, lse, p->num_sms, st);
     if (p->prof_on) p->hook.end(p, st);
     if (e != cudaSuccess) return COMB_ERR_CUDA;
     p->launches += 1;

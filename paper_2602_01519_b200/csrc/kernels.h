@@ -73,6 +73,6 @@ cudaError_t prefill_encode_q_map(const void *q, int64_t total_q, int num_q_heads
                                  TensorMapBlob *q_map);
 cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &maps,
                            const PrefillItem *items_dev, int num_items, int num_q_heads, float scale, void *out,
-                           float *lse, cudaStream_t stream);
+                           float *lse, int num_sms, cudaStream_t stream);
 
 }  // namespace comb

@@ -14,6 +14,7 @@
 
 #include <cuda.h>
 #include <cuda_bf16.h>
+#include <cstdlib>
 #include <cstring>
 
 namespace comb {
@@ -242,6 +243,322 @@ prefill_v0_kernel(const PrefillArgs a, const __grid_constant__ Maps maps) {
     if (warp == 0) ptx::tmem_dealloc(tmem, C::TMEM_COLS);
 }
 
+// ============================================================================================
+// v1: persistent, warp-specialised, two Q tiles in ping-pong per CTA.
+//   warps 0-3 : softmax + epilogue of Q tile 0 (one thread per row)      warp 8 : TMA loader (Q tiles, K/V ring)
+//   warps 4-7 : softmax + epilogue of Q tile 1                           warp 9 : tcgen05.mma issuer (one lane)
+// TMEM (512 columns): S0/P0 @0, S1/P1 @128, O0 @256, O1 @256+DV.  While the softmax warps of one tile work on
+// S_j, the tensor pipe runs P V_j and Q K_{j+1}^T of the other tile.  The running max is only advanced when it
+// grows by more than 2^8 (lazy rescale), so the accumulator in TMEM is almost never touched by the softmax warps.
+// ============================================================================================
+template <int DQK, int DV>
+struct V1Cfg {
+    static constexpr int KH = DQK / 64, VH = DV / 64;
+    static constexpr int HALF = kTileM * 128;  // [128 rows][64 bf16]
+    static constexpr int Q_BYTES = KH * HALF;
+    static constexpr int K_BYTES = KH * HALF, V_BYTES = VH * HALF;
+    static constexpr int SLOT = K_BYTES > V_BYTES ? K_BYTES : V_BYTES;  // K and V tiles alternate in one ring
+    static constexpr int SMEM_MAX = 232448;                             // 227 KB
+    static constexpr int NSLOT_RAW = (SMEM_MAX - 1024 - 512 - 2 * Q_BYTES) / SLOT;
+    static constexpr int NSLOT = NSLOT_RAW > 8 ? 8 : NSLOT_RAW;
+    static_assert(NSLOT >= 2, "need at least a K and a V slot");
+    static constexpr int SMEM = 1024 + 2 * Q_BYTES + NSLOT * SLOT + 512;
+    static constexpr int TMEM_COLS = 512;
+    static constexpr int THREADS = 384;  // 3 warpgroups: softmax 0, softmax 1, {loader, MMA issuer, 2 idle warps}
+};
+
+__device__ __forceinline__ float fmax3(float a, float b, float c) {
+    float d;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+    return d;
+}
+
+template <int DQK, int DV>
+__global__ void __launch_bounds__(384, 1)
+prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const int num_items) {
+    using C = V1Cfg<DQK, DV>;
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    unsigned char *sQ = smem;                    // [2 tiles][KH][128][64]
+    unsigned char *sKV = smem + 2 * C::Q_BYTES;  // ring of NSLOT tiles
+    uint64_t *bars = reinterpret_cast<uint64_t *>(sKV + C::NSLOT * C::SLOT);
+    uint64_t *q_full = bars, *q_empty = bars + 2, *s_full = bars + 4, *p_full = bars + 6, *o_done = bars + 8;
+    uint64_t *kv_full = bars + 10, *kv_empty = bars + 10 + C::NSLOT;
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(bars + 10 + 2 * C::NSLOT);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        for (int t = 0; t < 2; ++t) {
+            ptx::mbar_init(&q_full[t], 1);
+            ptx::mbar_init(&q_empty[t], 1);
+            ptx::mbar_init(&s_full[t], 1);
+            ptx::mbar_init(&p_full[t], 128);
+            ptx::mbar_init(&o_done[t], 1);
+        }
+        for (int s = 0; s < C::NSLOT; ++s) {
+            ptx::mbar_init(&kv_full[s], 1);
+            ptx::mbar_init(&kv_empty[s], 1);
+        }
+        ptx::fence_barrier_init();
+        ptx::tma_prefetch_desc(&maps.q);
+        ptx::tma_prefetch_desc(&maps.k);
+        ptx::tma_prefetch_desc(&maps.v);
+    }
+    if (warp == 8) {
+        ptx::tmem_alloc(tmem_slot, C::TMEM_COLS);
+        ptx::tmem_relinquish();
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    const int G = a.group, Hq = a.num_q_heads;
+    const int tok_per_tile = kTileM / G;
+
+    // register file: 384 x 168 at launch; the softmax warpgroups take what the third warpgroup gives up
+    // (2 x 128 x 208 + 128 x 88 = 384 x 168: asking for more than the CTA owns would block forever)
+    if (warp < 8) {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(208));
+    } else {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(88));
+    }
+
+    if (warp < 8) {
+        // ===================== softmax + epilogue of Q tile t =====================
+        const int t = warp >> 2;
+        const int row = (warp & 3) * 32 + lane;
+        const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
+        const uint32_t tS = tmem + lane_base + t * 128;
+        const uint32_t tO = tmem + lane_base + 256 + t * DV;
+        const int row_tok = row / G, row_head = row % G;
+        const float c = a.scale_log2;
+        const float2 c2 = make_float2(c, c);
+        uint32_t s_cnt = 0, o_cnt = 0;
+        for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
+            const PrefillItem it = a.items[idx];
+            const int tok_valid = it.q_rows - t * tok_per_tile;
+            if (tok_valid <= 0) continue;  // this item has no second Q tile
+            const int npages = a.page_indptr[it.request + 1] - a.page_indptr[it.request];
+            const int n_kv = (npages + kTilePages - 1) / kTilePages;
+            const int tile0 = a.tile_indptr[it.request];
+            const bool row_valid = row_tok < tok_valid;
+            const int tok = it.q_row0 + t * tok_per_tile + row_tok, head = it.kv_head * G + row_head;
+            __nv_bfloat16 *orow = a.out + ((size_t)tok * Hq + head) * DV;
+            if (n_kv == 0) {  // no contexts linked (reading I13): zero contribution, lse = -inf
+                if (row_valid) {
+                    for (int e = 0; e < DV / 8; ++e) reinterpret_cast<uint4 *>(orow)[e] = make_uint4(0, 0, 0, 0);
+                    if (a.lse) a.lse[(size_t)tok * Hq + head] = -INFINITY;
+                }
+                continue;
+            }
+            float m_used = -INFINITY, l_run = 0.f;
+            for (int j = 0; j < n_kv; ++j) {
+                const uint64_t ntok8 = a.tile_ntok[tile0 + j];
+                ptx::mbar_wait(&s_full[t], s_cnt & 1);
+                ++s_cnt;
+                ptx::tc_fence_after();
+                uint32_t r[kTileN];
+#pragma unroll
+                for (int q = 0; q < kTileN / 32; ++q)
+                    ptx::tmem_ld32(tS + q * 32, *reinterpret_cast<uint32_t(*)[32]>(&r[q * 32]));
+                ptx::tmem_wait_ld();
+                if (ntok8 != kFullTile) {  // interior partial pages / missing pages of the last tile
+#pragma unroll
+                    for (int e = 0; e < kTileN; ++e) {
+                        const int nt = (int)((ntok8 >> (8 * (e / kPage))) & 0xffu);
+                        if ((e % kPage) >= nt) r[e] = 0xff800000u;  // -inf
+                    }
+                }
+                float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+                for (int e = 0; e < kTileN; e += 2)
+                    mx4[(e >> 1) & 3] = fmax3(mx4[(e >> 1) & 3], __uint_as_float(r[e]), __uint_as_float(r[e + 1]));
+                const float m_new = fmaxf(fmax3(mx4[0], mx4[1], mx4[2]), fmaxf(mx4[3], m_used));
+                if (j == 0) {
+                    m_used = m_new;
+                } else if (__any_sync(0xffffffffu, (m_new - m_used) * c > 8.f)) {
+                    // rare: move the reference max and rescale this warp's rows of the accumulator
+                    ptx::mbar_wait(&o_done[t], (o_cnt + j - 1) & 1);  // P V_{j-1} has landed
+                    ptx::tc_fence_after();
+                    const float alpha = ptx::ex2((m_used - m_new) * c);
+                    l_run *= alpha;
+                    m_used = m_new;
+#pragma unroll
+                    for (int q = 0; q < DV / 32; ++q) {
+                        uint32_t o[32];
+                        ptx::tmem_ld32(tO + q * 32, o);
+                        ptx::tmem_wait_ld();
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
+                        ptx::tmem_st32(tO + q * 32, o);
+                    }
+                }
+                const float neg = -m_used * c;
+                const float2 neg2 = make_float2(neg, neg);
+                float2 sum4[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+#pragma unroll
+                for (int e = 0; e < kTileN; e += 2) {
+                    const float2 x = ptx::ffma2(make_float2(__uint_as_float(r[e]), __uint_as_float(r[e + 1])), c2, neg2);
+                    const float p0 = ptx::ex2(x.x), p1 = ptx::ex2(x.y);
+                    sum4[(e >> 1) & 3] = ptx::fadd2(sum4[(e >> 1) & 3], make_float2(p0, p1));
+                    r[e >> 1] = ptx::pack_bf16x2(p0, p1);
+                }
+                const float2 sA = ptx::fadd2(sum4[0], sum4[1]), sB = ptx::fadd2(sum4[2], sum4[3]);
+                l_run += (sA.x + sA.y) + (sB.x + sB.y);
+                ptx::tmem_st32(tS, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
+                ptx::tmem_st32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[32]));
+                ptx::tmem_wait_st();
+                ptx::tc_fence_before();
+                ptx::mbar_arrive(&p_full[t]);
+            }
+            // ---- epilogue: O / l -> bf16 ----
+            ptx::mbar_wait(&o_done[t], (o_cnt + n_kv - 1) & 1);
+            o_cnt += n_kv;
+            ptx::tc_fence_after();
+            const float inv = 1.f / l_run;
+#pragma unroll
+            for (int q = 0; q < DV / 32; ++q) {
+                uint32_t o[32];
+                ptx::tmem_ld32(tO + q * 32, o);
+                ptx::tmem_wait_ld();
+                if (row_valid) {
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        uint4 w;
+                        w.x = ptx::pack_bf16x2(__uint_as_float(o[8 * e + 0]) * inv, __uint_as_float(o[8 * e + 1]) * inv);
+                        w.y = ptx::pack_bf16x2(__uint_as_float(o[8 * e + 2]) * inv, __uint_as_float(o[8 * e + 3]) * inv);
+                        w.z = ptx::pack_bf16x2(__uint_as_float(o[8 * e + 4]) * inv, __uint_as_float(o[8 * e + 5]) * inv);
+                        w.w = ptx::pack_bf16x2(__uint_as_float(o[8 * e + 6]) * inv, __uint_as_float(o[8 * e + 7]) * inv);
+                        reinterpret_cast<uint4 *>(orow)[q * 4 + e] = w;
+                    }
+                }
+            }
+            if (row_valid && a.lse) a.lse[(size_t)tok * Hq + head] = (m_used * c + log2f(l_run)) * kLn2;
+            ptx::tc_fence_before();  // our reads of O precede the arrive that lets the next item's P V overwrite it
+        }
+    } else if (warp == 8) {
+        // ===================== TMA loader =====================
+        uint32_t slot = 0, phase = 0, qcnt[2] = {0, 0};
+        for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
+            const PrefillItem it = a.items[idx];
+            const int pbeg = a.page_indptr[it.request], npages = a.page_indptr[it.request + 1] - pbeg;
+            const int n_kv = (npages + kTilePages - 1) / kTilePages;
+            if (n_kv == 0) continue;
+            const int nq = it.q_rows > tok_per_tile ? 2 : 1;
+            for (int t = 0; t < nq; ++t) {
+                ptx::mbar_wait(&q_empty[t], (qcnt[t] & 1) ^ 1);
+                ++qcnt[t];
+                if (lane == 0) {
+                    ptx::mbar_expect_tx(&q_full[t], C::Q_BYTES);
+                    for (int h = 0; h < C::KH; ++h)
+                        ptx::tma_load_3d(sQ + t * C::Q_BYTES + h * C::HALF, &maps.q, h * 64, it.kv_head * G,
+                                         it.q_row0 + t * tok_per_tile, &q_full[t]);
+                }
+            }
+            for (int j = 0; j < n_kv; ++j) {
+                const int pages_here = min(kTilePages, npages - j * kTilePages);
+                int row0 = 0;
+                if (lane < pages_here) {
+                    const int pid = a.page_ids[pbeg + j * kTilePages + lane];
+                    row0 = a.layer_row0 + (pid * a.num_kv_heads + it.kv_head) * kPage;
+                }
+#pragma unroll
+                for (int kv = 0; kv < 2; ++kv) {  // K tile, then V tile
+                    ptx::mbar_wait(&kv_empty[slot], phase ^ 1);
+                    unsigned char *dst = sKV + slot * C::SLOT;
+                    if (lane == 0) ptx::mbar_expect_tx(&kv_full[slot], (uint32_t)pages_here * kPage * (kv == 0 ? DQK : DV) * 2);
+                    __syncwarp();
+                    if (lane < pages_here) {
+                        if (kv == 0) {
+#pragma unroll
+                            for (int h = 0; h < C::KH; ++h)
+                                ptx::tma_load_2d(dst + h * C::HALF + lane * 2048, &maps.k, h * 64, row0, &kv_full[slot]);
+                        } else {
+#pragma unroll
+                            for (int h = 0; h < C::VH; ++h)
+                                ptx::tma_load_2d(dst + h * C::HALF + lane * 2048, &maps.v, h * 64, row0, &kv_full[slot]);
+                        }
+                    }
+                    if (++slot == C::NSLOT) { slot = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 9 && lane == 0) {
+        // ===================== MMA issuer (one thread) =====================
+        constexpr uint32_t idesc_s = ptx::umma_idesc_bf16(kTileM, kTileN, false);
+        constexpr uint32_t idesc_o = ptx::umma_idesc_bf16(kTileM, DV, true);
+        // descriptors advance by adding (byte offset >> 4) to the 14-bit start-address field
+        const uint64_t dq0 = ptx::umma_desc_sw128(ptx::smem_u32(sQ), 16, 1024);
+        const uint64_t dk0 = ptx::umma_desc_sw128(ptx::smem_u32(sKV), 16, 1024);
+        const uint64_t dv0 = ptx::umma_desc_sw128(ptx::smem_u32(sKV), C::HALF, 1024);
+        uint32_t slot = 0, phase = 0, qcnt[2] = {0, 0}, pcnt[2] = {0, 0};
+        auto issue_s = [&](int t, uint32_t kslot) {
+            const uint64_t dq = dq0 + (uint64_t)((t * C::Q_BYTES) >> 4), dk = dk0 + (uint64_t)((kslot * C::SLOT) >> 4);
+#pragma unroll
+            for (int kk = 0; kk < DQK / 16; ++kk) {
+                const uint64_t off = (uint64_t)(((kk / 4) * C::HALF + (kk % 4) * 32) >> 4);
+                ptx::mma_ss(tmem + t * 128, dq + off, dk + off, idesc_s, kk > 0);
+            }
+        };
+        for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
+            const PrefillItem it = a.items[idx];
+            const int npages = a.page_indptr[it.request + 1] - a.page_indptr[it.request];
+            const int n_kv = (npages + kTilePages - 1) / kTilePages;
+            if (n_kv == 0) continue;
+            const int nq = it.q_rows > tok_per_tile ? 2 : 1;
+            // prologue: S_t = Q_t K_0^T
+            uint32_t kslot = slot;
+            ptx::mbar_wait(&kv_full[kslot], phase);
+            if (++slot == C::NSLOT) { slot = 0; phase ^= 1; }
+            for (int t = 0; t < nq; ++t) {
+                ptx::mbar_wait(&q_full[t], qcnt[t] & 1);
+                ++qcnt[t];
+                ptx::tc_fence_after();
+                issue_s(t, kslot);
+                ptx::mma_commit(&s_full[t]);
+                if (n_kv == 1) ptx::mma_commit(&q_empty[t]);
+            }
+            ptx::mma_commit(&kv_empty[kslot]);
+            for (int j = 0; j < n_kv; ++j) {
+                const int pages_here = min(kTilePages, npages - j * kTilePages);
+                const bool more = j + 1 < n_kv;
+                const uint32_t vslot = slot;
+                ptx::mbar_wait(&kv_full[vslot], phase);
+                if (++slot == C::NSLOT) { slot = 0; phase ^= 1; }
+                const uint32_t kphase = phase;
+                kslot = slot;
+                if (more && ++slot == C::NSLOT) { slot = 0; phase ^= 1; }
+                for (int t = 0; t < nq; ++t) {
+                    ptx::mbar_wait(&p_full[t], pcnt[t] & 1);
+                    ++pcnt[t];
+                    ptx::tc_fence_after();
+                    for (int ks = 0; ks < pages_here; ++ks)  // O_t += P_t V_j, one k-step of 16 keys per page
+                        ptx::mma_ts(tmem + 256 + t * DV, tmem + t * 128 + ks * 8,
+                                    dv0 + (uint64_t)((vslot * C::SLOT + ks * 2048) >> 4), idesc_o,
+                                    (j > 0 || ks > 0) ? 1u : 0u);
+                    ptx::mma_commit(&o_done[t]);
+                    if (more) {
+                        if (t == 0) {
+                            ptx::mbar_wait(&kv_full[kslot], kphase);
+                            ptx::tc_fence_after();
+                        }
+                        issue_s(t, kslot);
+                        ptx::mma_commit(&s_full[t]);
+                        if (j + 2 == n_kv) ptx::mma_commit(&q_empty[t]);
+                    }
+                }
+                ptx::mma_commit(&kv_empty[vslot]);
+                if (more) ptx::mma_commit(&kv_empty[kslot]);
+            }
+        }
+    }
+
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    if (warp == 8) ptx::tmem_dealloc(tmem, C::TMEM_COLS);
+}
+
 // ---------------------------------------------------------------- TMA descriptor encoding (host)
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -286,6 +603,25 @@ cudaError_t launch_v0(const PrefillArgs &a, const Maps &maps, int num_items, cud
     return cudaGetLastError();
 }
 
+template <int DQK, int DV>
+cudaError_t launch_v1(const PrefillArgs &a, const Maps &maps, int num_items, int num_sms, cudaStream_t st) {
+    using C = V1Cfg<DQK, DV>;
+    auto kern = prefill_v1_kernel<DQK, DV>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
+    if (e != cudaSuccess) return e;
+    const int grid = num_items < num_sms ? num_items : num_sms;
+    kern<<<grid, C::THREADS, C::SMEM, st>>>(a, maps, num_items);
+    return cudaGetLastError();
+}
+
+bool use_v0() {
+    static const bool v = [] {
+        const char *e = getenv("COMB_PREFILL_IMPL");
+        return e && e[0] == 'v' && e[1] == '0';
+    }();
+    return v;
+}
+
 }  // namespace
 
 bool prefill_supported(int group, int dqk, int dv) {
@@ -318,7 +654,7 @@ cudaError_t prefill_encode_q_map(const void *q, int64_t total_q, int num_q_heads
 
 cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &pm,
                            const PrefillItem *items_dev, int num_items, int num_q_heads, float scale, void *out,
-                           float *lse, cudaStream_t stream) {
+                           float *lse, int num_sms, cudaStream_t stream) {
     PrefillArgs a;
     a.items = items_dev;
     a.page_indptr = lv.page_indptr;
@@ -336,8 +672,10 @@ cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, con
     memcpy(&maps.q, &pm.q, sizeof(CUtensorMap));
     memcpy(&maps.k, &pm.k, sizeof(CUtensorMap));
     memcpy(&maps.v, &pm.v, sizeof(CUtensorMap));
-#define COMB_PREFILL_CASE(DQ, DVV) \
-    if (g.head_dim_qk == DQ && g.head_dim_v == DVV) return launch_v0<DQ, DVV>(a, maps, num_items, stream);
+#define COMB_PREFILL_CASE(DQ, DVV)                                                              \
+    if (g.head_dim_qk == DQ && g.head_dim_v == DVV)                                             \
+        return use_v0() ? launch_v0<DQ, DVV>(a, maps, num_items, stream)                        \
+                        : launch_v1<DQ, DVV>(a, maps, num_items, num_sms, stream);
     COMB_PREFILL_CASE(128, 128)
     COMB_PREFILL_CASE(64, 64)
     COMB_PREFILL_CASE(192, 128)
