@@ -53,11 +53,17 @@ def peaks():
     return {"hbm": FALLBACK_HBM_GBS, "tf_burst": FALLBACK_BF16_TFLOPS, "tf_sustained": 1400.0, "src": "fallback"}
 
 
-def ncu_traffic(kernel: str):
-    """DRAM bytes per launch from the committed ncu capture (profiles/ncu_traffic.json), or None."""
-    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
-    if os.path.exists(p):
-        return json.load(open(p)).get(kernel)
+def ncu_traffic(kernel: str, workload: str):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of `kernel` on `workload` from the
+    committed ncu --set full capture (profiles/ncu_traffic.csv), or None when that pair was not captured."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for line in f.read().splitlines()[1:]:
+            cols = line.split(",")
+            if len(cols) >= 3 and cols[0] == kernel and cols[1] == workload:
+                return int(cols[2])
     return None
 
 
@@ -203,7 +209,7 @@ def main():
     import torch.distributed as dist
 
     import paper_2602_01519_b200 as comb
-    from paper_2602_01519_b200 import harness
+    from paper_2602_01519_b200 import harness, replicas
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -221,11 +227,7 @@ def main():
         torch.cuda.synchronize()
 
     def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replicas.max_over_ranks(x, device="cuda")
 
     pk = peaks()
     extras = {}
@@ -318,15 +320,15 @@ def main():
         torch.cuda.empty_cache()
         return res
 
-    def roofline_hbm(r, kernel_name):
+    def roofline_hbm(r, kernel_name, wname):
         achieved = (r["kv_bytes"] + r["io_bytes"]) / (r["kernel_ms"] * 1e-3) / 1e9
         return {"bound": "hbm", "achieved": achieved, "peak": pk["hbm"], "unit": "GB/s", "frac": achieved / pk["hbm"],
                 "peak_source": pk["src"] + " copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
                 "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS, "kernel": kernel_name,
                 "kernel_ms": r["kernel_ms"], "algorithmic_bytes": r["kv_bytes"] + r["io_bytes"],
-                "traffic": ncu_traffic(kernel_name)}
+                "traffic": ncu_traffic(kernel_name, wname)}
 
-    def roofline_tensor(r, kernel_name):
+    def roofline_tensor(r, kernel_name, wname):
         achieved = r["flops"] / (r["kernel_ms"] * 1e-3) / 1e12
         sustained = r["timed_seconds"] >= 1.0
         peak = pk["tf_sustained"] if sustained else pk["tf_burst"]
@@ -334,7 +336,7 @@ def main():
                 "peak_source": "%s cuBLAS bf16 %s" % (pk["src"], "sustained" if sustained else "burst"),
                 "frac_of_burst": achieved / pk["tf_burst"], "frac_of_sustained": achieved / pk["tf_sustained"],
                 "frac_of_nominal_2250": achieved / NOMINAL_BF16_TFLOPS, "kernel": kernel_name,
-                "kernel_ms": r["kernel_ms"], "algorithmic_flops": r["flops"], "traffic": ncu_traffic(kernel_name)}
+                "kernel_ms": r["kernel_ms"], "algorithmic_flops": r["flops"], "traffic": ncu_traffic(kernel_name, wname)}
 
     # ------------------------------------------------------------------ primary workload
     if primary_prefill:
@@ -342,7 +344,7 @@ def main():
         r = bench_attention(w, "prefill", args.steps, args.warmup, fill="linked")
         value = world * r["flops"] / (r["ms_per_step"] * 1e-3) / 1e12
         unit, metric = "TFLOP/s", "prefill cross-attn TFLOP/s (BASELINE metric, prefill half)"
-        roof = roofline_tensor(r, "prefill")
+        roof = roofline_tensor(r, "prefill", "rag_prefill")
         e2e_val = world * r["flops"] / (r["e2e_ms"] * 1e-3) / 1e12
         dtype = "bf16"
     else:
@@ -350,7 +352,7 @@ def main():
         r = bench_attention(w, "decode", args.steps, args.warmup, fill="linked")
         value = world * r["kv_bytes"] / (r["ms_per_step"] * 1e-3) / 1e9
         unit, metric = "GB/s", METRIC
-        roof = roofline_hbm(r, "decode_split")
+        roof = roofline_hbm(r, "decode_split", "decode_link")
         e2e_val = world * r["kv_bytes"] / (r["e2e_ms"] * 1e-3) / 1e9
         dtype = "bf16"
     log("primary", json.dumps(r))
@@ -363,7 +365,7 @@ def main():
             extras[name] = {"workload": name, "ms_per_step": rr["ms_per_step"], "kernel_ms": rr["kernel_ms"],
                             "tflops": rr["flops"] / (rr["ms_per_step"] * 1e-3) / 1e12,
                             "q_tokens_per_s": rr["q_tokens"] / (rr["ms_per_step"] * 1e-3),
-                            "roofline": roofline_tensor(rr, "prefill"), "clocks": rr["clocks"],
+                            "roofline": roofline_tensor(rr, "prefill", name.replace("_prefill", "") if name != "rag_prefill" else name), "clocks": rr["clocks"],
                             "l2": "flushed between iterations" if flush else "inputs larger than L2"}
             log(name, json.dumps(extras[name]))
 
@@ -372,7 +374,7 @@ def main():
             extras[name] = {"workload": name, "ms_per_step": rr["ms_per_step"], "kernel_ms": rr["kernel_ms"],
                             "merge_ms": rr["merge_ms"],
                             "gbs_logical": rr["kv_bytes"] / (rr["ms_per_step"] * 1e-3) / 1e9,
-                            "roofline": roofline_hbm(rr, "decode_split"), "clocks": rr["clocks"],
+                            "roofline": roofline_hbm(rr, "decode_split", name.replace("_decode", "") if name != "decode_link" else name), "clocks": rr["clocks"],
                             "l2": "flushed between iterations" if flush else "inputs larger than L2"}
             log(name, json.dumps(extras[name]))
 
@@ -461,7 +463,7 @@ def bench_store(torch, comb, harness, w, pk):
             "kernel_ms": ms / cnt, "roofline": {"bound": "hbm", "achieved": achieved, "peak": pk["hbm"], "unit": "GB/s",
                                                  "frac": achieved / pk["hbm"], "algorithmic_bytes": nbytes,
                                                  "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
-                                                 "kernel": "store", "traffic": ncu_traffic("store")},
+                                                 "kernel": "store", "traffic": ncu_traffic("store", "long_fewshot")},
             "l2": "flushed between iterations"}
 
 
