@@ -68,6 +68,23 @@ def ncu_traffic(kernel: str, workload: str):
 
 
 # ------------------------------------------------------------------------------------------------
+class L2Flush:
+    """Evicts the 126 MB L2 between timed iterations: writes a 256 MB buffer, then reads a second 256 MB buffer, so
+    the cache is left holding CLEAN lines of unrelated data (after the write alone it would hold ~100 MB of dirty
+    lines whose write-back would be charged to the kernel under test)."""
+    HOW = "flushed between iterations (256 MB written, then 256 MB read: L2 left clean)"
+
+    def __init__(self, torch):
+        self.w = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        self.r = torch.zeros(64 << 20, dtype=torch.int32, device="cuda")
+        self.sink = torch.zeros((), dtype=torch.int64, device="cuda")
+
+    def __call__(self, i: int):
+        self.w.fill_(i & 0xff)
+        self.sink += self.r.sum()
+
+
+# ------------------------------------------------------------------------------------------------
 class ClockSampler:
     """Samples SM clock and throttle reasons DURING the timed region (NVML, every 10 ms)."""
 
@@ -250,7 +267,7 @@ def main():
         chunk_indptr, chunk_ids = w.chunk_indptr, w.chunk_ids_flat
         batch = ld.batch
         kid = comb.KERNEL_DECODE_SPLIT if phase == "decode" else comb.KERNEL_PREFILL
-        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if flush_l2 else None
+        flush = L2Flush(torch) if flush_l2 else None
 
         def step():
             if with_link:
@@ -269,7 +286,7 @@ def main():
         with ClockSampler(local) as clk:
             if flush_l2:
                 for i in range(steps):
-                    flush.fill_(i & 0xff)
+                    flush(i)
                     ev[2 * i].record()
                     step()
                     ev[2 * i + 1].record()
@@ -366,7 +383,7 @@ def main():
                             "tflops": rr["flops"] / (rr["ms_per_step"] * 1e-3) / 1e12,
                             "q_tokens_per_s": rr["q_tokens"] / (rr["ms_per_step"] * 1e-3),
                             "roofline": roofline_tensor(rr, "prefill", name.replace("_prefill", "") if name != "rag_prefill" else name), "clocks": rr["clocks"],
-                            "l2": "flushed between iterations" if flush else "inputs larger than L2"}
+                            "l2": L2Flush.HOW if flush else "inputs larger than L2"}
             log(name, json.dumps(extras[name]))
 
         def decode_extra(name, wk, steps, fill, flush=False):
@@ -375,7 +392,7 @@ def main():
                             "merge_ms": rr["merge_ms"],
                             "gbs_logical": rr["kv_bytes"] / (rr["ms_per_step"] * 1e-3) / 1e9,
                             "roofline": roofline_hbm(rr, "decode_split", name.replace("_decode", "") if name != "decode_link" else name), "clocks": rr["clocks"],
-                            "l2": "flushed between iterations" if flush else "inputs larger than L2"}
+                            "l2": L2Flush.HOW if flush else "inputs larger than L2"}
             log(name, json.dumps(extras[name]))
 
         try:
@@ -442,14 +459,14 @@ def bench_store(torch, comb, harness, w, pk):
     T = int(tok[-1])
     k = torch.randn((T, w.num_kv_heads, w.head_dim_qk), device="cuda").to(torch.bfloat16)
     v = torch.randn((T, w.num_kv_heads, w.head_dim_v), device="cuda").to(torch.bfloat16)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    flush = L2Flush(torch)
     comb.comb_profile_enable(pool.handle, True)
     comb.comb_profile_read(pool.handle, comb.KERNEL_STORE)
     n = 20
     for i in range(n + 3):
         for c in ids:
             comb.comb_chunk_free(pool.handle, c)
-        flush.fill_(i)
+        flush(i)
         if i == 3:
             torch.cuda.synchronize()
             comb.comb_profile_read(pool.handle, comb.KERNEL_STORE)
@@ -464,7 +481,7 @@ def bench_store(torch, comb, harness, w, pk):
                                                  "frac": achieved / pk["hbm"], "algorithmic_bytes": nbytes,
                                                  "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
                                                  "kernel": "store", "traffic": ncu_traffic("store", "long_fewshot")},
-            "l2": "flushed between iterations"}
+            "l2": L2Flush.HOW}
 
 
 def bench_link(torch, comb, harness, w):
