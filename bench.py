@@ -401,6 +401,10 @@ def main():
             else:
                 decode_extra("decode_link", cs.decode_link(seed=args.seed), 100, "linked")
             prefill_extra("rag_prefill_lq32", cs.rag_prefill(seed=args.seed, lq=32), 20, "linked")
+            # the paper's own regime (< 50 dynamic tokens) at a small batch: 32 work items for 148 SMs,
+            # so each request's KV is cut into ranges that run on different SMs and are merged by LSE
+            prefill_extra("rag_prefill_lq32_r4", cs.rag_prefill(seed=args.seed, lq=32, requests=4), 20, "linked",
+                          flush=True)
             prefill_extra("long_fewshot_prefill", cs.long_fewshot(seed=args.seed), 10, "all", flush=True)
             decode_extra("long_fewshot_decode", cs.long_fewshot(seed=args.seed), 50, "all", flush=True)
             prefill_extra("mla_shaped_prefill", cs.mla_shaped(seed=args.seed), 20, "linked")

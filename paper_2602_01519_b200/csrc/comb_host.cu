@@ -8,6 +8,7 @@
 #include "kernels.h"
 
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <unordered_map>
@@ -18,6 +19,7 @@ using namespace comb;
 namespace {
 
 constexpr int kRingSlots = 4;
+constexpr size_t kLinkInfoSlots = 8;
 
 struct Chunk {
     int32_t num_tokens;
@@ -49,6 +51,16 @@ struct comb_pool {
     bool kv_maps_ready = false;
     TensorMapBlob k_map, v_map;
     int64_t launches = 0;
+    // Host copy of the per-request page counts of the most recent links, keyed by their device buffer: lets the
+    // prefill planner cut long requests into KV ranges without reading the tables back from the device.
+    struct LinkInfo { const void *device_buf; std::vector<int32_t> pages; };
+    std::vector<LinkInfo> link_info;  // at most kLinkInfoSlots, oldest replaced first
+    size_t link_info_next = 0;
+    const std::vector<int32_t> *find_link_pages(const void *device_buf, int32_t R) const {
+        for (const LinkInfo &li : link_info)
+            if (li.device_buf == device_buf && (int32_t)li.pages.size() == R) return &li.pages;
+        return nullptr;
+    }
     // per-kernel timing (comb_profile_*)
     struct ProfRec { int id; cudaEvent_t a, b; };
     bool prof_on = false;
@@ -182,6 +194,33 @@ LinkLayout link_layout(int32_t R, int64_t total_pages, int64_t total_tiles) {
     L.off_page_ntok = o;   o = align_up(o + sizeof(int32_t) * (size_t)std::max<int64_t>(total_pages, 1), 16);
     L.bytes = o;
     return L;
+}
+
+// KV ranges per request for a prefill call that has `num_items` unsplit work items and whose longest request has
+// `max_tiles` 128-slot tiles. Ranges are only worth their fixed cost (pipeline fill per item, fp32 partial rows,
+// the merge pass) when the items cannot fill even one wave of the persistent grid: measured on B200, cutting a
+// 1.7-wave or 3.5-wave problem into ranges gained nothing (profiles/r01_bench.md). So: no ranges once there is an
+// item per SM; otherwise the largest count that still fits one wave, every range keeping at least two tiles.
+int plan_prefill_splits(size_t num_items, int max_tiles, int num_sms, int max_allowed) {
+    static const int cands[] = {1, 2, 3, 4, 6, 8, 12, 16};
+    static const int forced = [] {  // COMB_PREFILL_NSPLIT=n: measurement hook, overrides the policy (1 = never split)
+        const char *e = getenv("COMB_PREFILL_NSPLIT");
+        return e ? atoi(e) : 0;
+    }();
+    if (forced > 0) {
+        int ns = std::min(forced, max_allowed);
+        while (ns > 1 && prefill_tiles_per_split(max_tiles, ns) < 1) --ns;
+        return std::max(ns, 1);
+    }
+    if (num_items == 0 || num_items >= (size_t)num_sms) return 1;
+    int best = 1;
+    for (int ns : cands) {
+        if (ns > max_allowed) break;
+        if (ns > 1 && prefill_tiles_per_split(max_tiles, ns) < 2) break;
+        if (num_items * (size_t)ns > (size_t)num_sms) break;
+        best = ns;
+    }
+    return best;
 }
 
 LinkView view_of(const comb_link_t *l) {
@@ -480,6 +519,25 @@ int32_t comb_link(comb_pool_t *p, int32_t R, const int32_t *chunk_indptr, const 
     if (slot < 0) return COMB_ERR_CUDA;
     int32_t rc = comb_link_plan(p, R, chunk_indptr, chunk_ids, link, p->ring[slot].host);
     if (rc != COMB_OK) return rc;
+    {   // remember the page count of every request of this link (host side of page_indptr)
+        const int32_t *pi = (const int32_t *)((const char *)p->ring[slot].host +
+                                              ((const char *)link->page_indptr - (const char *)link->device_buf));
+        comb_pool::LinkInfo *li = nullptr;
+        for (comb_pool::LinkInfo &x : p->link_info)
+            if (x.device_buf == link->device_buf) li = &x;
+        if (!li) {
+            if (p->link_info.size() < kLinkInfoSlots) {
+                p->link_info.emplace_back();
+                li = &p->link_info.back();
+            } else {
+                li = &p->link_info[p->link_info_next];
+                p->link_info_next = (p->link_info_next + 1) % kLinkInfoSlots;
+            }
+            li->device_buf = link->device_buf;
+        }
+        li->pages.resize((size_t)R);
+        for (int32_t r = 0; r < R; ++r) li->pages[(size_t)r] = pi[r + 1] - pi[r];
+    }
     cudaStream_t st = (cudaStream_t)stream;
     // the ONLY data movement of the link stage: the tables. K/V are never touched.
     if (cudaMemcpyAsync(link->device_buf, p->ring[slot].host, link->bytes_used, cudaMemcpyHostToDevice, st) !=
@@ -497,8 +555,15 @@ size_t comb_workspace_bytes(const comb_pool_t *p, int32_t R, int32_t Hq, int64_t
     // prefill: one item per (request, kv-head, pair of 128-row tiles); rows per tile = 128 / G tokens
     const int G = std::max(1, Hq / p->cfg.num_kv_heads);
     const int tok_per_item = 2 * 128 / std::min(G, 128);
-    const size_t items = ((size_t)total_q / tok_per_item + (size_t)R + 1) * p->cfg.num_kv_heads;
-    const size_t pre = items * sizeof(PrefillItem);
+    const size_t items_hi = ((size_t)total_q / tok_per_item + (size_t)R + 1) * p->cfg.num_kv_heads;
+    const size_t items_lo = ((size_t)total_q + tok_per_item - 1) / tok_per_item * p->cfg.num_kv_heads;
+    // the planner sees the exact item count at call time; bound its answer over every count this shape allows
+    const int max_tiles = (max_pages + kTilePages - 1) / kTilePages;
+    int nsplit = 1;
+    for (size_t n = std::max<size_t>(items_lo, 1); n <= items_hi; n += (size_t)p->cfg.num_kv_heads)
+        nsplit = std::max(nsplit, plan_prefill_splits(n, max_tiles, p->num_sms, prefill_max_splits()));
+    const size_t pre = align_up(items_hi * (size_t)nsplit * sizeof(PrefillItem), 256) +
+                       (nsplit > 1 ? prefill_partial_bytes(nsplit, total_q, Hq, p->cfg.head_dim_v) : 0);
     return align_up(std::max(dec, pre), 256) + 256;
 }
 
@@ -555,14 +620,30 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     // BASELINE configs) make this the same as longest-first.
     for (int32_t r = 0; r < R; ++r) order.push_back(Req{r, (int64_t)q_indptr[r + 1] - q_indptr[r]});
     std::stable_sort(order.begin(), order.end(), [](const Req &a, const Req &b) { return a.cost > b.cost; });
-    size_t num_items = 0;
-    for (const Req &x : order) num_items += (size_t)((x.cost + tok_per_item - 1) / tok_per_item) * Hkv;
-    if (num_items == 0) return COMB_OK;
-    if (num_items > (size_t)INT32_MAX) return COMB_ERR_CAPACITY;
-    const size_t need = num_items * sizeof(PrefillItem);
-    if (!ws || ws_bytes < need) return COMB_ERR_CAPACITY;
-    cudaStream_t st = (cudaStream_t)stream;
+    size_t base_items = 0;
+    for (const Req &x : order) base_items += (size_t)((x.cost + tok_per_item - 1) / tok_per_item) * Hkv;
+    if (base_items == 0) return COMB_OK;
     p->probe_device();
+    // ---- KV ranges: only when the link's per-request page counts are known on the host (comb_link of this pool)
+    const std::vector<int32_t> *req_pages = p->find_link_pages(link->device_buf, R);
+    const int max_tiles = (link->max_pages_per_request + kTilePages - 1) / kTilePages;
+    const int nsplit = req_pages ? plan_prefill_splits(base_items, max_tiles, p->num_sms, prefill_max_splits()) : 1;
+    size_t num_items = 0;
+    for (const Req &x : order) {
+        int eff = 1;
+        if (nsplit > 1) {
+            const int n_kv = ((*req_pages)[(size_t)x.r] + kTilePages - 1) / kTilePages;
+            const int tps = prefill_tiles_per_split(n_kv, nsplit);
+            eff = tps > 0 ? (n_kv + tps - 1) / tps : 1;
+        }
+        num_items += (size_t)((x.cost + tok_per_item - 1) / tok_per_item) * Hkv * (size_t)eff;
+    }
+    if (num_items > (size_t)INT32_MAX) return COMB_ERR_CAPACITY;
+    const size_t items_bytes = align_up(num_items * sizeof(PrefillItem), 256);
+    const size_t part_bytes = nsplit > 1 ? prefill_partial_bytes(nsplit, total_q, Hq, p->cfg.head_dim_v) : 0;
+    const size_t need = items_bytes + part_bytes;
+    if (!ws || ws_bytes < need || (((uintptr_t)ws) & 15)) return COMB_ERR_CAPACITY;
+    cudaStream_t st = (cudaStream_t)stream;
     if (!p->kv_maps_ready) {
         if (prefill_encode_kv_maps(p->geom, &p->k_map, &p->v_map) != cudaSuccess) return COMB_ERR_CUDA;
         p->kv_maps_ready = true;
@@ -571,23 +652,37 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     maps.k = p->k_map;
     maps.v = p->v_map;
     if (prefill_encode_q_map(q, total_q, Hq, G, p->cfg.head_dim_qk, &maps.q) != cudaSuccess) return COMB_ERR_CUDA;
-    const int slot = p->acquire(need);
+    const int slot = p->acquire(num_items * sizeof(PrefillItem));
     if (slot < 0) return COMB_ERR_CUDA;
     PrefillItem *h = (PrefillItem *)p->ring[slot].host;
     size_t at = 0;
     for (const Req &x : order) {
         const int32_t row0 = q_indptr[x.r];
+        int n_kv = 0, tps = INT32_MAX / kTilePages, eff = 1;
+        if (nsplit > 1) {
+            n_kv = ((*req_pages)[(size_t)x.r] + kTilePages - 1) / kTilePages;
+            tps = prefill_tiles_per_split(n_kv, nsplit);
+            eff = tps > 0 ? (n_kv + tps - 1) / tps : 1;
+            if (eff <= 1) tps = INT32_MAX / kTilePages;
+        }
+        // the ranges of one (Q tile pair, kv-head) sit together, then the kv-heads: CTAs that stream the same K/V
+        // run at the same time (L2 reuse)
         for (int64_t t = 0; t < x.cost; t += tok_per_item)
             for (int g = 0; g < Hkv; ++g)
-                h[at++] = PrefillItem{x.r, g, row0 + (int32_t)t, (int32_t)std::min<int64_t>(tok_per_item, x.cost - t)};
+                for (int sidx = 0; sidx < eff; ++sidx)
+                    h[at++] = PrefillItem{x.r, g, row0 + (int32_t)t, (int32_t)std::min<int64_t>(tok_per_item, x.cost - t),
+                                          eff > 1 ? sidx * tps : 0, tps, eff > 1 ? sidx : -1, 0};
     }
-    if (cudaMemcpyAsync(ws, h, need, cudaMemcpyHostToDevice, st) != cudaSuccess) return COMB_ERR_CUDA;
+    if (cudaMemcpyAsync(ws, h, num_items * sizeof(PrefillItem), cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return COMB_ERR_CUDA;
     if (p->prof_on) p->hook.begin(p, kKernelPrefill, st);
+    int launches = 0;
     cudaError_t e = launch_prefill(p->geom, layer, view_of(link), maps, (const PrefillItem *)ws, (int)num_items, Hq,
-                                   scale, out, lse, p->num_sms, st);
+                                   scale, out, lse, nsplit, total_q, (char *)ws + items_bytes, p->num_sms, st,
+                                   &launches);
     if (p->prof_on) p->hook.end(p, st);
     if (e != cudaSuccess) return COMB_ERR_CUDA;
-    p->launches += 1;
+    p->launches += launches;
     if (!p->release(slot, st)) return COMB_ERR_CUDA;
     return COMB_OK;
 }

@@ -56,13 +56,23 @@ cudaError_t launch_decode(const PoolGeom &g, int layer, const LinkView &lv, int 
                           cudaStream_t stream, int *launches, const LaunchHook *hook);
 
 // ---- (a4) prefill -----------------------------------------------------------------------------
-// One CTA work item: up to two consecutive 128-row Q tiles of one (request, kv-head).
+// One CTA work item: up to two consecutive 128-row Q tiles of one (request, kv-head) against a range of the
+// request's 128-slot KV tiles. A request's KV is cut into `nsplit` ranges when there are too few items to fill the
+// GPU (low-parallelism shapes: few requests, few query tokens); the ranges' partial results are merged by LSE.
 struct PrefillItem {
     int32_t request;
     int32_t kv_head;
     int32_t q_row0;     // first query token row (absolute row in q) of tile 0
     int32_t q_rows;     // valid query tokens in this item (1 .. 2*128/G)
+    int32_t kv_tile0;   // first KV tile of this item (index inside the request)
+    int32_t kv_tiles;   // KV tiles of this item (clamped to the request's on the device)
+    int32_t split;      // -1: the item sees all of the request's KV and writes the final output; else its range index
+    int32_t pad;
 };
+// Splits of a request with n_kv tiles when the call uses `nsplit` ranges: ceil(n_kv / ceil(n_kv / nsplit)).
+inline int prefill_tiles_per_split(int n_kv, int nsplit) { return (n_kv + nsplit - 1) / nsplit; }
+int prefill_max_splits();  // 1 when the selected kernel cannot split (debug kernel), else 16
+size_t prefill_partial_bytes(int nsplit, int64_t total_q, int num_q_heads, int dv);
 bool prefill_supported(int group, int dqk, int dv);
 // CUtensorMap is 128 bytes, 64-byte aligned; kept opaque here so the runtime needs no cuda.h.
 struct alignas(64) TensorMapBlob { unsigned char bytes[128]; };
@@ -71,8 +81,10 @@ struct PrefillMaps { TensorMapBlob q, k, v; };
 cudaError_t prefill_encode_kv_maps(const PoolGeom &g, TensorMapBlob *k_map, TensorMapBlob *v_map);
 cudaError_t prefill_encode_q_map(const void *q, int64_t total_q, int num_q_heads, int group, int dqk,
                                  TensorMapBlob *q_map);
+// nsplit > 1: `partials` holds prefill_partial_bytes() bytes; a second kernel merges the ranges (*launches += 1).
 cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &maps,
                            const PrefillItem *items_dev, int num_items, int num_q_heads, float scale, void *out,
-                           float *lse, int num_sms, cudaStream_t stream);
+                           float *lse, int nsplit, int64_t total_q, void *partials, int num_sms, cudaStream_t stream,
+                           int *launches);
 
 }  // namespace comb

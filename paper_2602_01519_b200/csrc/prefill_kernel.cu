@@ -35,7 +35,26 @@ struct PrefillArgs {
     int num_q_heads, num_kv_heads, group;
     int layer_row0;      // first arena row of this layer = layer * num_pages * Hkv * 16
     float scale_log2;    // scale * log2(e)
+    // KV ranges (items with split >= 0): normalised partial rows and their log2-domain LSE, merged by a second kernel
+    float *part_o;       // [nsplit][sum lq][Hq][Dv]
+    float *part_lse;     // [nsplit][sum lq][Hq]   log2(sum_j 2^(s_j * scale_log2)) over the item's range
+    int64_t total_q;
+    int nsplit;
 };
+
+// The slice of a request's tables an item covers: first table entry, number of entries, first tile.
+struct ItemKv {
+    int pbeg, npages, tile0;
+};
+__device__ __forceinline__ ItemKv item_kv(const PrefillArgs &a, const PrefillItem &it) {
+    const int pb = a.page_indptr[it.request], np = a.page_indptr[it.request + 1] - pb;
+    ItemKv v;
+    const int skip = min(np, it.kv_tile0 * kTilePages);
+    v.pbeg = pb + skip;
+    v.npages = min(np - skip, it.kv_tiles * kTilePages);
+    v.tile0 = a.tile_indptr[it.request] + it.kv_tile0;
+    return v;
+}
 
 struct Maps {
     CUtensorMap q, k, v;
@@ -273,7 +292,7 @@ __device__ __forceinline__ float fmax3(float a, float b, float c) {
     return d;
 }
 
-template <int DQK, int DV>
+template <int DQK, int DV, bool RANGES>
 __global__ void __launch_bounds__(384, 1)
 prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const int num_items) {
     using C = V1Cfg<DQK, DV>;
@@ -338,9 +357,9 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
             const PrefillItem it = a.items[idx];
             const int tok_valid = it.q_rows - t * tok_per_tile;
             if (tok_valid <= 0) continue;  // this item has no second Q tile
-            const int npages = a.page_indptr[it.request + 1] - a.page_indptr[it.request];
-            const int n_kv = (npages + kTilePages - 1) / kTilePages;
-            const int tile0 = a.tile_indptr[it.request];
+            const ItemKv kv = item_kv(a, it);
+            const int n_kv = (kv.npages + kTilePages - 1) / kTilePages;
+            const int tile0 = kv.tile0;
             const bool row_valid = row_tok < tok_valid;
             const int tok = it.q_row0 + t * tok_per_tile + row_tok, head = it.kv_head * G + row_head;
             __nv_bfloat16 *orow = a.out + ((size_t)tok * Hq + head) * DV;
@@ -416,12 +435,14 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
             o_cnt += n_kv;
             ptx::tc_fence_after();
             const float inv = 1.f / l_run;
+            const bool partial = RANGES && it.split >= 0;  // one KV range of several (RANGES: compiled in only then)
+            const size_t prow = partial ? ((size_t)it.split * (size_t)a.total_q + (size_t)tok) * Hq + head : 0;
 #pragma unroll
             for (int q = 0; q < DV / 32; ++q) {
                 uint32_t o[32];
                 ptx::tmem_ld32(tO + q * 32, o);
                 ptx::tmem_wait_ld();
-                if (row_valid) {
+                if (row_valid && !partial) {
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
                         uint4 w;
@@ -431,9 +452,18 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
                         w.w = ptx::pack_bf16x2(__uint_as_float(o[8 * e + 6]) * inv, __uint_as_float(o[8 * e + 7]) * inv);
                         reinterpret_cast<uint4 *>(orow)[q * 4 + e] = w;
                     }
+                } else if (RANGES && row_valid) {  // fp32 partial row for the merge kernel
+                    float4 *prow_o = reinterpret_cast<float4 *>(a.part_o + prow * DV + q * 32);
+#pragma unroll
+                    for (int e = 0; e < 8; ++e)
+                        prow_o[e] = make_float4(__uint_as_float(o[4 * e + 0]) * inv, __uint_as_float(o[4 * e + 1]) * inv,
+                                                __uint_as_float(o[4 * e + 2]) * inv, __uint_as_float(o[4 * e + 3]) * inv);
                 }
             }
-            if (row_valid && a.lse) a.lse[(size_t)tok * Hq + head] = (m_used * c + log2f(l_run)) * kLn2;
+            if (row_valid) {
+                if (partial) a.part_lse[prow] = m_used * c + log2f(l_run);
+                else if (a.lse) a.lse[(size_t)tok * Hq + head] = (m_used * c + log2f(l_run)) * kLn2;
+            }
             ptx::tc_fence_before();  // our reads of O precede the arrive that lets the next item's P V overwrite it
         }
     } else if (warp == 8) {
@@ -441,7 +471,8 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
         uint32_t slot = 0, phase = 0, qcnt[2] = {0, 0};
         for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
             const PrefillItem it = a.items[idx];
-            const int pbeg = a.page_indptr[it.request], npages = a.page_indptr[it.request + 1] - pbeg;
+            const ItemKv kv = item_kv(a, it);
+            const int pbeg = kv.pbeg, npages = kv.npages;
             const int n_kv = (npages + kTilePages - 1) / kTilePages;
             if (n_kv == 0) continue;
             const int nq = it.q_rows > tok_per_tile ? 2 : 1;
@@ -502,7 +533,7 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
         };
         for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
             const PrefillItem it = a.items[idx];
-            const int npages = a.page_indptr[it.request + 1] - a.page_indptr[it.request];
+            const int npages = item_kv(a, it).npages;
             const int n_kv = (npages + kTilePages - 1) / kTilePages;
             if (n_kv == 0) continue;
             const int nq = it.q_rows > tok_per_tile ? 2 : 1;
@@ -559,6 +590,59 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
     if (warp == 8) ptx::tmem_dealloc(tmem, C::TMEM_COLS);
 }
 
+// ============================================================================================
+// Merge of KV ranges (SURVEY.md §8(c) pin P8): for the rows of every item with split == 0,
+//   out = sum_s w_s O_s / sum_s w_s,  w_s = 2^(lse2_s - max_s lse2_s),  lse = ln 2 * (max + log2 sum_s w_s).
+// Grid (item, row group): items with split != 0 return at once; a warp merges one row, a lane owns DV/32 columns.
+// Every load of a row is independent of the others (all ranges' LSEs first, then all partial rows), so a row costs
+// about two memory round trips.
+// ============================================================================================
+template <int DV>
+__global__ void __launch_bounds__(128) prefill_merge_kernel(const PrefillArgs a, const int num_items) {
+    const PrefillItem it = a.items[blockIdx.x];
+    if (it.split != 0) return;
+    const int G = a.group, Hq = a.num_q_heads;
+    const int np = a.page_indptr[it.request + 1] - a.page_indptr[it.request];
+    const int n_kv = (np + kTilePages - 1) / kTilePages;
+    const int nsp = (n_kv + it.kv_tiles - 1) / it.kv_tiles;  // ranges of this request (it.kv_tiles = tiles per range)
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    constexpr int CPL = DV / 32;  // columns per lane (2 or 4)
+    constexpr int kMaxSplits = 16;
+    const int row = blockIdx.y * 4 + warp;
+    if (row < it.q_rows * G && nsp <= kMaxSplits) {
+        const int tok = it.q_row0 + row / G, head = it.kv_head * G + row % G;
+        const size_t r0 = (size_t)tok * Hq + head, stride = (size_t)a.total_q * Hq;
+        float l2[kMaxSplits], m = -INFINITY;
+#pragma unroll
+        for (int s = 0; s < kMaxSplits; ++s) l2[s] = s < nsp ? a.part_lse[r0 + s * stride] : -INFINITY;
+#pragma unroll
+        for (int s = 0; s < kMaxSplits; ++s) m = fmaxf(m, l2[s]);
+        float acc[CPL];
+#pragma unroll
+        for (int e = 0; e < CPL; ++e) acc[e] = 0.f;
+        float wsum = 0.f;
+#pragma unroll 4
+        for (int s = 0; s < nsp; ++s) {
+            const float w = ptx::ex2(l2[s] - m);
+            wsum += w;
+            const float *po = a.part_o + (r0 + s * stride) * DV + lane * CPL;
+            if constexpr (CPL == 4) {
+                const float4 v = *reinterpret_cast<const float4 *>(po);
+                acc[0] += w * v.x; acc[1] += w * v.y; acc[2] += w * v.z; acc[3] += w * v.w;
+            } else {
+                const float2 v = *reinterpret_cast<const float2 *>(po);
+                acc[0] += w * v.x; acc[1] += w * v.y;
+            }
+        }
+        const float inv = 1.f / wsum;
+        __nv_bfloat16 *orow = a.out + r0 * DV + lane * CPL;
+#pragma unroll
+        for (int e = 0; e < CPL; e += 2)
+            *reinterpret_cast<uint32_t *>(orow + e) = ptx::pack_bf16x2(acc[e] * inv, acc[e + 1] * inv);
+        if (lane == 0 && a.lse) a.lse[r0] = (m + log2f(wsum)) * kLn2;
+    }
+}
+
 // ---------------------------------------------------------------- TMA descriptor encoding (host)
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -606,7 +690,7 @@ cudaError_t launch_v0(const PrefillArgs &a, const Maps &maps, int num_items, cud
 template <int DQK, int DV>
 cudaError_t launch_v1(const PrefillArgs &a, const Maps &maps, int num_items, int num_sms, cudaStream_t st) {
     using C = V1Cfg<DQK, DV>;
-    auto kern = prefill_v1_kernel<DQK, DV>;
+    auto kern = a.nsplit > 1 ? prefill_v1_kernel<DQK, DV, true> : prefill_v1_kernel<DQK, DV, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
     if (e != cudaSuccess) return e;
     const int grid = num_items < num_sms ? num_items : num_sms;
@@ -652,9 +736,16 @@ cudaError_t prefill_encode_q_map(const void *q, int64_t total_q, int num_q_heads
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
+int prefill_max_splits() { return use_v0() ? 1 : 16; }
+
+size_t prefill_partial_bytes(int nsplit, int64_t total_q, int num_q_heads, int dv) {
+    return (size_t)nsplit * (size_t)total_q * (size_t)num_q_heads * (size_t)(dv + 1) * sizeof(float);
+}
+
 cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &pm,
                            const PrefillItem *items_dev, int num_items, int num_q_heads, float scale, void *out,
-                           float *lse, int num_sms, cudaStream_t stream) {
+                           float *lse, int nsplit, int64_t total_q, void *partials, int num_sms, cudaStream_t stream,
+                           int *launches) {
     PrefillArgs a;
     a.items = items_dev;
     a.page_indptr = lv.page_indptr;
@@ -668,14 +759,20 @@ cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, con
     a.group = num_q_heads / g.num_kv_heads;
     a.layer_row0 = layer * g.num_pages * g.num_kv_heads * kPage;
     a.scale_log2 = scale * kLog2e;
+    a.total_q = total_q;
+    a.nsplit = nsplit;
+    a.part_o = nsplit > 1 ? (float *)partials : nullptr;
+    a.part_lse = nsplit > 1 ? a.part_o + (size_t)nsplit * (size_t)total_q * num_q_heads * g.head_dim_v : nullptr;
+    if (nsplit > 1 && (use_v0() || !partials)) return cudaErrorInvalidValue;
     Maps maps;
     memcpy(&maps.q, &pm.q, sizeof(CUtensorMap));
     memcpy(&maps.k, &pm.k, sizeof(CUtensorMap));
     memcpy(&maps.v, &pm.v, sizeof(CUtensorMap));
+    cudaError_t e = cudaErrorInvalidValue;
 #define COMB_PREFILL_CASE(DQ, DVV)                                                              \
     if (g.head_dim_qk == DQ && g.head_dim_v == DVV)                                             \
-        return use_v0() ? launch_v0<DQ, DVV>(a, maps, num_items, stream)                        \
-                        : launch_v1<DQ, DVV>(a, maps, num_items, num_sms, stream);
+        e = use_v0() ? launch_v0<DQ, DVV>(a, maps, num_items, stream)                           \
+                     : launch_v1<DQ, DVV>(a, maps, num_items, num_sms, stream);
     COMB_PREFILL_CASE(128, 128)
     COMB_PREFILL_CASE(64, 64)
     COMB_PREFILL_CASE(192, 128)
@@ -683,7 +780,16 @@ cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, con
     COMB_PREFILL_CASE(64, 128)
     COMB_PREFILL_CASE(192, 64)
 #undef COMB_PREFILL_CASE
-    return cudaErrorInvalidValue;
+    if (e != cudaSuccess) return e;
+    *launches += 1;
+    if (nsplit > 1) {
+        const dim3 mgrid(num_items, 2 * kTileM / 4);  // an item has at most 2 x 128 rows, a CTA merges 4
+        if (g.head_dim_v == 128) prefill_merge_kernel<128><<<mgrid, 128, 0, stream>>>(a, num_items);
+        else prefill_merge_kernel<64><<<mgrid, 128, 0, stream>>>(a, num_items);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        *launches += 1;
+    }
+    return cudaSuccess;
 }
 
 }  // namespace comb

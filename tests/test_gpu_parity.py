@@ -195,6 +195,28 @@ def test_prefill_tiny_config():
     check_attention(out, lse, *oracle.attention_for(w.peaked()), tag="tiny prefill peaked")
 
 
+@pytest.mark.parametrize("shape", [(32, 8, 128, 128), (16, 16, 192, 128), (8, 2, 64, 64)])
+def test_prefill_kv_ranges_low_parallelism(shape):
+    """Few work items for 148 SMs (the paper's regime: < 50 dynamic tokens): every request's KV is cut
+    into ranges that run on different SMs and are merged by LSE (pin P8). Requests of very different lengths (one
+    shorter than a range, one empty, interior partial pages) share the call."""
+    Hq, Hkv, Dqk, Dv = shape
+    lens = [700, 333, 512, 129, 16, 1000, 47, 800]
+    w = cs.custom("ranges", num_q_heads=Hq, num_kv_heads=Hkv, head_dim_qk=Dqk, head_dim_v=Dv, chunk_len=lens,
+                  links=[[0, 1, 2, 3, 5, 7, 6], [4], [], [5, 0, 7, 2, 1]], lq=[20, 7, 3, 33], seed=5)
+    for ww in (w, w.peaked()):
+        ld = H().load_workload(ww, sentinel=SENTINEL, shuffle_seed=13)
+        l0 = ld.pool.launches
+        out, lse = ld.pool.prefill(ld.batch, ld.q, ld.q_indptr, ww.scale)
+        torch.cuda.synchronize()
+        assert ld.pool.launches - l0 == 2, "expected the range kernel + the merge kernel"
+        out, lse = H().device_to_bits(out), lse.cpu().numpy().astype(np.float64)
+        check_attention(out, lse, *oracle.attention_for(ww), tag="kv ranges %s" % (shape,))
+        rows2 = slice(int(ww.q_indptr[2]), int(ww.q_indptr[3]))
+        assert np.all(out[rows2] == 0) and np.all(np.isneginf(lse[rows2]))
+        ld.pool.close()
+
+
 @pytest.mark.parametrize("shape", PREFILL_SHAPES)
 @pytest.mark.parametrize("peaked", [False, True])
 def test_prefill_ragged(shape, peaked):
