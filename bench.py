@@ -379,9 +379,15 @@ def main():
         # ---- the other configs (not bench lines; context for the BASELINE metric's prefill half) ----
         def prefill_extra(name, wk, steps, fill, flush=False):
             rr = bench_attention(wk, "prefill", steps, 3, fill=fill, flush_l2=flush, e2e=False)
+            # a prefill whose flops per logical KV byte sit under the ridge of the measured peaks is HBM-bound
+            # (no GQA or few query tokens: SURVEY.md 8(d)); it is then reported against the HBM roof first
+            ridge = pk["tf_burst"] * 1e12 / (pk["hbm"] * 1e9)
+            intensity = rr["flops"] / (rr["kv_bytes"] + rr["io_bytes"])
             extras[name] = {"workload": name, "ms_per_step": rr["ms_per_step"], "kernel_ms": rr["kernel_ms"],
                             "tflops": rr["flops"] / (rr["ms_per_step"] * 1e-3) / 1e12,
                             "q_tokens_per_s": rr["q_tokens"] / (rr["ms_per_step"] * 1e-3),
+                            "flop_per_logical_byte": intensity, "ridge_flop_per_byte": ridge,
+                            "roofline_hbm": roofline_hbm(rr, "prefill", "") if intensity < ridge else None,
                             "roofline": roofline_tensor(rr, "prefill", name.replace("_prefill", "") if name != "rag_prefill" else name), "clocks": rr["clocks"],
                             "l2": L2Flush.HOW if flush else "inputs larger than L2"}
             log(name, json.dumps(extras[name]))

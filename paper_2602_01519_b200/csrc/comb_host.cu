@@ -554,9 +554,10 @@ size_t comb_workspace_bytes(const comb_pool_t *p, int32_t R, int32_t Hq, int64_t
     const size_t dec = decode_workspace_bytes(R, Hq, p->cfg.head_dim_v, plan);
     // prefill: one item per (request, kv-head, pair of 128-row tiles); rows per tile = 128 / G tokens
     const int G = std::max(1, Hq / p->cfg.num_kv_heads);
-    const int tok_per_item = 2 * 128 / std::min(G, 128);
-    const size_t items_hi = ((size_t)total_q / tok_per_item + (size_t)R + 1) * p->cfg.num_kv_heads;
-    const size_t items_lo = ((size_t)total_q + tok_per_item - 1) / tok_per_item * p->cfg.num_kv_heads;
+    // an item covers one or two 128-row tiles (prefill_tiles_per_cta): bound the item count from both sides
+    const int tok_per_tile = 128 / std::min(G, 128);
+    const size_t items_hi = ((size_t)total_q / tok_per_tile + (size_t)R + 1) * p->cfg.num_kv_heads;
+    const size_t items_lo = ((size_t)total_q + 2 * tok_per_tile - 1) / (2 * tok_per_tile) * p->cfg.num_kv_heads;
     // the planner sees the exact item count at call time; bound its answer over every count this shape allows
     const int max_tiles = (max_pages + kTilePages - 1) / kTilePages;
     int nsplit = 1;
@@ -610,7 +611,15 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     // ---- work items: (request, kv-head, pair of Q tiles); the 2*Hkv.. items of one request sit together so
     // CTAs that stream the same K/V run at the same time (L2 reuse). Requests are ordered longest KV first
     // so the tail of the grid is made of short items.
-    const int tok_per_tile = 128 / G, tok_per_item = 2 * tok_per_tile;
+    int64_t max_lq = 0;
+    for (int32_t r = 0; r < R; ++r) max_lq = std::max<int64_t>(max_lq, q_indptr[r + 1] - q_indptr[r]);
+    const std::vector<int32_t> *req_pages = p->find_link_pages(link->device_buf, R);
+    int64_t nonempty = 0;
+    for (int32_t r = 0; r < R; ++r) nonempty += q_indptr[r + 1] > q_indptr[r];
+    p->probe_device();
+    const int tiles_per_cta = prefill_tiles_per_cta(G, p->cfg.head_dim_qk, p->cfg.head_dim_v, max_lq, nonempty * Hkv,
+                                                    p->num_sms);
+    const int tok_per_tile = 128 / G, tok_per_item = tiles_per_cta * tok_per_tile;
     struct Req { int32_t r; int64_t cost; };
     std::vector<Req> order;
     order.reserve(R);
@@ -625,8 +634,9 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     if (base_items == 0) return COMB_OK;
     p->probe_device();
     // ---- KV ranges: only when the link's per-request page counts are known on the host (comb_link of this pool)
-    const std::vector<int32_t> *req_pages = p->find_link_pages(link->device_buf, R);
     const int max_tiles = (link->max_pages_per_request + kTilePages - 1) / kTilePages;
+    // (one item per SM is the target even when two single-tile CTAs share an SM: measured, 256 ranges on 148 SMs
+    // were slower than 128)
     const int nsplit = req_pages ? plan_prefill_splits(base_items, max_tiles, p->num_sms, prefill_max_splits()) : 1;
     size_t num_items = 0;
     for (const Req &x : order) {
@@ -678,8 +688,8 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     if (p->prof_on) p->hook.begin(p, kKernelPrefill, st);
     int launches = 0;
     cudaError_t e = launch_prefill(p->geom, layer, view_of(link), maps, (const PrefillItem *)ws, (int)num_items, Hq,
-                                   scale, out, lse, nsplit, total_q, (char *)ws + items_bytes, p->num_sms, st,
-                                   &launches);
+                                   scale, out, lse, nsplit, total_q, (char *)ws + items_bytes, tiles_per_cta,
+                                   p->num_sms, st, &launches);
     if (p->prof_on) p->hook.end(p, st);
     if (e != cudaSuccess) return COMB_ERR_CUDA;
     p->launches += launches;

@@ -72,6 +72,9 @@ struct PrefillItem {
 // Splits of a request with n_kv tiles when the call uses `nsplit` ranges: ceil(n_kv / ceil(n_kv / nsplit)).
 inline int prefill_tiles_per_split(int n_kv, int nsplit) { return (n_kv + nsplit - 1) / nsplit; }
 int prefill_max_splits();  // 1 when the selected kernel cannot split (debug kernel), else 16
+// Q tiles per CTA (1 or 2) for a call whose longest request has max_q_tokens query tokens and that would have
+// num_items single-tile items; an item then covers up to that many 128-row tiles.
+int prefill_tiles_per_cta(int group, int dqk, int dv, int64_t max_q_tokens, int64_t num_items, int num_sms);
 size_t prefill_partial_bytes(int nsplit, int64_t total_q, int num_q_heads, int dv);
 bool prefill_supported(int group, int dqk, int dv);
 // CUtensorMap is 128 bytes, 64-byte aligned; kept opaque here so the runtime needs no cuda.h.
@@ -84,7 +87,7 @@ cudaError_t prefill_encode_q_map(const void *q, int64_t total_q, int num_q_heads
 // nsplit > 1: `partials` holds prefill_partial_bytes() bytes; a second kernel merges the ranges (*launches += 1).
 cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &maps,
                            const PrefillItem *items_dev, int num_items, int num_q_heads, float scale, void *out,
-                           float *lse, int nsplit, int64_t total_q, void *partials, int num_sms, cudaStream_t stream,
-                           int *launches);
+                           float *lse, int nsplit, int64_t total_q, void *partials, int tiles_per_cta, int num_sms,
+                           cudaStream_t stream, int *launches);
 
 }  // namespace comb

@@ -46,6 +46,24 @@ struct PrefillArgs {
 struct ItemKv {
     int pbeg, npages, tile0;
 };
+// What tile slot t of an item works on: consecutive query rows over the item's KV range.
+struct TileView {
+    int q_row0, tok_valid;  // first query token row, valid query tokens (<= 0: slot unused)
+    int pbeg, npages, tile0;  // KV: first table entry, entries, first tile
+    int split;              // -1: final output, else range index of the partial result
+};
+__device__ __forceinline__ TileView tile_view(const PrefillArgs &a, const PrefillItem &it, int t, int tok_per_tile) {
+    const int pb = a.page_indptr[it.request], np = a.page_indptr[it.request + 1] - pb;
+    const int skip = min(np, it.kv_tile0 * kTilePages);
+    TileView v;
+    v.pbeg = pb + skip;
+    v.npages = min(np - skip, it.kv_tiles * kTilePages);
+    v.tile0 = a.tile_indptr[it.request] + it.kv_tile0;
+    v.q_row0 = it.q_row0 + t * tok_per_tile;
+    v.tok_valid = it.q_rows - t * tok_per_tile;
+    v.split = it.split;
+    return v;
+}
 __device__ __forceinline__ ItemKv item_kv(const PrefillArgs &a, const PrefillItem &it) {
     const int pb = a.page_indptr[it.request], np = a.page_indptr[it.request + 1] - pb;
     ItemKv v;
@@ -270,20 +288,35 @@ prefill_v0_kernel(const PrefillArgs a, const __grid_constant__ Maps maps) {
 // S_j, the tensor pipe runs P V_j and Q K_{j+1}^T of the other tile.  The running max is only advanced when it
 // grows by more than 2^8 (lazy rescale), so the accumulator in TMEM is almost never touched by the softmax warps.
 // ============================================================================================
-template <int DQK, int DV>
+// NT = Q tiles per CTA. NT = 2 is the configuration described above (one CTA per SM). NT = 1 is for calls in
+// which no request has more than one 128-row tile per kv-head (the paper's regime, < 50 dynamic tokens): a CTA then
+// has a single softmax warpgroup, 256 TMEM columns and half the shared memory, so TWO CTAs share an SM and the
+// ping-pong happens between CTAs, each with its own K/V stream (inside one CTA a lone tile would leave the tensor
+// pipe idle during its softmax).
+template <int DQK, int DV, int NT>
 struct V1Cfg {
     static constexpr int KH = DQK / 64, VH = DV / 64;
     static constexpr int HALF = kTileM * 128;  // [128 rows][64 bf16]
     static constexpr int Q_BYTES = KH * HALF;
     static constexpr int K_BYTES = KH * HALF, V_BYTES = VH * HALF;
     static constexpr int SLOT = K_BYTES > V_BYTES ? K_BYTES : V_BYTES;  // K and V tiles alternate in one ring
-    static constexpr int SMEM_MAX = 232448;                             // 227 KB
-    static constexpr int NSLOT_RAW = (SMEM_MAX - 1024 - 512 - 2 * Q_BYTES) / SLOT;
+    // 227 KB for a CTA that owns the SM; half of 228 KB less the 1 KB the system reserves per CTA for two per SM.
+    // A single-tile CTA whose ring would not get two slots in half an SM (Dqk = 192) takes the whole SM instead
+    // and spends the second Q tile's space on a third ring slot.
+    static constexpr bool HALF_SM = NT == 1 && (115712 - 1024 - 512 - Q_BYTES) / SLOT >= 2;
+    static constexpr int CTAS_PER_SM = HALF_SM ? 2 : 1;
+    static constexpr int SMEM_MAX = HALF_SM ? 115712 : 232448;
+    static constexpr int NSLOT_RAW = (SMEM_MAX - 1024 - 512 - NT * Q_BYTES) / SLOT;
     static constexpr int NSLOT = NSLOT_RAW > 8 ? 8 : NSLOT_RAW;
-    static_assert(NSLOT >= 2, "need at least a K and a V slot");
-    static constexpr int SMEM = 1024 + 2 * Q_BYTES + NSLOT * SLOT + 512;
-    static constexpr int TMEM_COLS = 512;
-    static constexpr int THREADS = 384;  // 3 warpgroups: softmax 0, softmax 1, {loader, MMA issuer, 2 idle warps}
+    static constexpr bool FITS = NSLOT >= 2;  // at least a K and a V slot
+    static constexpr int SMEM = 1024 + NT * Q_BYTES + (FITS ? NSLOT : 2) * SLOT + 512;
+    static constexpr int TMEM_COLS = 256 * NT;           // S_t/P_t @ 128 t, O_t @ 128 NT + t DV
+    static constexpr int NSW = 4 * NT;                   // softmax warps; then the loader warp, then the issuer warp
+    static constexpr int THREADS = 128 * (NT + 1);       // + one warpgroup {loader, MMA issuer, 2 idle warps}
+    // register file per CTA = THREADS x the launch-bound count (168 at NT = 2, 128 at NT = 1); setmaxnreg moves it:
+    //   NT = 2: 2 x 128 x 208 + 128 x 88 = 384 x 168        NT = 1: 128 x 208 + 128 x 48 = 256 x 128
+    static constexpr int REG_SOFTMAX = 208;
+    static constexpr int REG_OTHER = NT == 2 ? 88 : 48;
 };
 
 __device__ __forceinline__ float fmax3(float a, float b, float c) {
@@ -292,14 +325,14 @@ __device__ __forceinline__ float fmax3(float a, float b, float c) {
     return d;
 }
 
-template <int DQK, int DV, bool RANGES>
-__global__ void __launch_bounds__(384, 1)
+template <int DQK, int DV, bool RANGES, int NT>
+__global__ void __launch_bounds__(V1Cfg<DQK, DV, NT>::THREADS, 3 - NT)  // registers: 168 (NT = 2) or 128 (NT = 1)
 prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const int num_items) {
-    using C = V1Cfg<DQK, DV>;
+    using C = V1Cfg<DQK, DV, NT>;
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     unsigned char *sQ = smem;                    // [2 tiles][KH][128][64]
-    unsigned char *sKV = smem + 2 * C::Q_BYTES;  // ring of NSLOT tiles
+    unsigned char *sKV = smem + NT * C::Q_BYTES;  // ring of NSLOT tiles
     uint64_t *bars = reinterpret_cast<uint64_t *>(sKV + C::NSLOT * C::SLOT);
     uint64_t *q_full = bars, *q_empty = bars + 2, *s_full = bars + 4, *p_full = bars + 6, *o_done = bars + 8;
     uint64_t *kv_full = bars + 10, *kv_empty = bars + 10 + C::NSLOT;
@@ -323,7 +356,7 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
         ptx::tma_prefetch_desc(&maps.k);
         ptx::tma_prefetch_desc(&maps.v);
     }
-    if (warp == 8) {
+    if (warp == C::NSW) {
         ptx::tmem_alloc(tmem_slot, C::TMEM_COLS);
         ptx::tmem_relinquish();
     }
@@ -336,32 +369,32 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
 
     // register file: 384 x 168 at launch; the softmax warpgroups take what the third warpgroup gives up
     // (2 x 128 x 208 + 128 x 88 = 384 x 168: asking for more than the CTA owns would block forever)
-    if (warp < 8) {
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(208));
+    if (warp < C::NSW) {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::REG_SOFTMAX));
     } else {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(88));
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::REG_OTHER));
     }
 
-    if (warp < 8) {
+    if (warp < C::NSW) {
         // ===================== softmax + epilogue of Q tile t =====================
         const int t = warp >> 2;
         const int row = (warp & 3) * 32 + lane;
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
         const uint32_t tS = tmem + lane_base + t * 128;
-        const uint32_t tO = tmem + lane_base + 256 + t * DV;
+        const uint32_t tO = tmem + lane_base + 128 * NT + t * DV;
         const int row_tok = row / G, row_head = row % G;
         const float c = a.scale_log2;
         const float2 c2 = make_float2(c, c);
         uint32_t s_cnt = 0, o_cnt = 0;
         for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
             const PrefillItem it = a.items[idx];
-            const int tok_valid = it.q_rows - t * tok_per_tile;
-            if (tok_valid <= 0) continue;  // this item has no second Q tile
-            const ItemKv kv = item_kv(a, it);
-            const int n_kv = (kv.npages + kTilePages - 1) / kTilePages;
-            const int tile0 = kv.tile0;
+            const TileView tv = tile_view(a, it, t, tok_per_tile);
+            const int tok_valid = tv.tok_valid;
+            if (tok_valid <= 0) continue;  // this item does not use the second tile slot
+            const int n_kv = (tv.npages + kTilePages - 1) / kTilePages;
+            const int tile0 = tv.tile0;
             const bool row_valid = row_tok < tok_valid;
-            const int tok = it.q_row0 + t * tok_per_tile + row_tok, head = it.kv_head * G + row_head;
+            const int tok = tv.q_row0 + row_tok, head = it.kv_head * G + row_head;
             __nv_bfloat16 *orow = a.out + ((size_t)tok * Hq + head) * DV;
             if (n_kv == 0) {  // no contexts linked (reading I13): zero contribution, lse = -inf
                 if (row_valid) {
@@ -435,8 +468,8 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
             o_cnt += n_kv;
             ptx::tc_fence_after();
             const float inv = 1.f / l_run;
-            const bool partial = RANGES && it.split >= 0;  // one KV range of several (RANGES: compiled in only then)
-            const size_t prow = partial ? ((size_t)it.split * (size_t)a.total_q + (size_t)tok) * Hq + head : 0;
+            const bool partial = RANGES && tv.split >= 0;  // one KV range of several (RANGES: compiled in only then)
+            const size_t prow = partial ? ((size_t)tv.split * (size_t)a.total_q + (size_t)tok) * Hq + head : 0;
 #pragma unroll
             for (int q = 0; q < DV / 32; ++q) {
                 uint32_t o[32];
@@ -466,55 +499,63 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
             }
             ptx::tc_fence_before();  // our reads of O precede the arrive that lets the next item's P V overwrite it
         }
-    } else if (warp == 8) {
+    } else if (warp == C::NSW) {
         // ===================== TMA loader =====================
         uint32_t slot = 0, phase = 0, qcnt[2] = {0, 0};
         for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
             const PrefillItem it = a.items[idx];
-            const ItemKv kv = item_kv(a, it);
-            const int pbeg = kv.pbeg, npages = kv.npages;
-            const int n_kv = (npages + kTilePages - 1) / kTilePages;
-            if (n_kv == 0) continue;
-            const int nq = it.q_rows > tok_per_tile ? 2 : 1;
-            for (int t = 0; t < nq; ++t) {
+            TileView tv[2];
+            int n_kv[2];
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                tv[t] = tile_view(a, it, t, tok_per_tile);
+                n_kv[t] = (t < NT && tv[t].tok_valid > 0) ? (tv[t].npages + kTilePages - 1) / kTilePages : 0;
+            }
+            if (n_kv[0] == 0) continue;
+#pragma unroll
+            for (int t = 0; t < NT; ++t) {
+                if (n_kv[t] == 0) continue;
                 ptx::mbar_wait(&q_empty[t], (qcnt[t] & 1) ^ 1);
                 ++qcnt[t];
                 if (lane == 0) {
                     ptx::mbar_expect_tx(&q_full[t], C::Q_BYTES);
                     for (int h = 0; h < C::KH; ++h)
                         ptx::tma_load_3d(sQ + t * C::Q_BYTES + h * C::HALF, &maps.q, h * 64, it.kv_head * G,
-                                         it.q_row0 + t * tok_per_tile, &q_full[t]);
+                                         tv[t].q_row0, &q_full[t]);
                 }
             }
-            for (int j = 0; j < n_kv; ++j) {
-                const int pages_here = min(kTilePages, npages - j * kTilePages);
+            // one K (is_v = false) or V tile of tile slot t's stream into the next ring slot
+            auto load_tile = [&](int t, int j, bool is_v) {
+                const int pages_here = min(kTilePages, tv[t].npages - j * kTilePages);
                 int row0 = 0;
                 if (lane < pages_here) {
-                    const int pid = a.page_ids[pbeg + j * kTilePages + lane];
+                    const int pid = a.page_ids[tv[t].pbeg + j * kTilePages + lane];
                     row0 = a.layer_row0 + (pid * a.num_kv_heads + it.kv_head) * kPage;
                 }
+                ptx::mbar_wait(&kv_empty[slot], phase ^ 1);
+                unsigned char *dst = sKV + slot * C::SLOT;
+                if (lane == 0)
+                    ptx::mbar_expect_tx(&kv_full[slot], (uint32_t)pages_here * kPage * (is_v ? DV : DQK) * 2);
+                __syncwarp();
+                if (lane < pages_here) {
+                    if (!is_v) {
 #pragma unroll
-                for (int kv = 0; kv < 2; ++kv) {  // K tile, then V tile
-                    ptx::mbar_wait(&kv_empty[slot], phase ^ 1);
-                    unsigned char *dst = sKV + slot * C::SLOT;
-                    if (lane == 0) ptx::mbar_expect_tx(&kv_full[slot], (uint32_t)pages_here * kPage * (kv == 0 ? DQK : DV) * 2);
-                    __syncwarp();
-                    if (lane < pages_here) {
-                        if (kv == 0) {
+                        for (int h = 0; h < C::KH; ++h)
+                            ptx::tma_load_2d(dst + h * C::HALF + lane * 2048, &maps.k, h * 64, row0, &kv_full[slot]);
+                    } else {
 #pragma unroll
-                            for (int h = 0; h < C::KH; ++h)
-                                ptx::tma_load_2d(dst + h * C::HALF + lane * 2048, &maps.k, h * 64, row0, &kv_full[slot]);
-                        } else {
-#pragma unroll
-                            for (int h = 0; h < C::VH; ++h)
-                                ptx::tma_load_2d(dst + h * C::HALF + lane * 2048, &maps.v, h * 64, row0, &kv_full[slot]);
-                        }
+                        for (int h = 0; h < C::VH; ++h)
+                            ptx::tma_load_2d(dst + h * C::HALF + lane * 2048, &maps.v, h * 64, row0, &kv_full[slot]);
                     }
-                    if (++slot == C::NSLOT) { slot = 0; phase ^= 1; }
                 }
+                if (++slot == C::NSLOT) { slot = 0; phase ^= 1; }
+            };
+            for (int j = 0; j < n_kv[0]; ++j) {  // both tile slots read the same stream: K_0 V_0 K_1 V_1 ...
+                load_tile(0, j, false);
+                load_tile(0, j, true);
             }
         }
-    } else if (warp == 9 && lane == 0) {
+    } else if (warp == C::NSW + 1 && lane == 0) {
         // ===================== MMA issuer (one thread) =====================
         constexpr uint32_t idesc_s = ptx::umma_idesc_bf16(kTileM, kTileN, false);
         constexpr uint32_t idesc_o = ptx::umma_idesc_bf16(kTileM, DV, true);
@@ -564,7 +605,7 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
                     ++pcnt[t];
                     ptx::tc_fence_after();
                     for (int ks = 0; ks < pages_here; ++ks)  // O_t += P_t V_j, one k-step of 16 keys per page
-                        ptx::mma_ts(tmem + 256 + t * DV, tmem + t * 128 + ks * 8,
+                        ptx::mma_ts(tmem + 128 * NT + t * DV, tmem + t * 128 + ks * 8,
                                     dv0 + (uint64_t)((vslot * C::SLOT + ks * 2048) >> 4), idesc_o,
                                     (j > 0 || ks > 0) ? 1u : 0u);
                     ptx::mma_commit(&o_done[t]);
@@ -587,7 +628,7 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
-    if (warp == 8) ptx::tmem_dealloc(tmem, C::TMEM_COLS);
+    if (warp == C::NSW) ptx::tmem_dealloc(tmem, C::TMEM_COLS);
 }
 
 // ============================================================================================
@@ -687,15 +728,20 @@ cudaError_t launch_v0(const PrefillArgs &a, const Maps &maps, int num_items, cud
     return cudaGetLastError();
 }
 
-template <int DQK, int DV>
+template <int DQK, int DV, int NT>
 cudaError_t launch_v1(const PrefillArgs &a, const Maps &maps, int num_items, int num_sms, cudaStream_t st) {
-    using C = V1Cfg<DQK, DV>;
-    auto kern = a.nsplit > 1 ? prefill_v1_kernel<DQK, DV, true> : prefill_v1_kernel<DQK, DV, false>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
-    if (e != cudaSuccess) return e;
-    const int grid = num_items < num_sms ? num_items : num_sms;
-    kern<<<grid, C::THREADS, C::SMEM, st>>>(a, maps, num_items);
-    return cudaGetLastError();
+    using C = V1Cfg<DQK, DV, NT>;
+    if constexpr (!C::FITS) {
+        return cudaErrorInvalidValue;
+    } else {
+        auto kern = a.nsplit > 1 ? prefill_v1_kernel<DQK, DV, true, NT> : prefill_v1_kernel<DQK, DV, false, NT>;
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
+        if (e != cudaSuccess) return e;
+        const int ctas = num_sms * C::CTAS_PER_SM;
+        const int grid = num_items < ctas ? num_items : ctas;
+        kern<<<grid, C::THREADS, C::SMEM, st>>>(a, maps, num_items);
+        return cudaGetLastError();
+    }
 }
 
 bool use_v0() {
@@ -738,14 +784,38 @@ cudaError_t prefill_encode_q_map(const void *q, int64_t total_q, int num_q_heads
 
 int prefill_max_splits() { return use_v0() ? 1 : 16; }
 
+// Q tiles per CTA for a call whose longest request has `max_q_tokens` query tokens: 1 (two CTAs per SM) when every
+// request fits one 128-row tile per kv-head and the shape's shared-memory budget allows it, else 2.
+int prefill_tiles_per_cta(int group, int dqk, int dv, int64_t max_q_tokens, int64_t num_items, int num_sms) {
+    if (use_v0() || max_q_tokens * group > kTileM) return 2;
+    static const bool off = [] { const char *e = getenv("COMB_PREFILL_NT"); return e && e[0] == '2'; }();
+    if (off) return 2;  // measurement hook: COMB_PREFILL_NT=2 keeps the two-tile kernel
+    // Two single-tile CTAs per SM only pay when CTAs really share SMs; a lone CTA is better off with the two-tile
+    // kernel's deeper K/V ring. The full-SM single-tile variant (Dqk = 192) has the deeper ring itself.
+#define COMB_NT1_CASE(DQ, DVV)                                              \
+    if (dqk == DQ && dv == DVV) {                                           \
+        using C1 = V1Cfg<DQ, DVV, 1>;                                       \
+        if (!C1::FITS) return 2;                                            \
+        return (!C1::HALF_SM || num_items > num_sms) ? 1 : 2;               \
+    }
+    COMB_NT1_CASE(128, 128)
+    COMB_NT1_CASE(64, 64)
+    COMB_NT1_CASE(192, 128)
+    COMB_NT1_CASE(128, 64)
+    COMB_NT1_CASE(64, 128)
+    COMB_NT1_CASE(192, 64)
+#undef COMB_NT1_CASE
+    return 2;
+}
+
 size_t prefill_partial_bytes(int nsplit, int64_t total_q, int num_q_heads, int dv) {
     return (size_t)nsplit * (size_t)total_q * (size_t)num_q_heads * (size_t)(dv + 1) * sizeof(float);
 }
 
 cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &pm,
                            const PrefillItem *items_dev, int num_items, int num_q_heads, float scale, void *out,
-                           float *lse, int nsplit, int64_t total_q, void *partials, int num_sms, cudaStream_t stream,
-                           int *launches) {
+                           float *lse, int nsplit, int64_t total_q, void *partials, int tiles_per_cta, int num_sms,
+                           cudaStream_t stream, int *launches) {
     PrefillArgs a;
     a.items = items_dev;
     a.page_indptr = lv.page_indptr;
@@ -772,7 +842,8 @@ cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, con
 #define COMB_PREFILL_CASE(DQ, DVV)                                                              \
     if (g.head_dim_qk == DQ && g.head_dim_v == DVV)                                             \
         e = use_v0() ? launch_v0<DQ, DVV>(a, maps, num_items, stream)                           \
-                     : launch_v1<DQ, DVV>(a, maps, num_items, num_sms, stream);
+            : tiles_per_cta == 1 ? launch_v1<DQ, DVV, 1>(a, maps, num_items, num_sms, stream)   \
+                                 : launch_v1<DQ, DVV, 2>(a, maps, num_items, num_sms, stream);
     COMB_PREFILL_CASE(128, 128)
     COMB_PREFILL_CASE(64, 64)
     COMB_PREFILL_CASE(192, 128)

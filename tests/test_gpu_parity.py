@@ -203,7 +203,7 @@ def test_prefill_kv_ranges_low_parallelism(shape):
     Hq, Hkv, Dqk, Dv = shape
     lens = [700, 333, 512, 129, 16, 1000, 47, 800]
     w = cs.custom("ranges", num_q_heads=Hq, num_kv_heads=Hkv, head_dim_qk=Dqk, head_dim_v=Dv, chunk_len=lens,
-                  links=[[0, 1, 2, 3, 5, 7, 6], [4], [], [5, 0, 7, 2, 1]], lq=[20, 7, 3, 33], seed=5)
+                  links=[[0, 1, 2, 3, 5, 7, 6], [4], [], [5, 0, 7, 2, 1]], lq=[20, 7, 3, 32], seed=5)
     for ww in (w, w.peaked()):
         ld = H().load_workload(ww, sentinel=SENTINEL, shuffle_seed=13)
         l0 = ld.pool.launches
