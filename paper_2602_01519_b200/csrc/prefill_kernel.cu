@@ -555,8 +555,11 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
                 load_tile(0, j, true);
             }
         }
-    } else if (warp == C::NSW + 1 && lane == 0) {
-        // ===================== MMA issuer (one thread) =====================
+    } else if (warp == C::NSW + 1) {
+        // ===================== MMA issuer =====================
+        // The whole warp runs the control flow (so descriptors and barrier addresses stay in uniform registers and
+        // no per-instruction waterfall loop is needed); one elected lane issues the tcgen05 instructions.
+        const bool leader = ptx::elect_one();
         constexpr uint32_t idesc_s = ptx::umma_idesc_bf16(kTileM, kTileN, false);
         constexpr uint32_t idesc_o = ptx::umma_idesc_bf16(kTileM, DV, true);
         // descriptors advance by adding (byte offset >> 4) to the 14-bit start-address field
@@ -569,7 +572,7 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
 #pragma unroll
             for (int kk = 0; kk < DQK / 16; ++kk) {
                 const uint64_t off = (uint64_t)(((kk / 4) * C::HALF + (kk % 4) * 32) >> 4);
-                ptx::mma_ss(tmem + t * 128, dq + off, dk + off, idesc_s, kk > 0);
+                if (leader) ptx::mma_ss(tmem + t * 128, dq + off, dk + off, idesc_s, kk > 0);
             }
         };
         for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
@@ -587,10 +590,10 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
                 ++qcnt[t];
                 ptx::tc_fence_after();
                 issue_s(t, kslot);
-                ptx::mma_commit(&s_full[t]);
-                if (n_kv == 1) ptx::mma_commit(&q_empty[t]);
+                if (leader) ptx::mma_commit(&s_full[t]);
+                if (n_kv == 1) if (leader) ptx::mma_commit(&q_empty[t]);
             }
-            ptx::mma_commit(&kv_empty[kslot]);
+            if (leader) ptx::mma_commit(&kv_empty[kslot]);
             for (int j = 0; j < n_kv; ++j) {
                 const int pages_here = min(kTilePages, npages - j * kTilePages);
                 const bool more = j + 1 < n_kv;
@@ -605,22 +608,22 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
                     ++pcnt[t];
                     ptx::tc_fence_after();
                     for (int ks = 0; ks < pages_here; ++ks)  // O_t += P_t V_j, one k-step of 16 keys per page
-                        ptx::mma_ts(tmem + 128 * NT + t * DV, tmem + t * 128 + ks * 8,
+                        if (leader) ptx::mma_ts(tmem + 128 * NT + t * DV, tmem + t * 128 + ks * 8,
                                     dv0 + (uint64_t)((vslot * C::SLOT + ks * 2048) >> 4), idesc_o,
                                     (j > 0 || ks > 0) ? 1u : 0u);
-                    ptx::mma_commit(&o_done[t]);
+                    if (leader) ptx::mma_commit(&o_done[t]);
                     if (more) {
                         if (t == 0) {
                             ptx::mbar_wait(&kv_full[kslot], kphase);
                             ptx::tc_fence_after();
                         }
                         issue_s(t, kslot);
-                        ptx::mma_commit(&s_full[t]);
-                        if (j + 2 == n_kv) ptx::mma_commit(&q_empty[t]);
+                        if (leader) ptx::mma_commit(&s_full[t]);
+                        if (j + 2 == n_kv) if (leader) ptx::mma_commit(&q_empty[t]);
                     }
                 }
-                ptx::mma_commit(&kv_empty[vslot]);
-                if (more) ptx::mma_commit(&kv_empty[kslot]);
+                if (leader) ptx::mma_commit(&kv_empty[vslot]);
+                if (more) if (leader) ptx::mma_commit(&kv_empty[kslot]);
             }
         }
     }

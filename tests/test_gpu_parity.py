@@ -195,6 +195,38 @@ def test_prefill_tiny_config():
     check_attention(out, lse, *oracle.attention_for(w.peaked()), tag="tiny prefill peaked")
 
 
+def test_layers_share_page_ids_but_not_data():
+    """L = 3 cross-attention layers over one page-id space (the paper interleaves 8 cross layers): a
+    chunk is stored once per layer with that layer's K/V, linked once, and every layer's prefill and decode read
+    their own arena slice."""
+    from dataclasses import replace
+    from paper_2602_01519_b200 import Pool
+    base = ragged_workload("layers", 8, 2, 128, 128, [9, 0, 2, 40], seed=3)
+    ws = [replace(base, seed=100 + l) for l in range(3)]  # same lengths and links, different K/V/Q values
+    pool = Pool(2, 128, 128, base.pool_pages, num_layers=3, shuffle_seed=21, sentinel=SENTINEL)
+    ids = list(range(base.num_chunks))
+    tok = np.zeros(base.num_chunks + 1, np.int32)
+    np.cumsum(base.chunk_len, out=tok[1:])
+    for l in (2, 0, 1):  # any layer order: the first store of a chunk allocates its page list
+        kv = [ws[l].chunk_kv(c) for c in ids]
+        pool.store_chunks(ids, tok, H().bits_to_device(np.concatenate([k for k, _ in kv]), "cuda"),
+                          H().bits_to_device(np.concatenate([v for _, v in kv]), "cuda"), layer=l)
+    assert pool.free_pages == 0
+    batch = pool.link([list(map(int, x)) for x in base.links])
+    for l in range(3):
+        q = H().bits_to_device(ws[l].all_q(), "cuda")
+        out, lse = pool.prefill(batch, q, base.q_indptr, base.scale, layer=l)
+        torch.cuda.synchronize()
+        check_attention(H().device_to_bits(out), lse.cpu().numpy().astype(np.float64), *oracle.attention_for(ws[l]),
+                        tag="prefill layer %d" % l)
+        wd = ws[l].decode_phase()
+        outd, lsed = pool.decode(batch, H().bits_to_device(wd.all_q(), "cuda"), wd.scale, layer=l)
+        torch.cuda.synchronize()
+        check_attention(H().device_to_bits(outd), lsed.cpu().numpy().astype(np.float64), *oracle.attention_for(wd),
+                        tag="decode layer %d" % l)
+    pool.close()
+
+
 @pytest.mark.parametrize("shape", [(32, 8, 128, 128), (16, 16, 192, 128), (8, 2, 64, 64)])
 def test_prefill_kv_ranges_low_parallelism(shape):
     """Few work items for 148 SMs (the paper's regime: < 50 dynamic tokens): every request's KV is cut
