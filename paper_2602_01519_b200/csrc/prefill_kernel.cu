@@ -334,9 +334,11 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
     unsigned char *sQ = smem;                    // [2 tiles][KH][128][64]
     unsigned char *sKV = smem + NT * C::Q_BYTES;  // ring of NSLOT tiles
     uint64_t *bars = reinterpret_cast<uint64_t *>(sKV + C::NSLOT * C::SLOT);
-    uint64_t *q_full = bars, *q_empty = bars + 2, *s_full = bars + 4, *p_full = bars + 6, *o_done = bars + 8;
-    uint64_t *kv_full = bars + 10, *kv_empty = bars + 10 + C::NSLOT;
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(bars + 10 + 2 * C::NSLOT);
+    // p_full is indexed [tile * 2 + half]: P goes to the tensor pipe in two 64-key halves, one barrier each (a parity
+    // wait cannot tell phase k from phase k - 2, so a barrier must never have two phases outstanding)
+    uint64_t *q_full = bars, *q_empty = bars + 2, *s_full = bars + 4, *p_full = bars + 6, *o_done = bars + 10;
+    uint64_t *kv_full = bars + 12, *kv_empty = bars + 12 + C::NSLOT;
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(bars + 12 + 2 * C::NSLOT);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
@@ -344,7 +346,8 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
             ptx::mbar_init(&q_full[t], 1);
             ptx::mbar_init(&q_empty[t], 1);
             ptx::mbar_init(&s_full[t], 1);
-            ptx::mbar_init(&p_full[t], 128);
+            ptx::mbar_init(&p_full[t * 2], 128);
+            ptx::mbar_init(&p_full[t * 2 + 1], 128);
             ptx::mbar_init(&o_done[t], 1);
         }
         for (int s = 0; s < C::NSLOT; ++s) {
@@ -449,19 +452,23 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
                 const float2 neg2 = make_float2(neg, neg);
                 float2 sum4[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
 #pragma unroll
-                for (int e = 0; e < kTileN; e += 2) {
-                    const float2 x = ptx::ffma2(make_float2(__uint_as_float(r[e]), __uint_as_float(r[e + 1])), c2, neg2);
-                    const float p0 = ptx::ex2(x.x), p1 = ptx::ex2(x.y);
-                    sum4[(e >> 1) & 3] = ptx::fadd2(sum4[(e >> 1) & 3], make_float2(p0, p1));
-                    r[e >> 1] = ptx::pack_bf16x2(p0, p1);
+                for (int half = 0; half < 2; ++half) {
+                    // P (bf16, written over S columns this thread has already consumed) is handed over in two 64-key
+                    // halves: the tensor pipe runs the first half of P V under the second half's exponentials
+#pragma unroll
+                    for (int e = half * 64; e < half * 64 + 64; e += 2) {
+                        const float2 x = ptx::ffma2(make_float2(__uint_as_float(r[e]), __uint_as_float(r[e + 1])), c2, neg2);
+                        const float p0 = ptx::ex2(x.x), p1 = ptx::ex2(x.y);
+                        sum4[(e >> 1) & 3] = ptx::fadd2(sum4[(e >> 1) & 3], make_float2(p0, p1));
+                        r[e >> 1] = ptx::pack_bf16x2(p0, p1);
+                    }
+                    ptx::tmem_st32(tS + half * 32, *reinterpret_cast<uint32_t(*)[32]>(&r[half * 32]));
+                    ptx::tmem_wait_st();
+                    ptx::tc_fence_before();
+                    ptx::mbar_arrive(&p_full[t * 2 + half]);
                 }
                 const float2 sA = ptx::fadd2(sum4[0], sum4[1]), sB = ptx::fadd2(sum4[2], sum4[3]);
                 l_run += (sA.x + sA.y) + (sB.x + sB.y);
-                ptx::tmem_st32(tS, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
-                ptx::tmem_st32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[32]));
-                ptx::tmem_wait_st();
-                ptx::tc_fence_before();
-                ptx::mbar_arrive(&p_full[t]);
             }
             // ---- epilogue: O / l -> bf16 ----
             ptx::mbar_wait(&o_done[t], (o_cnt + n_kv - 1) & 1);
@@ -604,13 +611,16 @@ prefill_v1_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const 
                 kslot = slot;
                 if (more && ++slot == C::NSLOT) { slot = 0; phase ^= 1; }
                 for (int t = 0; t < nq; ++t) {
-                    ptx::mbar_wait(&p_full[t], pcnt[t] & 1);
+#pragma unroll
+                    for (int half = 0; half < 2; ++half) {  // O_t += P_t V_j, one k-step of 16 keys per page
+                        ptx::mbar_wait(&p_full[t * 2 + half], pcnt[t] & 1);
+                        ptx::tc_fence_after();
+                        for (int ks = half * 4; ks < min(pages_here, half * 4 + 4); ++ks)
+                            if (leader) ptx::mma_ts(tmem + 128 * NT + t * DV, tmem + t * 128 + ks * 8,
+                                                    dv0 + (uint64_t)((vslot * C::SLOT + ks * 2048) >> 4), idesc_o,
+                                                    (j > 0 || ks > 0) ? 1u : 0u);
+                    }
                     ++pcnt[t];
-                    ptx::tc_fence_after();
-                    for (int ks = 0; ks < pages_here; ++ks)  // O_t += P_t V_j, one k-step of 16 keys per page
-                        if (leader) ptx::mma_ts(tmem + 128 * NT + t * DV, tmem + t * 128 + ks * 8,
-                                    dv0 + (uint64_t)((vslot * C::SLOT + ks * 2048) >> 4), idesc_o,
-                                    (j > 0 || ks > 0) ? 1u : 0u);
                     if (leader) ptx::mma_commit(&o_done[t]);
                     if (more) {
                         if (t == 0) {
