@@ -446,11 +446,13 @@ int32_t comb_link_plan(const comb_pool_t *p, int32_t R, const int32_t *chunk_ind
     // pass 1: lookups + sizes (nothing is written if any id is unknown)
     int64_t total_pages = 0, total_tiles = 0, total_tok = 0;
     int32_t max_pages = 0;
+    std::vector<const Chunk *> found((size_t)chunk_indptr[R]);  // one directory lookup per linked chunk
     for (int32_t r = 0; r < R; ++r) {
         int64_t pr = 0;
         for (int32_t e = chunk_indptr[r]; e < chunk_indptr[r + 1]; ++e) {
             auto it = p->dir.find(chunk_ids[e]);
             if (it == p->dir.end()) return COMB_ERR_UNKNOWN_CHUNK;
+            found[(size_t)e] = &it->second;
             pr += (int64_t)it->second.pages.size();
             total_tok += it->second.num_tokens;
         }
@@ -477,20 +479,20 @@ int32_t comb_link_plan(const comb_pool_t *p, int32_t R, const int32_t *chunk_ind
         const int64_t begin = at;
         int64_t kv = 0;
         for (int32_t e = chunk_indptr[r]; e < chunk_indptr[r + 1]; ++e) {
-            const Chunk &c = p->dir.find(chunk_ids[e])->second;
+            const Chunk &c = *found[(size_t)e];
             const int32_t np = (int32_t)c.pages.size();
-            for (int32_t j = 0; j < np; ++j) {
-                page_ids[at] = c.pages[j];
-                page_ntok[at] = (j + 1 < np) ? kPage : c.num_tokens - kPage * (np - 1);
-                ++at;
-            }
+            memcpy(page_ids + at, c.pages.data(), (size_t)np * sizeof(int32_t));
+            std::fill(page_ntok + at, page_ntok + at + np, (int32_t)kPage);
+            page_ntok[at + np - 1] = c.num_tokens - kPage * (np - 1);  // the chunk's last page may be partly filled
+            at += np;
             kv += c.num_tokens;
         }
         kv_len[r] = (int32_t)kv;
         page_indptr[r + 1] = (int32_t)at;
         for (int64_t t = begin; t < at; t += kTilePages) {
             uint64_t packed = 0;
-            for (int j = 0; j < kTilePages && t + j < at; ++j) packed |= (uint64_t)page_ntok[t + j] << (8 * j);
+            const int lim = (int)std::min<int64_t>(kTilePages, at - t);
+            for (int j = 0; j < lim; ++j) packed |= (uint64_t)page_ntok[t + j] << (8 * j);
             tile_ntok[tile_at++] = packed;
         }
         tile_indptr[r + 1] = (int32_t)tile_at;
