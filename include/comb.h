@@ -162,7 +162,12 @@ int32_t comb_link_plan(const comb_pool_t *pool, int32_t num_requests, const int3
  *             finite positive number (INVALID otherwise)
  *   workspace device, comb_workspace_bytes() bytes, 16-byte aligned
  * q-head h reads kv-head h / (Hq/Hkv). kv_len == 0 gives out = 0, lse = -inf. tcgen05/TMEM/TMA kernel.
- * Errors: INVALID, CAPACITY, CUDA. */
+ * When the call has fewer work items than the GPU has SMs (few requests with few query tokens — the paper's
+ * regime) and `link` was produced by comb_link of this pool, every request's KV is cut into ranges
+ * that run on different SMs; their fp32 partial rows live in `workspace` and a second kernel merges them by LSE.
+ * The result is the same function; only fp32 summation order differs.
+ * Errors: INVALID, CAPACITY (workspace smaller than comb_workspace_bytes() for this shape, or not 16-byte
+ * aligned), CUDA. */
 int32_t comb_cross_attn_prefill(comb_pool_t *pool, int32_t layer, const comb_link_t *link, int32_t num_requests,
                                 const void *q, const int32_t *q_indptr, int32_t num_q_heads, float scale, void *out,
                                 float *lse, void *workspace, size_t workspace_bytes, void *stream);
@@ -176,7 +181,8 @@ int32_t comb_cross_attn_decode(comb_pool_t *pool, int32_t layer, const comb_link
                                void *workspace, size_t workspace_bytes, void *stream);
 
 /* Workspace that suffices for either attention call: num_requests requests, num_q_heads heads, total_q
- * query rows, max_pages_per_request table entries in the longest request. */
+ * query rows, max_pages_per_request table entries in the longest request (pass comb_link_t.max_pages_per_request).
+ * Holds the decode split partials, or the prefill work-item list plus the partial rows of its KV ranges. */
 size_t comb_workspace_bytes(const comb_pool_t *pool, int32_t num_requests, int32_t num_q_heads, int64_t total_q,
                             int32_t max_pages_per_request);
 
