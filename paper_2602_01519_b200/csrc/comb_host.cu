@@ -565,6 +565,7 @@ size_t comb_workspace_bytes(const comb_pool_t *p, int32_t R, int32_t Hq, int64_t
     int nsplit = 1;
     for (size_t n = std::max<size_t>(items_lo, 1); n <= items_hi; n += (size_t)p->cfg.num_kv_heads)
         nsplit = std::max(nsplit, plan_prefill_splits(n, max_tiles, p->num_sms, prefill_max_splits()));
+    if (prefill_max_splits() > 1 && max_tiles >= 4) nsplit = std::max(nsplit, 4);  // last-wave ranges (up to 4)
     const size_t pre = align_up(items_hi * (size_t)nsplit * sizeof(PrefillItem), 256) +
                        (nsplit > 1 ? prefill_partial_bytes(nsplit, total_q, Hq, p->cfg.head_dim_v) : 0);
     return align_up(std::max(dec, pre), 256) + 256;
@@ -622,34 +623,70 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     const int tiles_per_cta = prefill_tiles_per_cta(G, p->cfg.head_dim_qk, p->cfg.head_dim_v, max_lq, nonempty * Hkv,
                                                     p->num_sms);
     const int tok_per_tile = 128 / G, tok_per_item = tiles_per_cta * tok_per_tile;
-    struct Req { int32_t r; int64_t cost; };
+    // ---- work items: (request, kv-head, one or two Q tiles) against the request's KV, or against a range of it.
+    // Requests are ordered by work (query rows x KV tiles when the link's page counts are known on the host, i.e.
+    // the link came from comb_link of this pool; else query rows) so the tail of the persistent grid is made of
+    // short items; the kv-heads of one Q tile group sit together so CTAs that stream the same K/V run at the same
+    // time (L2 reuse).
+    auto tiles_of = [&](int32_t r) {
+        return req_pages ? ((*req_pages)[(size_t)r] + kTilePages - 1) / kTilePages : 1;
+    };
+    struct Req { int32_t r; int64_t rows, cost; };
     std::vector<Req> order;
     order.reserve(R);
-    // kv length is known on the host only through the link summary per request? use the table sizes:
-    // page_indptr lives on the device, so order by lq (rows) only when lengths are unknown. The link call
-    // kept no per-request host copy, therefore sort by query rows (stable) — equal-length links (all
-    // BASELINE configs) make this the same as longest-first.
-    for (int32_t r = 0; r < R; ++r) order.push_back(Req{r, (int64_t)q_indptr[r + 1] - q_indptr[r]});
-    std::stable_sort(order.begin(), order.end(), [](const Req &a, const Req &b) { return a.cost > b.cost; });
-    size_t base_items = 0;
-    for (const Req &x : order) base_items += (size_t)((x.cost + tok_per_item - 1) / tok_per_item) * Hkv;
-    if (base_items == 0) return COMB_OK;
-    p->probe_device();
-    // ---- KV ranges: only when the link's per-request page counts are known on the host (comb_link of this pool)
-    const int max_tiles = (link->max_pages_per_request + kTilePages - 1) / kTilePages;
-    // (one item per SM is the target even when two single-tile CTAs share an SM: measured, 256 ranges on 148 SMs
-    // were slower than 128)
-    const int nsplit = req_pages ? plan_prefill_splits(base_items, max_tiles, p->num_sms, prefill_max_splits()) : 1;
-    size_t num_items = 0;
-    for (const Req &x : order) {
-        int eff = 1;
-        if (nsplit > 1) {
-            const int n_kv = ((*req_pages)[(size_t)x.r] + kTilePages - 1) / kTilePages;
-            const int tps = prefill_tiles_per_split(n_kv, nsplit);
-            eff = tps > 0 ? (n_kv + tps - 1) / tps : 1;
-        }
-        num_items += (size_t)((x.cost + tok_per_item - 1) / tok_per_item) * Hkv * (size_t)eff;
+    for (int32_t r = 0; r < R; ++r) {
+        const int64_t rows = (int64_t)q_indptr[r + 1] - q_indptr[r];
+        order.push_back(Req{r, rows, rows * std::max(1, tiles_of(r))});
     }
+    std::stable_sort(order.begin(), order.end(), [](const Req &a, const Req &b) { return a.cost > b.cost; });
+    std::vector<PrefillItem> base;
+    for (const Req &x : order)
+        for (int64_t t = 0; t < x.rows; t += tok_per_item)
+            for (int g = 0; g < Hkv; ++g)
+                base.push_back(PrefillItem{x.r, g, q_indptr[x.r] + (int32_t)t,
+                                           (int32_t)std::min<int64_t>(tok_per_item, x.rows - t), 0,
+                                           INT32_MAX / kTilePages, -1, 0});
+    if (base.empty()) return COMB_OK;
+    // ---- KV ranges (need the page counts): (1) fewer items than SMs: every request is cut so that items x ranges
+    // fill one wave; (2) several waves with a last wave at most half full: only the items of that last wave are cut
+    // (by up to 4), so it takes a fraction of an item's time instead of a whole one (cfg 4: 512 items on 148 SMs).
+    const int max_tiles = (link->max_pages_per_request + kTilePages - 1) / kTilePages;
+    const size_t ctas = (size_t)p->num_sms * (size_t)prefill_ctas_per_sm(tiles_per_cta, p->cfg.head_dim_qk,
+                                                                          p->cfg.head_dim_v);
+    int uniform = 1, tail_factor = 1;
+    size_t tail_from = base.size();
+    if (req_pages) {
+        // (one item per SM is the target even when two single-tile CTAs share an SM: measured, 256 ranges on 148
+        // SMs were slower than 128)
+        uniform = plan_prefill_splits(base.size(), max_tiles, p->num_sms, prefill_max_splits());
+        const size_t tail = base.size() % ctas;
+        if (uniform == 1 && base.size() > ctas && tail > 0 && 2 * tail <= ctas && prefill_max_splits() > 1) {
+            tail_factor = (int)std::min<size_t>(4, ctas / tail);
+            tail_from = base.size() - tail;
+        }
+    }
+    std::vector<PrefillItem> items;
+    items.reserve(base.size() * (size_t)std::max(uniform, 1) + (base.size() - tail_from) * (size_t)tail_factor);
+    int nsplit = 1;
+    for (size_t i = 0; i < base.size(); ++i) {
+        const int want = i >= tail_from ? tail_factor : uniform;
+        const int n_kv = want > 1 ? tiles_of(base[i].request) : 0;
+        const int tps = want > 1 ? std::max(2, prefill_tiles_per_split(n_kv, want)) : 0;  // >= 2 tiles per range
+        const int eff = tps > 0 ? (n_kv + tps - 1) / tps : 1;
+        if (eff <= 1) {
+            items.push_back(base[i]);
+            continue;
+        }
+        nsplit = std::max(nsplit, eff);
+        for (int sidx = 0; sidx < eff; ++sidx) {
+            PrefillItem it = base[i];
+            it.kv_tile0 = sidx * tps;
+            it.kv_tiles = tps;
+            it.split = sidx;
+            items.push_back(it);
+        }
+    }
+    const size_t num_items = items.size();
     if (num_items > (size_t)INT32_MAX) return COMB_ERR_CAPACITY;
     const size_t items_bytes = align_up(num_items * sizeof(PrefillItem), 256);
     const size_t part_bytes = nsplit > 1 ? prefill_partial_bytes(nsplit, total_q, Hq, p->cfg.head_dim_v) : 0;
@@ -667,24 +704,7 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     const int slot = p->acquire(num_items * sizeof(PrefillItem));
     if (slot < 0) return COMB_ERR_CUDA;
     PrefillItem *h = (PrefillItem *)p->ring[slot].host;
-    size_t at = 0;
-    for (const Req &x : order) {
-        const int32_t row0 = q_indptr[x.r];
-        int n_kv = 0, tps = INT32_MAX / kTilePages, eff = 1;
-        if (nsplit > 1) {
-            n_kv = ((*req_pages)[(size_t)x.r] + kTilePages - 1) / kTilePages;
-            tps = prefill_tiles_per_split(n_kv, nsplit);
-            eff = tps > 0 ? (n_kv + tps - 1) / tps : 1;
-            if (eff <= 1) tps = INT32_MAX / kTilePages;
-        }
-        // the ranges of one (Q tile pair, kv-head) sit together, then the kv-heads: CTAs that stream the same K/V
-        // run at the same time (L2 reuse)
-        for (int64_t t = 0; t < x.cost; t += tok_per_item)
-            for (int g = 0; g < Hkv; ++g)
-                for (int sidx = 0; sidx < eff; ++sidx)
-                    h[at++] = PrefillItem{x.r, g, row0 + (int32_t)t, (int32_t)std::min<int64_t>(tok_per_item, x.cost - t),
-                                          eff > 1 ? sidx * tps : 0, tps, eff > 1 ? sidx : -1, 0};
-    }
+    memcpy(h, items.data(), num_items * sizeof(PrefillItem));
     if (cudaMemcpyAsync(ws, h, num_items * sizeof(PrefillItem), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return COMB_ERR_CUDA;
     if (p->prof_on) p->hook.begin(p, kKernelPrefill, st);

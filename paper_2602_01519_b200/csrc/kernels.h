@@ -75,6 +75,7 @@ int prefill_max_splits();  // 1 when the selected kernel cannot split (debug ker
 // Q tiles per CTA (1 or 2) for a call whose longest request has max_q_tokens query tokens and that would have
 // num_items single-tile items; an item then covers up to that many 128-row tiles.
 int prefill_tiles_per_cta(int group, int dqk, int dv, int64_t max_q_tokens, int64_t num_items, int num_sms);
+int prefill_ctas_per_sm(int tiles_per_cta, int dqk, int dv);  // resident CTAs per SM of the kernel that choice selects
 size_t prefill_partial_bytes(int nsplit, int64_t total_q, int num_q_heads, int dv);
 bool prefill_supported(int group, int dqk, int dv);
 // CUtensorMap is 128 bytes, 64-byte aligned; kept opaque here so the runtime needs no cuda.h.

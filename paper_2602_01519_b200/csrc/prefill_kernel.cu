@@ -821,6 +821,20 @@ int prefill_tiles_per_cta(int group, int dqk, int dv, int64_t max_q_tokens, int6
     return 2;
 }
 
+int prefill_ctas_per_sm(int tiles_per_cta, int dqk, int dv) {
+    if (tiles_per_cta != 1) return 1;
+#define COMB_CPS_CASE(DQ, DVV) \
+    if (dqk == DQ && dv == DVV) return V1Cfg<DQ, DVV, 1>::CTAS_PER_SM;
+    COMB_CPS_CASE(128, 128)
+    COMB_CPS_CASE(64, 64)
+    COMB_CPS_CASE(192, 128)
+    COMB_CPS_CASE(128, 64)
+    COMB_CPS_CASE(64, 128)
+    COMB_CPS_CASE(192, 64)
+#undef COMB_CPS_CASE
+    return 1;
+}
+
 size_t prefill_partial_bytes(int nsplit, int64_t total_q, int num_q_heads, int dv) {
     return (size_t)nsplit * (size_t)total_q * (size_t)num_q_heads * (size_t)(dv + 1) * sizeof(float);
 }
