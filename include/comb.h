@@ -150,7 +150,9 @@ size_t comb_link_bytes(int32_t num_requests, int64_t total_pages);
 int32_t comb_link(comb_pool_t *pool, int32_t num_requests, const int32_t *chunk_indptr /* host [R+1] */,
                   const uint64_t *chunk_ids /* host, link order */, comb_link_t *link, void *stream);
 /* Same tables written into HOST memory `host_buf` (link->device_bytes bytes available); the pointers in
- * `link` are laid out as if host_buf were device_buf. No CUDA call — used by comb_link and by host tests. */
+ * `link` are laid out as if host_buf were device_buf. No CUDA call — used by comb_link and by host tests.
+ * Also notes, inside the pool and keyed by link->device_buf, how many pages every request links (the prefill
+ * planner's KV ranges need it; the directory and the free list are not touched). */
 int32_t comb_link_plan(const comb_pool_t *pool, int32_t num_requests, const int32_t *chunk_indptr,
                        const uint64_t *chunk_ids, comb_link_t *link, void *host_buf);
 

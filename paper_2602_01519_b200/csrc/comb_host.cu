@@ -510,6 +510,24 @@ int32_t comb_link_plan(const comb_pool_t *p, int32_t R, const int32_t *chunk_ind
     link->total_tiles = total_tiles;
     link->total_kv_tokens = total_tok;
     link->bytes_used = L.bytes;
+    {   // remember the page count of every request of this link (host side of page_indptr), keyed by its device buffer
+        comb_pool_t *pm = const_cast<comb_pool_t *>(p);  // bookkeeping only: the directory and free list are untouched
+        comb_pool::LinkInfo *li = nullptr;
+        for (comb_pool::LinkInfo &x : pm->link_info)
+            if (x.device_buf == link->device_buf) li = &x;
+        if (!li) {
+            if (pm->link_info.size() < kLinkInfoSlots) {
+                pm->link_info.emplace_back();
+                li = &pm->link_info.back();
+            } else {
+                li = &pm->link_info[pm->link_info_next];
+                pm->link_info_next = (pm->link_info_next + 1) % kLinkInfoSlots;
+            }
+            li->device_buf = link->device_buf;
+        }
+        li->pages.resize((size_t)R);
+        for (int32_t r = 0; r < R; ++r) li->pages[(size_t)r] = page_indptr[r + 1] - page_indptr[r];
+    }
     return COMB_OK;
 }
 
@@ -521,25 +539,6 @@ int32_t comb_link(comb_pool_t *p, int32_t R, const int32_t *chunk_indptr, const 
     if (slot < 0) return COMB_ERR_CUDA;
     int32_t rc = comb_link_plan(p, R, chunk_indptr, chunk_ids, link, p->ring[slot].host);
     if (rc != COMB_OK) return rc;
-    {   // remember the page count of every request of this link (host side of page_indptr)
-        const int32_t *pi = (const int32_t *)((const char *)p->ring[slot].host +
-                                              ((const char *)link->page_indptr - (const char *)link->device_buf));
-        comb_pool::LinkInfo *li = nullptr;
-        for (comb_pool::LinkInfo &x : p->link_info)
-            if (x.device_buf == link->device_buf) li = &x;
-        if (!li) {
-            if (p->link_info.size() < kLinkInfoSlots) {
-                p->link_info.emplace_back();
-                li = &p->link_info.back();
-            } else {
-                li = &p->link_info[p->link_info_next];
-                p->link_info_next = (p->link_info_next + 1) % kLinkInfoSlots;
-            }
-            li->device_buf = link->device_buf;
-        }
-        li->pages.resize((size_t)R);
-        for (int32_t r = 0; r < R; ++r) li->pages[(size_t)r] = pi[r + 1] - pi[r];
-    }
     cudaStream_t st = (cudaStream_t)stream;
     // the ONLY data movement of the link stage: the tables. K/V are never touched.
     if (cudaMemcpyAsync(link->device_buf, p->ring[slot].host, link->bytes_used, cudaMemcpyHostToDevice, st) !=

@@ -174,3 +174,46 @@ def test_product_does_not_import_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle\b", src, flags=re.M), f
                 assert "comb_oracle" not in src and "_work/" not in src, f
+
+
+def test_workspace_bound_covers_every_prefill_plan():
+    """comb_workspace_bytes() must suffice for whatever the prefill planner decides (KV ranges for sub-wave calls,
+    last-wave ranges, one or two Q tiles per CTA). Without a GPU the calls below stop at their first CUDA call
+    (COMB_ERR_CUDA) — but only after the capacity check, so COMB_ERR_CAPACITY here means the bound is too small."""
+    rng = np.random.default_rng(123)
+    shapes = [(32, 8, 128, 128), (16, 16, 192, 128), (8, 2, 64, 64), (8, 8, 128, 64)]
+    for trial in range(60):
+        Hq, Hkv, Dqk, Dv = shapes[trial % len(shapes)]
+        n_chunks = int(rng.integers(1, 40))
+        lens = rng.integers(1, 1200, size=n_chunks)
+        pages = int(((lens + 15) // 16).sum())
+        pool = make_pool(num_pages=pages, Hkv=Hkv, Dqk=Dqk, Dv=Dv, seed=trial)
+        for c in range(n_chunks):
+            comb.comb_chunk_alloc(pool, c, int(lens[c]))
+        R = int(rng.integers(1, 48))
+        lists = [list(rng.choice(n_chunks, size=int(rng.integers(0, min(n_chunks, 12) + 1)), replace=False))
+                 for _ in range(R)]
+        lq = rng.choice([0, 1, 7, 32, 33, 64, 128, 129, 300, 512], size=R)
+        q_indptr = np.zeros(R + 1, np.int32)
+        np.cumsum(lq, out=q_indptr[1:])
+        indptr = np.zeros(R + 1, np.int32)
+        np.cumsum([len(x) for x in lists], out=indptr[1:])
+        ids = np.array([c for l in lists for c in l], np.uint64)
+        total_pages = int(sum(((lens[c] + 15) // 16) for l in lists for c in l))
+        link = comb.Link()
+        link.device_buf = 0x7300_0000_0000
+        link.device_bytes = comb.comb_link_bytes(R, total_pages)
+        host = np.zeros(link.device_bytes, np.uint8)
+        comb.comb_link_plan(pool, indptr, ids, link, host)  # the host half of comb_link (tables + page counts)
+        total_q = int(q_indptr[-1])
+        ws_bytes = comb.comb_workspace_bytes(pool, R, Hq, total_q, int(link.max_pages_per_request))
+        st = _lib.lib.comb_cross_attn_prefill(pool, 0, C.byref(link), R, 0x7400_0000_0000, q_indptr.ctypes.data, Hq,
+                                              C.c_float(0.1), 0x7500_0000_0000, None, 0x7600_0000_0000, ws_bytes, None)
+        assert st != comb.COMB_ERR_CAPACITY, "trial %d: workspace bound %d too small" % (trial, ws_bytes)
+        assert st in (comb.COMB_OK, comb.COMB_ERR_CUDA)
+        if total_q > 0:  # and the check is really reached: a 16-byte workspace is refused
+            st = _lib.lib.comb_cross_attn_prefill(pool, 0, C.byref(link), R, 0x7400_0000_0000, q_indptr.ctypes.data,
+                                                  Hq, C.c_float(0.1), 0x7500_0000_0000, None, 0x7600_0000_0000, 16,
+                                                  None)
+            assert st == comb.COMB_ERR_CAPACITY
+        comb.comb_pool_destroy(pool)
