@@ -404,12 +404,25 @@ DecodePlan make_decode_plan(int R, int Hkv, int max_pages, int num_sms) {
         p.num_splits = 1;
         return p;
     }
-    // aim for >= 4 waves of 2 CTAs per SM, but never fewer than 16 pages (4 per warp) per split
+    // aim for ~4 waves of 2 CTAs per SM, but never fewer than 16 pages (4 per warp) per split; around that target
+    // take the split count whose CTA total fills its last wave best (8 requests x 8 kv-heads x 19 splits would run
+    // 4.1 waves, x 18 splits 3.9)
     const long units = (long)R * Hkv;
-    const long target = (long)num_sms * 2 * 4;
-    long nsplit = (target + units - 1) / units;
-    nsplit = std::max(1L, std::min(nsplit, (long)(max_pages + 15) / 16));
-    int chunk = (int)((max_pages + nsplit - 1) / nsplit);
+    const long wave = (long)num_sms * 2;
+    const long target = wave * 4;
+    const long cap = std::max(1L, (long)(max_pages + 15) / 16);
+    const long ns0 = std::max(1L, std::min((target + units - 1) / units, cap));
+    long best = ns0;
+    double best_eff = 0.0;
+    for (long ns = std::max(1L, ns0 - ns0 / 4); ns <= std::min(cap, ns0 + ns0 / 4); ++ns) {
+        int chunk = (int)((max_pages + ns - 1) / ns);
+        chunk = (chunk + kWarps - 1) / kWarps * kWarps;
+        const long eff_ns = (max_pages + chunk - 1) / chunk;  // splits the longest request really gets
+        const long ctas = units * eff_ns;
+        const double eff = (double)ctas / (double)((ctas + wave - 1) / wave * wave);
+        if (eff > best_eff + 1e-9) { best_eff = eff; best = ns; }
+    }
+    int chunk = (int)((max_pages + best - 1) / best);
     chunk = (chunk + kWarps - 1) / kWarps * kWarps;
     p.chunk_pages = chunk;
     p.num_splits = (max_pages + chunk - 1) / chunk;
