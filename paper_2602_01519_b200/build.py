@@ -43,7 +43,7 @@ def _compile(src: str, verbose: bool) -> str:
     obj = os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
     path = os.path.join(CSRC, src)
     if _stale(obj, [path] + HEADERS):
-        extra = os.environ.get("COMB_NVCC_EXTRA", "").split()  # tuning hook, e.g. -DCOMB_PREFILL_TUNE
+        extra = os.environ.get("COMB_NVCC_EXTRA", "").split()  # extra nvcc flags for experiments (e.g. -DNAME=value)
         cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", path, "-o", obj]
         p = subprocess.run(cmd, capture_output=True, text=True)
         if p.returncode != 0:
