@@ -251,9 +251,11 @@ def main():
     primary_prefill = args.workload == "rag_prefill"
 
     # ------------------------------------------------------------------ attention benches
-    def bench_attention(w, phase, steps, warmup, *, fill, flush_l2=False, with_link=True, e2e=True):
+    def bench_attention(w, phase, steps, warmup, *, fill, flush_l2=False, with_link=True, e2e=True, shuffle=None):
         """Returns a dict of timings for `steps` passes of (link +) attention on workload w."""
-        ld = harness.load_workload(w, fill=fill, shuffle_seed=2024 + rank, keep_host=False)
+        # free list: permuted (a chunk's pages scattered over the arena, as in a long-running server) unless told
+        ld = harness.load_workload(w, fill=fill, shuffle_seed=(2024 + rank) if shuffle is None else shuffle,
+                                   keep_host=False)
         pool = ld.pool
         if phase == "decode":
             wq = w.decode_phase() if int(w.lq.max()) > 1 else w
@@ -426,8 +428,8 @@ def main():
                             "l2": L2Flush.HOW if flush else "inputs larger than L2"}
             log(name, json.dumps(extras[name]))
 
-        def decode_extra(name, wk, steps, fill, flush=False):
-            rr = bench_attention(wk, "decode", steps, 3, fill=fill, flush_l2=flush, e2e=False)
+        def decode_extra(name, wk, steps, fill, flush=False, shuffle=None):
+            rr = bench_attention(wk, "decode", steps, 3, fill=fill, flush_l2=flush, e2e=False, shuffle=shuffle)
             extras[name] = {"workload": name, "ms_per_step": rr["ms_per_step"], "kernel_ms": rr["kernel_ms"],
                             "merge_ms": rr["merge_ms"],
                             "gbs_logical": rr["kv_bytes"] / (rr["ms_per_step"] * 1e-3) / 1e9,
@@ -440,6 +442,8 @@ def main():
                 prefill_extra("rag_prefill", cs.rag_prefill(seed=args.seed), 20, "linked")
             else:
                 decode_extra("decode_link", cs.decode_link(seed=args.seed), 100, "linked")
+            if not primary_prefill:  # the same primary workload with an ascending free list (contiguous chunks)
+                decode_extra("decode_link_contiguous_pages", cs.decode_link(seed=args.seed), 100, "linked", shuffle=0)
             prefill_extra("rag_prefill_lq32", cs.rag_prefill(seed=args.seed, lq=32), 20, "linked")
             # the paper's own regime (< 50 dynamic tokens) at a small batch: 32 work items for 148 SMs,
             # so each request's KV is cut into ranges that run on different SMs and are merged by LSE
