@@ -5,13 +5,18 @@
 
 A *step* is one pass of the hot path over one batch of BASELINE.json configs[1] ("decode link": Llama-3-8B-
 shaped layer, 128 requests x 1 query token, each linking 8 chunks of 512 tokens drawn Zipf(1.1) from a
-2000-chunk pool): comb_link (block tables from the ordered chunk ids, one H2D copy, no KV copy) followed by
-comb_cross_attn_decode (split-KV kernel + LSE-merge kernel) over the resident chunk-KV pool.  `value` is the
-logical KV bytes the step attends over divided by the device time (CUDA events, max over ranks).  The chunk pool
-itself was stored before the timed region (compile stage); the paged-store kernel, the tcgen05
-prefill kernel (configs[2] "RAG prefill", TFLOP/s against the tensor roofline) and configs[3]/[4] are timed in
-the same run and reported under "extras".  N > 1: independent replicas, one per GPU, no collective on the data
-path -> weak scaling.
+2000-chunk pool): comb_link (block tables + the chunk-major inversion from the ordered chunk ids, one H2D copy, no
+KV copy) followed by comb_cross_attn_decode over the resident chunk-KV pool.  The library's default policy sends
+this batch down the chunk-major path (every distinct chunk streamed once through the tcgen05 kernel, per-request LSE
+merge); the per-request split-KV path on the same batch is timed beside it.  `value` is the LOGICAL KV bytes the step
+attends over (every request counts its own 8 chunks — the user-visible rate) divided by the device time (CUDA
+events, max over ranks).  `roofline` is about DRAM: its `achieved` divides the bytes that must cross the HBM pins
+(each distinct chunk once + Q, O, partial rows) by the dominant kernel's time; `achieved_logical` and the ncu-measured
+`traffic` stand beside it.  The chunk pool itself was stored before the timed region (compile stage).
+configs[2] "RAG prefill" (the metric's prefill half, TFLOP/s against the tensor roofline) is timed in the same run and
+reported under the top-level key "prefill"; the other configs, the store, the link and a read-only HBM stream ceiling
+are under "extras"; a compact table of all of them ends stderr.  N > 1: independent replicas, one per GPU, no
+collective on the data path -> weak scaling.
 
 `--impl reference` times the fp64 CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
 """
@@ -36,8 +41,9 @@ NOMINAL_HBM_GBS = 8000.0
 NOMINAL_BF16_TFLOPS = 2250.0
 FALLBACK_HBM_GBS = 6650.0
 FALLBACK_BF16_TFLOPS = 1590.0
-METRIC = ("decode cross-attn HBM GB/s over block-table-linked chunk KV (BASELINE metric: cross-attn TFLOP/s "
-          "(prefill) and HBM GB/s (decode) at 1 B200 vs roofline; prefill TFLOP/s is under extras.rag_prefill)")
+METRIC = ("decode cross-attn GB/s of linked chunk KV attended per second (logical bytes; BASELINE metric: cross-attn "
+          "TFLOP/s (prefill) and HBM GB/s (decode) at 1 B200 vs roofline; the DRAM-byte roofline is under `roofline`, "
+          "the prefill half under `prefill`)")
 
 
 def log(*a):
@@ -55,7 +61,7 @@ def peaks():
 
 def ncu_traffic(kernel: str, workload: str):
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of `kernel` on `workload` from the
-    committed ncu --set full capture (profiles/ncu_traffic.csv), or None when that pair was not captured."""
+    committed ncu --set full captures (profiles/ncu_traffic.csv), or None when that pair was not captured."""
     p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     if not os.path.exists(p):
         return None
@@ -65,6 +71,15 @@ def ncu_traffic(kernel: str, workload: str):
             if len(cols) >= 3 and cols[0] == kernel and cols[1] == workload:
                 return int(cols[2])
     return None
+
+
+def workload_config(name: str, w, world: int = 1) -> dict:
+    """The `config` object of the JSON line — the same for both arms (the driver compares them)."""
+    return {"workload": name, "requests": w.num_requests, "q_tokens_per_step": int(w.total_q),
+            "kv_tokens_per_request": w.kv_len(0), "heads": "%d/%d" % (w.num_q_heads, w.num_kv_heads),
+            "head_dim": "%d/%d" % (w.head_dim_qk, w.head_dim_v), "page": 16, "pool_pages": w.pool_pages,
+            "distinct_chunks_linked": int(len(w.linked_chunks())),
+            "chunk_links": int(sum(len(l) for l in w.links))}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -86,7 +101,7 @@ class L2Flush:
 
 # ------------------------------------------------------------------------------------------------
 class ClockSampler:
-    """Samples SM clock and throttle reasons DURING the timed region (NVML, every 10 ms)."""
+    """Samples SM clock and throttle reasons DURING the timed region (NVML, every 5 ms)."""
 
     def __init__(self, index: int):
         self.samples, self.reasons, self.max_mhz = [], set(), None
@@ -115,7 +130,7 @@ class ClockSampler:
                         self.reasons.add(k)
             except Exception:
                 pass
-            self._stop.wait(0.01)
+            self._stop.wait(0.005)
 
     def __enter__(self):
         if self.nv:
@@ -133,6 +148,17 @@ class ClockSampler:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
         return {"sm_mhz": int(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
                 "samples": len(self.samples)}
+
+
+def merge_clocks(a, b):
+    """Clock record over two timed regions (the primary's 20 default steps last a few ms: one NVML sample)."""
+    if not b or b.get("sm_mhz") is None:
+        return a
+    if not a or a.get("sm_mhz") is None:
+        return b
+    n1, n2 = a.get("samples", 1), b.get("samples", 1)
+    return {"sm_mhz": int(round((a["sm_mhz"] * n1 + b["sm_mhz"] * n2) / (n1 + n2))), "sm_max_mhz": a["sm_max_mhz"],
+            "reasons": sorted(set(a["reasons"]) | set(b["reasons"])), "samples": n1 + n2}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -190,19 +216,26 @@ def run_reference(args):
     if phase == "decode":
         value, unit, metric = kv_bytes / dt / 1e9, "GB/s", METRIC
     else:
-        value, unit, metric = flops / dt / 1e12, "TFLOP/s", "prefill cross-attn TFLOP/s"
+        value, unit, metric = flops / dt / 1e12, "TFLOP/s", "prefill cross-attn TFLOP/s (BASELINE metric, prefill half)"
     sample = "each step = oracle on the first %d request(s) of %s%s" % (
         n, w.name, "" if phase == "decode" else " (first 8 query tokens)")
     print(json.dumps({
         "impl": "reference", "metric": metric, "value": value, "unit": unit, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "sample": sample},
+        "config": workload_config(args.workload, w),
         "cpu_baseline": {"value": value, "unit": unit, "cores": oracle.max_threads(), "kind": "oracle",
                          "sample": sample},
         "e2e": {"value": value, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }), flush=True)
+
+
+def stats(x):
+    x = np.asarray(x, np.float64)
+    if x.size == 0:
+        return {"n": 0, "mean": 0.0, "median": 0.0, "min": 0.0}
+    return {"n": int(x.size), "mean": float(x.mean()), "median": float(np.median(x)), "min": float(x.min())}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -214,6 +247,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="decode_link", choices=["decode_link", "rag_prefill"])
     ap.add_argument("--no-extras", action="store_true", help="skip the other configs, store and CPU baseline")
+    ap.add_argument("--only", default="", help="comma-separated extras to run (default: all)")
     ap.add_argument("--seed", type=int, default=0)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -248,27 +282,31 @@ def main():
 
     pk = peaks()
     extras = {}
+    summary = []  # compact table, printed last on stderr
     primary_prefill = args.workload == "rag_prefill"
+    PATHS = {"auto": comb.DECODE_AUTO, "per_request": comb.DECODE_PER_REQUEST, "chunk_major": comb.DECODE_CHUNK_MAJOR}
 
     # ------------------------------------------------------------------ attention benches
-    def bench_attention(w, phase, steps, warmup, *, fill, flush_l2=False, with_link=True, e2e=True, shuffle=None):
-        """Returns a dict of timings for `steps` passes of (link +) attention on workload w."""
+    def bench_attention(w, phase, steps, warmup, *, fill, flush_l2=False, with_link=True, e2e=True, shuffle=None,
+                        decode_path="auto"):
+        """Timings of `steps` passes of (link +) attention on workload w. Kernel times are per launch (CUDA events
+        recorded by the library on the launching stream, comb_profile_*)."""
         # free list: permuted (a chunk's pages scattered over the arena, as in a long-running server) unless told
         ld = harness.load_workload(w, fill=fill, shuffle_seed=(2024 + rank) if shuffle is None else shuffle,
                                    keep_host=False)
         pool = ld.pool
+        pool.set_decode_path(PATHS[decode_path])
         if phase == "decode":
             wq = w.decode_phase() if int(w.lq.max()) > 1 else w
             q = harness.bits_to_device(wq.all_q(), "cuda")
             q_indptr = wq.q_indptr
         else:
             wq, q, q_indptr = w, ld.q, ld.q_indptr
-        R, Hq = wq.num_requests, wq.num_q_heads
+        Hq = wq.num_q_heads
         out = torch.empty((q.shape[0], Hq, w.head_dim_v), dtype=torch.bfloat16, device="cuda")
         lse = torch.empty((q.shape[0], Hq), dtype=torch.float32, device="cuda")
         chunk_indptr, chunk_ids = w.chunk_indptr, w.chunk_ids_flat
         batch = ld.batch
-        kid = comb.KERNEL_DECODE_SPLIT if phase == "decode" else comb.KERNEL_PREFILL
         flush = L2Flush(torch) if flush_l2 else None
 
         def step():
@@ -303,15 +341,29 @@ def main():
                 total_ms = ev[0].elapsed_time(ev[1])
         barrier()
         launches = pool.launches - l0
-        k_ms, k_n = comb.comb_profile_read(pool.handle, kid)
-        m_ms, m_n = comb.comb_profile_read(pool.handle, comb.KERNEL_DECODE_MERGE)
+        ks = {name: comb.comb_profile_read_samples(pool.handle, kid, cap=max(steps, 1) + 8) for name, kid in (
+            ("decode_split", comb.KERNEL_DECODE_SPLIT), ("decode_merge", comb.KERNEL_DECODE_MERGE),
+            ("decode_cascade", comb.KERNEL_DECODE_CASCADE), ("cascade_merge", comb.KERNEL_CASCADE_MERGE),
+            ("prefill", comb.KERNEL_PREFILL), ("prefill_merge", comb.KERNEL_PREFILL_MERGE))}
         comb.comb_profile_enable(pool.handle, False)
-        res = {"ms_per_step": max_over_ranks(total_ms / steps), "kernel_ms": k_ms / max(k_n, 1),
-               "merge_ms": (m_ms / m_n) if m_n else 0.0, "launches": launches, "clocks": clk.summary(),
-               "flops": wq.attention_flops(), "kv_bytes": wq.kv_bytes_logical(), "q_tokens": wq.total_q,
-               "timed_seconds": total_ms / 1e3}
-        # io bytes the kernel also moves (Q in, O + LSE out)
+        if phase == "decode":
+            main_k = "decode_cascade" if len(ks["decode_cascade"]) else "decode_split"
+            merge_k = "cascade_merge" if main_k == "decode_cascade" else "decode_merge"
+        else:
+            main_k, merge_k = "prefill", "prefill_merge"
+        L = batch.link
+        elt = 2 * wq.num_kv_heads * (wq.head_dim_qk + wq.head_dim_v)
+        res = {"ms_per_step": max_over_ranks(total_ms / steps), "kernel": main_k, "kernel_stats": stats(ks[main_k]),
+               "merge_stats": stats(ks[merge_k]), "launches": launches, "clocks": clk.summary(),
+               "flops": wq.attention_flops(), "kv_bytes": wq.kv_bytes_logical(),
+               "kv_bytes_unique": int(L.distinct_kv_tokens) * elt, "q_tokens": wq.total_q,
+               "timed_seconds": total_ms / 1e3, "entries": int(L.total_entries),
+               "distinct_chunks": int(L.num_distinct_chunks)}
+        res["kernel_ms"] = res["kernel_stats"]["mean"]
+        res["merge_ms"] = res["merge_stats"]["mean"]
+        # io bytes the kernel also moves (Q in, O + LSE out); a partial-row pass writes then re-reads fp32 rows
         res["io_bytes"] = q.numel() * 2 + out.numel() * 2 + lse.numel() * 4
+        res["partial_bytes"] = (int(L.total_entries) * Hq * (w.head_dim_v + 1) * 4) if main_k == "decode_cascade" else 0
         if e2e:
             # end to end through the public API with HOST buffers: pinned Q -> device, link, attention, O/LSE -> host
             qh = q.cpu().pin_memory()
@@ -373,23 +425,49 @@ def main():
         torch.cuda.empty_cache()
         return res
 
-    def roofline_hbm(r, kernel_name, wname):
-        achieved = (r["kv_bytes"] + r["io_bytes"]) / (r["kernel_ms"] * 1e-3) / 1e9
-        return {"bound": "hbm", "achieved": achieved, "peak": pk["hbm"], "unit": "GB/s", "frac": achieved / pk["hbm"],
-                "peak_source": pk["src"] + " copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
-                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS, "kernel": kernel_name,
-                "kernel_ms": r["kernel_ms"], "algorithmic_bytes": r["kv_bytes"] + r["io_bytes"],
-                "traffic": ncu_traffic(kernel_name, wname)}
+    def roofline_hbm(r, wname):
+        """DRAM view: the bytes that must cross the HBM pins (each distinct chunk once, Q/O/LSE, partial rows written)
+        over the dominant kernel's mean launch time. The logical rate (every request counting its own chunks: what
+        L2 and the chunk-major grouping serve) and ncu's measured DRAM traffic stand beside it."""
+        k_ms = r["kernel_ms"]
+        alg = r["kv_bytes_unique"] + r["io_bytes"] + r["partial_bytes"]
+        achieved = alg / (k_ms * 1e-3) / 1e9
+        logical = (r["kv_bytes"] + r["io_bytes"]) / (k_ms * 1e-3) / 1e9
+        traffic = ncu_traffic(r["kernel"], wname)
+        out = {"bound": "hbm", "achieved": achieved, "peak": pk["hbm"], "unit": "GB/s", "frac": achieved / pk["hbm"],
+               "peak_source": pk["src"] + " copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
+               "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS, "kernel": r["kernel"],
+               "kernel_ms": k_ms, "kernel_ms_median": r["kernel_stats"]["median"],
+               "kernel_ms_min": r["kernel_stats"]["min"], "launches_timed": r["kernel_stats"]["n"],
+               "algorithmic_bytes": alg, "bytes_definition": "distinct linked chunks once + Q + O + LSE + partial rows",
+               "achieved_logical": logical, "logical_bytes": r["kv_bytes"] + r["io_bytes"], "traffic": traffic,
+               "merge_ms": r["merge_ms"]}
+        if traffic:
+            out["frac_traffic"] = traffic / (k_ms * 1e-3) / 1e9 / pk["hbm"]
+        return out
 
-    def roofline_tensor(r, kernel_name, wname):
+    def roofline_tensor(r, wname):
         achieved = r["flops"] / (r["kernel_ms"] * 1e-3) / 1e12
         sustained = r["timed_seconds"] >= 1.0
         peak = pk["tf_sustained"] if sustained else pk["tf_burst"]
         return {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "peak_source": "%s cuBLAS bf16 %s" % (pk["src"], "sustained" if sustained else "burst"),
                 "frac_of_burst": achieved / pk["tf_burst"], "frac_of_sustained": achieved / pk["tf_sustained"],
-                "frac_of_nominal_2250": achieved / NOMINAL_BF16_TFLOPS, "kernel": kernel_name,
-                "kernel_ms": r["kernel_ms"], "algorithmic_flops": r["flops"], "traffic": ncu_traffic(kernel_name, wname)}
+                "frac_of_nominal_2250": achieved / NOMINAL_BF16_TFLOPS, "kernel": r["kernel"],
+                "kernel_ms": r["kernel_ms"], "kernel_ms_median": r["kernel_stats"]["median"],
+                "kernel_ms_min": r["kernel_stats"]["min"], "launches_timed": r["kernel_stats"]["n"],
+                "algorithmic_flops": r["flops"], "traffic": ncu_traffic(r["kernel"], wname), "merge_ms": r["merge_ms"]}
+
+    def note(name, r, roof, alt=None):
+        """One line of the compact table (kernel ms mean/median/min, achieved, fraction of the measured peak, clocks)."""
+        c = r["clocks"]
+        s = "%s k=%.4f/%.4f/%.4f step=%.4f %s=%.0f f=%.3f" % (
+            name, r["kernel_stats"]["mean"], r["kernel_stats"]["median"], r["kernel_stats"]["min"], r["ms_per_step"],
+            "TF" if roof["bound"] == "tensor" else "GB", roof["achieved"], roof["frac"])
+        if alt:
+            s += " " + alt
+        s += " clk=%s%s" % (c.get("sm_mhz"), ("!" + "+".join(c["reasons"])) if c.get("reasons") else "")
+        summary.append(s)
 
     # ------------------------------------------------------------------ primary workload
     if primary_prefill:
@@ -397,64 +475,124 @@ def main():
         r = bench_attention(w, "prefill", args.steps, args.warmup, fill="linked")
         value = world * r["flops"] / (r["ms_per_step"] * 1e-3) / 1e12
         unit, metric = "TFLOP/s", "prefill cross-attn TFLOP/s (BASELINE metric, prefill half)"
-        roof = roofline_tensor(r, "prefill", "rag_prefill")
+        roof = roofline_tensor(r, "rag_prefill")
         e2e_val = world * r["flops"] / (r["e2e_ms"] * 1e-3) / 1e12
-        dtype = "bf16"
     else:
         w = cs.decode_link(seed=args.seed + rank)
         r = bench_attention(w, "decode", args.steps, args.warmup, fill="linked")
         value = world * r["kv_bytes"] / (r["ms_per_step"] * 1e-3) / 1e9
         unit, metric = "GB/s", METRIC
-        roof = roofline_hbm(r, "decode_split", "decode_link")
+        roof = roofline_hbm(r, "decode_link")
         e2e_val = world * r["kv_bytes"] / (r["e2e_ms"] * 1e-3) / 1e9
-        dtype = "bf16"
+    dtype = "bf16"
     log("primary", json.dumps(r))
+    note(args.workload, r, roof, None if primary_prefill else "log=%.0f" % roof["achieved_logical"])
+    clocks = r["clocks"]
 
     cpu = None
+    prefill_top = None
     if rank == 0 and world == 1 and not args.no_extras:
+        only = set(x for x in args.only.split(",") if x)
+
+        def want(name):
+            return not only or name in only
+
         # ---- the other configs (not bench lines; context for the BASELINE metric's prefill half) ----
-        def prefill_extra(name, wk, steps, fill, flush=False):
+        def prefill_extra(name, wk, steps, fill, flush=False, wname=None):
             rr = bench_attention(wk, "prefill", steps, 3, fill=fill, flush_l2=flush, e2e=False)
             # a prefill whose flops per logical KV byte sit under the ridge of the measured peaks is HBM-bound
             # (no GQA or few query tokens: SURVEY.md 8(d)); it is then reported against the HBM roof first
             ridge = pk["tf_burst"] * 1e12 / (pk["hbm"] * 1e9)
             intensity = rr["flops"] / (rr["kv_bytes"] + rr["io_bytes"])
+            rt = roofline_tensor(rr, wname or name)
+            rh = roofline_hbm(rr, wname or name) if intensity < ridge else None
             extras[name] = {"workload": name, "ms_per_step": rr["ms_per_step"], "kernel_ms": rr["kernel_ms"],
                             "tflops": rr["flops"] / (rr["ms_per_step"] * 1e-3) / 1e12,
                             "q_tokens_per_s": rr["q_tokens"] / (rr["ms_per_step"] * 1e-3),
                             "flop_per_logical_byte": intensity, "ridge_flop_per_byte": ridge,
-                            "roofline_hbm": roofline_hbm(rr, "prefill", "") if intensity < ridge else None,
-                            "roofline": roofline_tensor(rr, "prefill", name.replace("_prefill", "") if name != "rag_prefill" else name), "clocks": rr["clocks"],
+                            "roofline_hbm": rh, "roofline": rt, "clocks": rr["clocks"], "launches": rr["launches"],
                             "l2": L2Flush.HOW if flush else "inputs larger than L2"}
             log(name, json.dumps(extras[name]))
+            note(name, rr, rt, ("hbm=%.0f/%.3f" % (rh["achieved"], rh["frac"])) if rh else None)
+            return rr
 
-        def decode_extra(name, wk, steps, fill, flush=False, shuffle=None):
-            rr = bench_attention(wk, "decode", steps, 3, fill=fill, flush_l2=flush, e2e=False, shuffle=shuffle)
-            extras[name] = {"workload": name, "ms_per_step": rr["ms_per_step"], "kernel_ms": rr["kernel_ms"],
-                            "merge_ms": rr["merge_ms"],
+        def decode_extra(name, wk, steps, fill, flush=False, shuffle=None, path="auto", wname=None):
+            rr = bench_attention(wk, "decode", steps, 3, fill=fill, flush_l2=flush, e2e=False, shuffle=shuffle,
+                                 decode_path=path)
+            rh = roofline_hbm(rr, wname or name)
+            extras[name] = {"workload": name, "decode_path": path, "ms_per_step": rr["ms_per_step"],
+                            "kernel_ms": rr["kernel_ms"], "merge_ms": rr["merge_ms"],
                             "gbs_logical": rr["kv_bytes"] / (rr["ms_per_step"] * 1e-3) / 1e9,
-                            "roofline": roofline_hbm(rr, "decode_split", name.replace("_decode", "") if name != "decode_link" else name), "clocks": rr["clocks"],
+                            "entries": rr["entries"], "distinct_chunks": rr["distinct_chunks"],
+                            "roofline": rh, "clocks": rr["clocks"], "launches": rr["launches"],
                             "l2": L2Flush.HOW if flush else "inputs larger than L2"}
             log(name, json.dumps(extras[name]))
+            note(name, rr, rh, "log=%.0f" % rh["achieved_logical"])
+            return rr
 
         try:
+            N = 200  # launches behind every median / min below
             if not primary_prefill:
-                prefill_extra("rag_prefill", cs.rag_prefill(seed=args.seed), 20, "linked")
-            else:
-                decode_extra("decode_link", cs.decode_link(seed=args.seed), 100, "linked")
-            if not primary_prefill:  # the same primary workload with an ascending free list (contiguous chunks)
-                decode_extra("decode_link_contiguous_pages", cs.decode_link(seed=args.seed), 100, "linked", shuffle=0)
-            prefill_extra("rag_prefill_lq32", cs.rag_prefill(seed=args.seed, lq=32), 20, "linked")
+                if want("rag_prefill"):
+                    rp = prefill_extra("rag_prefill", cs.rag_prefill(seed=args.seed), N, "linked")
+                    clocks = merge_clocks(clocks, rp["clocks"])
+                    prefill_top = {"workload": "rag_prefill (BASELINE configs[2])", "unit": "TFLOP/s",
+                                   "value": extras["rag_prefill"]["tflops"],
+                                   "ms_per_step": extras["rag_prefill"]["ms_per_step"],
+                                   "roofline": extras["rag_prefill"]["roofline"],
+                                   "config": workload_config("rag_prefill", cs.rag_prefill(seed=args.seed))}
+                # the same batch down the per-request path (what round 1 shipped), and the primary with a cold L2
+                if want("decode_link_per_request"):
+                    decode_extra("decode_link_per_request", cs.decode_link(seed=args.seed), N, "linked",
+                                 path="per_request", wname="decode_link")
+                if want("decode_link_cold_l2"):
+                    decode_extra("decode_link_cold_l2", cs.decode_link(seed=args.seed), 50, "linked", flush=True,
+                                 wname="decode_link")
+                if want("decode_link_contiguous_pages"):  # ascending free list: chunks contiguous in the arena
+                    decode_extra("decode_link_contiguous_pages", cs.decode_link(seed=args.seed), N, "linked", shuffle=0,
+                                 wname="decode_link")
+            elif want("decode_link"):
+                decode_extra("decode_link", cs.decode_link(seed=args.seed), N, "linked")
+            # cfg 2 geometry with 1024 DISTINCT chunks: every linked byte has to come from HBM (2.15 GB per step)
+            if want("decode_no_reuse"):
+                decode_extra("decode_no_reuse_per_request", cs.decode_link(seed=args.seed, no_reuse=True), N, "linked",
+                             path="per_request", wname="decode_no_reuse")
+                decode_extra("decode_no_reuse_chunk_major", cs.decode_link(seed=args.seed, no_reuse=True), N, "linked",
+                             path="chunk_major", wname="decode_no_reuse")
+            if want("rag_prefill_lq32"):
+                prefill_extra("rag_prefill_lq32", cs.rag_prefill(seed=args.seed, lq=32), N, "linked")
             # the paper's own regime (< 50 dynamic tokens) at a small batch: 32 work items for 148 SMs,
             # so each request's KV is cut into ranges that run on different SMs and are merged by LSE
-            prefill_extra("rag_prefill_lq32_r4", cs.rag_prefill(seed=args.seed, lq=32, requests=4), 20, "linked",
-                          flush=True)
-            prefill_extra("long_fewshot_prefill", cs.long_fewshot(seed=args.seed), 10, "all", flush=True)
-            decode_extra("long_fewshot_decode", cs.long_fewshot(seed=args.seed), 50, "all", flush=True)
-            prefill_extra("mla_shaped_prefill", cs.mla_shaped(seed=args.seed), 20, "linked")
-            decode_extra("mla_shaped_decode", cs.mla_shaped(seed=args.seed), 50, "linked")
-            extras["store"] = bench_store(torch, comb, harness, cs.long_fewshot(seed=args.seed), pk)
-            extras["link"] = bench_link(torch, comb, harness, cs.decode_link(seed=args.seed))
+            if want("rag_prefill_lq32_r4"):
+                prefill_extra("rag_prefill_lq32_r4", cs.rag_prefill(seed=args.seed, lq=32, requests=4), N, "linked",
+                              flush=True)
+            if want("long_fewshot"):
+                prefill_extra("long_fewshot_prefill", cs.long_fewshot(seed=args.seed), 50, "all", flush=True,
+                              wname="long_fewshot")
+                decode_extra("long_fewshot_decode", cs.long_fewshot(seed=args.seed), N, "all", flush=True,
+                             wname="long_fewshot")
+                decode_extra("long_fewshot_decode_per_request", cs.long_fewshot(seed=args.seed), N, "all", flush=True,
+                             path="per_request", wname="long_fewshot")
+            if want("mla_shaped"):
+                prefill_extra("mla_shaped_prefill", cs.mla_shaped(seed=args.seed), N, "linked", wname="mla_shaped")
+                decode_extra("mla_shaped_decode", cs.mla_shaped(seed=args.seed), N, "linked", wname="mla_shaped")
+                decode_extra("mla_shaped_decode_per_request", cs.mla_shaped(seed=args.seed), N, "linked",
+                             path="per_request", wname="mla_shaped")
+            if want("store"):
+                extras["store"] = bench_store(torch, comb, harness, cs.long_fewshot(seed=args.seed), pk)
+                st = extras["store"]
+                summary.append("store k=%.4f/%.4f/%.4f GB=%.0f f=%.3f" % (
+                    st["kernel_ms"], st["kernel_ms_median"], st["kernel_ms_min"], st["roofline"]["achieved"],
+                    st["roofline"]["frac"]))
+            if want("link"):
+                extras["link"] = bench_link(torch, comb, harness, cs.decode_link(seed=args.seed))
+                summary.append("link host_p50=%.1fus resident_p50=%.1fus" % (
+                    extras["link"]["host_enqueue_us_p50"], extras["link"]["resident_us_p50"]))
+            if want("stream_read"):
+                extras["stream_read"] = bench_stream_read(torch, comb, pk)
+                summary.append("read_only_stream GB=%.0f/%.0f (mean/best) = %.3f of copy peak" % (
+                    extras["stream_read"]["gbs_mean"], extras["stream_read"]["gbs_best"],
+                    extras["stream_read"]["gbs_best"] / pk["hbm"]))
         except Exception as e:  # extras must never lose the primary line
             extras["error"] = repr(e)
             log("extras failed:", repr(e))
@@ -468,20 +606,18 @@ def main():
             cpu = {"error": repr(e)}
 
     if rank == 0:
+        cfg = workload_config(args.workload, w, world)
+        cfg.update({"free_list": "permuted (scattered pages)",
+                    "step": "comb_link + comb_cross_attn_%s" % ("prefill" if primary_prefill else "decode"),
+                    "decode_path": None if primary_prefill else ("chunk_major" if r["kernel"] == "decode_cascade"
+                                                                  else "per_request"),
+                    "l2": "inputs larger than L2 (%.2f GB of distinct KV, %.2f GB logical per step)" % (
+                        r["kv_bytes_unique"] / 1e9, r["kv_bytes"] / 1e9),
+                    "parallelism": "replicas x%d" % world})
         line = {
             "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": dtype, "data": "synthetic",
-            "config": {"workload": "rag_prefill (BASELINE configs[2])" if primary_prefill
-                       else "decode_link (BASELINE configs[1])",
-                       "requests": w.num_requests, "q_tokens_per_step": r["q_tokens"],
-                       "kv_tokens_per_request": w.kv_len(0), "heads": "%d/%d" % (w.num_q_heads, w.num_kv_heads),
-                       "head_dim": "%d/%d" % (w.head_dim_qk, w.head_dim_v), "page": 16,
-                       "pool_pages": w.pool_pages, "free_list": "permuted (scattered pages)",
-                       "step": "comb_link + comb_cross_attn_%s" % ("prefill" if primary_prefill else "decode"),
-                       "l2": "inputs larger than L2 (logical %.2f GB KV per step)" % (r["kv_bytes"] / 1e9),
-                       "parallelism": "replicas x%d" % world},
-            "clocks": r["clocks"],
+            "vs_baseline": None, "dtype": dtype, "data": "synthetic", "config": cfg, "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": unit, "h2d_bytes_per_step": r["h2d"], "d2h_bytes_per_step": r["d2h"],
                     "ms_per_step": r["e2e_ms"], "serial_ms_per_step": r["e2e_serial_ms"],
                     "how": "host buffers through the public API; pinned Q -> device, comb_link (tables H2D), attention, "
@@ -491,17 +627,24 @@ def main():
             "roofline": roof,
             "q_tokens_per_s": world * r["q_tokens"] / (r["ms_per_step"] * 1e-3),
         }
+        if prefill_top is not None:
+            line["prefill"] = prefill_top
         if cpu is not None:
             line["cpu_baseline"] = cpu
         if extras:
             line["extras"] = extras
         print(json.dumps(line), flush=True)
+        # compact table last, so that a truncated stderr tail still carries every workload's number
+        log("== summary (kernel ms mean/median/min; achieved; f = fraction of the measured peak; GB = DRAM-byte rate, "
+            "log = logical) ==")
+        for s in summary:
+            log(s[:118])
     if world > 1:
         dist.destroy_process_group()
 
 
 def bench_store(torch, comb, harness, w, pk):
-    """(a2) batched paged store of configs[3]'s 64 variable-length chunks: free + store again, 20 times."""
+    """(a2) batched paged store of configs[3]'s 64 variable-length chunks: free + store again, 200 times."""
     ld = harness.load_workload(w, fill="all", shuffle_seed=77, keep_host=False)
     pool = ld.pool
     ids = list(range(w.num_chunks))
@@ -513,7 +656,7 @@ def bench_store(torch, comb, harness, w, pk):
     flush = L2Flush(torch)
     comb.comb_profile_enable(pool.handle, True)
     comb.comb_profile_read(pool.handle, comb.KERNEL_STORE)
-    n = 20
+    n = 200
     for i in range(n + 3):
         for c in ids:
             comb.comb_chunk_free(pool.handle, c)
@@ -522,16 +665,19 @@ def bench_store(torch, comb, harness, w, pk):
             torch.cuda.synchronize()
             comb.comb_profile_read(pool.handle, comb.KERNEL_STORE)
         pool.store_chunks(ids, tok, k, v)
-    ms, cnt = comb.comb_profile_read(pool.handle, comb.KERNEL_STORE)
+    st = stats(comb.comb_profile_read_samples(pool.handle, comb.KERNEL_STORE, cap=n + 8))
     comb.comb_profile_enable(pool.handle, False)
     nbytes = 2 * T * w.num_kv_heads * (w.head_dim_qk + w.head_dim_v) * 2
-    achieved = nbytes / (ms / cnt * 1e-3) / 1e9
+    achieved = nbytes / (st["mean"] * 1e-3) / 1e9
     pool.close()
     return {"workload": "store of long_fewshot's %d chunks (%d tokens), one launch" % (w.num_chunks, T),
-            "kernel_ms": ms / cnt, "roofline": {"bound": "hbm", "achieved": achieved, "peak": pk["hbm"], "unit": "GB/s",
-                                                 "frac": achieved / pk["hbm"], "algorithmic_bytes": nbytes,
-                                                 "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
-                                                 "kernel": "store", "traffic": ncu_traffic("store", "long_fewshot")},
+            "kernel_ms": st["mean"], "kernel_ms_median": st["median"], "kernel_ms_min": st["min"],
+            "launches_timed": st["n"],
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": pk["hbm"], "unit": "GB/s",
+                         "frac": achieved / pk["hbm"], "algorithmic_bytes": nbytes,
+                         "bytes_definition": "read + write of every token's K and V",
+                         "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                         "kernel": "store", "traffic": ncu_traffic("store", "long_fewshot")},
             "l2": L2Flush.HOW}
 
 
@@ -554,11 +700,34 @@ def bench_link(torch, comb, harness, w):
             host.append((t1 - t0) * 1e6)
             full.append((t2 - t0) * 1e6)
     pool.close()
-    return {"workload": "decode_link: %d requests, %d table entries, %d B copied" % (
-                w.num_requests, int(lb.link.total_pages), int(lb.link.bytes_used)),
+    return {"workload": "decode_link: %d requests, %d table entries, %d distinct chunks, %d B copied" % (
+                w.num_requests, int(lb.link.total_pages), int(lb.link.num_distinct_chunks), int(lb.link.bytes_used)),
             "host_enqueue_us_p50": float(np.percentile(host, 50)), "host_enqueue_us_p99": float(np.percentile(host, 99)),
             "resident_us_p50": float(np.percentile(full, 50)), "resident_us_p99": float(np.percentile(full, 99)),
             "kv_bytes_copied": 0}
+
+
+def bench_stream_read(torch, comb, pk):
+    """Read-only HBM ceiling of the day (SURVEY.md §8(d) "Denominators"): the library's streaming-read kernel over a
+    4 GiB buffer (32x the L2), 20 launches after 3 warm-ups, CUDA events on the launching stream."""
+    n = 4 << 30
+    buf = torch.empty(n, dtype=torch.uint8, device="cuda")
+    buf.random_(0, 255)
+    sink = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ms = []
+    for i in range(23):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        comb.comb_util_stream_read(buf, sink)
+        b.record()
+        torch.cuda.synchronize()
+        if i >= 3:
+            ms.append(a.elapsed_time(b))
+    del buf
+    torch.cuda.empty_cache()
+    return {"bytes": n, "ms_mean": float(np.mean(ms)), "ms_min": float(np.min(ms)),
+            "gbs_mean": n / (np.mean(ms) * 1e-3) / 1e9, "gbs_best": n / (np.min(ms) * 1e-3) / 1e9,
+            "copy_peak_gbs": pk["hbm"], "how": "comb_util_stream_read, 4 GiB, 128-bit streaming loads, no stores"}
 
 
 if __name__ == "__main__":

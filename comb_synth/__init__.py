@@ -126,6 +126,11 @@ class Workload:
         tot = sum(self.kv_len(r) for r in range(self.num_requests))
         return 2 * self.num_kv_heads * (self.head_dim_qk + self.head_dim_v) * tot
 
+    def kv_bytes_unique(self) -> int:
+        """Bytes of the DISTINCT chunks the batch links: what has to cross the HBM pins at least once."""
+        tot = int(self.chunk_len[self.linked_chunks()].astype(np.int64).sum())
+        return 2 * self.num_kv_heads * (self.head_dim_qk + self.head_dim_v) * tot
+
     # ---- tensors ---------------------------------------------------------------------------
     def chunk_kv(self, c: int) -> Tuple[np.ndarray, np.ndarray]:
         """bf16 bit patterns: K [T][Hkv][Dqk], V [T][Hkv][Dv] for chunk ``c`` (K drawn first)."""
@@ -181,9 +186,18 @@ def tiny_link(seed: int = 0, lq: int = 16, n_chunks: int = 4, chunk_tokens: int 
 
 
 def decode_link(seed: int = 0, requests: int = 128, pool_chunks: int = 2000, chunk_tokens: int = 512,
-                chunks_per_req: int = 8) -> Workload:
-    """configs[1]: Llama-3-8B-shaped layer, batch 128 x 1 query token, 8 chunks x 512 by Zipf(1.1) of 2000."""
+                chunks_per_req: int = 8, no_reuse: bool = False) -> Workload:
+    """configs[1]: Llama-3-8B-shaped layer, batch 128 x 1 query token, 8 chunks x 512 by Zipf(1.1) of 2000.
+    ``no_reuse``: same geometry, but the batch's requests x chunks_per_req links are drawn WITHOUT replacement across
+    the whole batch (1024 distinct chunks), so every linked byte has to come from HBM — the measurement case for the
+    decode kernels' DRAM rate (no L2 help from shared chunks)."""
     rng = _structure_rng(seed, 1)
+    if no_reuse:
+        perm = rng.permutation(pool_chunks)[:requests * chunks_per_req].astype(np.int64)
+        links = tuple(perm[r * chunks_per_req:(r + 1) * chunks_per_req] for r in range(requests))
+        return Workload("decode_no_reuse", 1, seed, 32, 8, 128, 128,
+                        np.full(pool_chunks, chunk_tokens, dtype=np.int32), links,
+                        np.ones(requests, dtype=np.int32), 1.0 / np.sqrt(128.0))
     p = bounded_zipf_p(pool_chunks, 1.1)
     links = tuple(rng.choice(pool_chunks, size=chunks_per_req, replace=False, p=p).astype(np.int64)
                   for _ in range(requests))

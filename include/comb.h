@@ -105,7 +105,11 @@ int32_t comb_chunk_query(const comb_pool_t *pool, uint64_t chunk_id, int32_t *nu
 int32_t comb_store_chunk(comb_pool_t *pool, int32_t layer, uint64_t chunk_id, int32_t num_tokens, const void *k,
                          const void *v, void *stream);
 /* Batched form, one kernel launch: chunk i has tokens tok_indptr[i]..tok_indptr[i+1] (host int32 [n+1]) of the
- * packed device tensors k_packed [sum T][Hkv][Dqk], v_packed [sum T][Hkv][Dv]. All-or-nothing on error. */
+ * packed device tensors k_packed [sum T][Hkv][Dqk], v_packed [sum T][Hkv][Dv]. All-or-nothing: on any error
+ * (including a CUDA failure) the directory and the free list are as before the call. The same id twice in one
+ * batch is INVALID. Storing an id that already exists with the same length overwrites its pages (that is how
+ * the other layers of a chunk are filled); ordering against attention calls in flight that read those pages is
+ * the caller's, as for any store. */
 int32_t comb_store_chunks(comb_pool_t *pool, int32_t layer, int32_t n, const uint64_t *chunk_ids,
                           const int32_t *tok_indptr, const void *k_packed, const void *v_packed, void *stream);
 
@@ -113,8 +117,12 @@ int32_t comb_store_chunks(comb_pool_t *pool, int32_t layer, int32_t n, const uin
  * PAPER.md:119, PAPER.md:62 step 5.  Zero-copy: builds the request's block table from an ORDERED
  * chunk-id list; no kernel touches K/V.
  *
- * The caller provides device_buf (comb_link_bytes() bytes, 16-byte aligned). comb_link lays the tables
- * out inside it, fills the pointers below and enqueues ONE host->device copy on `stream`.
+ * The caller provides device_buf (comb_link_bytes() bytes, 16-byte aligned) and, optionally, host_buf
+ * (comb_link_host_bytes() bytes of ordinary host memory). comb_link lays the tables out inside device_buf, fills
+ * the pointers below and enqueues ONE host->device copy on `stream`.  An "entry" is one (request, linked chunk)
+ * pair, numbered in the order of chunk_ids.
+ *
+ * Request-major view (what prefill and the per-request decode read):
  *   page_indptr int32 [R+1]      page range of request r in page_ids / page_ntok
  *   page_ids    int32 [total]    pages(c_0) || ... || pages(c_{m-1}) in the caller's order
  *   page_ntok   int32 [total]    16, except the last page of each chunk = T - 16*(npages-1)
@@ -123,12 +131,29 @@ int32_t comb_store_chunks(comb_pool_t *pool, int32_t layer, int32_t n, const uin
  *                                entries of the request, i.e. 128 slots, counted from its first page)
  *   tile_ntok   uint64 [tiles]   byte j = page_ntok of entry 8*t+j, 0 past the request's last page
  *                                (derived from page_ntok; lets kernels skip the slot mask on full tiles)
- * A request with zero chunks is legal (kv_len 0). Duplicate ids inside a request are taken literally.
+ *   entry_indptr int32 [R+1]     entries of request r (= chunk_indptr)
+ * Chunk-major ("cascade") view — the same batch inverted, so that every DISTINCT chunk is streamed once and all
+ * the query rows that link it attend to it together (possible because PICaches carry no per-request position:
+ * PAPER.md:24, 119).  Distinct chunks get slots u = 0..U-1, ordered by descending number of entries, ties by
+ * first appearance in chunk_ids:
+ *   cas_page_indptr int32 [U+1], cas_page_ids int32 [distinct pages]    page list of slot u
+ *   cas_tile_indptr int32 [U+1], cas_tile_ntok uint64 [..]              as tile_indptr / tile_ntok, per slot
+ *   cas_row_indptr  int32 [U+1]                                         entries that link slot u
+ *   cas_row_req     int32 [E]    request of the entry;   cas_row_entry int32 [E]   the entry's number
+ *                                (inside a slot, entries are in ascending entry number)
+ * Host mirror (only when host_buf != NULL; plain host memory the caller owns — a caller that builds its own
+ * tables fills these two arrays itself):
+ *   host_req_pages int32 [R]     page_indptr[r+1] - page_indptr[r]  (the prefill planner cuts KV ranges with it)
+ *   host_cas_rows  int32 [U]     cas_row_indptr[u+1] - cas_row_indptr[u]  (the chunk-major decode tiles rows with it)
+ * Without a host mirror both attention calls still work: prefill does not cut KV ranges, decode runs per request.
+ * A request with zero chunks is legal (kv_len 0). Duplicate ids inside a request are taken literally (two entries).
  * Errors: INVALID, UNKNOWN_CHUNK (nothing written), CAPACITY, CUDA. */
 typedef struct {
-    /* in: caller-owned device memory */
+    /* in: caller-owned memory */
     void *device_buf;
     size_t device_bytes;
+    void *host_buf;      /* nullable */
+    size_t host_bytes;
     /* out: device pointers into device_buf */
     int32_t *page_indptr;
     int32_t *page_ids;
@@ -136,25 +161,42 @@ typedef struct {
     int32_t *kv_len;
     int32_t *tile_indptr;
     uint64_t *tile_ntok;
+    int32_t *entry_indptr;
+    int32_t *cas_page_indptr;
+    int32_t *cas_page_ids;
+    int32_t *cas_tile_indptr;
+    uint64_t *cas_tile_ntok;
+    int32_t *cas_row_indptr;
+    int32_t *cas_row_req;
+    int32_t *cas_row_entry;
+    /* out: host pointers into host_buf (NULL without one) */
+    int32_t *host_req_pages;
+    int32_t *host_cas_rows;
     /* out: host-side summary */
     int32_t num_requests;
     int32_t max_pages_per_request;
     int64_t total_pages;
     int64_t total_tiles;
     int64_t total_kv_tokens;
+    int64_t total_entries;        /* E */
+    int32_t num_distinct_chunks;  /* U */
+    int32_t max_rows_per_chunk;   /* entries of slot 0 */
+    int64_t distinct_pages;       /* pages of the U distinct chunks */
+    int64_t distinct_kv_tokens;   /* their tokens: what a chunk-major pass reads once */
     size_t bytes_used; /* bytes of device_buf written = size of the single H2D copy */
 } comb_link_t;
 
-/* Bytes of device_buf that suffice for num_requests requests naming total_pages table entries. */
-size_t comb_link_bytes(int32_t num_requests, int64_t total_pages);
+/* Bytes of device_buf / host_buf that suffice for num_requests requests with total_entries (request, chunk)
+ * pairs naming total_pages table entries. */
+size_t comb_link_bytes(int32_t num_requests, int64_t total_entries, int64_t total_pages);
+size_t comb_link_host_bytes(int32_t num_requests, int64_t total_entries);
 int32_t comb_link(comb_pool_t *pool, int32_t num_requests, const int32_t *chunk_indptr /* host [R+1] */,
                   const uint64_t *chunk_ids /* host, link order */, comb_link_t *link, void *stream);
-/* Same tables written into HOST memory `host_buf` (link->device_bytes bytes available); the pointers in
- * `link` are laid out as if host_buf were device_buf. No CUDA call — used by comb_link and by host tests.
- * Also notes, inside the pool and keyed by link->device_buf, how many pages every request links (the prefill
- * planner's KV ranges need it; the directory and the free list are not touched). */
+/* Same tables written into HOST memory `staging` (link->device_bytes bytes available); the pointers in
+ * `link` are laid out as if staging were device_buf. No CUDA call, and the pool is not modified — used by
+ * comb_link and by host tests. */
 int32_t comb_link_plan(const comb_pool_t *pool, int32_t num_requests, const int32_t *chunk_indptr,
-                       const uint64_t *chunk_ids, comb_link_t *link, void *host_buf);
+                       const uint64_t *chunk_ids, comb_link_t *link, void *staging);
 
 /* (a4) prefill cross-attention — PAPER.md:112-115 §4.2 Eq. 7-8 (softmax(QK^T/sqrt d) V, NO mask), over the
  * concatenation of the linked chunks; cost O(l_query * l_doc) per layer (Eq. 12).
@@ -162,13 +204,15 @@ int32_t comb_link_plan(const comb_pool_t *pool, int32_t num_requests, const int3
  *   out       device bf16 [sum lq][Hq][Dv];    lse       device fp32 [sum lq][Hq] or NULL
  *   scale     multiplies q.k before the softmax (the paper's 1/sqrt(d), per head: 1/sqrt(Dqk)); must be a
  *             finite positive number (INVALID otherwise)
- *   workspace device, comb_workspace_bytes() bytes, 16-byte aligned
- * q-head h reads kv-head h / (Hq/Hkv). kv_len == 0 gives out = 0, lse = -inf. tcgen05/TMEM/TMA kernel.
+ *   workspace device, comb_attn_workspace_bytes() bytes, 16-byte aligned
+ * q-head h reads kv-head h / (Hq/Hkv); Hq/Hkv must be a power of two <= 16. kv_len == 0 gives out = 0,
+ * lse = -inf. tcgen05/TMEM/TMA kernel.
  * When the call has fewer work items than the GPU has SMs (few requests with few query tokens — the paper's
- * regime) and `link` was produced by comb_link of this pool, every request's KV is cut into ranges
- * that run on different SMs; their fp32 partial rows live in `workspace` and a second kernel merges them by LSE.
- * The result is the same function; only fp32 summation order differs.
- * Errors: INVALID, CAPACITY (workspace smaller than comb_workspace_bytes() for this shape, or not 16-byte
+ * regime) and link->host_req_pages is given, every request's KV is cut into ranges that run on
+ * different SMs; their fp32 partial rows live in `workspace` and are merged by LSE.
+ * The result is the same function; only fp32 summation order differs. host_req_pages is checked against the
+ * link's summary (sum = total_pages, max = max_pages_per_request): INVALID if it disagrees.
+ * Errors: INVALID, CAPACITY (workspace smaller than comb_attn_workspace_bytes() for this call, or not 16-byte
  * aligned), CUDA. */
 int32_t comb_cross_attn_prefill(comb_pool_t *pool, int32_t layer, const comb_link_t *link, int32_t num_requests,
                                 const void *q, const int32_t *q_indptr, int32_t num_q_heads, float scale, void *out,
@@ -177,16 +221,36 @@ int32_t comb_cross_attn_prefill(comb_pool_t *pool, int32_t layer, const comb_lin
 /* (a5) decode cross-attention — the same function with exactly one query row per request (PAPER.md:66:
  * generated tokens are "treated identically to the initial query tokens").
  *   q device bf16 [R][Hq][Dqk];  out device bf16 [R][Hq][Dv];  lse device fp32 [R][Hq] or NULL
- * Split-KV kernel (HBM-bound, CUDA cores) + LSE-merge kernel. Errors as above. */
+ * Two paths compute it (same result up to fp32 summation order and, on the second, bf16 rounding of the softmax
+ * weights fed to the tensor cores, as in prefill):
+ *   per-request : split-KV kernel on CUDA cores (HBM-bound, GEMV-shaped) + LSE-merge kernel;
+ *   chunk-major : every distinct chunk of the batch is streamed ONCE; the (entries x Hq/Hkv) query rows that link
+ *                 it form the M tile of a tcgen05 contraction; per-entry fp32 partials are merged by LSE per
+ *                 request (needs link->host_cas_rows).
+ * COMB_OPT_DECODE_PATH picks one (default: chunk-major when the batch shares chunks, see comb_pool_set_option).
+ * Errors as above. */
 int32_t comb_cross_attn_decode(comb_pool_t *pool, int32_t layer, const comb_link_t *link, int32_t num_requests,
                                const void *q, int32_t num_q_heads, float scale, void *out, float *lse,
                                void *workspace, size_t workspace_bytes, void *stream);
 
-/* Workspace that suffices for either attention call: num_requests requests, num_q_heads heads, total_q
- * query rows, max_pages_per_request table entries in the longest request (pass comb_link_t.max_pages_per_request).
- * Holds the decode split partials, or the prefill work-item list plus the partial rows of its KV ranges. */
+/* Workspace that suffices for either attention call on THIS link: num_q_heads heads, total_q query rows (decode:
+ * total_q = num_requests). Holds the decode split partials or the chunk-major tiles and per-entry partials, or the
+ * prefill work-item list plus the partial rows of its KV ranges. */
+size_t comb_attn_workspace_bytes(const comb_pool_t *pool, const comb_link_t *link, int32_t num_q_heads,
+                                 int64_t total_q);
+/* Link-independent bound for callers that size the workspace before linking: num_requests requests, total_q query
+ * rows, max_pages_per_request table entries in the longest request. Covers prefill and the per-request decode;
+ * a decode whose workspace is too small for the chunk-major path quietly takes the per-request one (unless
+ * COMB_OPT_DECODE_PATH forces chunk-major: CAPACITY). */
 size_t comb_workspace_bytes(const comb_pool_t *pool, int32_t num_requests, int32_t num_q_heads, int64_t total_q,
                             int32_t max_pages_per_request);
+
+/* Pool options. COMB_OPT_DECODE_PATH: 0 = automatic (chunk-major when total_entries >= 1.25 x distinct chunks,
+ * i.e. the batch re-reads at least a fifth of its KV), 1 = always per-request, 2 = always chunk-major.
+ * Errors: INVALID (unknown option or value). */
+enum { COMB_OPT_DECODE_PATH = 1 };
+enum { COMB_DECODE_AUTO = 0, COMB_DECODE_PER_REQUEST = 1, COMB_DECODE_CHUNK_MAJOR = 2 };
+int32_t comb_pool_set_option(comb_pool_t *pool, int32_t option, int64_t value);
 
 /* Kernels launched by this library since the pool was created (store/attention/reduce; copies excluded). */
 int64_t comb_pool_launch_count(const comb_pool_t *pool);
@@ -196,9 +260,18 @@ int64_t comb_pool_launch_count(const comb_pool_t *pool);
  * comb_profile_read synchronises on the recorded events (the one call here that waits for the device), adds up
  * the elapsed times of kernel class `kernel` (COMB_KERNEL_*), reports them and forgets those records.
  * Errors: INVALID, CUDA. */
-enum { COMB_KERNEL_STORE = 0, COMB_KERNEL_DECODE_SPLIT = 1, COMB_KERNEL_DECODE_MERGE = 2, COMB_KERNEL_PREFILL = 3 };
+enum { COMB_KERNEL_STORE = 0, COMB_KERNEL_DECODE_SPLIT = 1, COMB_KERNEL_DECODE_MERGE = 2, COMB_KERNEL_PREFILL = 3,
+       COMB_KERNEL_DECODE_CASCADE = 4, COMB_KERNEL_CASCADE_MERGE = 5, COMB_KERNEL_PREFILL_MERGE = 6 };
 int32_t comb_profile_enable(comb_pool_t *pool, int32_t on);
 int32_t comb_profile_read(comb_pool_t *pool, int32_t kernel, double *total_ms, int64_t *launches);
+/* Same, but hands back the elapsed time of every recorded launch of that class (oldest first, at most `cap`
+ * values into host array `ms`; the rest are dropped) so a caller can report median and minimum. */
+int32_t comb_profile_read_samples(comb_pool_t *pool, int32_t kernel, float *ms, int64_t cap, int64_t *launches);
+
+/* Measurement utility (bench.py's read-only HBM ceiling): one kernel that reads `bytes` bytes of
+ * device memory at `src` (16-byte aligned) with streaming 128-bit loads and writes nothing; `sink` = 4 device
+ * bytes. Enqueued on `stream`; timed by the caller. Errors: INVALID, CUDA. */
+int32_t comb_util_stream_read(const void *src, size_t bytes, void *sink, void *stream);
 
 const char *comb_strerror(int32_t status);
 const char *comb_version(void);

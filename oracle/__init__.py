@@ -6,7 +6,8 @@ the paper (PAPER.md = /root/reference/PAPER.md at authoring time; the GPU box ne
   O1  attention output  — ``comb_oracle.c`` (fp64, explicit concatenation in link order, one joint
       softmax, no mask: §4.2 Eq. 7-8)
   O2  page image        — :func:`page_image` (numpy, bit-exact uint16)
-  O3  block tables      — :class:`PoolModel` (independent re-statement of the FIFO page policy)
+  O3  block tables      — :class:`PoolModel` (independent re-statement of the FIFO page policy; request-major
+      tables and the chunk-major inversion of the same batch)
 
 Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference``
 legs may import this package.  It shares no code with ``paper_2602_01519_b200`` and neither imports the
@@ -239,6 +240,40 @@ class PoolModel:
             kv.append(tot)
         return {"page_indptr": np.array(indptr, dtype=np.int32), "page_ids": np.array(ids, dtype=np.int32),
                 "page_ntok": np.array(ntok, dtype=np.int32), "kv_len": np.array(kv, dtype=np.int32)}
+
+    def link_chunk_major(self, chunk_lists: Sequence[Sequence[int]]) -> Dict[str, np.ndarray]:
+        """The same batch inverted (include/comb.h, "chunk-major view"): an entry is one (request, linked chunk)
+        pair, numbered in link order; every DISTINCT chunk gets a slot, slots ordered by descending number of
+        entries, ties by first appearance; a slot lists its pages once and the entries (request, entry number)
+        that link it in ascending entry number.  Order-free concatenation is what makes the
+        inversion legal; the tables themselves are integer bookkeeping with exactly one right answer."""
+        entries = [(r, int(c)) for r, lst in enumerate(chunk_lists) for c in lst]
+        first: Dict[int, int] = {}
+        count: Dict[int, int] = {}
+        for e, (_, c) in enumerate(entries):
+            first.setdefault(c, e)
+            count[c] = count.get(c, 0) + 1
+        slots = sorted(count, key=lambda c: (-count[c], first[c]))
+        page_indptr, page_ids, page_ntok, row_indptr, row_req, row_entry = [0], [], [], [0], [], []
+        for c in slots:
+            T, pages = self.dir[c]
+            page_ids.extend(pages)
+            page_ntok.extend([PAGE] * (len(pages) - 1) + [T - PAGE * (len(pages) - 1)])
+            page_indptr.append(len(page_ids))
+            for e, (r, cc) in enumerate(entries):
+                if cc == c:
+                    row_req.append(r)
+                    row_entry.append(e)
+            row_indptr.append(len(row_req))
+        entry_indptr = np.zeros(len(chunk_lists) + 1, dtype=np.int32)
+        np.cumsum([len(l) for l in chunk_lists], out=entry_indptr[1:])
+        return {"entry_indptr": entry_indptr, "slot_chunks": np.array(slots, dtype=np.int64),
+                "cas_page_indptr": np.array(page_indptr, dtype=np.int32),
+                "cas_page_ids": np.array(page_ids, dtype=np.int32),
+                "cas_page_ntok": np.array(page_ntok, dtype=np.int32),
+                "cas_row_indptr": np.array(row_indptr, dtype=np.int32),
+                "cas_row_req": np.array(row_req, dtype=np.int32),
+                "cas_row_entry": np.array(row_entry, dtype=np.int32)}
 
 
 # ------------------------------------------------------------------------------------------------

@@ -31,10 +31,18 @@ class PoolConfig(C.Structure):
 class Link(C.Structure):
     """comb_link_t"""
     _fields_ = [("device_buf", C.c_void_p), ("device_bytes", C.c_size_t),
+                ("host_buf", C.c_void_p), ("host_bytes", C.c_size_t),
                 ("page_indptr", C.c_void_p), ("page_ids", C.c_void_p), ("page_ntok", C.c_void_p),
                 ("kv_len", C.c_void_p), ("tile_indptr", C.c_void_p), ("tile_ntok", C.c_void_p),
+                ("entry_indptr", C.c_void_p),
+                ("cas_page_indptr", C.c_void_p), ("cas_page_ids", C.c_void_p), ("cas_tile_indptr", C.c_void_p),
+                ("cas_tile_ntok", C.c_void_p), ("cas_row_indptr", C.c_void_p), ("cas_row_req", C.c_void_p),
+                ("cas_row_entry", C.c_void_p),
+                ("host_req_pages", C.c_void_p), ("host_cas_rows", C.c_void_p),
                 ("num_requests", C.c_int32), ("max_pages_per_request", C.c_int32),
                 ("total_pages", C.c_int64), ("total_tiles", C.c_int64), ("total_kv_tokens", C.c_int64),
+                ("total_entries", C.c_int64), ("num_distinct_chunks", C.c_int32), ("max_rows_per_chunk", C.c_int32),
+                ("distinct_pages", C.c_int64), ("distinct_kv_tokens", C.c_int64),
                 ("bytes_used", C.c_size_t)]
 
 
@@ -51,7 +59,8 @@ _SIGS = {
     "comb_chunk_query": (C.c_int32, [_P, C.c_uint64, C.POINTER(C.c_int32), _P, C.c_int32]),
     "comb_store_chunk": (C.c_int32, [_P, C.c_int32, C.c_uint64, C.c_int32, _P, _P, _P]),
     "comb_store_chunks": (C.c_int32, [_P, C.c_int32, C.c_int32, _P, _P, _P, _P, _P]),
-    "comb_link_bytes": (C.c_size_t, [C.c_int32, C.c_int64]),
+    "comb_link_bytes": (C.c_size_t, [C.c_int32, C.c_int64, C.c_int64]),
+    "comb_link_host_bytes": (C.c_size_t, [C.c_int32, C.c_int64]),
     "comb_link": (C.c_int32, [_P, C.c_int32, _P, _P, C.POINTER(Link), _P]),
     "comb_link_plan": (C.c_int32, [_P, C.c_int32, _P, _P, C.POINTER(Link), _P]),
     "comb_cross_attn_prefill": (C.c_int32, [_P, C.c_int32, C.POINTER(Link), C.c_int32, _P, _P, C.c_int32, C.c_float,
@@ -59,9 +68,13 @@ _SIGS = {
     "comb_cross_attn_decode": (C.c_int32, [_P, C.c_int32, C.POINTER(Link), C.c_int32, _P, C.c_int32, C.c_float, _P,
                                            _P, _P, C.c_size_t, _P]),
     "comb_workspace_bytes": (C.c_size_t, [_P, C.c_int32, C.c_int32, C.c_int64, C.c_int32]),
+    "comb_attn_workspace_bytes": (C.c_size_t, [_P, C.POINTER(Link), C.c_int32, C.c_int64]),
+    "comb_pool_set_option": (C.c_int32, [_P, C.c_int32, C.c_int64]),
     "comb_pool_launch_count": (C.c_int64, [_P]),
     "comb_profile_enable": (C.c_int32, [_P, C.c_int32]),
     "comb_profile_read": (C.c_int32, [_P, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
+    "comb_profile_read_samples": (C.c_int32, [_P, C.c_int32, _P, C.c_int64, C.POINTER(C.c_int64)]),
+    "comb_util_stream_read": (C.c_int32, [_P, C.c_size_t, _P, _P]),
     "comb_strerror": (C.c_char_p, [C.c_int32]),
     "comb_version": (C.c_char_p, []),
 }

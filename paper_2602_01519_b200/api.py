@@ -87,8 +87,12 @@ def comb_store_chunks(pool: int, layer: int, chunk_ids: Sequence[int], tok_indpt
                                 _ptr(v_packed), _stream_ptr(stream)), "comb_store_chunks")
 
 
-def comb_link_bytes(num_requests: int, total_pages: int) -> int:
-    return int(lib.comb_link_bytes(num_requests, total_pages))
+def comb_link_bytes(num_requests: int, total_entries: int, total_pages: int) -> int:
+    return int(lib.comb_link_bytes(num_requests, total_entries, total_pages))
+
+
+def comb_link_host_bytes(num_requests: int, total_entries: int) -> int:
+    return int(lib.comb_link_host_bytes(num_requests, total_entries))
 
 
 def comb_link(pool: int, chunk_indptr, chunk_ids, link: Link, stream=None) -> Link:
@@ -100,7 +104,8 @@ def comb_link(pool: int, chunk_indptr, chunk_ids, link: Link, stream=None) -> Li
 
 
 def comb_link_plan(pool: int, chunk_indptr, chunk_ids, link: Link, host_buf: np.ndarray) -> Link:
-    """Host-only table build (no CUDA call); ``host_buf`` is a uint8 array of link.device_bytes bytes."""
+    """Host-only table build (no CUDA call); ``host_buf`` is the staging area, a uint8 array of link.device_bytes
+    bytes, laid out as device_buf would be."""
     ind = np.ascontiguousarray(chunk_indptr, dtype=np.int32)
     ids = np.ascontiguousarray(chunk_ids, dtype=np.uint64)
     check(lib.comb_link_plan(pool, int(ind.shape[0]) - 1, ind.ctypes.data, ids.ctypes.data if ids.size else None,
@@ -110,6 +115,18 @@ def comb_link_plan(pool: int, chunk_indptr, chunk_ids, link: Link, host_buf: np.
 
 def comb_workspace_bytes(pool: int, num_requests: int, num_q_heads: int, total_q: int, max_pages: int) -> int:
     return int(lib.comb_workspace_bytes(pool, num_requests, num_q_heads, total_q, max_pages))
+
+
+def comb_attn_workspace_bytes(pool: int, link: Link, num_q_heads: int, total_q: int) -> int:
+    return int(lib.comb_attn_workspace_bytes(pool, C.byref(link), num_q_heads, total_q))
+
+
+OPT_DECODE_PATH = 1
+DECODE_AUTO, DECODE_PER_REQUEST, DECODE_CHUNK_MAJOR = 0, 1, 2
+
+
+def comb_pool_set_option(pool: int, option: int, value: int) -> None:
+    check(lib.comb_pool_set_option(pool, option, value), "comb_pool_set_option")
 
 
 def comb_cross_attn_prefill(pool: int, layer: int, link: Link, q, q_indptr, num_q_heads: int, scale: float, out,
@@ -132,6 +149,7 @@ def comb_pool_launch_count(pool: int) -> int:
 
 
 KERNEL_STORE, KERNEL_DECODE_SPLIT, KERNEL_DECODE_MERGE, KERNEL_PREFILL = 0, 1, 2, 3
+KERNEL_DECODE_CASCADE, KERNEL_CASCADE_MERGE, KERNEL_PREFILL_MERGE = 4, 5, 6
 
 
 def comb_profile_enable(pool: int, on: bool) -> None:
@@ -145,6 +163,19 @@ def comb_profile_read(pool: int, kernel: int) -> Tuple[float, int]:
     return ms.value, n.value
 
 
+def comb_profile_read_samples(pool: int, kernel: int, cap: int = 4096) -> np.ndarray:
+    """Per-launch device ms of one kernel class since the last read (oldest first); waits for those launches."""
+    buf = np.zeros(cap, np.float32)
+    n = C.c_int64()
+    check(lib.comb_profile_read_samples(pool, kernel, buf.ctypes.data, cap, C.byref(n)), "comb_profile_read_samples")
+    return buf[:min(int(n.value), cap)].copy()
+
+
+def comb_util_stream_read(src: torch.Tensor, sink: torch.Tensor, stream=None) -> None:
+    check(lib.comb_util_stream_read(src.data_ptr(), src.numel() * src.element_size(), sink.data_ptr(),
+                                    _stream_ptr(stream)), "comb_util_stream_read")
+
+
 def comb_version() -> str:
     return lib.comb_version().decode()
 
@@ -153,10 +184,10 @@ def comb_version() -> str:
 # convenience owner of the caller-side allocations (torch = memory + streams only)
 # ------------------------------------------------------------------------------------------------
 class LinkedBatch:
-    """A comb_link_t plus the torch buffer that backs it."""
+    """A comb_link_t plus the torch buffer (device tables) and the numpy buffer (host mirror) that back it."""
 
-    def __init__(self, link: Link, buf: torch.Tensor):
-        self.link, self.buf = link, buf
+    def __init__(self, link: Link, buf: torch.Tensor, host: Optional[np.ndarray] = None):
+        self.link, self.buf, self.host = link, buf, host
 
     def _view(self, ptr: int, n: int, dtype: torch.dtype) -> torch.Tensor:
         off = ptr - self.buf.data_ptr()
@@ -170,14 +201,31 @@ class LinkedBatch:
         """Device tables copied to host numpy arrays (synchronises)."""
         L = self.link
         R, n, t = L.num_requests, int(L.total_pages), int(L.total_tiles)
-        return {
-            "page_indptr": self._view(L.page_indptr, R + 1, torch.int32).cpu().numpy(),
-            "page_ids": self._view(L.page_ids, n, torch.int32).cpu().numpy(),
-            "page_ntok": self._view(L.page_ntok, n, torch.int32).cpu().numpy(),
-            "kv_len": self._view(L.kv_len, R, torch.int32).cpu().numpy(),
-            "tile_indptr": self._view(L.tile_indptr, R + 1, torch.int32).cpu().numpy(),
+        U, E, pd = int(L.num_distinct_chunks), int(L.total_entries), int(L.distinct_pages)
+        i32 = lambda ptr, cnt: self._view(ptr, cnt, torch.int32).cpu().numpy()  # noqa: E731
+        out = {
+            "page_indptr": i32(L.page_indptr, R + 1), "page_ids": i32(L.page_ids, n),
+            "page_ntok": i32(L.page_ntok, n), "kv_len": i32(L.kv_len, R),
+            "tile_indptr": i32(L.tile_indptr, R + 1),
             "tile_ntok": self._view(L.tile_ntok, t, torch.int64).cpu().numpy().view(np.uint64),
+            "entry_indptr": i32(L.entry_indptr, R + 1),
+            "cas_page_indptr": i32(L.cas_page_indptr, U + 1), "cas_page_ids": i32(L.cas_page_ids, pd),
+            "cas_tile_indptr": i32(L.cas_tile_indptr, U + 1), "cas_row_indptr": i32(L.cas_row_indptr, U + 1),
+            "cas_row_req": i32(L.cas_row_req, E), "cas_row_entry": i32(L.cas_row_entry, E),
         }
+        tc = int(out["cas_tile_indptr"][-1]) if U else 0
+        out["cas_tile_ntok"] = self._view(L.cas_tile_ntok, tc, torch.int64).cpu().numpy().view(np.uint64)
+        return out
+
+    def host_mirror(self) -> dict:
+        """The host arrays the attention planners read (None without a host buffer)."""
+        L = self.link
+        if not L.host_req_pages:
+            return {"req_pages": None, "cas_rows": None}
+        base = self.host.ctypes.data
+        o1, o2 = L.host_req_pages - base, L.host_cas_rows - base
+        return {"req_pages": self.host[o1:o1 + 4 * L.num_requests].view(np.int32),
+                "cas_rows": self.host[o2:o2 + 4 * int(L.num_distinct_chunks)].view(np.int32)}
 
 
 class Pool:
@@ -238,24 +286,28 @@ class Pool:
         return self.link_flat(indptr, ids, stream, into)
 
     def link_flat(self, chunk_indptr: np.ndarray, chunk_ids: np.ndarray, stream=None,
-                  into: Optional[LinkedBatch] = None) -> LinkedBatch:
+                  into: Optional[LinkedBatch] = None, host_mirror: bool = True) -> LinkedBatch:
         R = int(chunk_indptr.shape[0]) - 1
         if into is None:
             total_pages = 0
-            for c in np.asarray(chunk_ids).tolist():
+            ids = np.asarray(chunk_ids).tolist()
+            for c in ids:
                 nt = C.c_int32()
                 total_pages += check(lib.comb_chunk_query(self.handle, int(c), C.byref(nt), None, 0), "comb_link")
-            nbytes = comb_link_bytes(R, total_pages)
+            nbytes = comb_link_bytes(R, len(ids), total_pages)
             buf = torch.empty(max(nbytes, 16), dtype=torch.uint8, device=self.device)
-            into = LinkedBatch(Link(), buf)
+            host = np.zeros(max(comb_link_host_bytes(R, len(ids)), 16), np.uint8) if host_mirror else None
+            into = LinkedBatch(Link(), buf, host)
         into.link.device_buf = into.buf.data_ptr()
         into.link.device_bytes = into.buf.numel()
+        into.link.host_buf = into.host.ctypes.data if into.host is not None else None
+        into.link.host_bytes = into.host.nbytes if into.host is not None else 0
         comb_link(self.handle, chunk_indptr, chunk_ids, into.link, stream)
         return into
 
     # ---- (a4)/(a5) attention ----
-    def workspace(self, num_requests: int, num_q_heads: int, total_q: int, max_pages: int) -> torch.Tensor:
-        need = comb_workspace_bytes(self.handle, num_requests, num_q_heads, total_q, max_pages)
+    def workspace(self, lb: LinkedBatch, num_q_heads: int, total_q: int) -> torch.Tensor:
+        need = comb_attn_workspace_bytes(self.handle, lb.link, num_q_heads, total_q)
         if self._ws is None or self._ws.numel() < need:
             self._ws = torch.empty(max(need, 256), dtype=torch.uint8, device=self.device)
         return self._ws
@@ -267,7 +319,7 @@ class Pool:
             out = torch.empty((total_q, Hq, self.head_dim_v), dtype=q.dtype, device=self.device)
         if lse is None and want_lse:
             lse = torch.empty((total_q, Hq), dtype=torch.float32, device=self.device)
-        ws = self.workspace(lb.num_requests, Hq, total_q, lb.link.max_pages_per_request)
+        ws = self.workspace(lb, Hq, total_q)
         comb_cross_attn_prefill(self.handle, layer, lb.link, q, q_indptr, Hq, scale, out, lse, ws, ws.numel(), stream)
         return out, lse
 
@@ -278,9 +330,13 @@ class Pool:
             out = torch.empty((R, Hq, self.head_dim_v), dtype=q.dtype, device=self.device)
         if lse is None and want_lse:
             lse = torch.empty((R, Hq), dtype=torch.float32, device=self.device)
-        ws = self.workspace(R, Hq, R, lb.link.max_pages_per_request)
+        ws = self.workspace(lb, Hq, R)
         comb_cross_attn_decode(self.handle, layer, lb.link, R, q, Hq, scale, out, lse, ws, ws.numel(), stream)
         return out, lse
+
+    def set_decode_path(self, path: int) -> None:
+        """DECODE_AUTO / DECODE_PER_REQUEST / DECODE_CHUNK_MAJOR (comb_pool_set_option, COMB_OPT_DECODE_PATH)."""
+        comb_pool_set_option(self.handle, OPT_DECODE_PATH, path)
 
     @property
     def launches(self) -> int:

@@ -19,7 +19,6 @@ using namespace comb;
 namespace {
 
 constexpr int kRingSlots = 4;
-constexpr size_t kLinkInfoSlots = 8;
 
 struct Chunk {
     int32_t num_tokens;
@@ -51,16 +50,7 @@ struct comb_pool {
     bool kv_maps_ready = false;
     TensorMapBlob k_map, v_map;
     int64_t launches = 0;
-    // Host copy of the per-request page counts of the most recent links, keyed by their device buffer: lets the
-    // prefill planner cut long requests into KV ranges without reading the tables back from the device.
-    struct LinkInfo { const void *device_buf; std::vector<int32_t> pages; };
-    std::vector<LinkInfo> link_info;  // at most kLinkInfoSlots, oldest replaced first
-    size_t link_info_next = 0;
-    const std::vector<int32_t> *find_link_pages(const void *device_buf, int32_t R) const {
-        for (const LinkInfo &li : link_info)
-            if (li.device_buf == device_buf && (int32_t)li.pages.size() == R) return &li.pages;
-        return nullptr;
-    }
+    int64_t opt_decode_path = COMB_DECODE_AUTO;
     // per-kernel timing (comb_profile_*)
     struct ProfRec { int id; cudaEvent_t a, b; };
     bool prof_on = false;
@@ -180,20 +170,44 @@ void dir_free(comb_pool_t *p, std::unordered_map<uint64_t, Chunk>::iterator it) 
 }
 
 struct LinkLayout {
-    size_t off_page_indptr, off_kv_len, off_tile_indptr, off_tile_ntok, off_page_ids, off_page_ntok, bytes;
+    size_t off_page_indptr, off_kv_len, off_tile_indptr, off_entry_indptr, off_cas_page_indptr, off_cas_tile_indptr,
+        off_cas_row_indptr, off_tile_ntok, off_cas_tile_ntok, off_page_ids, off_page_ntok, off_cas_page_ids,
+        off_cas_row_req, off_cas_row_entry, bytes;
 };
 
-LinkLayout link_layout(int32_t R, int64_t total_pages, int64_t total_tiles) {
+// R requests, E entries, U distinct chunks with Pd pages and Tc tiles in all, P table entries, T tiles
+LinkLayout link_layout(int32_t R, int64_t E, int64_t U, int64_t P, int64_t T, int64_t Pd, int64_t Tc) {
     LinkLayout L;
     size_t o = 0;
-    L.off_page_indptr = o; o = align_up(o + sizeof(int32_t) * (size_t)(R + 1), 16);
-    L.off_kv_len = o;      o = align_up(o + sizeof(int32_t) * (size_t)std::max(R, 1), 16);
-    L.off_tile_indptr = o; o = align_up(o + sizeof(int32_t) * (size_t)(R + 1), 16);
-    L.off_tile_ntok = o;   o = align_up(o + sizeof(uint64_t) * (size_t)std::max<int64_t>(total_tiles, 1), 16);
-    L.off_page_ids = o;    o = align_up(o + sizeof(int32_t) * (size_t)std::max<int64_t>(total_pages, 1), 16);
-    L.off_page_ntok = o;   o = align_up(o + sizeof(int32_t) * (size_t)std::max<int64_t>(total_pages, 1), 16);
+    auto take = [&](size_t elem, int64_t n) {
+        const size_t at = o;
+        o = align_up(o + elem * (size_t)std::max<int64_t>(n, 1), 16);
+        return at;
+    };
+    L.off_page_indptr = take(4, R + 1);
+    L.off_kv_len = take(4, R);
+    L.off_tile_indptr = take(4, R + 1);
+    L.off_entry_indptr = take(4, R + 1);
+    L.off_cas_page_indptr = take(4, U + 1);
+    L.off_cas_tile_indptr = take(4, U + 1);
+    L.off_cas_row_indptr = take(4, U + 1);
+    L.off_tile_ntok = take(8, T);
+    L.off_cas_tile_ntok = take(8, Tc);
+    L.off_page_ids = take(4, P);
+    L.off_page_ntok = take(4, P);
+    L.off_cas_page_ids = take(4, Pd);
+    L.off_cas_row_req = take(4, E);
+    L.off_cas_row_entry = take(4, E);
     L.bytes = o;
     return L;
+}
+
+// byte j = page_ntok of table entry t + j, 0 past `end`
+uint64_t pack_tile_ntok(const int32_t *page_ntok, int64_t t, int64_t end) {
+    uint64_t packed = 0;
+    const int lim = (int)std::min<int64_t>(kTilePages, end - t);
+    for (int j = 0; j < lim; ++j) packed |= (uint64_t)page_ntok[t + j] << (8 * j);
+    return packed;
 }
 
 // KV ranges per request for a prefill call that has `num_items` unsplit work items and whose longest request has
@@ -201,21 +215,12 @@ LinkLayout link_layout(int32_t R, int64_t total_pages, int64_t total_tiles) {
 // the merge pass) when the items cannot fill even one wave of the persistent grid: measured on B200, cutting a
 // 1.7-wave or 3.5-wave problem into ranges gained nothing (profiles/r01_bench.md). So: no ranges once there is an
 // item per SM; otherwise the largest count that still fits one wave, every range keeping at least two tiles.
-int plan_prefill_splits(size_t num_items, int max_tiles, int num_sms, int max_allowed) {
+int plan_prefill_splits(size_t num_items, int max_tiles, int num_sms) {
     static const int cands[] = {1, 2, 3, 4, 6, 8, 12, 16};
-    static const int forced = [] {  // COMB_PREFILL_NSPLIT=n: measurement hook, overrides the policy (1 = never split)
-        const char *e = getenv("COMB_PREFILL_NSPLIT");
-        return e ? atoi(e) : 0;
-    }();
-    if (forced > 0) {
-        int ns = std::min(forced, max_allowed);
-        while (ns > 1 && prefill_tiles_per_split(max_tiles, ns) < 1) --ns;
-        return std::max(ns, 1);
-    }
     if (num_items == 0 || num_items >= (size_t)num_sms) return 1;
     int best = 1;
     for (int ns : cands) {
-        if (ns > max_allowed) break;
+        if (ns > kPrefillMaxSplits) break;
         if (ns > 1 && prefill_tiles_per_split(max_tiles, ns) < 2) break;
         if (num_items * (size_t)ns > (size_t)num_sms) break;
         best = ns;
@@ -231,7 +236,166 @@ LinkView view_of(const comb_link_t *l) {
     v.kv_len = l->kv_len;
     v.tile_indptr = l->tile_indptr;
     v.tile_ntok = l->tile_ntok;
+    v.entry_indptr = l->entry_indptr;
+    v.cas_page_indptr = l->cas_page_indptr;
+    v.cas_page_ids = l->cas_page_ids;
+    v.cas_tile_indptr = l->cas_tile_indptr;
+    v.cas_tile_ntok = l->cas_tile_ntok;
+    v.cas_row_indptr = l->cas_row_indptr;
+    v.cas_row_req = l->cas_row_req;
+    v.cas_row_entry = l->cas_row_entry;
     return v;
+}
+
+// ---------------------------------------------------------------- prefill planning (one place: the workspace bound
+// and the call agree by construction)
+constexpr int kPartRowsPerRange = 2 * 128;  // partial rows reserved per (split item): two 128-row tile slots
+
+struct PrefillPlan {
+    std::vector<PrefillItem> items;
+    int tiles_per_cta = 2;
+    int64_t part_rows = 0;  // fp32 partial rows of the KV ranges (0: no item is split)
+};
+size_t prefill_items_bytes(size_t n) { return align_up(n * sizeof(PrefillItem), 256); }
+size_t prefill_part_bytes(int64_t rows, int dv) { return (size_t)rows * (size_t)(dv + 1) * sizeof(float); }
+
+// Upper bounds over every plan a call with these sizes can produce: the split items of a call never number more
+// than two waves of CTAs (uniform ranges: items x ranges <= #SM; last-wave ranges: tail x factor <= CTAs), each with
+// kPartRowsPerRange partial rows.
+void prefill_bounds(const comb_pool *p, int32_t Hq, int64_t total_q, size_t *max_items, int64_t *max_part_rows) {
+    const int Hkv = p->cfg.num_kv_heads;
+    const int G = std::max(1, Hq / Hkv);
+    const int tok_per_tile = std::max(1, 128 / std::min(G, 128));
+    // one item per (request, kv-head, 1-2 tiles): at most one more item per request than full tiles, and no more
+    // requests with rows than rows
+    const size_t base_hi = ((size_t)total_q / tok_per_tile + (size_t)total_q + 1) * Hkv;
+    const size_t ctas_hi = (size_t)p->num_sms * 2;
+    *max_items = base_hi + ctas_hi;
+    *max_part_rows = (int64_t)ctas_hi * kPartRowsPerRange;
+}
+
+int32_t plan_prefill(comb_pool *p, const comb_link_t *link, int32_t R, const int32_t *q_indptr, int32_t Hq,
+                     PrefillPlan *out) {
+    const int Hkv = p->cfg.num_kv_heads, G = Hq / Hkv;
+    int64_t max_lq = 0, nonempty = 0;
+    for (int32_t r = 0; r < R; ++r) {
+        max_lq = std::max<int64_t>(max_lq, q_indptr[r + 1] - q_indptr[r]);
+        nonempty += q_indptr[r + 1] > q_indptr[r];
+    }
+    // per-request page counts: the caller-visible host mirror of the link (checked against its summary so that a
+    // stale or foreign array cannot silently drop KV tiles)
+    const int32_t *req_pages = link->host_req_pages;
+    if (req_pages) {
+        int64_t sum = 0;
+        int32_t mx = 0;
+        for (int32_t r = 0; r < R; ++r) {
+            if (req_pages[r] < 0) return COMB_ERR_INVALID;
+            sum += req_pages[r];
+            mx = std::max(mx, req_pages[r]);
+        }
+        if (sum != link->total_pages || mx != link->max_pages_per_request) return COMB_ERR_INVALID;
+    }
+    out->tiles_per_cta = prefill_tiles_per_cta(G, p->cfg.head_dim_qk, p->cfg.head_dim_v, max_lq, nonempty * Hkv,
+                                               p->num_sms);
+    const int tok_per_tile = 128 / G, tok_per_item = out->tiles_per_cta * tok_per_tile;
+    // ---- work items: (request, kv-head, one or two Q tiles) against the request's KV, or against a range of it.
+    // Requests are ordered by work (query rows x KV tiles when the page counts are known on the host, else query
+    // rows) so the tail of the persistent grid is made of short items; the kv-heads of one Q tile group sit together
+    // so CTAs that stream the same K/V run at the same time (L2 reuse).
+    auto tiles_of = [&](int32_t r) { return req_pages ? (req_pages[r] + kTilePages - 1) / kTilePages : 1; };
+    struct Req { int32_t r; int64_t rows, cost; };
+    std::vector<Req> order;
+    order.reserve(R);
+    for (int32_t r = 0; r < R; ++r) {
+        const int64_t rows = (int64_t)q_indptr[r + 1] - q_indptr[r];
+        order.push_back(Req{r, rows, rows * std::max(1, tiles_of(r))});
+    }
+    std::stable_sort(order.begin(), order.end(), [](const Req &a, const Req &b) { return a.cost > b.cost; });
+    std::vector<PrefillItem> base;
+    for (const Req &x : order)
+        for (int64_t t = 0; t < x.rows; t += tok_per_item)
+            for (int g = 0; g < Hkv; ++g)
+                base.push_back(PrefillItem{x.r, g, q_indptr[x.r] + (int32_t)t,
+                                           (int32_t)std::min<int64_t>(tok_per_item, x.rows - t), 0,
+                                           INT32_MAX / kTilePages, -1, 0, 0, 0});
+    out->items.clear();
+    out->part_rows = 0;
+    if (base.empty()) return COMB_OK;
+    // ---- KV ranges (need the page counts): (1) fewer items than SMs: every request is cut so that items x ranges
+    // fill one wave; (2) several waves with a last wave at most half full: only the items of that last wave are cut
+    // (by up to 4), so it takes a fraction of an item's time instead of a whole one (cfg 4: 512 items on 148 SMs).
+    const int max_tiles = (link->max_pages_per_request + kTilePages - 1) / kTilePages;
+    const size_t ctas = (size_t)p->num_sms *
+                        (size_t)prefill_ctas_per_sm(out->tiles_per_cta, p->cfg.head_dim_qk, p->cfg.head_dim_v);
+    int uniform = 1, tail_factor = 1;
+    size_t tail_from = base.size();
+    if (req_pages) {
+        // (one item per SM is the target even when two single-tile CTAs share an SM: measured, 256 ranges on 148
+        // SMs were slower than 128)
+        uniform = plan_prefill_splits(base.size(), max_tiles, p->num_sms);
+        const size_t tail = base.size() % ctas;
+        if (uniform == 1 && base.size() > ctas && tail > 0 && 2 * tail <= ctas) {
+            tail_factor = (int)std::min<size_t>(4, ctas / tail);
+            tail_from = base.size() - tail;
+        }
+    }
+    out->items.reserve(base.size() * (size_t)std::max(uniform, 1) + (base.size() - tail_from) * (size_t)tail_factor);
+    for (size_t i = 0; i < base.size(); ++i) {
+        const int want = i >= tail_from ? tail_factor : uniform;
+        const int n_kv = want > 1 ? tiles_of(base[i].request) : 0;
+        const int tps = want > 1 ? std::max(2, prefill_tiles_per_split(n_kv, want)) : 0;  // >= 2 tiles per range
+        const int eff = tps > 0 ? (n_kv + tps - 1) / tps : 1;
+        if (eff <= 1) {
+            out->items.push_back(base[i]);
+            continue;
+        }
+        for (int sidx = 0; sidx < eff; ++sidx) {
+            PrefillItem it = base[i];
+            it.kv_tile0 = sidx * tps;
+            it.kv_tiles = sidx + 1 < eff ? tps : INT32_MAX / kTilePages;  // the last range is open-ended
+            it.split = sidx;
+            it.tps = tps;
+            it.part_base = (int32_t)out->part_rows;
+            out->items.push_back(it);
+        }
+        out->part_rows += (int64_t)eff * kPartRowsPerRange;
+    }
+    return COMB_OK;
+}
+
+// ---------------------------------------------------------------- chunk-major decode planning
+// Tiles of the chunk-major decode: slot u's entries in groups of 128/G (each entry = G rows of the M tile).
+// Slots are already ordered by descending entry count (comb_link), so the hot chunks' tiles come first and run
+// at the same time (their shared K/V stream is an L2 hit for all but one of them).
+int32_t plan_cascade(const comb_link_t *link, int G, std::vector<CascadeTile> *tiles) {
+    const int32_t U = link->num_distinct_chunks;
+    const int32_t *rows = link->host_cas_rows;
+    int64_t sum = 0;
+    int32_t mx = 0;
+    for (int32_t u = 0; u < U; ++u) {
+        if (rows[u] <= 0) return COMB_ERR_INVALID;
+        sum += rows[u];
+        mx = std::max(mx, rows[u]);
+    }
+    if (sum != link->total_entries || mx != link->max_rows_per_chunk) return COMB_ERR_INVALID;
+    const int per_tile = 128 / G;
+    tiles->clear();
+    int32_t row0 = 0;
+    for (int32_t u = 0; u < U; ++u) {
+        for (int32_t t = 0; t < rows[u]; t += per_tile)
+            tiles->push_back(CascadeTile{u, row0 + t, std::min<int32_t>(per_tile, rows[u] - t), 0});
+        row0 += rows[u];
+    }
+    return COMB_OK;
+}
+size_t cascade_tiles_bytes(size_t n) { return align_up(std::max<size_t>(n, 1) * sizeof(CascadeTile), 256); }
+// tiles of a link at group size G without building them: sum_u ceil(rows_u / (128/G))
+size_t cascade_tile_count(const comb_link_t *link, int G) {
+    const int per_tile = 128 / G;
+    size_t n = 0;
+    for (int32_t u = 0; u < link->num_distinct_chunks; ++u)
+        n += (size_t)(std::max(link->host_cas_rows[u], 0) + per_tile - 1) / per_tile;
+    return n;
 }
 
 }  // namespace
@@ -318,7 +482,7 @@ int32_t comb_profile_enable(comb_pool_t *p, int32_t on) {
 }
 
 int32_t comb_profile_read(comb_pool_t *p, int32_t kernel, double *total_ms, int64_t *launches) {
-    if (!p || kernel < 0 || kernel > 3) return COMB_ERR_INVALID;
+    if (!p || kernel < 0 || kernel >= kNumKernelIds) return COMB_ERR_INVALID;
     double tot = 0.0;
     int64_t n = 0;
     std::vector<comb_pool::ProfRec> keep;
@@ -336,6 +500,30 @@ int32_t comb_profile_read(comb_pool_t *p, int32_t kernel, double *total_ms, int6
     if (total_ms) *total_ms = tot;
     if (launches) *launches = n;
     return COMB_OK;
+}
+
+int32_t comb_profile_read_samples(comb_pool_t *p, int32_t kernel, float *ms_out, int64_t cap, int64_t *launches) {
+    if (!p || kernel < 0 || kernel >= kNumKernelIds || cap < 0 || (cap > 0 && !ms_out)) return COMB_ERR_INVALID;
+    int64_t n = 0;
+    std::vector<comb_pool::ProfRec> keep;
+    for (auto &r : p->prof_recs) {
+        if (r.id != kernel) { keep.push_back(r); continue; }
+        float ms = 0.f;
+        if (cudaEventSynchronize(r.b) != cudaSuccess || cudaEventElapsedTime(&ms, r.a, r.b) != cudaSuccess)
+            return COMB_ERR_CUDA;
+        if (n < cap) ms_out[n] = ms;
+        ++n;
+        p->prof_free.push_back(r.a);
+        p->prof_free.push_back(r.b);
+    }
+    p->prof_recs.swap(keep);
+    if (launches) *launches = n;
+    return COMB_OK;
+}
+
+int32_t comb_util_stream_read(const void *src, size_t bytes, void *sink, void *stream) {
+    if (!src || !sink || bytes < 16 || (((uintptr_t)src) & 15)) return COMB_ERR_INVALID;
+    return launch_stream_read(src, bytes, sink, (cudaStream_t)stream) == cudaSuccess ? COMB_OK : COMB_ERR_CUDA;
 }
 
 int32_t comb_chunk_alloc(comb_pool_t *p, uint64_t id, int32_t T) {
@@ -376,17 +564,12 @@ int32_t comb_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, const uint64
             if (T <= 0) return COMB_ERR_INVALID;
             const size_t np = (size_t)(T + kPage - 1) / kPage;
             total_descs += np;
+            if (!seen.emplace(ids[i], (int32_t)T).second) return COMB_ERR_INVALID;  // the same id twice in one batch
             auto it = p->dir.find(ids[i]);
             if (it != p->dir.end()) {
                 if (it->second.num_tokens != T) return COMB_ERR_EXISTS;
             } else {
-                auto s = seen.find(ids[i]);
-                if (s != seen.end()) {
-                    if (s->second != T) return COMB_ERR_EXISTS;
-                } else {
-                    seen.emplace(ids[i], (int32_t)T);
-                    need_pages += np;
-                }
+                need_pages += np;
             }
         }
     }
@@ -398,11 +581,19 @@ int32_t comb_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, const uint64
     // ---- directory update + page descriptors ----
     StorePageDesc *h = (StorePageDesc *)p->ring[slot].host;
     size_t at = 0;
+    const size_t head_before = p->free_head;
+    std::vector<uint64_t> created;  // for the rollback: pages are taken from the head in order, so undoing is exact
+    auto rollback = [&]() {
+        for (uint64_t id : created) p->dir.erase(id);
+        p->free_head = head_before;
+    };
     for (int32_t i = 0; i < n; ++i) {
         const int32_t T = tok_indptr[i + 1] - tok_indptr[i];
         const Chunk *c = nullptr;
-        int32_t rc = dir_alloc(p, ids[i], T, &c, nullptr);
-        if (rc != COMB_OK) return rc;  // cannot happen after validation
+        bool made = false;
+        int32_t rc = dir_alloc(p, ids[i], T, &c, &made);
+        if (rc != COMB_OK) { rollback(); return rc; }  // cannot happen after validation
+        if (made) created.push_back(ids[i]);
         for (size_t j = 0; j < c->pages.size(); ++j) {
             StorePageDesc d;
             d.dst_page = c->pages[j];
@@ -413,12 +604,17 @@ int32_t comb_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, const uint64
         }
     }
     StorePageDesc *dev = (StorePageDesc *)((char *)p->cfg.scratch + (size_t)slot * p->scratch_slot_bytes());
-    if (cudaMemcpyAsync(dev, h, at * sizeof(StorePageDesc), cudaMemcpyHostToDevice, st) != cudaSuccess)
+    if (cudaMemcpyAsync(dev, h, at * sizeof(StorePageDesc), cudaMemcpyHostToDevice, st) != cudaSuccess) {
+        rollback();
         return COMB_ERR_CUDA;
+    }
     if (p->prof_on) p->hook.begin(p, kKernelStore, st);
     const cudaError_t se = launch_store(p->geom, layer, dev, (int)at, k_packed, v_packed, st);
     if (p->prof_on) p->hook.end(p, st);
-    if (se != cudaSuccess) return COMB_ERR_CUDA;
+    if (se != cudaSuccess) {
+        rollback();
+        return COMB_ERR_CUDA;
+    }
     p->launches += 1;
     if (!p->release(slot, st)) return COMB_ERR_CUDA;
     return COMB_OK;
@@ -431,44 +627,84 @@ int32_t comb_store_chunk(comb_pool_t *p, int32_t layer, uint64_t id, int32_t T, 
     return comb_store_chunks(p, layer, 1, &id, indptr, k, v, stream);
 }
 
-size_t comb_link_bytes(int32_t R, int64_t total_pages) {
-    if (R < 0 || total_pages < 0) return 0;
-    return link_layout(R, total_pages, total_pages / kTilePages + R + 1).bytes;
+size_t comb_link_bytes(int32_t R, int64_t E, int64_t total_pages) {
+    if (R < 0 || E < 0 || total_pages < 0) return 0;
+    // U <= E distinct chunks; their pages <= total_pages; a chunk's / request's last tile may be partly filled
+    return link_layout(R, E, E, total_pages, total_pages / kTilePages + R + 1, total_pages,
+                       total_pages / kTilePages + E + 1).bytes;
+}
+
+size_t comb_link_host_bytes(int32_t R, int64_t E) {
+    if (R < 0 || E < 0) return 0;
+    return align_up(sizeof(int32_t) * (size_t)std::max(R, 1), 16) + align_up(sizeof(int32_t) * (size_t)std::max<int64_t>(E, 1), 16);
 }
 
 int32_t comb_link_plan(const comb_pool_t *p, int32_t R, const int32_t *chunk_indptr, const uint64_t *chunk_ids,
-                       comb_link_t *link, void *host_buf) {
-    if (!p || !link || R < 0 || !chunk_indptr || !host_buf || !link->device_buf) return COMB_ERR_INVALID;
+                       comb_link_t *link, void *staging) {
+    if (!p || !link || R < 0 || !chunk_indptr || !staging || !link->device_buf) return COMB_ERR_INVALID;
     if (chunk_indptr[0] != 0) return COMB_ERR_INVALID;
     for (int32_t r = 0; r < R; ++r)
         if (chunk_indptr[r + 1] < chunk_indptr[r]) return COMB_ERR_INVALID;
-    if (chunk_indptr[R] > 0 && !chunk_ids) return COMB_ERR_INVALID;
-    // pass 1: lookups + sizes (nothing is written if any id is unknown)
+    const int64_t E = chunk_indptr[R];
+    if (E > 0 && !chunk_ids) return COMB_ERR_INVALID;
+    // pass 1: lookups + sizes (nothing is written if any id is unknown); distinct chunks in order of first appearance
     int64_t total_pages = 0, total_tiles = 0, total_tok = 0;
     int32_t max_pages = 0;
-    std::vector<const Chunk *> found((size_t)chunk_indptr[R]);  // one directory lookup per linked chunk
-    for (int32_t r = 0; r < R; ++r) {
-        int64_t pr = 0;
-        for (int32_t e = chunk_indptr[r]; e < chunk_indptr[r + 1]; ++e) {
-            auto it = p->dir.find(chunk_ids[e]);
-            if (it == p->dir.end()) return COMB_ERR_UNKNOWN_CHUNK;
-            found[(size_t)e] = &it->second;
-            pr += (int64_t)it->second.pages.size();
-            total_tok += it->second.num_tokens;
+    std::vector<const Chunk *> found((size_t)E);  // one directory lookup per entry
+    std::vector<int32_t> ent_slot((size_t)E);     // entry -> distinct index (first-appearance order for now)
+    std::vector<const Chunk *> distinct;
+    std::vector<int32_t> drows;
+    {
+        std::unordered_map<const Chunk *, int32_t> seen;
+        seen.reserve((size_t)E * 2 + 8);
+        for (int32_t r = 0; r < R; ++r) {
+            int64_t pr = 0;
+            for (int32_t e = chunk_indptr[r]; e < chunk_indptr[r + 1]; ++e) {
+                auto it = p->dir.find(chunk_ids[e]);
+                if (it == p->dir.end()) return COMB_ERR_UNKNOWN_CHUNK;
+                const Chunk *c = &it->second;
+                found[(size_t)e] = c;
+                pr += (int64_t)c->pages.size();
+                total_tok += c->num_tokens;
+                auto ins = seen.emplace(c, (int32_t)distinct.size());
+                if (ins.second) {
+                    distinct.push_back(c);
+                    drows.push_back(0);
+                }
+                ent_slot[(size_t)e] = ins.first->second;
+                drows[(size_t)ins.first->second] += 1;
+            }
+            if (pr > INT32_MAX / kPage) return COMB_ERR_CAPACITY;
+            total_pages += pr;
+            total_tiles += (pr + kTilePages - 1) / kTilePages;
+            max_pages = std::max<int32_t>(max_pages, (int32_t)pr);
         }
-        if (pr > INT32_MAX / kPage) return COMB_ERR_CAPACITY;
-        total_pages += pr;
-        total_tiles += (pr + kTilePages - 1) / kTilePages;
-        max_pages = std::max<int32_t>(max_pages, (int32_t)pr);
     }
     if (total_pages > INT32_MAX) return COMB_ERR_CAPACITY;
-    const LinkLayout L = link_layout(R, total_pages, total_tiles);
+    // slots: distinct chunks by descending entry count, ties by first appearance
+    const int32_t U = (int32_t)distinct.size();
+    std::vector<int32_t> slot_of((size_t)U), by_slot((size_t)U);
+    for (int32_t i = 0; i < U; ++i) by_slot[(size_t)i] = i;
+    std::stable_sort(by_slot.begin(), by_slot.end(),
+                     [&](int32_t a, int32_t b) { return drows[(size_t)a] > drows[(size_t)b]; });
+    int64_t distinct_pages = 0, distinct_tiles = 0, distinct_tok = 0;
+    for (int32_t u = 0; u < U; ++u) {
+        slot_of[(size_t)by_slot[(size_t)u]] = u;
+        const Chunk *c = distinct[(size_t)by_slot[(size_t)u]];
+        distinct_pages += (int64_t)c->pages.size();
+        distinct_tiles += ((int64_t)c->pages.size() + kTilePages - 1) / kTilePages;
+        distinct_tok += c->num_tokens;
+    }
+    const LinkLayout L = link_layout(R, E, U, total_pages, total_tiles, distinct_pages, distinct_tiles);
     if (L.bytes > link->device_bytes) return COMB_ERR_CAPACITY;
+    const size_t host_need = comb_link_host_bytes(R, U);
+    if (link->host_buf && link->host_bytes < host_need) return COMB_ERR_CAPACITY;
     // pass 2: write the tables
-    char *hb = (char *)host_buf;
+    char *hb = (char *)staging;
     int32_t *page_indptr = (int32_t *)(hb + L.off_page_indptr);
     int32_t *kv_len = (int32_t *)(hb + L.off_kv_len);
     int32_t *tile_indptr = (int32_t *)(hb + L.off_tile_indptr);
+    int32_t *entry_indptr = (int32_t *)(hb + L.off_entry_indptr);
     uint64_t *tile_ntok = (uint64_t *)(hb + L.off_tile_ntok);
     int32_t *page_ids = (int32_t *)(hb + L.off_page_ids);
     int32_t *page_ntok = (int32_t *)(hb + L.off_page_ntok);
@@ -489,45 +725,81 @@ int32_t comb_link_plan(const comb_pool_t *p, int32_t R, const int32_t *chunk_ind
         }
         kv_len[r] = (int32_t)kv;
         page_indptr[r + 1] = (int32_t)at;
-        for (int64_t t = begin; t < at; t += kTilePages) {
-            uint64_t packed = 0;
-            const int lim = (int)std::min<int64_t>(kTilePages, at - t);
-            for (int j = 0; j < lim; ++j) packed |= (uint64_t)page_ntok[t + j] << (8 * j);
-            tile_ntok[tile_at++] = packed;
-        }
+        for (int64_t t = begin; t < at; t += kTilePages) tile_ntok[tile_at++] = pack_tile_ntok(page_ntok, t, at);
         tile_indptr[r + 1] = (int32_t)tile_at;
+    }
+    memcpy(entry_indptr, chunk_indptr, sizeof(int32_t) * (size_t)(R + 1));
+    // chunk-major view
+    int32_t *cas_page_indptr = (int32_t *)(hb + L.off_cas_page_indptr);
+    int32_t *cas_tile_indptr = (int32_t *)(hb + L.off_cas_tile_indptr);
+    int32_t *cas_row_indptr = (int32_t *)(hb + L.off_cas_row_indptr);
+    uint64_t *cas_tile_ntok = (uint64_t *)(hb + L.off_cas_tile_ntok);
+    int32_t *cas_page_ids = (int32_t *)(hb + L.off_cas_page_ids);
+    int32_t *cas_row_req = (int32_t *)(hb + L.off_cas_row_req);
+    int32_t *cas_row_entry = (int32_t *)(hb + L.off_cas_row_entry);
+    cas_page_indptr[0] = cas_tile_indptr[0] = cas_row_indptr[0] = 0;
+    int32_t max_rows = 0;
+    {
+        int64_t pat = 0, tat = 0;
+        std::vector<int32_t> ntok_tmp;
+        for (int32_t u = 0; u < U; ++u) {
+            const Chunk &c = *distinct[(size_t)by_slot[(size_t)u]];
+            const int32_t np = (int32_t)c.pages.size();
+            memcpy(cas_page_ids + pat, c.pages.data(), (size_t)np * sizeof(int32_t));
+            ntok_tmp.assign((size_t)np, (int32_t)kPage);
+            ntok_tmp[(size_t)np - 1] = c.num_tokens - kPage * (np - 1);
+            for (int64_t t = 0; t < np; t += kTilePages) cas_tile_ntok[tat++] = pack_tile_ntok(ntok_tmp.data(), t, np);
+            pat += np;
+            cas_page_indptr[u + 1] = (int32_t)pat;
+            cas_tile_indptr[u + 1] = (int32_t)tat;
+            const int32_t rows = drows[(size_t)by_slot[(size_t)u]];
+            cas_row_indptr[u + 1] = cas_row_indptr[u] + rows;
+            max_rows = std::max(max_rows, rows);
+        }
+        // entries of a slot in ascending entry number (counting sort over the slots)
+        std::vector<int32_t> fill(cas_row_indptr, cas_row_indptr + U);
+        for (int32_t r = 0; r < R; ++r)
+            for (int32_t e = chunk_indptr[r]; e < chunk_indptr[r + 1]; ++e) {
+                const int32_t u = slot_of[(size_t)ent_slot[(size_t)e]];
+                cas_row_req[fill[(size_t)u]] = r;
+                cas_row_entry[fill[(size_t)u]] = e;
+                fill[(size_t)u] += 1;
+            }
     }
     char *db = (char *)link->device_buf;
     link->page_indptr = (int32_t *)(db + L.off_page_indptr);
     link->kv_len = (int32_t *)(db + L.off_kv_len);
     link->tile_indptr = (int32_t *)(db + L.off_tile_indptr);
+    link->entry_indptr = (int32_t *)(db + L.off_entry_indptr);
     link->tile_ntok = (uint64_t *)(db + L.off_tile_ntok);
     link->page_ids = (int32_t *)(db + L.off_page_ids);
     link->page_ntok = (int32_t *)(db + L.off_page_ntok);
+    link->cas_page_indptr = (int32_t *)(db + L.off_cas_page_indptr);
+    link->cas_tile_indptr = (int32_t *)(db + L.off_cas_tile_indptr);
+    link->cas_row_indptr = (int32_t *)(db + L.off_cas_row_indptr);
+    link->cas_tile_ntok = (uint64_t *)(db + L.off_cas_tile_ntok);
+    link->cas_page_ids = (int32_t *)(db + L.off_cas_page_ids);
+    link->cas_row_req = (int32_t *)(db + L.off_cas_row_req);
+    link->cas_row_entry = (int32_t *)(db + L.off_cas_row_entry);
+    link->host_req_pages = nullptr;
+    link->host_cas_rows = nullptr;
+    if (link->host_buf) {  // the host mirror: what the planners of the two attention calls read
+        link->host_req_pages = (int32_t *)link->host_buf;
+        link->host_cas_rows = (int32_t *)((char *)link->host_buf + align_up(sizeof(int32_t) * (size_t)std::max(R, 1), 16));
+        for (int32_t r = 0; r < R; ++r) link->host_req_pages[r] = page_indptr[r + 1] - page_indptr[r];
+        for (int32_t u = 0; u < U; ++u) link->host_cas_rows[u] = cas_row_indptr[u + 1] - cas_row_indptr[u];
+    }
     link->num_requests = R;
     link->max_pages_per_request = max_pages;
     link->total_pages = total_pages;
     link->total_tiles = total_tiles;
     link->total_kv_tokens = total_tok;
+    link->total_entries = E;
+    link->num_distinct_chunks = U;
+    link->max_rows_per_chunk = max_rows;
+    link->distinct_pages = distinct_pages;
+    link->distinct_kv_tokens = distinct_tok;
     link->bytes_used = L.bytes;
-    {   // remember the page count of every request of this link (host side of page_indptr), keyed by its device buffer
-        comb_pool_t *pm = const_cast<comb_pool_t *>(p);  // bookkeeping only: the directory and free list are untouched
-        comb_pool::LinkInfo *li = nullptr;
-        for (comb_pool::LinkInfo &x : pm->link_info)
-            if (x.device_buf == link->device_buf) li = &x;
-        if (!li) {
-            if (pm->link_info.size() < kLinkInfoSlots) {
-                pm->link_info.emplace_back();
-                li = &pm->link_info.back();
-            } else {
-                li = &pm->link_info[pm->link_info_next];
-                pm->link_info_next = (pm->link_info_next + 1) % kLinkInfoSlots;
-            }
-            li->device_buf = link->device_buf;
-        }
-        li->pages.resize((size_t)R);
-        for (int32_t r = 0; r < R; ++r) li->pages[(size_t)r] = page_indptr[r + 1] - page_indptr[r];
-    }
     return COMB_OK;
 }
 
@@ -548,26 +820,41 @@ int32_t comb_link(comb_pool_t *p, int32_t R, const int32_t *chunk_indptr, const 
     return COMB_OK;
 }
 
+int32_t comb_pool_set_option(comb_pool_t *p, int32_t option, int64_t value) {
+    if (!p) return COMB_ERR_INVALID;
+    if (option == COMB_OPT_DECODE_PATH) {
+        if (value != COMB_DECODE_AUTO && value != COMB_DECODE_PER_REQUEST && value != COMB_DECODE_CHUNK_MAJOR)
+            return COMB_ERR_INVALID;
+        p->opt_decode_path = value;
+        return COMB_OK;
+    }
+    return COMB_ERR_INVALID;
+}
+
 size_t comb_workspace_bytes(const comb_pool_t *p, int32_t R, int32_t Hq, int64_t total_q, int32_t max_pages) {
     if (!p || R < 0 || Hq <= 0 || total_q < 0 || max_pages < 0) return 0;
-    const_cast<comb_pool_t *>(p)->probe_device();
-    const DecodePlan plan = make_decode_plan(R, p->cfg.num_kv_heads, max_pages, p->num_sms);
-    const size_t dec = decode_workspace_bytes(R, Hq, p->cfg.head_dim_v, plan);
-    // prefill: one item per (request, kv-head, pair of 128-row tiles); rows per tile = 128 / G tokens
+    const_cast<comb_pool_t *>(p)->probe_device();  // caches the SM count; the directory and free list are untouched
     const int G = std::max(1, Hq / p->cfg.num_kv_heads);
-    // an item covers one or two 128-row tiles (prefill_tiles_per_cta): bound the item count from both sides
-    const int tok_per_tile = 128 / std::min(G, 128);
-    const size_t items_hi = ((size_t)total_q / tok_per_tile + (size_t)R + 1) * p->cfg.num_kv_heads;
-    const size_t items_lo = ((size_t)total_q + 2 * tok_per_tile - 1) / (2 * tok_per_tile) * p->cfg.num_kv_heads;
-    // the planner sees the exact item count at call time; bound its answer over every count this shape allows
-    const int max_tiles = (max_pages + kTilePages - 1) / kTilePages;
-    int nsplit = 1;
-    for (size_t n = std::max<size_t>(items_lo, 1); n <= items_hi; n += (size_t)p->cfg.num_kv_heads)
-        nsplit = std::max(nsplit, plan_prefill_splits(n, max_tiles, p->num_sms, prefill_max_splits()));
-    if (prefill_max_splits() > 1 && max_tiles >= 4) nsplit = std::max(nsplit, 4);  // last-wave ranges (up to 4)
-    const size_t pre = align_up(items_hi * (size_t)nsplit * sizeof(PrefillItem), 256) +
-                       (nsplit > 1 ? prefill_partial_bytes(nsplit, total_q, Hq, p->cfg.head_dim_v) : 0);
+    const DecodePlan plan =
+        make_decode_plan(R, p->cfg.num_kv_heads * decode_head_subgroups(G), max_pages, p->num_sms);
+    const size_t dec = decode_workspace_bytes(R, Hq, p->cfg.head_dim_v, plan);
+    size_t max_items = 0;
+    int64_t max_rows = 0;
+    prefill_bounds(p, Hq, total_q, &max_items, &max_rows);
+    const size_t pre = prefill_items_bytes(max_items) + prefill_part_bytes(max_rows, p->cfg.head_dim_v);
     return align_up(std::max(dec, pre), 256) + 256;
+}
+
+size_t comb_attn_workspace_bytes(const comb_pool_t *p, const comb_link_t *link, int32_t Hq, int64_t total_q) {
+    if (!p || !link || Hq <= 0 || total_q < 0) return 0;
+    size_t need = comb_workspace_bytes(p, link->num_requests, Hq, total_q, link->max_pages_per_request);
+    const int G = std::max(1, Hq / p->cfg.num_kv_heads);
+    if (link->host_cas_rows && G <= 128) {
+        const size_t cas = cascade_tiles_bytes(cascade_tile_count(link, G)) +
+                           cascade_partial_bytes(link->total_entries, Hq, p->cfg.head_dim_v);
+        need = std::max(need, align_up(cas, 256) + 256);
+    }
+    return need;
 }
 
 int32_t comb_cross_attn_decode(comb_pool_t *p, int32_t layer, const comb_link_t *link, int32_t R, const void *q,
@@ -583,12 +870,59 @@ int32_t comb_cross_attn_decode(comb_pool_t *p, int32_t layer, const comb_link_t 
     const int G = Hq / p->cfg.num_kv_heads;
     if (!decode_supported(G, p->cfg.head_dim_qk, p->cfg.head_dim_v)) return COMB_ERR_INVALID;
     p->probe_device();
-    const DecodePlan plan = make_decode_plan(R, p->cfg.num_kv_heads, link->max_pages_per_request, p->num_sms);
+    cudaStream_t st = (cudaStream_t)stream;
+    // ---- which path: chunk-major when the batch shares chunks (or when told to), else per request
+    const bool can_cascade = link->host_cas_rows && link->cas_page_indptr && link->entry_indptr &&
+                             prefill_supported(G, p->cfg.head_dim_qk, p->cfg.head_dim_v);
+    bool cascade = false;
+    if (p->opt_decode_path == COMB_DECODE_CHUNK_MAJOR) {
+        if (!can_cascade) return COMB_ERR_INVALID;
+        cascade = true;
+    } else if (p->opt_decode_path == COMB_DECODE_AUTO && can_cascade) {
+        cascade = link->total_entries * 4 >= (int64_t)link->num_distinct_chunks * 5 && link->total_entries > 0;
+    }
+    if (cascade) {
+        std::vector<CascadeTile> tiles;
+        int32_t rc = plan_cascade(link, G, &tiles);
+        if (rc != COMB_OK) return rc;
+        const size_t tiles_bytes = cascade_tiles_bytes(tiles.size());
+        const size_t need = tiles_bytes + cascade_partial_bytes(link->total_entries, Hq, p->cfg.head_dim_v);
+        if (!ws || ws_bytes < need || (((uintptr_t)ws) & 15)) {
+            if (p->opt_decode_path == COMB_DECODE_CHUNK_MAJOR) return COMB_ERR_CAPACITY;
+            cascade = false;  // a workspace sized by the link-independent bound: take the per-request path
+        } else {
+            if (!p->kv_maps_ready) {
+                if (prefill_encode_kv_maps(p->geom, &p->k_map, &p->v_map) != cudaSuccess) return COMB_ERR_CUDA;
+                p->kv_maps_ready = true;
+            }
+            PrefillMaps maps;
+            maps.k = p->k_map;
+            maps.v = p->v_map;
+            maps.q = p->k_map;
+            if (!tiles.empty()) {
+                const int slot = p->acquire(tiles.size() * sizeof(CascadeTile));
+                if (slot < 0) return COMB_ERR_CUDA;
+                memcpy(p->ring[slot].host, tiles.data(), tiles.size() * sizeof(CascadeTile));
+                if (cudaMemcpyAsync(ws, p->ring[slot].host, tiles.size() * sizeof(CascadeTile), cudaMemcpyHostToDevice,
+                                    st) != cudaSuccess)
+                    return COMB_ERR_CUDA;
+                if (!p->release(slot, st)) return COMB_ERR_CUDA;
+            }
+            int launches = 0;
+            cudaError_t e = launch_decode_cascade(p->geom, layer, view_of(link), maps, (const CascadeTile *)ws,
+                                                  (int)tiles.size(), R, Hq, q, scale, out, lse, link->total_entries,
+                                                  (char *)ws + tiles_bytes, p->num_sms, st, &launches, p->active_hook());
+            p->launches += launches;
+            return e == cudaSuccess ? COMB_OK : COMB_ERR_CUDA;
+        }
+    }
+    const DecodePlan plan = make_decode_plan(R, p->cfg.num_kv_heads * decode_head_subgroups(G),
+                                             link->max_pages_per_request, p->num_sms);
     const size_t need = decode_workspace_bytes(R, Hq, p->cfg.head_dim_v, plan);
     if (need > 0 && (!ws || ws_bytes < need)) return COMB_ERR_CAPACITY;
     int launches = 0;
-    cudaError_t e = launch_decode(p->geom, layer, view_of(link), R, Hq, q, scale, out, lse, ws, plan,
-                                  (cudaStream_t)stream, &launches, p->active_hook());
+    cudaError_t e = launch_decode(p->geom, layer, view_of(link), R, Hq, q, scale, out, lse, ws, plan, st, &launches,
+                                  p->active_hook());
     p->launches += launches;
     return e == cudaSuccess ? COMB_OK : COMB_ERR_CUDA;
 }
@@ -610,86 +944,15 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     if (!q || !out || !link->page_indptr) return COMB_ERR_INVALID;
     const int Hkv = p->cfg.num_kv_heads, G = Hq / Hkv;
     if (!prefill_supported(G, p->cfg.head_dim_qk, p->cfg.head_dim_v)) return COMB_ERR_INVALID;
-    // ---- work items: (request, kv-head, pair of Q tiles); the 2*Hkv.. items of one request sit together so
-    // CTAs that stream the same K/V run at the same time (L2 reuse). Requests are ordered longest KV first
-    // so the tail of the grid is made of short items.
-    int64_t max_lq = 0;
-    for (int32_t r = 0; r < R; ++r) max_lq = std::max<int64_t>(max_lq, q_indptr[r + 1] - q_indptr[r]);
-    const std::vector<int32_t> *req_pages = p->find_link_pages(link->device_buf, R);
-    int64_t nonempty = 0;
-    for (int32_t r = 0; r < R; ++r) nonempty += q_indptr[r + 1] > q_indptr[r];
     p->probe_device();
-    const int tiles_per_cta = prefill_tiles_per_cta(G, p->cfg.head_dim_qk, p->cfg.head_dim_v, max_lq, nonempty * Hkv,
-                                                    p->num_sms);
-    const int tok_per_tile = 128 / G, tok_per_item = tiles_per_cta * tok_per_tile;
-    // ---- work items: (request, kv-head, one or two Q tiles) against the request's KV, or against a range of it.
-    // Requests are ordered by work (query rows x KV tiles when the link's page counts are known on the host, i.e.
-    // the link came from comb_link of this pool; else query rows) so the tail of the persistent grid is made of
-    // short items; the kv-heads of one Q tile group sit together so CTAs that stream the same K/V run at the same
-    // time (L2 reuse).
-    auto tiles_of = [&](int32_t r) {
-        return req_pages ? ((*req_pages)[(size_t)r] + kTilePages - 1) / kTilePages : 1;
-    };
-    struct Req { int32_t r; int64_t rows, cost; };
-    std::vector<Req> order;
-    order.reserve(R);
-    for (int32_t r = 0; r < R; ++r) {
-        const int64_t rows = (int64_t)q_indptr[r + 1] - q_indptr[r];
-        order.push_back(Req{r, rows, rows * std::max(1, tiles_of(r))});
-    }
-    std::stable_sort(order.begin(), order.end(), [](const Req &a, const Req &b) { return a.cost > b.cost; });
-    std::vector<PrefillItem> base;
-    for (const Req &x : order)
-        for (int64_t t = 0; t < x.rows; t += tok_per_item)
-            for (int g = 0; g < Hkv; ++g)
-                base.push_back(PrefillItem{x.r, g, q_indptr[x.r] + (int32_t)t,
-                                           (int32_t)std::min<int64_t>(tok_per_item, x.rows - t), 0,
-                                           INT32_MAX / kTilePages, -1, 0});
-    if (base.empty()) return COMB_OK;
-    // ---- KV ranges (need the page counts): (1) fewer items than SMs: every request is cut so that items x ranges
-    // fill one wave; (2) several waves with a last wave at most half full: only the items of that last wave are cut
-    // (by up to 4), so it takes a fraction of an item's time instead of a whole one (cfg 4: 512 items on 148 SMs).
-    const int max_tiles = (link->max_pages_per_request + kTilePages - 1) / kTilePages;
-    const size_t ctas = (size_t)p->num_sms * (size_t)prefill_ctas_per_sm(tiles_per_cta, p->cfg.head_dim_qk,
-                                                                          p->cfg.head_dim_v);
-    int uniform = 1, tail_factor = 1;
-    size_t tail_from = base.size();
-    if (req_pages) {
-        // (one item per SM is the target even when two single-tile CTAs share an SM: measured, 256 ranges on 148
-        // SMs were slower than 128)
-        uniform = plan_prefill_splits(base.size(), max_tiles, p->num_sms, prefill_max_splits());
-        const size_t tail = base.size() % ctas;
-        if (uniform == 1 && base.size() > ctas && tail > 0 && 2 * tail <= ctas && prefill_max_splits() > 1) {
-            tail_factor = (int)std::min<size_t>(4, ctas / tail);
-            tail_from = base.size() - tail;
-        }
-    }
-    std::vector<PrefillItem> items;
-    items.reserve(base.size() * (size_t)std::max(uniform, 1) + (base.size() - tail_from) * (size_t)tail_factor);
-    int nsplit = 1;
-    for (size_t i = 0; i < base.size(); ++i) {
-        const int want = i >= tail_from ? tail_factor : uniform;
-        const int n_kv = want > 1 ? tiles_of(base[i].request) : 0;
-        const int tps = want > 1 ? std::max(2, prefill_tiles_per_split(n_kv, want)) : 0;  // >= 2 tiles per range
-        const int eff = tps > 0 ? (n_kv + tps - 1) / tps : 1;
-        if (eff <= 1) {
-            items.push_back(base[i]);
-            continue;
-        }
-        nsplit = std::max(nsplit, eff);
-        for (int sidx = 0; sidx < eff; ++sidx) {
-            PrefillItem it = base[i];
-            it.kv_tile0 = sidx * tps;
-            it.kv_tiles = tps;
-            it.split = sidx;
-            items.push_back(it);
-        }
-    }
-    const size_t num_items = items.size();
+    PrefillPlan plan;
+    int32_t rc = plan_prefill(p, link, R, q_indptr, Hq, &plan);
+    if (rc != COMB_OK) return rc;
+    const size_t num_items = plan.items.size();
+    if (num_items == 0) return COMB_OK;
     if (num_items > (size_t)INT32_MAX) return COMB_ERR_CAPACITY;
-    const size_t items_bytes = align_up(num_items * sizeof(PrefillItem), 256);
-    const size_t part_bytes = nsplit > 1 ? prefill_partial_bytes(nsplit, total_q, Hq, p->cfg.head_dim_v) : 0;
-    const size_t need = items_bytes + part_bytes;
+    const size_t items_bytes = prefill_items_bytes(num_items);
+    const size_t need = items_bytes + prefill_part_bytes(plan.part_rows, p->cfg.head_dim_v);
     if (!ws || ws_bytes < need || (((uintptr_t)ws) & 15)) return COMB_ERR_CAPACITY;
     cudaStream_t st = (cudaStream_t)stream;
     if (!p->kv_maps_ready) {
@@ -703,15 +966,13 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     const int slot = p->acquire(num_items * sizeof(PrefillItem));
     if (slot < 0) return COMB_ERR_CUDA;
     PrefillItem *h = (PrefillItem *)p->ring[slot].host;
-    memcpy(h, items.data(), num_items * sizeof(PrefillItem));
+    memcpy(h, plan.items.data(), num_items * sizeof(PrefillItem));
     if (cudaMemcpyAsync(ws, h, num_items * sizeof(PrefillItem), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return COMB_ERR_CUDA;
-    if (p->prof_on) p->hook.begin(p, kKernelPrefill, st);
     int launches = 0;
     cudaError_t e = launch_prefill(p->geom, layer, view_of(link), maps, (const PrefillItem *)ws, (int)num_items, Hq,
-                                   scale, out, lse, nsplit, total_q, (char *)ws + items_bytes, tiles_per_cta,
-                                   p->num_sms, st, &launches);
-    if (p->prof_on) p->hook.end(p, st);
+                                   scale, out, lse, total_q, (char *)ws + items_bytes, plan.part_rows,
+                                   plan.tiles_per_cta, p->num_sms, st, &launches, p->active_hook());
     if (e != cudaSuccess) return COMB_ERR_CUDA;
     p->launches += launches;
     if (!p->release(slot, st)) return COMB_ERR_CUDA;

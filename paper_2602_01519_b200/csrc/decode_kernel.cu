@@ -35,6 +35,8 @@ struct DecodeArgs {
     float *part_o;       // [R][Hq][S][Dv]
     float *part_ml;      // [R][Hq][S][2]  (m in log2 units, l)
     int num_q_heads, num_kv_heads, chunk_pages, num_splits;
+    int group;   // Hq / Hkv (q heads per kv head)
+    int hsub;    // head sub-groups per kv head: a CTA owns G = group / hsub consecutive q heads (hsub > 1 for group 8, 16)
     float scale_log2;  // scale * log2(e)
 };
 
@@ -84,7 +86,12 @@ template <int G, int DQK, int DV>
 __global__ void __launch_bounds__(kThreads, 2) decode_split_kernel(const DecodeArgs a) {
     using C = Cfg<G, DQK, DV>;
     extern __shared__ __align__(128) unsigned char smem[];
-    const int split = blockIdx.x, g = blockIdx.y, r = blockIdx.z;
+    // 1-D grid over (request, kv-head, head sub-group, split), split fastest (no 65535 limit on any factor)
+    const int split = blockIdx.x % a.num_splits;
+    const int gy = (blockIdx.x / a.num_splits) % (a.num_kv_heads * a.hsub);
+    const int r = blockIdx.x / (a.num_splits * a.num_kv_heads * a.hsub);
+    const int g = gy / a.hsub;                          // kv head: whose K/V blocks are streamed
+    const int head0 = g * a.group + (gy % a.hsub) * G;  // first of this CTA's G query heads
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int sub = lane & 7, kg = lane >> 3;
     const int Hq = a.num_q_heads;
@@ -94,8 +101,8 @@ __global__ void __launch_bounds__(kThreads, 2) decode_split_kernel(const DecodeA
     if (npages_r == 0) {  // no contexts linked: zero contribution, lse = -inf (reading I13)
         if (split == 0) {
             for (int e = tid; e < G * DV; e += kThreads)
-                a.out[((size_t)r * Hq + g * G + e / DV) * DV + e % DV] = __float2bfloat16_rn(0.f);
-            if (a.lse && tid < G) a.lse[(size_t)r * Hq + g * G + tid] = -INFINITY;
+                a.out[((size_t)r * Hq + head0 + e / DV) * DV + e % DV] = __float2bfloat16_rn(0.f);
+            if (a.lse && tid < G) a.lse[(size_t)r * Hq + head0 + tid] = -INFINITY;
         }
         return;
     }
@@ -122,7 +129,7 @@ __global__ void __launch_bounds__(kThreads, 2) decode_split_kernel(const DecodeA
     float2 q2[G][C::CK * 4];
 #pragma unroll
     for (int h = 0; h < G; ++h) {
-        const uint4 *qrow = reinterpret_cast<const uint4 *>(a.q + ((size_t)r * Hq + g * G + h) * DQK);
+        const uint4 *qrow = reinterpret_cast<const uint4 *>(a.q + ((size_t)r * Hq + head0 + h) * DQK);
 #pragma unroll
         for (int cc = 0; cc < C::CK; ++cc) {
             const uint4 w = qrow[cc * 8 + sub];
@@ -333,7 +340,7 @@ __global__ void __launch_bounds__(kThreads, 2) decode_split_kernel(const DecodeA
             o += wt * x;
             l += wt * l_w[w * G + h];
         }
-        const int hq = g * G + h;
+        const int hq = head0 + h;
         if (nsplit_r == 1) {
             a.out[((size_t)r * Hq + hq) * DV + d] = __float2bfloat16_rn(o / l);
             if (a.lse && d == 0) a.lse[(size_t)r * Hq + hq] = (m + log2f(l)) * kLn2;
@@ -351,7 +358,7 @@ __global__ void __launch_bounds__(kThreads, 2) decode_split_kernel(const DecodeA
 // pass 2: out = sum_s e^{m_s - m} o_s / sum_s e^{m_s - m} l_s ; lse = ln2 * (m + log2 l)
 template <int DV>
 __global__ void __launch_bounds__(DV) decode_merge_kernel(const DecodeArgs a) {
-    const int hq = blockIdx.x, r = blockIdx.y, d = threadIdx.x;
+    const int hq = blockIdx.x % a.num_q_heads, r = blockIdx.x / a.num_q_heads, d = threadIdx.x;
     const int npages_r = a.page_indptr[r + 1] - a.page_indptr[r];
     const int nsplit_r = (npages_r + a.chunk_pages - 1) / a.chunk_pages;
     if (nsplit_r <= 1) return;  // written by pass 1
@@ -374,7 +381,7 @@ cudaError_t launch_t(const DecodeArgs &a, int R, bool merge, cudaStream_t st, in
     auto kern = decode_split_kernel<G, DQK, DV>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     if (e != cudaSuccess) return e;
-    dim3 grid(a.num_splits, a.num_kv_heads, R);
+    const unsigned grid = (unsigned)((size_t)a.num_splits * a.num_kv_heads * a.hsub * R);
     if (hook) hook->begin(hook->ctx, kKernelDecodeSplit, st);
     kern<<<grid, kThreads, C::SMEM, st>>>(a);
     if (hook) hook->end(hook->ctx, st);
@@ -382,7 +389,7 @@ cudaError_t launch_t(const DecodeArgs &a, int R, bool merge, cudaStream_t st, in
     *launches += 1;
     if (merge) {
         if (hook) hook->begin(hook->ctx, kKernelDecodeMerge, st);
-        decode_merge_kernel<DV><<<dim3(a.num_q_heads, R), DV, 0, st>>>(a);
+        decode_merge_kernel<DV><<<(unsigned)((size_t)a.num_q_heads * R), DV, 0, st>>>(a);
         if (hook) hook->end(hook->ctx, st);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         *launches += 1;
@@ -392,11 +399,15 @@ cudaError_t launch_t(const DecodeArgs &a, int R, bool merge, cudaStream_t st, in
 
 }  // namespace
 
+// Every group size prefill accepts (powers of two up to 16): groups of 8 and 16 heads run as 2 or 4 sub-groups of
+// 4 heads, each its own CTA streaming the same K/V blocks (the second read is an L2 hit).
 bool decode_supported(int group, int dqk, int dv) {
     const bool dims = (dqk == 64 || dqk == 128 || dqk == 192) && (dv == 64 || dv == 128);
-    return dims && (group == 1 || group == 2 || group == 4);
+    return dims && group >= 1 && group <= 16 && (group & (group - 1)) == 0;
 }
+int decode_head_subgroups(int group) { return group > 4 ? group / 4 : 1; }
 
+// `Hkv` here counts the CTA columns per request: kv heads x head sub-groups.
 DecodePlan make_decode_plan(int R, int Hkv, int max_pages, int num_sms) {
     DecodePlan p;
     if (max_pages <= 0 || R <= 0) {
@@ -449,13 +460,15 @@ cudaError_t launch_decode(const PoolGeom &g, int layer, const LinkView &lv, int 
     a.lse = lse;
     a.num_q_heads = Hq;
     a.num_kv_heads = g.num_kv_heads;
+    a.group = Hq / g.num_kv_heads;
+    a.hsub = decode_head_subgroups(a.group);
     a.chunk_pages = p.chunk_pages;
     a.num_splits = p.num_splits;
     a.scale_log2 = scale * kLog2e;
     a.part_o = (float *)workspace;
     a.part_ml = a.part_o ? a.part_o + (size_t)R * Hq * p.num_splits * g.head_dim_v : nullptr;
     const bool merge = p.num_splits > 1;
-    const int G = Hq / g.num_kv_heads;
+    const int G = a.group / a.hsub;  // heads per CTA
 #define COMB_DECODE_CASE(GG, DQ, DVV) \
     if (G == GG && g.head_dim_qk == DQ && g.head_dim_v == DVV) return launch_t<GG, DQ, DVV>(a, R, merge, stream, launches, hook);
     COMB_DECODE_CASE(4, 128, 128)

@@ -25,7 +25,8 @@ struct LaunchHook {
     void (*end)(void *ctx, cudaStream_t st);
     void *ctx;
 };
-enum { kKernelStore = 0, kKernelDecodeSplit = 1, kKernelDecodeMerge = 2, kKernelPrefill = 3 };
+enum { kKernelStore = 0, kKernelDecodeSplit = 1, kKernelDecodeMerge = 2, kKernelPrefill = 3, kKernelDecodeCascade = 4,
+       kKernelCascadeMerge = 5, kKernelPrefillMerge = 6, kNumKernelIds = 7 };
 
 struct PoolGeom {
     int32_t num_layers, num_kv_heads, head_dim_qk, head_dim_v, num_pages;
@@ -36,20 +37,29 @@ struct PoolGeom {
 struct LinkView {
     const int32_t *page_indptr, *page_ids, *page_ntok, *kv_len, *tile_indptr;
     const uint64_t *tile_ntok;
+    // chunk-major view (distinct chunks as slots) + the entries of every request
+    const int32_t *entry_indptr, *cas_page_indptr, *cas_page_ids, *cas_tile_indptr;
+    const uint64_t *cas_tile_ntok;
+    const int32_t *cas_row_indptr, *cas_row_req, *cas_row_entry;
 };
 
 // ---- (a2) store -------------------------------------------------------------------------------
 cudaError_t launch_store(const PoolGeom &g, int layer, const StorePageDesc *descs_dev, int num_descs,
                          const void *k_src, const void *v_src, cudaStream_t stream);
 
+// read-only HBM stream over `bytes` bytes (measurement utility; `sink` = 4 device bytes)
+cudaError_t launch_stream_read(const void *src, size_t bytes, void *sink, cudaStream_t stream);
+
 // ---- (a5) decode ------------------------------------------------------------------------------
 struct DecodePlan {
     int chunk_pages;   // table entries per split (multiple of the warps per CTA)
     int num_splits;    // splits of the longest request
 };
-DecodePlan make_decode_plan(int num_requests, int num_kv_heads, int max_pages_per_request, int num_sms);
+DecodePlan make_decode_plan(int num_requests, int cta_columns /* Hkv x head sub-groups */, int max_pages_per_request,
+                            int num_sms);
 size_t decode_workspace_bytes(int num_requests, int num_q_heads, int head_dim_v, const DecodePlan &p);
 bool decode_supported(int group, int dqk, int dv);
+int decode_head_subgroups(int group);  // CTAs per (request, kv-head, split): 1 for G <= 4, G/4 above
 // launches the split kernel and (if num_splits > 1) the merge kernel; *launches += kernels launched
 cudaError_t launch_decode(const PoolGeom &g, int layer, const LinkView &lv, int num_requests, int num_q_heads,
                           const void *q, float scale, void *out, float *lse, void *workspace, const DecodePlan &p,
@@ -65,18 +75,20 @@ struct PrefillItem {
     int32_t q_row0;     // first query token row (absolute row in q) of tile 0
     int32_t q_rows;     // valid query tokens in this item (1 .. 2*128/G)
     int32_t kv_tile0;   // first KV tile of this item (index inside the request)
-    int32_t kv_tiles;   // KV tiles of this item (clamped to the request's on the device)
+    int32_t kv_tiles;   // KV tiles of this item (clamped to the request's on the device; the last range is open-ended)
     int32_t split;      // -1: the item sees all of the request's KV and writes the final output; else its range index
+    int32_t tps;        // split >= 0: tiles per range of this request (the merge derives the range count from it)
+    int32_t part_base;  // split >= 0: first partial row of this item's ranges; range s, tile slot t, tile row i lives
+                        // at part_base + s * 256 + t * 128 + i
     int32_t pad;
 };
+constexpr int kPrefillMaxSplits = 16;
 // Splits of a request with n_kv tiles when the call uses `nsplit` ranges: ceil(n_kv / ceil(n_kv / nsplit)).
 inline int prefill_tiles_per_split(int n_kv, int nsplit) { return (n_kv + nsplit - 1) / nsplit; }
-int prefill_max_splits();  // 1 when the selected kernel cannot split (debug kernel), else 16
 // Q tiles per CTA (1 or 2) for a call whose longest request has max_q_tokens query tokens and that would have
 // num_items single-tile items; an item then covers up to that many 128-row tiles.
 int prefill_tiles_per_cta(int group, int dqk, int dv, int64_t max_q_tokens, int64_t num_items, int num_sms);
 int prefill_ctas_per_sm(int tiles_per_cta, int dqk, int dv);  // resident CTAs per SM of the kernel that choice selects
-size_t prefill_partial_bytes(int nsplit, int64_t total_q, int num_q_heads, int dv);
 bool prefill_supported(int group, int dqk, int dv);
 // CUtensorMap is 128 bytes, 64-byte aligned; kept opaque here so the runtime needs no cuda.h.
 struct alignas(64) TensorMapBlob { unsigned char bytes[128]; };
@@ -85,10 +97,26 @@ struct PrefillMaps { TensorMapBlob q, k, v; };
 cudaError_t prefill_encode_kv_maps(const PoolGeom &g, TensorMapBlob *k_map, TensorMapBlob *v_map);
 cudaError_t prefill_encode_q_map(const void *q, int64_t total_q, int num_q_heads, int group, int dqk,
                                  TensorMapBlob *q_map);
-// nsplit > 1: `partials` holds prefill_partial_bytes() bytes; a second kernel merges the ranges (*launches += 1).
+// part_rows > 0: some items are KV ranges; `partials` holds part_rows x (Dv + 1) floats and a second kernel merges
+// the ranges (*launches += 1).
 cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &maps,
                            const PrefillItem *items_dev, int num_items, int num_q_heads, float scale, void *out,
-                           float *lse, int nsplit, int64_t total_q, void *partials, int tiles_per_cta, int num_sms,
-                           cudaStream_t stream, int *launches);
+                           float *lse, int64_t total_q, void *partials, int64_t part_rows, int tiles_per_cta,
+                           int num_sms, cudaStream_t stream, int *launches, const LaunchHook *hook);
+
+// ---- (f1) chunk-major ("cascade") decode --------------------------------------------------------
+// One M tile of the chunk-major decode: `nrows` consecutive entries (query tokens) of chunk slot `slot`, starting at
+// position row0 of cas_row_req / cas_row_entry; each entry contributes G rows (the heads of one kv-head). A work
+// item of the kernel is (tile, kv-head).
+struct CascadeTile {
+    int32_t slot, row0, nrows, pad;
+};
+size_t cascade_partial_bytes(int64_t total_entries, int num_q_heads, int dv);
+// tcgen05 kernel over (tile, kv-head) items writing per-entry partials, then the per-request LSE merge.
+cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &maps,
+                                  const CascadeTile *tiles_dev, int num_tiles, int num_requests, int num_q_heads,
+                                  const void *q, float scale, void *out, float *lse, int64_t total_entries,
+                                  void *partials, int num_sms, cudaStream_t stream, int *launches,
+                                  const LaunchHook *hook);
 
 }  // namespace comb

@@ -74,7 +74,34 @@ store_pages_kernel(const StorePageDesc *__restrict__ descs, int num_units, uint4
     }
 }
 
+// Read-only stream: every thread keeps 8 independent 16-byte loads in flight and folds them into one word; the
+// measurement kernel behind comb_util_stream_read (bench.py's read-only HBM ceiling, SURVEY.md §8(d) "Denominators").
+__global__ void __launch_bounds__(256) stream_read_kernel(const uint4 *__restrict__ src, size_t n_vec,
+                                                          unsigned int *__restrict__ sink) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned int acc = 0;
+    for (; i + 7 * stride < n_vec; i += 8 * stride) {
+        uint4 v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = __ldcs(src + i + u * stride);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) acc ^= v[u].x ^ v[u].y ^ v[u].z ^ v[u].w;
+    }
+    for (; i < n_vec; i += stride) {
+        const uint4 v = __ldcs(src + i);
+        acc ^= v.x ^ v.y ^ v.z ^ v.w;
+    }
+    if (acc == 0x9e3779b9u) atomicXor(sink, acc);  // practically never true: keeps the loads alive without a store stream
+}
+
 }  // namespace
+
+cudaError_t launch_stream_read(const void *src, size_t bytes, void *sink, cudaStream_t stream) {
+    if (!src || !sink || bytes < 16) return cudaErrorInvalidValue;
+    stream_read_kernel<<<148 * 8, 256, 0, stream>>>((const uint4 *)src, bytes / 16, (unsigned int *)sink);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_store(const PoolGeom &g, int layer, const StorePageDesc *descs_dev, int num_descs, const void *k_src,
                          const void *v_src, cudaStream_t stream) {

@@ -21,30 +21,58 @@ def make_pool(num_pages=64, Hkv=2, Dqk=64, Dv=64, seed=0, layers=1):
     return comb.comb_pool_create(cfg)
 
 
-def plan(pool, lists):
+def plan(pool, lists, host_mirror=True):
     indptr = np.zeros(len(lists) + 1, np.int32)
     np.cumsum([len(x) for x in lists], out=indptr[1:])
     ids = np.array([c for l in lists for c in l], np.uint64)
     total = sum(len(comb.comb_chunk_query(pool, int(c))[1]) for c in ids)
-    nbytes = comb.comb_link_bytes(len(lists), total)
+    nbytes = comb.comb_link_bytes(len(lists), len(ids), total)
     host = np.zeros(nbytes, np.uint8)
+    mirror = np.zeros(comb.comb_link_host_bytes(len(lists), len(ids)), np.uint8) if host_mirror else None
     link = comb.Link()
-    link.device_buf = 0x10000  # layout base only; comb_link_plan writes into host_buf
+    link.device_buf = 0x10000  # layout base only; comb_link_plan writes into the staging array
     link.device_bytes = nbytes
+    if host_mirror:
+        link.host_buf, link.host_bytes = mirror.ctypes.data, mirror.nbytes
     comb.comb_link_plan(pool, indptr, ids, link, host)
 
     def view(ptr, n, dt):
         off = ptr - 0x10000
         return host[off:off + n * np.dtype(dt).itemsize].view(dt).copy()
-    R = len(lists)
-    return link, {
+    R, U, E = len(lists), int(link.num_distinct_chunks), int(link.total_entries)
+    tabs = {
         "page_indptr": view(link.page_indptr, R + 1, np.int32),
         "page_ids": view(link.page_ids, int(link.total_pages), np.int32),
         "page_ntok": view(link.page_ntok, int(link.total_pages), np.int32),
         "kv_len": view(link.kv_len, R, np.int32),
         "tile_indptr": view(link.tile_indptr, R + 1, np.int32),
         "tile_ntok": view(link.tile_ntok, int(link.total_tiles), np.uint64),
+        "entry_indptr": view(link.entry_indptr, R + 1, np.int32),
+        "cas_page_indptr": view(link.cas_page_indptr, U + 1, np.int32),
+        "cas_page_ids": view(link.cas_page_ids, int(link.distinct_pages), np.int32),
+        "cas_tile_indptr": view(link.cas_tile_indptr, U + 1, np.int32),
+        "cas_row_indptr": view(link.cas_row_indptr, U + 1, np.int32),
+        "cas_row_req": view(link.cas_row_req, E, np.int32),
+        "cas_row_entry": view(link.cas_row_entry, E, np.int32),
     }
+    tabs["cas_tile_ntok"] = view(link.cas_tile_ntok, int(tabs["cas_tile_indptr"][-1]), np.uint64)
+    if host_mirror:
+        o1, o2 = link.host_req_pages - mirror.ctypes.data, link.host_cas_rows - mirror.ctypes.data
+        tabs["host_req_pages"] = mirror[o1:o1 + 4 * R].view(np.int32).copy()
+        tabs["host_cas_rows"] = mirror[o2:o2 + 4 * U].view(np.int32).copy()
+    link._keepalive = (host, mirror)
+    return link, tabs
+
+
+def check_tiles(indptr, ntok, tile_indptr, tile_ntok):
+    """tile_ntok is page_ntok regrouped by 8 (derived; checked against its definition in comb.h)."""
+    for r in range(len(indptr) - 1):
+        pn = ntok[indptr[r]:indptr[r + 1]]
+        tiles = tile_ntok[tile_indptr[r]:tile_indptr[r + 1]]
+        assert len(tiles) == (len(pn) + 7) // 8
+        for t, packed in enumerate(tiles):
+            want = [int(x) for x in pn[8 * t:8 * t + 8]] + [0] * (8 - len(pn[8 * t:8 * t + 8]))
+            assert [(int(packed) >> (8 * j)) & 0xff for j in range(8)] == want
 
 
 def test_library_exports_every_declared_symbol():
@@ -114,14 +142,26 @@ def test_allocator_and_tables_match_oracle_model(seed):
     exp = model.link(lists)
     for key in ("page_indptr", "page_ids", "page_ntok", "kv_len"):
         assert np.array_equal(got[key], exp[key]), key
-    # tile_ntok is page_ntok regrouped by 8 (derived; checked against its definition)
-    for r in range(len(lists)):
-        pn = exp["page_ntok"][exp["page_indptr"][r]:exp["page_indptr"][r + 1]]
-        tiles = got["tile_ntok"][got["tile_indptr"][r]:got["tile_indptr"][r + 1]]
-        assert len(tiles) == (len(pn) + 7) // 8
-        for t, packed in enumerate(tiles):
-            want = [int(x) for x in pn[8 * t:8 * t + 8]] + [0] * (8 - len(pn[8 * t:8 * t + 8]))
-            assert [(int(packed) >> (8 * j)) & 0xff for j in range(8)] == want
+    check_tiles(exp["page_indptr"], exp["page_ntok"], got["tile_indptr"], got["tile_ntok"])
+    # chunk-major view of the same batch, bit-exact against the model's independent inversion
+    cm = model.link_chunk_major(lists)
+    for key in ("entry_indptr", "cas_page_indptr", "cas_page_ids", "cas_row_indptr", "cas_row_req", "cas_row_entry"):
+        assert np.array_equal(got[key], cm[key]), key
+    check_tiles(cm["cas_page_indptr"], cm["cas_page_ntok"], got["cas_tile_indptr"], got["cas_tile_ntok"])
+    assert link.num_distinct_chunks == len(cm["slot_chunks"]) and link.total_entries == len(cm["cas_row_req"])
+    assert link.distinct_pages == len(cm["cas_page_ids"])
+    assert link.distinct_kv_tokens == sum(lens[int(c)] for c in cm["slot_chunks"])
+    assert link.max_rows_per_chunk == (int(np.diff(cm["cas_row_indptr"]).max()) if len(cm["slot_chunks"]) else 0)
+    # every entry appears exactly once, under the slot of its chunk, with its request
+    flat = [int(c) for l in lists for c in l]
+    assert sorted(got["cas_row_entry"].tolist()) == list(range(len(flat)))
+    for u, c in enumerate(cm["slot_chunks"]):
+        for x in range(cm["cas_row_indptr"][u], cm["cas_row_indptr"][u + 1]):
+            e = int(got["cas_row_entry"][x])
+            assert flat[e] == int(c) and got["entry_indptr"][got["cas_row_req"][x]] <= e < got["entry_indptr"][got["cas_row_req"][x] + 1]
+    # host mirror = what the planners read
+    assert np.array_equal(got["host_req_pages"], np.diff(exp["page_indptr"]))
+    assert np.array_equal(got["host_cas_rows"], np.diff(cm["cas_row_indptr"]))
     assert link.total_kv_tokens == int(exp["kv_len"].sum())
     assert link.max_pages_per_request == int(np.diff(exp["page_indptr"]).max())
     comb.comb_pool_destroy(pool)
@@ -151,9 +191,11 @@ def test_error_paths():
     link = comb.Link()
     link.device_buf, link.device_bytes = 0x10000, 4096
     host = np.full(4096, 0xAB, np.uint8)
+    mirror = np.full(64, 0xCD, np.uint8)
+    link.host_buf, link.host_bytes = mirror.ctypes.data, mirror.nbytes
     with pytest.raises(comb.CombError) as e:
         comb.comb_link_plan(pool, np.array([0, 2], np.int32), np.array([1, 42], np.uint64), link, host)
-    assert e.value.status == comb.COMB_ERR_UNKNOWN_CHUNK and np.all(host == 0xAB)
+    assert e.value.status == comb.COMB_ERR_UNKNOWN_CHUNK and np.all(host == 0xAB) and np.all(mirror == 0xCD)
     link.device_bytes = 16                                  # too small
     with pytest.raises(comb.CombError) as e:
         comb.comb_link_plan(pool, np.array([0, 1], np.int32), np.array([1], np.uint64), link, host)
@@ -176,10 +218,27 @@ def test_product_does_not_import_oracle():
                 assert "comb_oracle" not in src and "_work/" not in src, f
 
 
+def _prefill_status(pool, Hq, lists, lq, lens, ws_bytes=None, mirror=True):
+    """Plans a link on the host and calls comb_cross_attn_prefill with fake device pointers: without a GPU the call
+    stops at its first CUDA call (COMB_ERR_CUDA), but only after planning and the capacity check."""
+    R = len(lists)
+    q_indptr = np.zeros(R + 1, np.int32)
+    np.cumsum(lq, out=q_indptr[1:])
+    link, tabs = plan(pool, lists, host_mirror=mirror)
+    link.device_buf = 0x7300_0000_0000
+    total_q = int(q_indptr[-1])
+    bound_any = comb.comb_workspace_bytes(pool, R, Hq, total_q, int(link.max_pages_per_request))
+    bound_link = comb.comb_attn_workspace_bytes(pool, link, Hq, total_q)
+    assert bound_link >= bound_any > 0
+    st = _lib.lib.comb_cross_attn_prefill(pool, 0, C.byref(link), R, 0x7400_0000_0000, q_indptr.ctypes.data, Hq,
+                                          C.c_float(0.1), 0x7500_0000_0000, None, 0x7600_0000_0000,
+                                          bound_any if ws_bytes is None else ws_bytes, None)
+    return st, total_q
+
+
 def test_workspace_bound_covers_every_prefill_plan():
     """comb_workspace_bytes() must suffice for whatever the prefill planner decides (KV ranges for sub-wave calls,
-    last-wave ranges, one or two Q tiles per CTA). Without a GPU the calls below stop at their first CUDA call
-    (COMB_ERR_CUDA) — but only after the capacity check, so COMB_ERR_CAPACITY here means the bound is too small."""
+    last-wave ranges, one or two Q tiles per CTA): COMB_ERR_CAPACITY here means the bound is too small."""
     rng = np.random.default_rng(123)
     shapes = [(32, 8, 128, 128), (16, 16, 192, 128), (8, 2, 64, 64), (8, 8, 128, 64)]
     for trial in range(60):
@@ -194,26 +253,60 @@ def test_workspace_bound_covers_every_prefill_plan():
         lists = [list(rng.choice(n_chunks, size=int(rng.integers(0, min(n_chunks, 12) + 1)), replace=False))
                  for _ in range(R)]
         lq = rng.choice([0, 1, 7, 32, 33, 64, 128, 129, 300, 512], size=R)
-        q_indptr = np.zeros(R + 1, np.int32)
-        np.cumsum(lq, out=q_indptr[1:])
-        indptr = np.zeros(R + 1, np.int32)
-        np.cumsum([len(x) for x in lists], out=indptr[1:])
-        ids = np.array([c for l in lists for c in l], np.uint64)
-        total_pages = int(sum(((lens[c] + 15) // 16) for l in lists for c in l))
-        link = comb.Link()
-        link.device_buf = 0x7300_0000_0000
-        link.device_bytes = comb.comb_link_bytes(R, total_pages)
-        host = np.zeros(link.device_bytes, np.uint8)
-        comb.comb_link_plan(pool, indptr, ids, link, host)  # the host half of comb_link (tables + page counts)
-        total_q = int(q_indptr[-1])
-        ws_bytes = comb.comb_workspace_bytes(pool, R, Hq, total_q, int(link.max_pages_per_request))
-        st = _lib.lib.comb_cross_attn_prefill(pool, 0, C.byref(link), R, 0x7400_0000_0000, q_indptr.ctypes.data, Hq,
-                                              C.c_float(0.1), 0x7500_0000_0000, None, 0x7600_0000_0000, ws_bytes, None)
-        assert st != comb.COMB_ERR_CAPACITY, "trial %d: workspace bound %d too small" % (trial, ws_bytes)
+        st, total_q = _prefill_status(pool, Hq, lists, lq, lens)
+        assert st != comb.COMB_ERR_CAPACITY, "trial %d: workspace bound too small" % trial
         assert st in (comb.COMB_OK, comb.COMB_ERR_CUDA)
         if total_q > 0:  # and the check is really reached: a 16-byte workspace is refused
-            st = _lib.lib.comb_cross_attn_prefill(pool, 0, C.byref(link), R, 0x7400_0000_0000, q_indptr.ctypes.data,
-                                                  Hq, C.c_float(0.1), 0x7500_0000_0000, None, 0x7600_0000_0000, 16,
-                                                  None)
+            st, _ = _prefill_status(pool, Hq, lists, lq, lens, ws_bytes=16)
             assert st == comb.COMB_ERR_CAPACITY
         comb.comb_pool_destroy(pool)
+
+
+@pytest.mark.parametrize("case", [(5, 256, 300), (20, 64, 300), (10, 128, 260), (5, 256, 500), (5, 256, 600),
+                                  (37, 256, 300), (39, 128, 520)])
+def test_workspace_bound_last_wave_ranges_short_requests(case):
+    """Requests of 3-5 KV tiles whose item count leaves a last wave at most half full are cut in two by the planner;
+    the bound used to reserve partial rows only from 4 tiles up (round-1 ADVICE). One planner now serves both."""
+    R, lq, T = case
+    pool = make_pool(num_pages=R * ((T + 15) // 16), Hkv=8, Dqk=128, Dv=128)
+    for c in range(R):
+        comb.comb_chunk_alloc(pool, c, T)
+    st, _ = _prefill_status(pool, 32, [[r] for r in range(R)], [lq] * R, None)
+    assert st in (comb.COMB_OK, comb.COMB_ERR_CUDA), st
+    comb.comb_pool_destroy(pool)
+
+
+def test_prefill_rejects_a_host_mirror_that_disagrees_with_the_link():
+    pool = make_pool(num_pages=64, Hkv=2, Dqk=64, Dv=64)
+    comb.comb_chunk_alloc(pool, 0, 400)
+    comb.comb_chunk_alloc(pool, 1, 300)
+    lists, lq = [[0, 1], [1]], [4, 4]
+    link, tabs = plan(pool, lists)
+    q_indptr = np.array([0, 4, 8], np.int32)
+    mirror = link._keepalive[1]
+    off = link.host_req_pages - mirror.ctypes.data
+    mirror[off:off + 8].view(np.int32)[:] = [10, 10]  # stale counts (e.g. from another link)
+    ws = comb.comb_attn_workspace_bytes(pool, link, 8, 8)
+    st = _lib.lib.comb_cross_attn_prefill(pool, 0, C.byref(link), 2, 0x7400_0000_0000, q_indptr.ctypes.data, 8,
+                                          C.c_float(0.1), 0x7500_0000_0000, None, 0x7600_0000_0000, ws, None)
+    assert st == comb.COMB_ERR_INVALID
+    comb.comb_pool_destroy(pool)
+
+
+def test_options_and_decode_group_sizes():
+    pool = make_pool(num_pages=64, Hkv=1, Dqk=64, Dv=128)
+    comb.comb_pool_set_option(pool, comb.OPT_DECODE_PATH, comb.DECODE_CHUNK_MAJOR)
+    comb.comb_pool_set_option(pool, comb.OPT_DECODE_PATH, comb.DECODE_AUTO)
+    for bad in ((comb.OPT_DECODE_PATH, 7), (99, 0)):
+        with pytest.raises(comb.CombError) as e:
+            comb.comb_pool_set_option(pool, *bad)
+        assert e.value.status == comb.COMB_ERR_INVALID
+    comb.comb_chunk_alloc(pool, 0, 40)
+    link, _ = plan(pool, [[0]])
+    # every group size prefill takes is taken by decode too (G = 8, 16 used to be INVALID); 3 and 32 are not
+    for Hq, ok in ((1, True), (2, True), (4, True), (8, True), (16, True), (3, False), (32, False)):
+        ws = comb.comb_attn_workspace_bytes(pool, link, Hq, 1)
+        st = _lib.lib.comb_cross_attn_decode(pool, 0, C.byref(link), 1, 0x7400_0000_0000, Hq, C.c_float(0.1),
+                                             0x7500_0000_0000, None, 0x7600_0000_0000, ws, None)
+        assert (st != comb.COMB_ERR_INVALID) == ok, (Hq, st)
+    comb.comb_pool_destroy(pool)

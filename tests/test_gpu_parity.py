@@ -1,10 +1,13 @@
 """GPU parity tests (run with -m gpu on a B200): every step of the hot path, called through the C ABI
 (paper_2602_01519_b200.api -> libcomb.so), against the fp64 oracle on the same seeded inputs.
 
-Bars (BASELINE.json north_star): block tables and page contents bit-exact; attention outputs
-max abs <= 2e-2 and mean abs <= 2e-3; additionally relative L2 <= 1e-2 and |LSE error| <= 2e-3 so the claim
-means something on the small outputs N(0,1) inputs give."""
+Bars (BASELINE.json north_star; DESIGN.md §2 "Tolerances"): block tables and page contents bit-exact; attention
+outputs max abs <= 2e-2 and mean abs <= 2e-3; additionally relative L2 <= 1e-2 and |LSE error| <= 2e-4 (SURVEY.md
+§8(c) asks for 1e-3; the fp32 statistics give ~1e-6) so the claim means something on the small outputs N(0,1)
+inputs give."""
+import json
 import math
+import os
 
 import numpy as np
 import pytest
@@ -16,6 +19,18 @@ pytestmark = pytest.mark.gpu
 
 torch = pytest.importorskip("torch")
 SENTINEL = 0x7FC0  # bf16 NaN: any unmasked read of an unowned slot poisons the output (pin P15)
+LSE_TOL = 2e-4
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def record(tag, **kw):
+    """Measured worst cases, appended to gpurun_out/parity_measured.jsonl (evidence for DESIGN.md §2; not read back)."""
+    try:
+        os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+        with open(os.path.join(ROOT, "gpurun_out", "parity_measured.jsonl"), "a") as f:
+            f.write(json.dumps(dict(tag=tag, **{k: float(v) for k, v in kw.items()})) + "\n")
+    except OSError:
+        pass
 
 
 def H():
@@ -28,7 +43,12 @@ def check_attention(out_bits, lse, O, L, tag=""):
     assert np.all(np.isfinite(got)), tag + ": non-finite output"
     err = np.abs(got - O)
     rel = math.sqrt(float((err ** 2).sum()) / max(float((O ** 2).sum()), 1e-300))
-    assert err.max() <= 2e-2, "%s: max abs %.3e" % (tag, err.max())
+    # BASELINE's bar is absolute (2e-2) and fits its N(0,1) inputs, whose outputs stay below 0.5.  The peaked variants
+    # reach |O| > 4, where half a bf16 ulp of the OUTPUT alone is 2^-8 |O| = 0.0156: the bar grows by the bf16 unit
+    # roundoff for the part of |O| above 2 (never reached by BASELINE's inputs; DESIGN.md §2 "Tolerances").
+    excess = err - (2e-2 + 2.0 ** -8 * np.maximum(np.abs(O) - 2.0, 0.0))
+    assert excess.max() <= 0, "%s: max abs %.3e (|O| there %.3f)" % (tag, err.flat[excess.argmax()],
+                                                                       abs(O.flat[excess.argmax()]))
     assert err.mean() <= 2e-3, "%s: mean abs %.3e" % (tag, err.mean())
     assert rel <= 1e-2, "%s: rel L2 %.3e" % (tag, rel)
     if lse is not None:
@@ -36,18 +56,26 @@ def check_attention(out_bits, lse, O, L, tag=""):
         assert np.array_equal(np.isneginf(lse), np.isneginf(L)), tag + ": -inf pattern of LSE"
         if fin.any():
             e = np.abs(lse[fin] - L[fin]).max()
-            assert e <= 2e-3, "%s: LSE err %.3e" % (tag, e)
+            assert e <= LSE_TOL, "%s: LSE err %.3e" % (tag, e)
+            record(tag, max_abs=err.max(), mean_abs=err.mean(), rel_l2=rel, lse=e)
     return err.max(), err.mean(), rel
 
 
-def close_in_ulps(a, b, tag=""):
-    """Two GPU results for the same mathematical value (other tile partition, other kernel). They differ by the
-    bf16 rounding of the output (<= 2^-8 relative each) and of the P weights fed to the PV contraction (each weight
-    2^-9 relative, so about 2^-9 * sum_j p_j |v_j| / l ~ 2e-3 absolute for N(0,1) values), and by fp32 reassociation."""
+def close_in_ulps(a, b, tag="", peaked=False):
+    """Two GPU results for the same mathematical value (other tile partition, other kernel, other link order).
+    Bound (derived in DESIGN.md §2 "Tolerances"): each is its own fp32 value rounded to bf16 (2^-9 |a| each, 2^-8
+    together), and the fp32 values differ by the bf16 rounding of the softmax weights fed to the P.V contraction:
+    every weight carries an independent relative error of at most 2^-9 (std 2^-9/sqrt 3), so an element moves by about
+    2^-9/sqrt 3 * sqrt(sum_j p_j^2 v_j^2) / l ~ 1.1e-3 * v_rms / sqrt(n_eff), n_eff = l^2 / sum p^2 the effective number
+    of keys.  N(0,1) inputs: n_eff >= ~30 => sigma <= 2e-4, worst of ~1e5 elements (4.5 sigma) ~ 9e-4: floor 1.5e-3
+    (measured worst 8.9e-4, mean 1.3e-4).  Peaked inputs (Q x 4): n_eff down to 2-3 on the shortest requests =>
+    sigma up to 7e-4 and |v| up to 4: floor 8e-3 (measured worst 4.1e-3, mean 2.7e-4)."""
     d = np.abs(a - b)
-    assert np.all(d <= 2.0 ** -7 * np.abs(a) + 2.5e-3), "%s: worst excess %.3e" % (
-        tag, (d - 2.0 ** -7 * np.abs(a)).max())
-    assert d.mean() <= 3e-4, "%s: mean |a-b| = %.3e" % (tag, d.mean())
+    worst = float((d - 2.0 ** -7 * np.abs(a)).max())
+    record("ulps " + tag, worst_excess=worst, mean=d.mean())
+    floor, mean = (8e-3, 6e-4) if peaked else (1.5e-3, 3e-4)
+    assert worst <= floor, "%s: worst excess %.3e" % (tag, worst)
+    assert d.mean() <= mean, "%s: mean |a-b| = %.3e" % (tag, d.mean())
 
 
 def run_prefill(w, **kw):
@@ -279,7 +307,7 @@ def test_prefill_closed_forms():
     got = cs.bf16_bits_to_f64(out)
     for h in range(4):
         assert np.abs(got[:, h] - vs[h // 2]).max() <= 2 ** -8 * np.abs(vs).max() + 1e-6
-    assert np.abs(lse - math.log(259)).max() <= 1e-4
+    assert np.abs(lse - math.log(259)).max() <= 1e-5
 
 
 def test_prefill_permutation_and_split_invariance():
@@ -315,7 +343,7 @@ def test_prefill_permutation_and_split_invariance():
         res.append((cs.bf16_bits_to_f64(H().device_to_bits(out)), lse.cpu().numpy()))
         pool.close()
     close_in_ulps(res[0][0], res[1][0], "split vs whole")
-    assert np.abs(res[0][1] - res[1][1]).max() <= 1e-4
+    assert np.abs(res[0][1] - res[1][1]).max() <= 2e-5
 
 
 def test_prefill_row_equals_decode():
@@ -327,74 +355,432 @@ def test_prefill_row_equals_decode():
     a = cs.bf16_bits_to_f64(out_p[:6])
     b = cs.bf16_bits_to_f64(H().device_to_bits(out_d))
     close_in_ulps(a, b, "prefill row vs decode")
-    assert np.abs(lse_p[:6] - lse_d.cpu().numpy()).max() <= 1e-3
+    assert np.abs(lse_p[:6] - lse_d.cpu().numpy()).max() <= 2e-5
+
+
 
 
 # ------------------------------------------------------------------------------------------------
-# full BASELINE sizes, in the launch configuration bench.py times: sampled outputs against O1
+# closed forms and invariants on the GPU, prefill and both decode paths (pins P3-P5, P9, P10, P12 of SURVEY.md §8(c))
 # ------------------------------------------------------------------------------------------------
-def sampled_check(w, ld, out_bits, lse, n_per_req=6, reqs=(0, 1, -1)):
+def run_custom(Hq, Hkv, chunks, links, q, scale, shuffle_seed=9):
+    """chunks: list of (K float [T][Hkv][Dqk], V float [T][Hkv][Dv]) with bf16-exact values; q float [R][lq][Hq][Dqk].
+    Returns {"prefill" | "decode_split" | "decode_cascade": (O float64 [sum lq or R][Hq][Dv], LSE)}; the decode calls
+    use row 0 of every request."""
+    import paper_2602_01519_b200 as comb
+    Dqk, Dv = chunks[0][0].shape[2], chunks[0][1].shape[2]
+    pages = sum((k.shape[0] + 15) // 16 for k, _ in chunks)
+    pool = comb.Pool(Hkv, Dqk, Dv, pages + 3, shuffle_seed=shuffle_seed, sentinel=SENTINEL)
+    for c, (k, v) in enumerate(chunks):
+        kb, vb = cs.f32_to_bf16_bits(k), cs.f32_to_bf16_bits(v)
+        assert np.array_equal(cs.bf16_bits_to_f32(kb), k.astype(np.float32)), "test values must be bf16-exact"
+        assert np.array_equal(cs.bf16_bits_to_f32(vb), v.astype(np.float32))
+        pool.store_chunk(c, H().bits_to_device(kb, "cuda"), H().bits_to_device(vb, "cuda"))
+    lb = pool.link(links)
+    R = len(links)
+    lq = [x.shape[0] for x in q]
+    q_indptr = np.zeros(R + 1, np.int32)
+    np.cumsum(lq, out=q_indptr[1:])
+    qd = H().bits_to_device(cs.f32_to_bf16_bits(np.concatenate(q, 0)), "cuda")
+    res = {}
+    out, lse = pool.prefill(lb, qd, q_indptr, scale)
+    torch.cuda.synchronize()
+    res["prefill"] = (cs.bf16_bits_to_f64(H().device_to_bits(out)), lse.cpu().numpy().astype(np.float64))
+    q1 = H().bits_to_device(cs.f32_to_bf16_bits(np.stack([x[0] for x in q], 0)), "cuda")
+    for name, path in (("decode_split", comb.DECODE_PER_REQUEST), ("decode_cascade", comb.DECODE_CHUNK_MAJOR)):
+        pool.set_decode_path(path)
+        out, lse = pool.decode(lb, q1, scale)
+        torch.cuda.synchronize()
+        res[name] = (cs.bf16_bits_to_f64(H().device_to_bits(out)), lse.cpu().numpy().astype(np.float64))
+    pool.close()
+    return res, q_indptr
+
+
+@pytest.mark.parametrize("n1,n0", [(64, 64), (96, 32), (3, 1), (300, 100)])
+def test_two_level_closed_form_on_gpu(n1, n0):
+    """P5: scale 1, q = e_0, n1 keys k = e_0 (score 1) with V = 1 and n0 keys k = 0 (score 0) with V = 0, split over
+    three chunks: every output component = e n1 / (e n1 + n0) (= e/(e+1), 3e/(3e+1) for the ratios here) and
+    LSE = ln(e n1 + n0).  GPU within 2^-8 relative (bf16 output rounding + bf16 softmax weights)."""
+    Hq, Hkv, D = 4, 2, 64
+    K = np.zeros((n1 + n0, Hkv, D), np.float32)
+    V = np.zeros((n1 + n0, Hkv, D), np.float32)
+    order = np.random.default_rng(5).permutation(n1 + n0)
+    hot = order[:n1]
+    K[hot, :, 0] = 1.0
+    V[hot] = 1.0
+    cut = [0, (n1 + n0) // 3, (n1 + n0) // 3 + 1, n1 + n0]
+    chunks = [(K[cut[i]:cut[i + 1]], V[cut[i]:cut[i + 1]]) for i in range(3) if cut[i + 1] > cut[i]]
+    q = np.zeros((2, Hq, D), np.float32)
+    q[:, :, 0] = 1.0
+    res, _ = run_custom(Hq, Hkv, chunks, [list(range(len(chunks)))[::-1], list(range(len(chunks)))], [q, q[:1]], 1.0)
+    want = math.e * n1 / (math.e * n1 + n0)
+    gold = {}
+    with open(os.path.join(ROOT, "tests", "golden", "closed_forms.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                gold[line.split()[0]] = float(line.split()[1])
+    if n1 == n0:
+        assert abs(want - gold["sigmoid_1"]) < 1e-15           # e/(e+1)
+    if n1 == 3 * n0:
+        assert abs(want - gold["two_level_3_to_1"]) < 1e-15    # 3e/(3e+1)
+    for name, (O, L) in res.items():
+        assert np.abs(O - want).max() <= 2.0 ** -8 * want, "%s: %.6f vs %.6f" % (name, O.flat[np.abs(O - want).argmax()], want)
+        assert np.abs(L - math.log(math.e * n1 + n0)).max() <= 2e-5, name
+        record("p5 %s %d:%d" % (name, n1, n0), rel=np.abs(O - want).max() / want)
+
+
+def test_single_key_equal_scores_and_empty_link_on_gpu():
+    """P3: one key => O = V exactly, LSE = its score.  P4: q = 0 => O = mean V, LSE = ln n.  P12: no chunk => O = 0,
+    LSE = -inf.  All three in one batch, prefill and both decode paths (the single key sits in a page with 15
+    masked slots; the mean runs over an interior partial page)."""
+    Hq, Hkv, Dqk, Dv = 8, 2, 128, 128
+    rng = np.random.default_rng(11)
+    small = lambda *shape: rng.integers(-8, 9, size=shape).astype(np.float32) / 4.0  # noqa: E731  bf16-exact
+    chunks = [(small(1, Hkv, Dqk), small(1, Hkv, Dv)), (small(37, Hkv, Dqk), small(37, Hkv, Dv)),
+              (small(150, Hkv, Dqk), small(150, Hkv, Dv))]
+    q0 = small(3, Hq, Dqk)
+    links = [[0], [1, 2], [], [2, 1]]
+    q = [q0, np.zeros((2, Hq, Dqk), np.float32), q0[:1], np.zeros((1, Hq, Dqk), np.float32)]
+    scale = 0.125
+    res, qi = run_custom(Hq, Hkv, chunks, links, q, scale)
+    G = Hq // Hkv
+    vmean = np.concatenate([chunks[1][1], chunks[2][1]], 0).astype(np.float64).mean(0)  # [Hkv][Dv]
+    for name, (O, L) in res.items():
+        rows = (lambda r: slice(int(qi[r]), int(qi[r + 1]))) if name == "prefill" else (lambda r: slice(r, r + 1))
+        qq = (lambda r: q[r]) if name == "prefill" else (lambda r: q[r][:1])
+        for h in range(Hq):
+            assert np.array_equal(O[rows(0), h], np.broadcast_to(chunks[0][1][0, h // G].astype(np.float64), O[rows(0), h].shape)), name
+            s0 = scale * (qq(0)[:, h].astype(np.float64) @ chunks[0][0][0, h // G].astype(np.float64))
+            assert np.abs(L[rows(0), h] - s0).max() <= 1e-5, name
+            for r in (1, 3):
+                assert np.abs(O[rows(r), h] - vmean[h // G]).max() <= 2.0 ** -8 * np.abs(vmean).max() + 1e-6, name
+                assert np.abs(L[rows(r), h] - math.log(187)).max() <= 1e-5, name
+        assert np.all(O[rows(2)] == 0) and np.all(np.isneginf(L[rows(2)])), name
+
+
+def test_shift_invariance_and_v_affinity_on_gpu():
+    """P9: adding one vector c to every key shifts row i's scores by q_i.c: O unchanged, LSE + scale q_i.c (small
+    integers: sums exact).  P10: V constant => O = that constant; O is linear in V."""
+    Hq, Hkv, Dqk, Dv = 4, 1, 64, 64
+    rng = np.random.default_rng(3)
+    T = [40, 100, 17]
+    K = [rng.integers(-2, 3, size=(t, Hkv, Dqk)).astype(np.float32) for t in T]
+    V1 = [rng.integers(-4, 5, size=(t, Hkv, Dv)).astype(np.float32) for t in T]
+    V2 = [rng.integers(-4, 5, size=(t, Hkv, Dv)).astype(np.float32) for t in T]
+    q = [rng.integers(-1, 2, size=(5, Hq, Dqk)).astype(np.float32) for _ in range(2)]
+    cvec = rng.integers(-1, 2, size=(Dqk,)).astype(np.float32)
+    links, scale = [[0, 1, 2], [2, 0]], 0.0625
+    base, qi = run_custom(Hq, Hkv, list(zip(K, V1)), links, q, scale)
+    shifted, _ = run_custom(Hq, Hkv, [(k + cvec, v) for k, v in zip(K, V1)], links, q, scale)
+    const, _ = run_custom(Hq, Hkv, [(k, np.full_like(v, 1.5)) for k, v in zip(K, V1)], links, q, scale)
+    other, _ = run_custom(Hq, Hkv, list(zip(K, V2)), links, q, scale)
+    both, _ = run_custom(Hq, Hkv, [(k, a + b) for k, a, b in zip(K, V1, V2)], links, q, scale)
+    for name in base:
+        O, L = base[name]
+        qrows = np.concatenate(q, 0) if name == "prefill" else np.stack([x[0] for x in q], 0)
+        dl = scale * (qrows.astype(np.float64) @ cvec.astype(np.float64))      # [rows][Hq]
+        assert np.abs(shifted[name][1] - (L + dl)).max() <= 2e-5, name
+        close_in_ulps(O, shifted[name][0], "P9 %s" % name)
+        assert np.abs(const[name][0] - 1.5).max() <= 1.5 * 2.0 ** -8, name            # P10: constant V
+        lin = np.abs(both[name][0] - (O + other[name][0]))
+        assert lin.max() <= 2.0 ** -7 * np.abs(both[name][0]).max() + 2.5e-3 and lin.mean() <= 1e-3, name   # P10: linear in V
+
+
+# ------------------------------------------------------------------------------------------------
+# (f1) chunk-major decode: element by element against the oracle and against the per-request path
+# ------------------------------------------------------------------------------------------------
+def decode_both_paths(w, **kw):
+    import paper_2602_01519_b200 as comb
+    ld = H().load_workload(w, sentinel=SENTINEL, **kw)
+    res = {}
+    for name, path in (("split", comb.DECODE_PER_REQUEST), ("cascade", comb.DECODE_CHUNK_MAJOR)):
+        ld.pool.set_decode_path(path)
+        l0 = ld.pool.launches
+        out, lse = ld.pool.decode(ld.batch, ld.q, w.scale)
+        torch.cuda.synchronize()
+        res[name] = (H().device_to_bits(out), lse.cpu().numpy().astype(np.float64), ld.pool.launches - l0)
+    return ld, res
+
+
+def shared_workload(name, Hq, Hkv, Dqk, Dv, R=40, seed=0, hot=3):
+    """Requests share a few hot chunks (Zipf-like), one request links a chunk twice (I14), one links nothing (I13), one
+    links a single one-token chunk (P3 geometry), one hot chunk is linked by more than 128/G requests (several M
+    tiles of the same chunk)."""
+    rng = np.random.default_rng([seed, 31])
+    lens = rng.integers(1, 400, size=30).astype(np.int32)
+    lens[:5] = [1, 16, 17, 255, 300]
+    links = []
+    for r in range(R):
+        m = int(rng.integers(1, 6))
+        cold = rng.choice(np.arange(5 + hot, 30), size=m, replace=False)
+        links.append(np.concatenate([[5 + (r % hot)] if r % 4 else [], cold, [4]]).astype(np.int64))  # chunk 4: hot for all
+        rng.shuffle(links[-1])
+    links[1] = np.zeros(0, np.int64)
+    links[2] = np.array([0])
+    links[3] = np.array([7, 4, 7])
+    return cs.custom(name, k=8, seed=seed, num_q_heads=Hq, num_kv_heads=Hkv, head_dim_qk=Dqk, head_dim_v=Dv,
+                     chunk_len=lens, links=links, lq=[1] * R)
+
+
+@pytest.mark.parametrize("shape", [(32, 8, 128, 128), (16, 16, 192, 128), (8, 2, 64, 64), (8, 1, 64, 128),
+                                   (16, 1, 128, 128), (4, 2, 128, 64)])
+@pytest.mark.parametrize("peaked", [False, True])
+def test_decode_chunk_major_matches_oracle_and_per_request_path(shape, peaked):
+    Hq, Hkv, Dqk, Dv = shape
+    G = Hq // Hkv
+    w = shared_workload("cascade", Hq, Hkv, Dqk, Dv, R=40 if G < 16 else 12)
+    if peaked:
+        w = w.peaked()
+    ld, res = decode_both_paths(w, shuffle_seed=17)
+    O, L = oracle.attention_for(w)
+    for name, (out, lse, launches) in res.items():
+        check_attention(out, lse, O, L, "decode %s %s peaked=%s" % (name, shape, peaked))
+        assert np.all(out[1] == 0) and np.all(np.isneginf(lse[1]))             # empty link
+        v0 = ld.stored_host[0][1][0]
+        for h in range(Hq):                                                       # single key: bit-exact
+            assert np.array_equal(out[2, h], v0[h // G]), name
+    assert res["cascade"][2] == 2, "chunk-major = the tcgen05 kernel + the per-request merge"
+    close_in_ulps(cs.bf16_bits_to_f64(res["split"][0]), cs.bf16_bits_to_f64(res["cascade"][0]),
+                  "split vs cascade %s peaked=%s" % (shape, peaked), peaked=peaked)
+    assert np.abs(res["split"][1][np.isfinite(L)] - res["cascade"][1][np.isfinite(L)]).max() <= 2e-5
+    ld.pool.close()
+
+
+def test_decode_chunk_major_is_order_invariant_and_auto_policy():
+    """P6 on the chunk-major path ("in any order/position"): permuting every request's links changes the
+    entry numbering and the partial-row placement, not the result.  And the automatic policy: chunk-major when the
+    batch shares chunks (entries >= 1.25 x distinct chunks), per-request otherwise."""
+    import paper_2602_01519_b200 as comb
+    w = shared_workload("order", 32, 8, 128, 128, R=24, seed=2)
+    rng = np.random.default_rng(0)
+    wp = cs.custom("order", k=8, seed=2, num_q_heads=32, num_kv_heads=8, head_dim_qk=128, head_dim_v=128,
+                   chunk_len=w.chunk_len, links=[rng.permutation(l) for l in w.links], lq=[1] * 24)
+    outs = []
+    for ww in (w, wp):
+        ld = H().load_workload(ww, sentinel=SENTINEL, shuffle_seed=4)
+        l0 = ld.pool.launches
+        out, lse = ld.pool.decode(ld.batch, ld.q, ww.scale)           # automatic: this batch shares chunks
+        torch.cuda.synchronize()
+        assert ld.batch.link.total_entries * 4 >= ld.batch.link.num_distinct_chunks * 5
+        assert ld.pool.launches - l0 == 2
+        outs.append((cs.bf16_bits_to_f64(H().device_to_bits(out)), lse.cpu().numpy()))
+        # no sharing: every request its own chunk -> the per-request split kernel (1 or 2 launches, never the pair above)
+        lb = ld.pool.link([[10 + r] for r in range(8)])
+        assert lb.link.total_entries == lb.link.num_distinct_chunks
+        comb.comb_profile_enable(ld.pool.handle, True)
+        ld.pool.decode(lb, ld.q[:8], ww.scale)
+        torch.cuda.synchronize()
+        assert comb.comb_profile_read(ld.pool.handle, comb.KERNEL_DECODE_SPLIT)[1] == 1
+        assert comb.comb_profile_read(ld.pool.handle, comb.KERNEL_DECODE_CASCADE)[1] == 0
+        comb.comb_profile_enable(ld.pool.handle, False)
+        ld.pool.close()
+    fin = np.isfinite(outs[0][1])
+    close_in_ulps(outs[0][0], outs[1][0], "chunk-major, permuted links")
+    assert np.abs(outs[0][1][fin] - outs[1][1][fin]).max() <= 2e-5
+
+
+@pytest.mark.parametrize("group", [8, 16])
+def test_decode_large_groups_take_the_per_request_path_too(group):
+    """A pool prefill accepts (G = 8, 16) used to be INVALID for decode (round-1 VERDICT): groups run as sub-groups of 4."""
+    w = ragged_workload("g%d" % group, group * 2, 2, 128, 128, [1] * 6, seed=group)
+    ld, res = decode_both_paths(w, shuffle_seed=3)
+    O, L = oracle.attention_for(w)
+    for name, (out, lse, _) in res.items():
+        check_attention(out, lse, O, L, "decode G=%d %s" % (group, name))
+    ld2, out_p, lse_p = run_prefill(w, shuffle_seed=3)
+    check_attention(out_p, lse_p, O, L, "prefill G=%d" % group)
+
+
+# ------------------------------------------------------------------------------------------------
+# the persistent prefill kernel with several items per CTA, and the last-wave KV ranges, every element
+# ------------------------------------------------------------------------------------------------
+def test_prefill_many_items_per_cta_all_elements():
+    """37 requests x 130 tokens, 32/8 heads: 3 items per (request, kv-head) = 888 items = exactly 6 waves of 148
+    CTAs (no last-wave ranges), so every CTA of the unsplit persistent kernel runs 6 items back to back (K/V ring
+    phase, q_empty and o_cnt carry over from item to item)."""
+    rng = np.random.default_rng(41)
+    lens = rng.integers(60, 260, size=12).astype(np.int32)
+    links = [rng.choice(12, size=6, replace=False) for _ in range(37)]
+    w = cs.custom("multi_item", k=7, num_q_heads=32, num_kv_heads=8, head_dim_qk=128, head_dim_v=128, chunk_len=lens,
+                  links=links, lq=[130] * 37)
+    ld = H().load_workload(w, sentinel=SENTINEL, shuffle_seed=8)
+    l0 = ld.pool.launches
+    out, lse = ld.pool.prefill(ld.batch, ld.q, ld.q_indptr, w.scale)
+    torch.cuda.synchronize()
+    if torch.cuda.get_device_properties(0).multi_processor_count == 148:
+        assert ld.pool.launches - l0 == 1, "unsplit path: one kernel"
+    check_attention(H().device_to_bits(out), lse.cpu().numpy().astype(np.float64), *oracle.attention_for(w),
+                    tag="prefill multi-item")
+    ld.pool.close()
+
+
+@pytest.mark.parametrize("case", [(5, 256, 300), (20, 64, 300), (5, 256, 1500)])
+def test_prefill_last_wave_ranges_all_elements(case):
+    """Item counts that leave a last wave at most half full (160 items on 148 SMs): only those items are cut into KV
+    ranges (2 ranges of a 3-tile request; up to 4 of a 12-tile one) and merged; the others write final rows."""
+    R, lq, T = case
+    w = cs.custom("tailcut", k=6, num_q_heads=32, num_kv_heads=8, head_dim_qk=128, head_dim_v=128,
+                  chunk_len=[T - 100, 100] * R, links=[[2 * r, 2 * r + 1] for r in range(R)], lq=[lq] * R)
+    for ww in (w, w.peaked()):
+        ld = H().load_workload(ww, sentinel=SENTINEL, shuffle_seed=8)
+        sms = torch.cuda.get_device_properties(0).multi_processor_count
+        l0 = ld.pool.launches
+        out, lse = ld.pool.prefill(ld.batch, ld.q, ld.q_indptr, ww.scale)
+        torch.cuda.synchronize()
+        if sms == 148:
+            assert ld.pool.launches - l0 == 2, "expected last-wave ranges + merge on a 148-SM part"
+        check_attention(H().device_to_bits(out), lse.cpu().numpy().astype(np.float64), *oracle.attention_for(ww),
+                        tag="prefill tail cut %s" % (case,))
+        ld.pool.close()
+
+
+def test_prefill_through_a_caller_written_table():
+    """The link tables are plain arrays: a caller may write them itself (here: numpy, from the oracle's table model)
+    and still gets KV ranges, because the page counts the planner needs travel in the link (host_req_pages), not
+    in a cache inside the pool (round-1 VERDICT item 4)."""
+    import ctypes as C
+    import paper_2602_01519_b200 as comb
+    w = cs.custom("caller", k=5, num_q_heads=8, num_kv_heads=2, head_dim_qk=128, head_dim_v=128,
+                  chunk_len=[700, 333, 512, 129], links=[[0, 1, 2], [3, 0]], lq=[20, 9])
+    ld = H().load_workload(w, sentinel=SENTINEL, shuffle_seed=13)
+    model = oracle.PoolModel(w.pool_pages, 13)
+    for c in range(w.num_chunks):
+        model.store(c, int(w.chunk_len[c]))
+    t = model.link([list(map(int, l)) for l in w.links])
+    R = 2
+    npages = np.diff(t["page_indptr"]).astype(np.int32)
+    tile_indptr = np.zeros(R + 1, np.int32)
+    np.cumsum((npages + 7) // 8, out=tile_indptr[1:])
+    tile_ntok = np.zeros(int(tile_indptr[-1]), np.uint64)
+    for r in range(R):
+        pn = t["page_ntok"][t["page_indptr"][r]:t["page_indptr"][r + 1]]
+        for i in range(0, len(pn), 8):
+            tile_ntok[tile_indptr[r] + i // 8] = sum(int(x) << (8 * j) for j, x in enumerate(pn[i:i + 8]))
+    parts = [t["page_indptr"], t["page_ids"], t["page_ntok"], t["kv_len"], tile_indptr]
+    offs, blob = [], b""
+    for a in parts + [tile_ntok]:
+        blob += b"\0" * ((-len(blob)) % 16)
+        offs.append(len(blob))
+        blob += a.tobytes()
+    dev = torch.from_numpy(np.frombuffer(blob, np.uint8).copy()).cuda()
+    link = comb.Link()
+    link.device_buf, link.device_bytes = dev.data_ptr(), dev.numel()
+    base = dev.data_ptr()
+    (link.page_indptr, link.page_ids, link.page_ntok, link.kv_len, link.tile_indptr, link.tile_ntok) = [base + o for o in offs]
+    link.num_requests, link.max_pages_per_request = R, int(npages.max())
+    link.total_pages, link.total_tiles = int(npages.sum()), int(tile_indptr[-1])
+    link.total_kv_tokens = int(t["kv_len"].sum())
+    link.host_req_pages = npages.ctypes.data
+    lb = comb.LinkedBatch(link, dev, None)
+    l0 = ld.pool.launches
+    out, lse = ld.pool.prefill(lb, ld.q, ld.q_indptr, w.scale)
+    torch.cuda.synchronize()
+    assert ld.pool.launches - l0 == 2, "KV ranges + merge expected for 16 items on a B200"
+    check_attention(H().device_to_bits(out), lse.cpu().numpy().astype(np.float64), *oracle.attention_for(w),
+                    tag="caller-written table")
+    # the per-request decode needs nothing but the request-major tables either
+    wd = w.decode_phase()
+    outd, lsed = ld.pool.decode(lb, H().bits_to_device(wd.all_q(), "cuda"), wd.scale)
+    torch.cuda.synchronize()
+    check_attention(H().device_to_bits(outd), lsed.cpu().numpy().astype(np.float64), *oracle.attention_for(wd),
+                    tag="caller-written table, decode")
+    ld.pool.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# full BASELINE sizes, in the launch configuration bench.py times
+#   decode (cfg 2, 4, 5): EVERY output element, per-request and chunk-major paths
+#   prefill (cfg 3, 4, 5): one row of every work item (request, kv-head, Q-tile pair) + one whole request (or, for
+#   cfg 4, one whole 128-token block of a request whose items are cut into last-wave KV ranges)
+# ------------------------------------------------------------------------------------------------
+def per_item_samples(w, ld, out_bits, lse, tok_per_item, whole, tag):
+    """whole = (request, first token, tokens): every (row, head) of that block; plus, for every request, one random
+    row inside every `tok_per_item`-token block paired with one random head of every kv-head."""
     rng = np.random.default_rng(123)
-    R = w.num_requests
-    for r in [x % R for x in reqs]:
-        lo, hi = int(w.q_indptr[r]), int(w.q_indptr[r + 1])
-        rows = rng.integers(lo, hi, size=n_per_req).astype(np.int32)
-        heads = rng.integers(0, w.num_q_heads, size=n_per_req).astype(np.int32)
+    R, Hq, Hkv = w.num_requests, w.num_q_heads, w.num_kv_heads
+    G = Hq // Hkv
+    q_all = H().device_to_bits(ld.q)
+    qi = np.asarray(w.q_indptr, np.int32)
+    worst = dict(max_abs=0.0, mean_abs=0.0, lse=0.0, n=0)
+    for r in range(R):
+        lo, hi = int(qi[r]), int(qi[r + 1])
+        rows, heads = [], []
+        for b0 in range(lo, hi, tok_per_item):
+            for g in range(Hkv):
+                rows.append(int(rng.integers(b0, min(b0 + tok_per_item, hi))))
+                heads.append(g * G + int(rng.integers(0, G)))
+        if whole is not None and whole[0] == r:
+            for t in range(lo + whole[1], lo + whole[1] + whole[2]):
+                rows += [t] * Hq
+                heads += list(range(Hq))
+        if not rows:
+            continue
         ks, vs, sel = [], [], []
         for c in w.links[r]:
             k, v = ld.stored_host[int(c)]
             sel.append(len(ks))
             ks.append(k)
             vs.append(v)
-        qi = np.zeros(R + 1, np.int32)
-        qi[:] = w.q_indptr
         ci = np.zeros(R + 1, np.int32)
         ci[r + 1:] = len(sel)
-        q_all = H().device_to_bits(ld.q)
+        rows, heads = np.array(rows, np.int32), np.array(heads, np.int32)
         O, L = oracle.attention_samples(r, q_all, qi, ks, vs, ci, np.array(sel, np.int32), w.scale, rows, heads)
         got = cs.bf16_bits_to_f64(out_bits[rows, heads])
         err = np.abs(got - O)
-        assert err.max() <= 2e-2 and err.mean() <= 2e-3, (r, err.max(), err.mean())
+        assert np.all(np.isfinite(got))
+        assert err.max() <= 2e-2 and err.mean() <= 2e-3, (tag, r, err.max(), err.mean())
         rel = math.sqrt(float((err ** 2).sum()) / float((O ** 2).sum()))
-        assert rel <= 1e-2, (r, rel)
-        assert np.abs(lse[rows, heads] - L).max() <= 2e-3
+        assert rel <= 1e-2, (tag, r, rel)
+        le = np.abs(lse[rows, heads] - L).max()
+        assert le <= LSE_TOL, (tag, r, le)
+        worst = dict(max_abs=max(worst["max_abs"], err.max()), mean_abs=max(worst["mean_abs"], err.mean()),
+                     lse=max(worst["lse"], le), n=worst["n"] + len(rows))
+    record(tag, **worst)
 
 
-def test_full_size_decode_link_sampled():
-    w = cs.decode_link()
-    ld, out, lse = run_decode(w, fill="linked", shuffle_seed=2024)
-    assert np.all(np.isfinite(cs.bf16_bits_to_f64(out)))
-    sampled_check(w, ld, out, lse)
+def full_decode_check(w, fill, tag):
+    wd = w.decode_phase() if int(w.lq.max()) > 1 else w
+    ld, res = decode_both_paths(wd, fill=fill, shuffle_seed=2024)
+    O, L = oracle.attention_for(wd)
+    for name, (out, lse, _) in res.items():
+        check_attention(out, lse, O, L, "%s decode %s (every element)" % (tag, name))
+    close_in_ulps(cs.bf16_bits_to_f64(res["split"][0]), cs.bf16_bits_to_f64(res["cascade"][0]), tag + " split vs cascade")
+    ld.pool.close()
 
 
-def test_full_size_rag_prefill_sampled():
+def test_full_size_decode_link_every_element():
+    full_decode_check(cs.decode_link(), "linked", "cfg2")
+
+
+def test_full_size_long_fewshot_decode_every_element():
+    full_decode_check(cs.long_fewshot(), "all", "cfg4")
+
+
+def test_full_size_mla_decode_every_element():
+    full_decode_check(cs.mla_shaped(), "linked", "cfg5")
+
+
+def test_full_size_rag_prefill_every_item_and_a_whole_request():
     w = cs.rag_prefill()
     ld, out, lse = run_prefill(w, fill="linked", shuffle_seed=2024)
     assert np.all(np.isfinite(cs.bf16_bits_to_f64(out)))
-    sampled_check(w, ld, out, lse)
+    per_item_samples(w, ld, out, lse, 64, (5, 0, 256), "cfg3 prefill")      # item = 2 tiles x 32 tokens
+    ld.pool.close()
 
 
-def test_full_size_long_fewshot_sampled():
+def test_full_size_long_fewshot_prefill_every_item_and_a_whole_block():
     w = cs.long_fewshot()
     ld, out, lse = run_prefill(w, shuffle_seed=2024)
     assert np.all(np.isfinite(cs.bf16_bits_to_f64(out)))
-    sampled_check(w, ld, out, lse, n_per_req=4, reqs=(0, -1))
-    wd = w.decode_phase()
-    qd = H().bits_to_device(wd.all_q(), "cuda")
-    out_d, lse_d = ld.pool.decode(ld.batch, qd, wd.scale)
-    torch.cuda.synchronize()
-    ld.q = qd
-    sampled_check(wd, ld, H().device_to_bits(out_d), lse_d.cpu().numpy().astype(np.float64), n_per_req=4, reqs=(0, -1))
+    # the planner orders requests by work and cuts the LAST wave's items (512 items on 148 CTAs: the last 68) into
+    # KV ranges; with equal work per request those are the items of the highest request ids: take the block there
+    per_item_samples(w, ld, out, lse, 64, (7, 384, 128), "cfg4 prefill")
+    ld.pool.close()
 
 
-def test_full_size_mla_sampled():
+def test_full_size_mla_prefill_every_item_and_a_whole_request():
     w = cs.mla_shaped()
     ld, out, lse = run_prefill(w, fill="linked", shuffle_seed=2024)
     assert np.all(np.isfinite(cs.bf16_bits_to_f64(out)))
-    sampled_check(w, ld, out, lse, n_per_req=4, reqs=(0, -1))
-    wd = w.decode_phase()
-    qd = H().bits_to_device(wd.all_q(), "cuda")
-    out_d, lse_d = ld.pool.decode(ld.batch, qd, wd.scale)
-    torch.cuda.synchronize()
-    ld.q = qd
-    sampled_check(wd, ld, H().device_to_bits(out_d), lse_d.cpu().numpy().astype(np.float64), n_per_req=4, reqs=(0, -1))
+    per_item_samples(w, ld, out, lse, 128, (9, 0, 128), "cfg5 prefill")     # item = 1 tile x 128 tokens (G = 1)
+    ld.pool.close()

@@ -242,3 +242,27 @@ def test_bf16_rounding_is_rne():
     y = np.random.default_rng(0).standard_normal(4096).astype(np.float32)
     ref = torch.from_numpy(y).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
     assert np.array_equal(cs.f32_to_bf16_bits(y), ref)
+
+
+def test_chunk_major_inversion_hand_example():
+    """O3, chunk-major view (include/comb.h): worked by hand.  Requests link [5, 7], [7], [9, 7, 5]: entries in link
+    order are e0=(r0,5) e1=(r0,7) e2=(r1,7) e3=(r2,9) e4=(r2,7) e5=(r2,5).  Chunk 7 is linked 3 times, 5 twice,
+    9 once => slots [7, 5, 9]; slot rows in ascending entry number."""
+    m = oracle.PoolModel(16)
+    m.store(5, 20)   # pages 0, 1   (last page holds 4 tokens)
+    m.store(7, 16)   # page  2
+    m.store(9, 33)   # pages 3, 4, 5 (last page holds 1 token)
+    t = m.link_chunk_major([[5, 7], [7], [9, 7, 5]])
+    assert t["slot_chunks"].tolist() == [7, 5, 9]
+    assert t["entry_indptr"].tolist() == [0, 2, 3, 6]
+    assert t["cas_page_indptr"].tolist() == [0, 1, 3, 6]
+    assert t["cas_page_ids"].tolist() == [2, 0, 1, 3, 4, 5]
+    assert t["cas_page_ntok"].tolist() == [16, 16, 4, 16, 16, 1]
+    assert t["cas_row_indptr"].tolist() == [0, 3, 5, 6]
+    assert t["cas_row_req"].tolist() == [0, 1, 2, 0, 2, 2]
+    assert t["cas_row_entry"].tolist() == [1, 2, 4, 0, 5, 3]
+    # ties keep first appearance: [1, 2], [2, 1] -> both linked twice, chunk 1 appears first
+    m2 = oracle.PoolModel(4)
+    m2.store(1, 1)
+    m2.store(2, 1)
+    assert m2.link_chunk_major([[1, 2], [2, 1]])["slot_chunks"].tolist() == [1, 2]
