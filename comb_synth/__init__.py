@@ -259,3 +259,31 @@ def custom(name: str, *, k: int = 9, seed: int = 0, num_q_heads: int, num_kv_hea
         scale = 1.0 / float(np.sqrt(head_dim_qk))
     return Workload(name, k, seed, num_q_heads, num_kv_heads, head_dim_qk, head_dim_v, chunk_len, links, lq,
                     float(scale), q_gain)
+
+
+# --------------------------------------------------------------------------------------------
+# inputs of the steps either side of the attention: encoder hidden states, decoder rows
+# and projection weights.  Data only: N(0, std) float32 -> bf16 bits, one generator per tensor.
+# --------------------------------------------------------------------------------------------
+def normal_bf16(seed: int, tag: int, index: int, shape, std: float = 1.0) -> np.ndarray:
+    """bf16 bit patterns of N(0, std) values from ``default_rng([seed, 99, tag, index])``."""
+    rng = np.random.default_rng([seed, 99, int(tag), int(index)])
+    x = rng.standard_normal(tuple(int(s) for s in shape), dtype=np.float32) * np.float32(std)
+    return f32_to_bf16_bits(x)
+
+
+def hidden_states(seed: int, chunk: int, tokens: int, d_model: int) -> np.ndarray:
+    """H^E of one chunk, bf16 bits [tokens][d_model] (unit variance, like a normalised residual stream)."""
+    return normal_bf16(seed, 1, chunk, (tokens, d_model))
+
+
+def decoder_rows(seed: int, request: int, rows: int, d_model: int) -> np.ndarray:
+    """X^D rows of one request, bf16 bits [rows][d_model]."""
+    return normal_bf16(seed, 2, request, (rows, d_model))
+
+
+def projection_weight(seed: int, kind: int, layer: int, out_features: int, in_features: int,
+                      gain: float = 1.0) -> np.ndarray:
+    """nn.Linear-layout weight [out][in], N(0, gain / sqrt(in)) so that outputs of unit-variance inputs have
+    variance gain^2.  kind: 0 = W_KV, 1 = W_Q, 2 = W_O."""
+    return normal_bf16(seed, 10 + kind, layer, (out_features, in_features), gain / float(np.sqrt(in_features)))

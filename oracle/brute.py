@@ -52,3 +52,29 @@ def attention_brute(q_bits: np.ndarray, k_chunks: Sequence[np.ndarray], v_chunks
             O[i].append([math.fsum(w * v[c] for w, v in zip(weights, values)) / z for c in range(Dv)])
             L[i].append(math.log(z))
     return O, L
+
+
+def attention_request(q: np.ndarray, kcat: np.ndarray, vcat: np.ndarray, scale: float):
+    """The same brute force on fp64 inputs, keys already concatenated: q [lq][Hq][Dqk], kcat [kv][Hkv][Dqk],
+    vcat [kv][Hkv][Dv] -> (O [lq][Hq][Dv], LSE [lq][Hq]) as numpy arrays.  Pins oracle/layer.py::attention_f64."""
+    lq, Hq, Dqk = q.shape
+    kv, Hkv, Dv = vcat.shape
+    G = Hq // Hkv
+    O = np.zeros((lq, Hq, Dv))
+    L = np.full((lq, Hq), -math.inf)
+    for i in range(lq):
+        for h in range(Hq):
+            g = h // G
+            weights = []
+            for t in range(kv):
+                s = 0.0
+                for c in range(Dqk):
+                    s += float(q[i, h, c]) * float(kcat[t, g, c])
+                weights.append(math.exp(scale * s))
+            if not weights:
+                continue
+            z = math.fsum(weights)
+            for c in range(Dv):
+                O[i, h, c] = math.fsum(w * float(vcat[t, g, c]) for t, w in enumerate(weights)) / z
+            L[i, h] = math.log(z)
+    return O, L

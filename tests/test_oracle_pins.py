@@ -266,3 +266,124 @@ def test_chunk_major_inversion_hand_example():
     m2.store(1, 1)
     m2.store(2, 1)
     assert m2.link_chunk_major([[1, 2], [2, 1]])["slot_chunks"].tolist() == [1, 2]
+
+
+# ------------------------------------------------------------------------------------------------
+# oracle/layer.py — the projections and the sub-layer around the attention
+# ------------------------------------------------------------------------------------------------
+from oracle import layer as ol  # noqa: E402
+
+
+def _small_layer(seed=0, Hq=4, Hkv=2, Dqk=8, Dv=4, d_model=12):
+    rng = np.random.default_rng(seed)
+    lens = [5, 1, 7]
+    ck = [rng.standard_normal((t, Hkv, Dqk)) for t in lens]
+    cv = [rng.standard_normal((t, Hkv, Dv)) for t in lens]
+    links = [[2, 0], [], [1, 0, 2]]
+    q_indptr = np.array([0, 3, 5, 6], np.int32)
+    x = rng.standard_normal((6, d_model))
+    w_q = rng.standard_normal((Hq * Dqk, d_model)) / 3.0
+    w_o = rng.standard_normal((d_model, Hq * Dv)) / 3.0
+    return dict(x=x, q_indptr=q_indptr, w_q=w_q, w_o=w_o, Hq=Hq, ck=ck, cv=cv, links=links, scale=0.3)
+
+
+def test_project_kv_brute_force_and_identity():
+    """Eq. 5-6 by explicit loops; and with W = identity blocks the projection hands the hidden state through."""
+    rng = np.random.default_rng(1)
+    T, d_model, Hkv, Dqk, Dv = 5, 6, 2, 3, 2
+    h = rng.standard_normal((T, d_model))
+    w = rng.standard_normal((Hkv * (Dqk + Dv), d_model))
+    K, V = ol.project_kv(h, w, Hkv, Dqk, Dv)
+    for t in range(T):
+        for g in range(Hkv):
+            for d in range(Dqk):
+                assert abs(K[t, g, d] - sum(h[t, c] * w[g * Dqk + d, c] for c in range(d_model))) < 1e-13
+            for d in range(Dv):
+                assert abs(V[t, g, d] - sum(h[t, c] * w[Hkv * Dqk + g * Dv + d, c] for c in range(d_model))) < 1e-13
+    eye = np.zeros((Hkv * (Dqk + Dv), 10))
+    eye[np.arange(10), np.arange(10)] = 1.0
+    h10 = rng.standard_normal((T, 10))
+    K, V = ol.project_kv(h10, eye, Hkv, Dqk, Dv)
+    assert np.array_equal(K.reshape(T, -1), h10[:, :6]) and np.array_equal(V.reshape(T, -1), h10[:, 6:])
+
+
+def test_attention_f64_agrees_with_the_c_oracle_and_brute_force():
+    """Two independently written statements of Eq. 7-8 (C loops over bf16 inputs; numpy matmuls over fp64 inputs) on
+    bf16-exact values, plus the no-max-subtraction brute force; empty link gives O = 0, LSE = -inf."""
+    w = cs.custom("pin", num_q_heads=4, num_kv_heads=2, head_dim_qk=64, head_dim_v=64, chunk_len=[20, 37, 3],
+                  links=[[1, 0, 2], [], [2]], lq=[3, 2, 4])
+    O, L = oracle.attention_for(w)
+    for r in range(3):
+        q = ol.bf16_to_f64(w.request_q(r))
+        lst = [int(c) for c in w.links[r]]
+        kc = np.concatenate([ol.bf16_to_f64(w.chunk_kv(c)[0]) for c in lst], 0) if lst else np.zeros((0, 2, 64))
+        vc = np.concatenate([ol.bf16_to_f64(w.chunk_kv(c)[1]) for c in lst], 0) if lst else np.zeros((0, 2, 64))
+        o, l = ol.attention_f64(q, kc, vc, w.scale)
+        lo, hi = int(w.q_indptr[r]), int(w.q_indptr[r + 1])
+        assert np.abs(o - O[lo:hi]).max() <= 1e-12
+        if lst:
+            assert np.abs(l - L[lo:hi]).max() <= 1e-12
+            ob, lb = brute.attention_request(q, kc, vc, w.scale)
+            assert np.abs(o - ob).max() <= 1e-12 and np.abs(l - lb).max() <= 1e-12
+        else:
+            assert np.all(o == 0) and np.all(np.isneginf(l))
+
+
+def test_cross_layer_special_weights():
+    """PAPER.md:117 + 30: the sub-layer only ADDS to the decoder row, so W_O = 0 recovers it exactly (the plug-in
+    property); W_Q = 0 makes every score equal, so the attention is the mean of the linked V (P4) pushed through W_O;
+    the result is linear in W_O; a request that links nothing keeps its rows."""
+    a = _small_layer()
+    y = ol.cross_layer(a["x"], a["q_indptr"], a["w_q"], a["w_o"], a["Hq"], a["ck"], a["cv"], a["links"], a["scale"])
+    y0 = ol.cross_layer(a["x"], a["q_indptr"], a["w_q"], 0 * a["w_o"], a["Hq"], a["ck"], a["cv"], a["links"], a["scale"])
+    assert np.array_equal(y0, a["x"])
+    assert np.array_equal(y[3:5], a["x"][3:5])                       # request 1 links nothing
+    y2 = ol.cross_layer(a["x"], a["q_indptr"], a["w_q"], 2 * a["w_o"], a["Hq"], a["ck"], a["cv"], a["links"], a["scale"])
+    assert np.abs((y2 - a["x"]) - 2 * (y - a["x"])).max() <= 1e-13
+    yq = ol.cross_layer(a["x"], a["q_indptr"], 0 * a["w_q"], a["w_o"], a["Hq"], a["ck"], a["cv"], a["links"], a["scale"])
+    G = a["Hq"] // 2
+    for r, rows in ((0, range(0, 3)), (2, range(5, 6))):
+        vmean = np.concatenate([a["cv"][c] for c in a["links"][r]], 0).mean(0)     # [Hkv][Dv]
+        heads = np.concatenate([vmean[h // G] for h in range(a["Hq"])])             # [Hq*Dv]
+        for i in rows:
+            assert np.abs(yq[i] - (a["x"][i] + a["w_o"] @ heads)).max() <= 1e-13
+
+
+def test_cross_layer_brute_force():
+    """Eq. 4 + 7-8 + output projection by explicit loops and the brute-force attention (no max subtraction)."""
+    a = _small_layer(seed=3)
+    y = ol.cross_layer(a["x"], a["q_indptr"], a["w_q"], a["w_o"], a["Hq"], a["ck"], a["cv"], a["links"], a["scale"])
+    Hq, Dqk, Dv = a["Hq"], 8, 4
+    for r, lst in enumerate(a["links"]):
+        for i in range(a["q_indptr"][r], a["q_indptr"][r + 1]):
+            q = np.array([[sum(a["x"][i, c] * a["w_q"][h * Dqk + d, c] for c in range(12)) for d in range(Dqk)]
+                          for h in range(Hq)])
+            if lst:
+                kc = np.concatenate([a["ck"][c] for c in lst], 0)
+                vc = np.concatenate([a["cv"][c] for c in lst], 0)
+                o, _ = brute.attention_request(q[None], kc, vc, a["scale"])
+                o = o[0].reshape(-1)
+            else:
+                o = np.zeros(Hq * Dv)
+            want = a["x"][i] + np.array([sum(o[j] * a["w_o"][c, j] for j in range(Hq * Dv)) for c in range(12)])
+            assert np.abs(y[i] - want).max() <= 1e-12
+
+
+def test_cross_stack_is_the_layers_in_order():
+    a = _small_layer(seed=5)
+    wq = [a["w_q"], a["w_q"][::-1].copy()]
+    wo = [a["w_o"], a["w_o"][:, ::-1].copy()]
+    ck, cv = [a["ck"], [k[::-1].copy() for k in a["ck"]]], [a["cv"], [v * 0.5 for v in a["cv"]]]
+    st = ol.cross_stack(a["x"], a["q_indptr"], wq, wo, a["Hq"], ck, cv, a["links"], a["scale"])
+    y1 = ol.cross_layer(a["x"], a["q_indptr"], wq[0], wo[0], a["Hq"], ck[0], cv[0], a["links"], a["scale"])
+    y2 = ol.cross_layer(y1, a["q_indptr"], wq[1], wo[1], a["Hq"], ck[1], cv[1], a["links"], a["scale"])
+    assert np.array_equal(st[0], y1) and np.array_equal(st[1], y2)
+
+
+def test_bf16_rounding_helpers():
+    """bf16 keeps 8 significant bits: the spacing at 1.0 is 2^-7.  Hand-worked round-to-nearest-even cases."""
+    x = np.array([1.0, 1.0 + 2.0 ** -7, 1.0 + 2.0 ** -8, 1.0 + 3 * 2.0 ** -8, 1.0 + 2.0 ** -8 + 2.0 ** -20, -2.5, 0.0])
+    b = ol.f64_to_bf16_bits(x)
+    assert [hex(v) for v in b] == ["0x3f80", "0x3f81", "0x3f80", "0x3f82", "0x3f81", "0xc020", "0x0"]
+    #        exact     exact      tie -> even (down)  tie -> even (up)  just above the tie
+    assert np.array_equal(ol.bf16_to_f64(b), [1.0, 1.0078125, 1.0, 1.015625, 1.0078125, -2.5, 0.0])
