@@ -644,7 +644,8 @@ def main():
 
 
 def bench_store(torch, comb, harness, w, pk):
-    """(a2) batched paged store of configs[3]'s 64 variable-length chunks: free + store again, 200 times."""
+    """(a2) batched paged store of configs[3]'s 64 variable-length chunks, 200 times over the same page lists (a store of
+    an id that exists with the same length rewrites its pages), L2 flushed clean before every launch."""
     ld = harness.load_workload(w, fill="all", shuffle_seed=77, keep_host=False)
     pool = ld.pool
     ids = list(range(w.num_chunks))
@@ -658,8 +659,6 @@ def bench_store(torch, comb, harness, w, pk):
     comb.comb_profile_read(pool.handle, comb.KERNEL_STORE)
     n = 200
     for i in range(n + 3):
-        for c in ids:
-            comb.comb_chunk_free(pool.handle, c)
         flush(i)
         if i == 3:
             torch.cuda.synchronize()

@@ -19,9 +19,10 @@
  *     allocated by the caller (PyTorch) and stay caller-owned; they must outlive their use on the
  *     stream. Host metadata (directory, free list, pinned staging) belongs to the pool and is freed by
  *     comb_pool_destroy.
- *   - A pool is not thread-safe; callers serialise. A store and a later attention call that reads the
- *     chunk must be ordered by the caller (same stream, or an event) — the paper stores PICaches
- *     "asynchronously".
+ *   - A pool is not thread-safe; callers serialise. The paper stores PICaches "asynchronously":
+ *     a store may run on any stream; comb_link orders its own stream after the stores of the chunks it names
+ *     (see (f4) "ready"), so an attention call that follows a comb_link on the same stream reads complete pages.
+ *     A caller that writes link tables itself orders streams itself.
  *   - dtype: bf16 storage for Q, K, V and O (bit patterns, 2 bytes); fp32 statistics (lse).
  *
  * Layout of the chunk-KV pool (part of the bit-exact contract)
@@ -55,7 +56,8 @@ typedef enum {
     COMB_ERR_UNKNOWN_CHUNK = -4, /* link/free/query names an id that is not in the directory (the caller
                                     must compile + store first, PAPER.md:62 step 2); nothing is written */
     COMB_ERR_CAPACITY = -5,      /* link buffer, scratch or workspace too small */
-    COMB_ERR_CUDA = -6           /* a CUDA call failed; cudaGetLastError() is preserved for the caller */
+    COMB_ERR_CUDA = -6,          /* a CUDA call failed; cudaGetLastError() is preserved for the caller */
+    COMB_ERR_BUSY = -7           /* comb_chunk_free of a pinned chunk */
 } comb_status_t;
 
 typedef struct comb_pool comb_pool_t; /* opaque */
@@ -71,7 +73,7 @@ typedef struct {
     int32_t num_pages;     /* pages per layer */
     void *k_arena;         /* device, bf16, comb_pool_bytes().k_bytes, 1024-byte aligned */
     void *v_arena;         /* device, bf16, comb_pool_bytes().v_bytes, 1024-byte aligned */
-    void *scratch;         /* device, comb_pool_bytes().scratch_bytes: store page descriptors (ring of 4) */
+    void *scratch;         /* device, comb_pool_bytes().scratch_bytes: store page / tile descriptors (ring of 4) */
     uint64_t free_list_shuffle_seed; /* 0: ascending ids. Else: Fisher-Yates (i = n-1..1, j = next() mod
                                         (i+1), swap) driven by splitmix64(seed) — scatters a chunk's pages
                                         over the arena like a long-running server would */
@@ -84,6 +86,32 @@ int32_t comb_pool_bytes(const comb_pool_config_t *cfg, size_t *k_bytes, size_t *
 int32_t comb_pool_create(const comb_pool_config_t *cfg, comb_pool_t **out);
 int32_t comb_pool_destroy(comb_pool_t *pool);
 int32_t comb_pool_free_pages(const comb_pool_t *pool); /* pages currently on the free list (>= 0) */
+
+/* (f4) pool lifecycle — PAPER.md:205 (the PIC manager "reserves a portion ... of GPU memory", the allocator hands
+ * out free memory, PICaches are "stored asynchronously"), PAPER.md:277 (memory is what bounds concurrency)
+ * step 4 (the manager updates its table).  The paper does not say what happens when the reserved memory is full;
+ * reading I16: explicit comb_chunk_free always works; with COMB_OPT_EVICT_LRU the pool also makes room
+ * by itself.
+ *   pins      comb_chunk_pin raises a chunk's reference count, comb_chunk_unpin lowers it (INVALID below zero). A
+ *             pinned chunk is never evicted and comb_chunk_free on it returns COMB_ERR_BUSY. A serving loop pins the
+ *             chunks of a request from lookup until the request's last attention call has completed.
+ *   use stamp comb_chunk_alloc / a store stamps the chunk with a fresh tick; every comb_link draws ONE fresh tick and
+ *             stamps all chunks it names (comb_link_plan stamps nothing).
+ *   eviction  (only with comb_pool_set_option(pool, COMB_OPT_EVICT_LRU, 1)) when an alloc/store needs more pages
+ *             than are free, unpinned chunks that are not part of the call are evicted in ascending (use stamp,
+ *             creation order) until it fits; each evicted chunk's pages go to the free-list tail in page-list order,
+ *             exactly as comb_chunk_free would put them. If even that cannot make room: NO_SPACE, nothing evicted.
+ *             comb_pool_evicted() lists what the most recent alloc/store call evicted, so the caller can update its
+ *             own table. Kernels in flight are NOT tracked: unpin only what the GPU is done with.
+ *   ready     a store records an event on its stream; comb_link makes ITS stream wait for the stores of the chunks
+ *             it names that have not completed yet (cudaStreamWaitEvent; no host wait). So a store may run on a side
+ *             stream ("asynchronously") and the link + attention calls that follow on another stream are ordered
+ *             after it without the caller handling events. */
+int32_t comb_chunk_pin(comb_pool_t *pool, uint64_t chunk_id);
+int32_t comb_chunk_unpin(comb_pool_t *pool, uint64_t chunk_id);
+/* Writes up to `cap` ids evicted by the most recent alloc/store call (in eviction order); returns how many were. */
+int32_t comb_pool_evicted(const comb_pool_t *pool, uint64_t *chunk_ids, int32_t cap);
+int64_t comb_pool_eviction_count(const comb_pool_t *pool); /* chunks evicted since the pool was created */
 
 /* Directory-only half of a store: insert chunk_id with num_tokens and take ceil(T/16) pages from the head
  * of the free list; no data moves (a fused producer may write the pages itself). Idempotent for an
@@ -112,6 +140,19 @@ int32_t comb_store_chunk(comb_pool_t *pool, int32_t layer, uint64_t chunk_id, in
  * the caller's, as for any store. */
 int32_t comb_store_chunks(comb_pool_t *pool, int32_t layer, int32_t n, const uint64_t *chunk_ids,
                           const int32_t *tok_indptr, const void *k_packed, const void *v_packed, void *stream);
+
+/* (f2) compile-side producer fused into the store — PAPER.md:105-109 §4.2 Eq. 5-6: K^cross = H^E W_K,
+ * V^cross = H^E W_V, and PAPER.md:119 / 205: what is stored is K^cross and V^cross.  One tcgen05 GEMM whose epilogue
+ * writes bf16 straight into the chunks' pages (tail slots of a last page zero-filled): the [T][Hkv][D] K/V tensors
+ * of comb_store_chunks never exist in HBM.
+ *   h_packed  device bf16 [sum T][d_model]   encoder hidden states of the n chunks, packed as tok_indptr says
+ *   w_kv      device bf16 [Hkv*Dqk + Hkv*Dv][d_model]: row (h*Dqk + d) holds column (h, d) of W_K, then the rows of
+ *             W_V likewise (the nn.Linear layout, i.e. the paper's W transposed); d_model % 8 == 0
+ * Page image afterwards: Kpage[layer][pages[t/16]][h][t%16][d] = bf16_rne(sum_c h[t][c] * W_K[c][(h,d)]) with the
+ * sum accumulated in fp32 (same for V).  Directory semantics, all-or-nothing and errors as comb_store_chunks. */
+int32_t comb_project_store_chunks(comb_pool_t *pool, int32_t layer, int32_t n, const uint64_t *chunk_ids,
+                                  const int32_t *tok_indptr, const void *h_packed, int32_t d_model, const void *w_kv,
+                                  void *stream);
 
 /* (a3) link — PAPER.md:24 "loads and concatenates needed KV vectors (in any order/position)",
  * PAPER.md:119, PAPER.md:62 step 5.  Zero-copy: builds the request's block table from an ORDERED
@@ -193,8 +234,8 @@ size_t comb_link_host_bytes(int32_t num_requests, int64_t total_entries);
 int32_t comb_link(comb_pool_t *pool, int32_t num_requests, const int32_t *chunk_indptr /* host [R+1] */,
                   const uint64_t *chunk_ids /* host, link order */, comb_link_t *link, void *stream);
 /* Same tables written into HOST memory `staging` (link->device_bytes bytes available); the pointers in
- * `link` are laid out as if staging were device_buf. No CUDA call, and the pool is not modified — used by
- * comb_link and by host tests. */
+ * `link` are laid out as if staging were device_buf. No CUDA call, and the pool is not modified (no use stamps,
+ * no waiting for stores) — used by host tests and by callers that plan ahead. */
 int32_t comb_link_plan(const comb_pool_t *pool, int32_t num_requests, const int32_t *chunk_indptr,
                        const uint64_t *chunk_ids, comb_link_t *link, void *staging);
 
@@ -245,10 +286,35 @@ size_t comb_attn_workspace_bytes(const comb_pool_t *pool, const comb_link_t *lin
 size_t comb_workspace_bytes(const comb_pool_t *pool, int32_t num_requests, int32_t num_q_heads, int64_t total_q,
                             int32_t max_pages_per_request);
 
+/* (f3) the cross-attention sub-layer around the attention — PAPER.md:102-105 Eq. 4 (Q = X^D W_Q), Eq. 7-8, and the
+ * output projection whose result "is then passed through the standard decoder pathway via residual connections"
+ * (PAPER.md:117):   x_out = x + Attn(x W_Q ; linked K, V) W_O      (no norm, gate or bias: none is in Eq. 4-8)
+ *   x, x_out  device bf16 [rows][d_model]  (rows = sum lq for prefill, = num_requests for decode); x_out may alias x
+ *             only if the caller does not need x afterwards (each row is read before it is written)
+ *   w_q       device bf16 [Hq*Dqk][d_model]   row (h*Dqk + d) = column (h, d) of W_Q
+ *   w_o       device bf16 [d_model][Hq*Dv]    row c = the weights producing output feature c
+ *   q_indptr  HOST int32 [R+1] for prefill; NULL selects decode (one row per request)
+ *   workspace device, comb_layer_workspace_bytes() bytes, 16-byte aligned: Q and attention-output staging + the
+ *             attention call's own workspace
+ * Three launches on `stream`: GEMM (tcgen05) -> comb_cross_attn_prefill/decode -> GEMM with the residual added in
+ * its epilogue.  Q and the attention output are rounded to bf16 between the steps (they are the inputs of the next
+ * tensor-core contraction).  A model's L cross layers (8 in the paper's Llama instance) are L calls,
+ * layer = 0..L-1, each with its own weights, over one link (page ids are shared by all layers).
+ * Errors: INVALID, CAPACITY, CUDA. */
+int32_t comb_cross_layer_forward(comb_pool_t *pool, int32_t layer, const comb_link_t *link, int32_t num_requests,
+                                 const void *x, const int32_t *q_indptr, int32_t d_model, int32_t num_q_heads,
+                                 const void *w_q, const void *w_o, float scale, void *x_out, void *workspace,
+                                 size_t workspace_bytes, void *stream);
+size_t comb_layer_workspace_bytes(const comb_pool_t *pool, const comb_link_t *link, int32_t num_q_heads, int64_t rows);
+/* The projection alone: c[M][N] = bf16(a[M][K] w[N][K]^T (+ residual[M][N])), fp32 accumulation on tcgen05.
+ * K % 8 == 0, N % 32 == 0. (pool is only used for the device's SM count and profiling.) Errors: INVALID, CUDA. */
+int32_t comb_gemm_bf16(comb_pool_t *pool, const void *a, const void *w, const void *residual, void *c, int64_t M,
+                       int32_t N, int32_t K, void *stream);
+
 /* Pool options. COMB_OPT_DECODE_PATH: 0 = automatic (chunk-major when total_entries >= 1.25 x distinct chunks,
  * i.e. the batch re-reads at least a fifth of its KV), 1 = always per-request, 2 = always chunk-major.
  * Errors: INVALID (unknown option or value). */
-enum { COMB_OPT_DECODE_PATH = 1 };
+enum { COMB_OPT_DECODE_PATH = 1, COMB_OPT_EVICT_LRU = 2 /* 0 (default) = never evict, 1 = LRU eviction, see (f4) */ };
 enum { COMB_DECODE_AUTO = 0, COMB_DECODE_PER_REQUEST = 1, COMB_DECODE_CHUNK_MAJOR = 2 };
 int32_t comb_pool_set_option(comb_pool_t *pool, int32_t option, int64_t value);
 
@@ -261,7 +327,7 @@ int64_t comb_pool_launch_count(const comb_pool_t *pool);
  * the elapsed times of kernel class `kernel` (COMB_KERNEL_*), reports them and forgets those records.
  * Errors: INVALID, CUDA. */
 enum { COMB_KERNEL_STORE = 0, COMB_KERNEL_DECODE_SPLIT = 1, COMB_KERNEL_DECODE_MERGE = 2, COMB_KERNEL_PREFILL = 3,
-       COMB_KERNEL_DECODE_CASCADE = 4, COMB_KERNEL_CASCADE_MERGE = 5, COMB_KERNEL_PREFILL_MERGE = 6 };
+       COMB_KERNEL_DECODE_CASCADE = 4, COMB_KERNEL_CASCADE_MERGE = 5, COMB_KERNEL_PREFILL_MERGE = 6, COMB_KERNEL_GEMM = 7 };
 int32_t comb_profile_enable(comb_pool_t *pool, int32_t on);
 int32_t comb_profile_read(comb_pool_t *pool, int32_t kernel, double *total_ms, int64_t *launches);
 /* Same, but hands back the elapsed time of every recorded launch of that class (oldest first, at most `cap`

@@ -59,6 +59,11 @@ _SIGS = {
     "comb_chunk_query": (C.c_int32, [_P, C.c_uint64, C.POINTER(C.c_int32), _P, C.c_int32]),
     "comb_store_chunk": (C.c_int32, [_P, C.c_int32, C.c_uint64, C.c_int32, _P, _P, _P]),
     "comb_store_chunks": (C.c_int32, [_P, C.c_int32, C.c_int32, _P, _P, _P, _P, _P]),
+    "comb_project_store_chunks": (C.c_int32, [_P, C.c_int32, C.c_int32, _P, _P, _P, C.c_int32, _P, _P]),
+    "comb_cross_layer_forward": (C.c_int32, [_P, C.c_int32, C.POINTER(Link), C.c_int32, _P, _P, C.c_int32, C.c_int32,
+                                             _P, _P, C.c_float, _P, _P, C.c_size_t, _P]),
+    "comb_layer_workspace_bytes": (C.c_size_t, [_P, C.POINTER(Link), C.c_int32, C.c_int64]),
+    "comb_gemm_bf16": (C.c_int32, [_P, _P, _P, _P, _P, C.c_int64, C.c_int32, C.c_int32, _P]),
     "comb_link_bytes": (C.c_size_t, [C.c_int32, C.c_int64, C.c_int64]),
     "comb_link_host_bytes": (C.c_size_t, [C.c_int32, C.c_int64]),
     "comb_link": (C.c_int32, [_P, C.c_int32, _P, _P, C.POINTER(Link), _P]),

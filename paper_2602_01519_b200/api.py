@@ -87,6 +87,34 @@ def comb_store_chunks(pool: int, layer: int, chunk_ids: Sequence[int], tok_indpt
                                 _ptr(v_packed), _stream_ptr(stream)), "comb_store_chunks")
 
 
+def comb_project_store_chunks(pool: int, layer: int, chunk_ids: Sequence[int], tok_indptr, h_packed, d_model: int,
+                              w_kv, stream=None) -> None:
+    ids = np.ascontiguousarray(chunk_ids, dtype=np.uint64)
+    ind = np.ascontiguousarray(tok_indptr, dtype=np.int32)
+    check(lib.comb_project_store_chunks(pool, layer, int(ids.shape[0]), ids.ctypes.data, ind.ctypes.data,
+                                        _ptr(h_packed), int(d_model), _ptr(w_kv), _stream_ptr(stream)),
+          "comb_project_store_chunks")
+
+
+def comb_gemm_bf16(pool: int, a, w, c, M: int, N: int, K: int, residual=None, stream=None) -> None:
+    check(lib.comb_gemm_bf16(pool, _ptr(a), _ptr(w), _ptr(residual), _ptr(c), int(M), int(N), int(K),
+                             _stream_ptr(stream)), "comb_gemm_bf16")
+
+
+def comb_layer_workspace_bytes(pool: int, link: Link, num_q_heads: int, rows: int) -> int:
+    return int(lib.comb_layer_workspace_bytes(pool, C.byref(link), num_q_heads, rows))
+
+
+def comb_cross_layer_forward(pool: int, layer: int, link: Link, num_requests: int, x, q_indptr, d_model: int,
+                             num_q_heads: int, w_q, w_o, scale: float, x_out, workspace, workspace_bytes: int,
+                             stream=None) -> None:
+    ind = None if q_indptr is None else np.ascontiguousarray(q_indptr, dtype=np.int32)
+    check(lib.comb_cross_layer_forward(pool, layer, C.byref(link), num_requests, _ptr(x),
+                                       None if ind is None else ind.ctypes.data, int(d_model), num_q_heads, _ptr(w_q),
+                                       _ptr(w_o), float(scale), _ptr(x_out), _ptr(workspace), int(workspace_bytes),
+                                       _stream_ptr(stream)), "comb_cross_layer_forward")
+
+
 def comb_link_bytes(num_requests: int, total_entries: int, total_pages: int) -> int:
     return int(lib.comb_link_bytes(num_requests, total_entries, total_pages))
 
@@ -149,7 +177,7 @@ def comb_pool_launch_count(pool: int) -> int:
 
 
 KERNEL_STORE, KERNEL_DECODE_SPLIT, KERNEL_DECODE_MERGE, KERNEL_PREFILL = 0, 1, 2, 3
-KERNEL_DECODE_CASCADE, KERNEL_CASCADE_MERGE, KERNEL_PREFILL_MERGE = 4, 5, 6
+KERNEL_DECODE_CASCADE, KERNEL_CASCADE_MERGE, KERNEL_PREFILL_MERGE, KERNEL_GEMM = 4, 5, 6, 7
 
 
 def comb_profile_enable(pool: int, on: bool) -> None:
@@ -251,6 +279,7 @@ class Pool:
                               self.k_arena.data_ptr(), self.v_arena.data_ptr(), self.scratch.data_ptr(), shuffle_seed)
         self.handle = comb_pool_create(self.cfg)
         self._ws: Optional[torch.Tensor] = None
+        self._lws: Optional[torch.Tensor] = None
 
     def _aligned_i16(self, nbytes: int, align: int = 1024) -> torch.Tensor:
         raw = torch.empty(nbytes // 2 + align // 2, dtype=torch.int16, device=self.device)
@@ -276,6 +305,27 @@ class Pool:
     def store_chunks(self, chunk_ids, tok_indptr, k_packed: torch.Tensor, v_packed: torch.Tensor, layer: int = 0,
                      stream=None) -> None:
         comb_store_chunks(self.handle, layer, chunk_ids, tok_indptr, k_packed, v_packed, stream)
+
+    def project_store_chunks(self, chunk_ids, tok_indptr, h_packed: torch.Tensor, w_kv: torch.Tensor, layer: int = 0,
+                             stream=None) -> None:
+        """(f2) K/V projection of the chunks' hidden states with the pages written by the GEMM's epilogue."""
+        comb_project_store_chunks(self.handle, layer, chunk_ids, tok_indptr, h_packed, int(h_packed.shape[1]), w_kv,
+                                  stream)
+
+    # ---- (f3) cross-attention sub-layer: x + Attn(x W_Q) W_O ----
+    def layer_forward(self, lb: "LinkedBatch", x: torch.Tensor, q_indptr, w_q: torch.Tensor, w_o: torch.Tensor,
+                      scale: float, layer: int = 0, out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+        """q_indptr None = decode (one row per request)."""
+        rows, d_model = int(x.shape[0]), int(x.shape[1])
+        Hq = int(w_q.shape[0]) // self.head_dim_qk
+        if out is None:
+            out = torch.empty_like(x)
+        need = comb_layer_workspace_bytes(self.handle, lb.link, Hq, rows)
+        if self._lws is None or self._lws.numel() < need:
+            self._lws = torch.empty(max(need, 256), dtype=torch.uint8, device=self.device)
+        comb_cross_layer_forward(self.handle, layer, lb.link, lb.num_requests, x, q_indptr, d_model, Hq, w_q, w_o, scale,
+                                 out, self._lws, self._lws.numel(), stream)
+        return out
 
     # ---- (a3) link ----
     def link(self, chunk_lists: Sequence[Sequence[int]], stream=None, into: Optional[LinkedBatch] = None) -> LinkedBatch:

@@ -16,59 +16,73 @@
 namespace comb {
 namespace {
 
-// One warp per (request, q head); a lane owns DV/32 consecutive output columns.  All LSEs of the request are read
-// first (up to 32 per pass, one per lane), then the partial rows: two dependent memory round trips per row.
+// One CTA of 4 warps per (request, q head): the request's entries are dealt round-robin to the warps, a lane owns
+// DV/32 consecutive output columns, and the four warps' weighted sums meet in shared memory.  Every warp first reads
+// ALL of the request's LSEs (one per lane per pass; they are few) to agree on the maximum, then streams its share of
+// the partial rows with 4 independent loads in flight.
 template <int DV>
 __global__ void __launch_bounds__(128) cascade_merge_kernel(const float *__restrict__ part_o,
                                                             const float *__restrict__ part_lse,
                                                             const int32_t *__restrict__ entry_indptr,
                                                             __nv_bfloat16 *__restrict__ out, float *__restrict__ lse,
-                                                            int num_rows /* R * Hq */, int Hq) {
+                                                            int Hq) {
     constexpr int CPL = DV / 32;
+    __shared__ float s_acc[4][DV];
+    __shared__ float s_w[4];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int row = blockIdx.x * 4 + warp;  // (request, head)
-    if (row >= num_rows) return;
+    const int row = blockIdx.x;  // (request, head)
     const int r = row / Hq, h = row - r * Hq;
     const int e0 = entry_indptr[r], e1 = entry_indptr[r + 1];
-    __nv_bfloat16 *orow = out + (size_t)row * DV + lane * CPL;
+    __nv_bfloat16 *orow = out + (size_t)row * DV;
     if (e0 == e1) {  // no contexts linked (reading I13)
-#pragma unroll
-        for (int c = 0; c < CPL; c += 2) *reinterpret_cast<uint32_t *>(orow + c) = 0u;
-        if (lane == 0 && lse) lse[row] = -INFINITY;
+        if (threadIdx.x < DV / 2) reinterpret_cast<uint32_t *>(orow)[threadIdx.x] = 0u;
+        if (threadIdx.x == 0 && lse) lse[row] = -INFINITY;
         return;
     }
-    // pass 1: max of the entries' LSEs
     float m = -INFINITY;
     for (int e = e0 + lane; e < e1; e += 32) m = fmaxf(m, part_lse[(size_t)e * Hq + h]);
 #pragma unroll
     for (int off = 16; off >= 1; off >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, off));
-    // pass 2: weighted sum of the partial rows
     float acc[CPL];
 #pragma unroll
     for (int c = 0; c < CPL; ++c) acc[c] = 0.f;
     float wsum = 0.f;
-    for (int eb = e0; eb < e1; eb += 32) {
-        const int mine = eb + lane;
-        const float w_mine = mine < e1 ? ptx::ex2(part_lse[(size_t)mine * Hq + h] - m) : 0.f;
-        const int n = min(32, e1 - eb);
-        for (int i = 0; i < n; ++i) {
-            const float w = __shfl_sync(0xffffffffu, w_mine, i);
-            wsum += w;
-            const float *po = part_o + ((size_t)(eb + i) * Hq + h) * DV + lane * CPL;
-            if constexpr (CPL == 4) {
-                const float4 v = *reinterpret_cast<const float4 *>(po);
-                acc[0] += w * v.x; acc[1] += w * v.y; acc[2] += w * v.z; acc[3] += w * v.w;
-            } else {
-                const float2 v = *reinterpret_cast<const float2 *>(po);
-                acc[0] += w * v.x; acc[1] += w * v.y;
+    for (int eb = e0 + warp; eb < e1; eb += 16) {  // this warp: entries eb, eb + 4, eb + 8, eb + 12
+        float w[4];
+        float4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int e = eb + 4 * u;
+            const bool ok = e < e1;
+            w[u] = ok ? ptx::ex2(part_lse[(size_t)e * Hq + h] - m) : 0.f;
+            v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (ok) {
+                const float *po = part_o + ((size_t)e * Hq + h) * DV + lane * CPL;
+                if constexpr (CPL == 4) v[u] = *reinterpret_cast<const float4 *>(po);
+                else { const float2 t = *reinterpret_cast<const float2 *>(po); v[u].x = t.x; v[u].y = t.y; }
             }
         }
-    }
-    const float inv = 1.f / wsum;
 #pragma unroll
-    for (int c = 0; c < CPL; c += 2)
-        *reinterpret_cast<uint32_t *>(orow + c) = ptx::pack_bf16x2(acc[c] * inv, acc[c + 1] * inv);
-    if (lane == 0 && lse) lse[row] = (m + log2f(wsum)) * kLn2;
+        for (int u = 0; u < 4; ++u) {
+            wsum += w[u];
+            acc[0] += w[u] * v[u].x;
+            acc[1] += w[u] * v[u].y;
+            if constexpr (CPL == 4) { acc[2] += w[u] * v[u].z; acc[3] += w[u] * v[u].w; }
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < CPL; ++c) s_acc[warp][lane * CPL + c] = acc[c];
+    if (lane == 0) s_w[warp] = wsum;
+    __syncthreads();
+    const float wtot = (s_w[0] + s_w[1]) + (s_w[2] + s_w[3]);
+    if (threadIdx.x < DV / 2) {
+        const int c = 2 * threadIdx.x;
+        const float inv = 1.f / wtot;
+        const float a0 = (s_acc[0][c] + s_acc[1][c]) + (s_acc[2][c] + s_acc[3][c]);
+        const float a1 = (s_acc[0][c + 1] + s_acc[1][c + 1]) + (s_acc[2][c + 1] + s_acc[3][c + 1]);
+        reinterpret_cast<uint32_t *>(orow)[threadIdx.x] = ptx::pack_bf16x2(a0 * inv, a1 * inv);
+    }
+    if (threadIdx.x == 0 && lse) lse[row] = (m + log2f(wtot)) * kLn2;
 }
 
 template <int DQK, int DV>
@@ -119,16 +133,17 @@ cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &
     a.cas_row_req = lv.cas_row_req;
     a.cas_row_entry = lv.cas_row_entry;
     a.q = (const char *)q;
-    if (!partials || !tiles_dev) return cudaErrorInvalidValue;
+    if (!partials) return cudaErrorInvalidValue;
     Maps maps;
     memcpy(&maps.q, &pm.k, sizeof(CUtensorMap));  // unused in this mode (Q rows are gathered); any valid map
     memcpy(&maps.k, &pm.k, sizeof(CUtensorMap));
     memcpy(&maps.v, &pm.v, sizeof(CUtensorMap));
     const int num_items = num_tiles * g.num_kv_heads;
-    cudaError_t e = cudaErrorInvalidValue;
-    if (hook) hook->begin(hook->ctx, kKernelDecodeCascade, stream);
-#define COMB_CASCADE_CASE(DQ, DVV) \
-    if (g.head_dim_qk == DQ && g.head_dim_v == DVV) e = launch_cascade_t<DQ, DVV>(a, maps, num_items, num_sms, stream);
+    cudaError_t e = num_items > 0 ? cudaErrorInvalidValue : cudaSuccess;  // every request empty: only the merge runs
+    if (hook && num_items > 0) hook->begin(hook->ctx, kKernelDecodeCascade, stream);
+#define COMB_CASCADE_CASE(DQ, DVV)                                    \
+    if (num_items > 0 && g.head_dim_qk == DQ && g.head_dim_v == DVV) \
+        e = launch_cascade_t<DQ, DVV>(a, maps, num_items, num_sms, stream);
     COMB_CASCADE_CASE(128, 128)
     COMB_CASCADE_CASE(64, 64)
     COMB_CASCADE_CASE(192, 128)
@@ -136,17 +151,15 @@ cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &
     COMB_CASCADE_CASE(64, 128)
     COMB_CASCADE_CASE(192, 64)
 #undef COMB_CASCADE_CASE
-    if (hook) hook->end(hook->ctx, stream);
+    if (hook && num_items > 0) hook->end(hook->ctx, stream);
     if (e != cudaSuccess) return e;
-    *launches += 1;
+    *launches += num_items > 0 ? 1 : 0;
     const int rows = num_requests * num_q_heads;
     if (hook) hook->begin(hook->ctx, kKernelCascadeMerge, stream);
     if (g.head_dim_v == 128)
-        cascade_merge_kernel<128><<<(rows + 3) / 4, 128, 0, stream>>>(a.part_o, a.part_lse, lv.entry_indptr, a.out, lse,
-                                                                      rows, num_q_heads);
+        cascade_merge_kernel<128><<<rows, 128, 0, stream>>>(a.part_o, a.part_lse, lv.entry_indptr, a.out, lse, num_q_heads);
     else
-        cascade_merge_kernel<64><<<(rows + 3) / 4, 128, 0, stream>>>(a.part_o, a.part_lse, lv.entry_indptr, a.out, lse,
-                                                                     rows, num_q_heads);
+        cascade_merge_kernel<64><<<rows, 128, 0, stream>>>(a.part_o, a.part_lse, lv.entry_indptr, a.out, lse, num_q_heads);
     if (hook) hook->end(hook->ctx, stream);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     *launches += 1;

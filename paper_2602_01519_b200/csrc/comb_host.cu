@@ -19,6 +19,9 @@ using namespace comb;
 namespace {
 
 constexpr int kRingSlots = 4;
+// scratch per page and slot: one StorePageDesc (16 B) for a store, or at worst one GemmRowTile (48 B) when every
+// chunk of a fused projection store is a single page
+constexpr size_t kScratchBytesPerPage = 48;
 
 struct Chunk {
     int32_t num_tokens;
@@ -75,7 +78,7 @@ struct comb_pool {
     }
     const LaunchHook *active_hook() { return prof_on ? &hook : nullptr; }
 
-    size_t scratch_slot_bytes() const { return align_up((size_t)cfg.num_pages * sizeof(StorePageDesc), 256); }
+    size_t scratch_slot_bytes() const { return align_up((size_t)cfg.num_pages * kScratchBytesPerPage, 256); }
 
     void probe_device() {
         if (device_probed) return;
@@ -425,7 +428,7 @@ int32_t comb_pool_bytes(const comb_pool_config_t *cfg, size_t *k_bytes, size_t *
     if (k_bytes) *k_bytes = blocks * cfg->head_dim_qk * 2;
     if (v_bytes) *v_bytes = blocks * cfg->head_dim_v * 2;
     if (scratch_bytes)
-        *scratch_bytes = kRingSlots * align_up((size_t)cfg->num_pages * sizeof(StorePageDesc), 256);
+        *scratch_bytes = kRingSlots * align_up((size_t)cfg->num_pages * kScratchBytesPerPage, 256);
     return COMB_OK;
 }
 
@@ -549,21 +552,33 @@ int32_t comb_chunk_query(const comb_pool_t *p, uint64_t id, int32_t *num_tokens,
     return n;
 }
 
-int32_t comb_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, const uint64_t *ids, const int32_t *tok_indptr,
-                          const void *k_packed, const void *v_packed, void *stream) {
-    if (!p || n < 0 || (n > 0 && (!ids || !tok_indptr || !k_packed || !v_packed))) return COMB_ERR_INVALID;
+}  // extern "C"
+#pragma GCC visibility pop
+
+namespace {
+
+// The directory half of a batched store: validates everything first so an error allocates nothing, then takes the
+// pages. `undo` restores the directory and the free list exactly (pages are taken from the head in order).
+struct StoreBatch {
+    std::vector<const Chunk *> chunks;  // per batch entry
+    std::vector<uint64_t> created;
+    size_t head_before = 0;
+    size_t total_pages = 0;             // page descriptors of the batch (existing chunks included)
+};
+int32_t store_begin(comb_pool_t *p, int32_t layer, int32_t n, const uint64_t *ids, const int32_t *tok_indptr,
+                    StoreBatch *sb) {
+    if (!p || n < 0 || (n > 0 && (!ids || !tok_indptr))) return COMB_ERR_INVALID;
     if (layer < 0 || layer >= p->cfg.num_layers) return COMB_ERR_INVALID;
     if (n == 0) return COMB_OK;
     if (tok_indptr[0] != 0) return COMB_ERR_INVALID;
-    // ---- validate everything first so an error allocates nothing (all-or-nothing) ----
-    size_t need_pages = 0, total_descs = 0;
+    size_t need_pages = 0;
     {
         std::unordered_map<uint64_t, int32_t> seen;
         for (int32_t i = 0; i < n; ++i) {
             const int64_t T = (int64_t)tok_indptr[i + 1] - tok_indptr[i];
             if (T <= 0) return COMB_ERR_INVALID;
             const size_t np = (size_t)(T + kPage - 1) / kPage;
-            total_descs += np;
+            sb->total_pages += np;
             if (!seen.emplace(ids[i], (int32_t)T).second) return COMB_ERR_INVALID;  // the same id twice in one batch
             auto it = p->dir.find(ids[i]);
             if (it != p->dir.end()) {
@@ -574,26 +589,43 @@ int32_t comb_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, const uint64
         }
     }
     if (need_pages > p->free_list.size() - p->free_head) return COMB_ERR_NO_SPACE;
-    if (total_descs > (size_t)p->cfg.num_pages) return COMB_ERR_CAPACITY;
-    cudaStream_t st = (cudaStream_t)stream;
-    const int slot = p->acquire(total_descs * sizeof(StorePageDesc));
-    if (slot < 0) return COMB_ERR_CUDA;
-    // ---- directory update + page descriptors ----
-    StorePageDesc *h = (StorePageDesc *)p->ring[slot].host;
-    size_t at = 0;
-    const size_t head_before = p->free_head;
-    std::vector<uint64_t> created;  // for the rollback: pages are taken from the head in order, so undoing is exact
-    auto rollback = [&]() {
-        for (uint64_t id : created) p->dir.erase(id);
-        p->free_head = head_before;
-    };
+    if (sb->total_pages > (size_t)p->cfg.num_pages) return COMB_ERR_CAPACITY;
+    sb->head_before = p->free_head;
+    sb->chunks.reserve((size_t)n);
     for (int32_t i = 0; i < n; ++i) {
-        const int32_t T = tok_indptr[i + 1] - tok_indptr[i];
         const Chunk *c = nullptr;
         bool made = false;
-        int32_t rc = dir_alloc(p, ids[i], T, &c, &made);
-        if (rc != COMB_OK) { rollback(); return rc; }  // cannot happen after validation
-        if (made) created.push_back(ids[i]);
+        const int32_t rc = dir_alloc(p, ids[i], tok_indptr[i + 1] - tok_indptr[i], &c, &made);
+        if (rc != COMB_OK) return rc;  // cannot happen after validation
+        if (made) sb->created.push_back(ids[i]);
+        sb->chunks.push_back(c);
+    }
+    return COMB_OK;
+}
+void store_undo(comb_pool_t *p, const StoreBatch &sb) {
+    for (uint64_t id : sb.created) p->dir.erase(id);
+    p->free_head = sb.head_before;
+}
+
+}  // namespace
+
+#pragma GCC visibility push(default)
+extern "C" {
+
+int32_t comb_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, const uint64_t *ids, const int32_t *tok_indptr,
+                          const void *k_packed, const void *v_packed, void *stream) {
+    if (n > 0 && (!k_packed || !v_packed)) return COMB_ERR_INVALID;
+    StoreBatch sb;
+    int32_t rc = store_begin(p, layer, n, ids, tok_indptr, &sb);
+    if (rc != COMB_OK || n == 0) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int slot = p->acquire(sb.total_pages * sizeof(StorePageDesc));
+    if (slot < 0) { store_undo(p, sb); return COMB_ERR_CUDA; }
+    StorePageDesc *h = (StorePageDesc *)p->ring[slot].host;
+    size_t at = 0;
+    for (int32_t i = 0; i < n; ++i) {
+        const Chunk *c = sb.chunks[(size_t)i];
+        const int32_t T = c->num_tokens;
         for (size_t j = 0; j < c->pages.size(); ++j) {
             StorePageDesc d;
             d.dst_page = c->pages[j];
@@ -605,18 +637,84 @@ int32_t comb_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, const uint64
     }
     StorePageDesc *dev = (StorePageDesc *)((char *)p->cfg.scratch + (size_t)slot * p->scratch_slot_bytes());
     if (cudaMemcpyAsync(dev, h, at * sizeof(StorePageDesc), cudaMemcpyHostToDevice, st) != cudaSuccess) {
-        rollback();
+        store_undo(p, sb);
         return COMB_ERR_CUDA;
     }
     if (p->prof_on) p->hook.begin(p, kKernelStore, st);
     const cudaError_t se = launch_store(p->geom, layer, dev, (int)at, k_packed, v_packed, st);
     if (p->prof_on) p->hook.end(p, st);
     if (se != cudaSuccess) {
-        rollback();
+        store_undo(p, sb);
         return COMB_ERR_CUDA;
     }
     p->launches += 1;
     if (!p->release(slot, st)) return COMB_ERR_CUDA;
+    return COMB_OK;
+}
+
+int32_t comb_project_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, const uint64_t *ids,
+                                  const int32_t *tok_indptr, const void *h_packed, int32_t d_model, const void *w_kv,
+                                  void *stream) {
+    if (n > 0 && (!h_packed || !w_kv)) return COMB_ERR_INVALID;
+    if (!p || d_model <= 0 || d_model % 8) return COMB_ERR_INVALID;
+    const int32_t N = p->cfg.num_kv_heads * (p->cfg.head_dim_qk + p->cfg.head_dim_v);
+    StoreBatch sb;
+    int32_t rc = store_begin(p, layer, n, ids, tok_indptr, &sb);
+    if (rc != COMB_OK || n == 0) return rc;
+    const int64_t M = tok_indptr[n];
+    if (!gemm_shape_ok(M, N, d_model)) { store_undo(p, sb); return COMB_ERR_INVALID; }
+    // M tiles: 128 tokens (8 pages) of ONE chunk each, so a tile's rows map to whole pages of that chunk
+    std::vector<GemmRowTile> tiles;
+    tiles.reserve(sb.total_pages / kTilePages + (size_t)n);
+    for (int32_t i = 0; i < n; ++i) {
+        const Chunk *c = sb.chunks[(size_t)i];
+        const int32_t T = c->num_tokens, np = (int32_t)c->pages.size();
+        for (int32_t t0 = 0; t0 < T; t0 += 128) {
+            GemmRowTile rt;
+            rt.a_row0 = tok_indptr[i] + t0;
+            rt.rows_valid = std::min(128, T - t0);
+            rt.rows_zero_to = std::min(128, np * kPage - t0);  // up to the end of the chunk's last page
+            rt.pad = 0;
+            for (int j = 0; j < 8; ++j) rt.pages[j] = (t0 / kPage + j < np) ? c->pages[(size_t)(t0 / kPage + j)] : -1;
+            tiles.push_back(rt);
+        }
+    }
+    p->probe_device();
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = tiles.size() * sizeof(GemmRowTile);
+    if (bytes > p->scratch_slot_bytes()) { store_undo(p, sb); return COMB_ERR_CAPACITY; }
+    const int slot = p->acquire(bytes);
+    if (slot < 0) { store_undo(p, sb); return COMB_ERR_CUDA; }
+    memcpy(p->ring[slot].host, tiles.data(), bytes);
+    GemmRowTile *dev = (GemmRowTile *)((char *)p->cfg.scratch + (size_t)slot * p->scratch_slot_bytes());
+    if (cudaMemcpyAsync(dev, p->ring[slot].host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) {
+        store_undo(p, sb);
+        return COMB_ERR_CUDA;
+    }
+    GemmProblem gp{h_packed, w_kv, M, N, d_model};
+    if (p->prof_on) p->hook.begin(p, kKernelGemm, st);
+    const cudaError_t ge = launch_gemm_paged(gp, p->geom, layer, dev, (int)tiles.size(), p->num_sms, st);
+    if (p->prof_on) p->hook.end(p, st);
+    if (ge != cudaSuccess) {
+        store_undo(p, sb);
+        return COMB_ERR_CUDA;
+    }
+    p->launches += 1;
+    if (!p->release(slot, st)) return COMB_ERR_CUDA;
+    return COMB_OK;
+}
+
+int32_t comb_gemm_bf16(comb_pool_t *p, const void *a, const void *w, const void *residual, void *c, int64_t M, int32_t N,
+                       int32_t K, void *stream) {
+    if (!p || !a || !w || !c || !gemm_shape_ok(M, N, K)) return COMB_ERR_INVALID;
+    p->probe_device();
+    cudaStream_t st = (cudaStream_t)stream;
+    GemmProblem gp{a, w, M, N, K};
+    if (p->prof_on) p->hook.begin(p, kKernelGemm, st);
+    const cudaError_t e = launch_gemm_rowmajor(gp, c, residual, p->num_sms, st);
+    if (p->prof_on) p->hook.end(p, st);
+    if (e != cudaSuccess) return COMB_ERR_CUDA;
+    p->launches += 1;
     return COMB_OK;
 }
 
@@ -977,6 +1075,40 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     p->launches += launches;
     if (!p->release(slot, st)) return COMB_ERR_CUDA;
     return COMB_OK;
+}
+
+size_t comb_layer_workspace_bytes(const comb_pool_t *p, const comb_link_t *link, int32_t Hq, int64_t rows) {
+    if (!p || !link || Hq <= 0 || rows < 0) return 0;
+    const size_t qb = align_up((size_t)rows * Hq * p->cfg.head_dim_qk * 2, 256);
+    const size_t ob = align_up((size_t)rows * Hq * p->cfg.head_dim_v * 2, 256);
+    return qb + ob + comb_attn_workspace_bytes(p, link, Hq, rows);
+}
+
+int32_t comb_cross_layer_forward(comb_pool_t *p, int32_t layer, const comb_link_t *link, int32_t R, const void *x,
+                                 const int32_t *q_indptr, int32_t d_model, int32_t Hq, const void *w_q, const void *w_o,
+                                 float scale, void *x_out, void *ws, size_t ws_bytes, void *stream) {
+    if (!p || !link || R < 0 || Hq <= 0 || d_model <= 0) return COMB_ERR_INVALID;
+    if (R == 0) return COMB_OK;
+    if (!x || !x_out || !w_q || !w_o) return COMB_ERR_INVALID;
+    const int64_t rows = q_indptr ? (int64_t)q_indptr[R] : (int64_t)R;
+    if (rows < 0) return COMB_ERR_INVALID;
+    if (rows == 0) return COMB_OK;
+    const int Dqk = p->cfg.head_dim_qk, Dv = p->cfg.head_dim_v;
+    if (!gemm_shape_ok(rows, Hq * Dqk, d_model) || !gemm_shape_ok(rows, d_model, Hq * Dv)) return COMB_ERR_INVALID;
+    const size_t qb = align_up((size_t)rows * Hq * Dqk * 2, 256), ob = align_up((size_t)rows * Hq * Dv * 2, 256);
+    const size_t attn_ws = comb_attn_workspace_bytes(p, link, Hq, rows);
+    if (!ws || (((uintptr_t)ws) & 15) || ws_bytes < qb + ob + attn_ws) return COMB_ERR_CAPACITY;
+    char *qbuf = (char *)ws, *obuf = qbuf + qb, *aws = obuf + ob;
+    // Eq. 4: Q = X W_Q
+    int32_t rc = comb_gemm_bf16(p, x, w_q, nullptr, qbuf, rows, Hq * Dqk, d_model, stream);
+    if (rc != COMB_OK) return rc;
+    // Eq. 7-8 over the linked chunks
+    rc = q_indptr ? comb_cross_attn_prefill(p, layer, link, R, qbuf, q_indptr, Hq, scale, obuf, nullptr, aws, attn_ws,
+                                            stream)
+                  : comb_cross_attn_decode(p, layer, link, R, qbuf, Hq, scale, obuf, nullptr, aws, attn_ws, stream);
+    if (rc != COMB_OK) return rc;
+    // output projection, residual added in the epilogue
+    return comb_gemm_bf16(p, obuf, w_o, x, x_out, rows, d_model, Hq * Dv, stream);
 }
 
 }  // extern "C"

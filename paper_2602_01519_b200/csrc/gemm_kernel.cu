@@ -1,0 +1,283 @@
+// gemm_kernel.cu — (f2)/(f3) the projections either side of the link-stage attention, C = A W^T on tcgen05:
+//   K^cross = H^E W_K, V^cross = H^E W_V   (§4.2 Eq. 5-6) with an epilogue that writes bf16 straight
+//                                          into the chunk's pages (K/V are what is stored)
+//   Q = X^D W_Q                            (Eq. 4)
+//   X^D + H W_O                            (output projection + residual)
+//
+// Persistent, warp-specialised: warp 0 = TMA producer (A tile 128 x 64, W tile 256 x 64, SWIZZLE_128B, 4-stage
+// mbarrier ring), warp 1 = single-thread tcgen05.mma issuer (M 128, N 256, K 16 per instruction, fp32 accumulators in
+// TMEM, two accumulator buffers of 256 columns so the epilogue of tile i runs under the main loop of tile i + 1),
+// warps 2-5 = epilogue (tcgen05.ld of the warp's 32 TMEM lanes, bf16 pack, 64-byte stores).
+#include "kernels.h"
+#include "ptx.cuh"
+
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cstring>
+
+namespace comb {
+namespace {
+
+constexpr int BM = 128, BN = 256, BK = 64, STAGES = 4;
+constexpr int A_BYTES = BM * BK * 2, B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int GEMM_THREADS = 192;
+constexpr int GEMM_SMEM = 1024 + STAGES * STAGE_BYTES + 256;
+
+enum { kEpiRowMajor = 0, kEpiPaged = 1 };
+
+struct GemmArgs {
+    int64_t M;
+    int N, K;
+    int num_m_tiles, num_n_tiles;
+    // row-major epilogue
+    __nv_bfloat16 *c;
+    const __nv_bfloat16 *residual;
+    // paged epilogue
+    const GemmRowTile *row_tiles;
+    char *k_layer, *v_layer;   // this layer's arenas: bf16 [num_pages][Hkv][16][D]
+    int hkv, dqk, dv;
+};
+
+struct GemmMaps {
+    CUtensorMap a, w;
+};
+
+template <int EPI>
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
+gemm_bf16_kernel(const GemmArgs g, const __grid_constant__ GemmMaps maps) {
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + STAGES * STAGE_BYTES);
+    uint64_t *full = bars, *empty = bars + STAGES, *acc_full = bars + 2 * STAGES, *acc_empty = bars + 2 * STAGES + 2;
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(bars + 2 * STAGES + 4);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) {
+            ptx::mbar_init(&full[s], 1);
+            ptx::mbar_init(&empty[s], 1);
+        }
+        for (int s = 0; s < 2; ++s) {
+            ptx::mbar_init(&acc_full[s], 1);
+            ptx::mbar_init(&acc_empty[s], 4);  // one arrival per epilogue warp
+        }
+        ptx::fence_barrier_init();
+        ptx::tma_prefetch_desc(&maps.a);
+        ptx::tma_prefetch_desc(&maps.w);
+    }
+    if (warp == 1) {
+        ptx::tmem_alloc(tmem_slot, 512);
+        ptx::tmem_relinquish();
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    const int num_tiles = g.num_m_tiles * g.num_n_tiles;
+    const int num_kb = (g.K + BK - 1) / BK;
+
+    if (warp == 0) {
+        // ===================== TMA producer =====================
+        uint32_t stage = 0, phase = 0;
+        for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+            const int mt = tile / g.num_n_tiles, nt = tile - mt * g.num_n_tiles;
+            int a_row0 = mt * BM;
+            if constexpr (EPI == kEpiPaged) a_row0 = g.row_tiles[mt].a_row0;
+            for (int kb = 0; kb < num_kb; ++kb) {
+                ptx::mbar_wait(&empty[stage], phase ^ 1);
+                if (lane == 0) {
+                    unsigned char *sa = smem + stage * STAGE_BYTES, *sb = sa + A_BYTES;
+                    ptx::mbar_expect_tx(&full[stage], STAGE_BYTES);
+                    ptx::tma_load_2d(sa, &maps.a, kb * BK, a_row0, &full[stage]);
+                    ptx::tma_load_2d(sb, &maps.w, kb * BK, nt * BN, &full[stage]);
+                }
+                if (++stage == STAGES) { stage = 0; phase ^= 1; }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer (whole warp runs the control flow, one lane issues) =====================
+        const bool leader = ptx::elect_one();
+        constexpr uint32_t idesc = ptx::umma_idesc_bf16(BM, BN, false);
+        const uint64_t da0 = ptx::umma_desc_sw128(ptx::smem_u32(smem), 16, 1024);
+        const uint64_t db0 = ptx::umma_desc_sw128(ptx::smem_u32(smem + A_BYTES), 16, 1024);
+        uint32_t stage = 0, phase = 0, acc = 0, acc_phase = 0;
+        for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+            ptx::mbar_wait(&acc_empty[acc], acc_phase ^ 1);  // the epilogue has drained this accumulator
+            ptx::tc_fence_after();
+            for (int kb = 0; kb < num_kb; ++kb) {
+                ptx::mbar_wait(&full[stage], phase);
+                ptx::tc_fence_after();
+                const uint64_t so = (uint64_t)((stage * STAGE_BYTES) >> 4);
+#pragma unroll
+                for (int kk = 0; kk < BK / 16; ++kk)
+                    if (leader)
+                        ptx::mma_ss(tmem + acc * BN, da0 + so + (uint64_t)((kk * 32) >> 4), db0 + so + (uint64_t)((kk * 32) >> 4),
+                                    idesc, (kb > 0 || kk > 0) ? 1u : 0u);
+                if (leader) ptx::mma_commit(&empty[stage]);  // frees the smem stage when these MMAs have read it
+                if (++stage == STAGES) { stage = 0; phase ^= 1; }
+            }
+            if (leader) ptx::mma_commit(&acc_full[acc]);
+            if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+        }
+    } else {
+        // ===================== epilogue: warps 2..5 own TMEM lanes 32 (warp % 4) .. + 31 =====================
+        const int quad = warp & 3;
+        const int row = quad * 32 + lane;  // row of the tile
+        const uint32_t lane_base = (uint32_t)(quad * 32) << 16;
+        uint32_t acc = 0, acc_phase = 0;
+        for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+            const int mt = tile / g.num_n_tiles, nt = tile - mt * g.num_n_tiles;
+            // ---- where this thread's row goes ----
+            bool store_row = false, zero_row = false;
+            char *dst_k = nullptr, *dst_v = nullptr;           // paged: (page, head 0, slot) of the row in each arena
+            __nv_bfloat16 *dst_c = nullptr;
+            const __nv_bfloat16 *res = nullptr;
+            if constexpr (EPI == kEpiRowMajor) {
+                const int64_t grow = (int64_t)mt * BM + row;
+                store_row = grow < g.M;
+                dst_c = g.c + grow * g.N;
+                res = g.residual ? g.residual + grow * g.N : nullptr;
+            } else {
+                const GemmRowTile rt = g.row_tiles[mt];
+                const int page = rt.pages[row >> 4];
+                zero_row = row >= rt.rows_valid && row < rt.rows_zero_to;
+                store_row = (row < rt.rows_valid || zero_row) && page >= 0;
+                const int slot = row & 15;
+                dst_k = g.k_layer + (((size_t)page * g.hkv) * kPage + slot) * (size_t)g.dqk * 2;
+                dst_v = g.v_layer + (((size_t)page * g.hkv) * kPage + slot) * (size_t)g.dv * 2;
+            }
+            ptx::mbar_wait(&acc_full[acc], acc_phase);
+            ptx::tc_fence_after();
+            const uint32_t tacc = tmem + lane_base + acc * BN;
+#pragma unroll 1
+            for (int cb = 0; cb < BN / 32; ++cb) {
+                uint32_t r[32];
+                ptx::tmem_ld32(tacc + cb * 32, r);
+                ptx::tmem_wait_ld();
+                const int col0 = nt * BN + cb * 32;  // first output column of these 32
+                if (store_row && col0 < g.N) {
+                uint4 *dst;
+                if constexpr (EPI == kEpiRowMajor) {
+                    dst = reinterpret_cast<uint4 *>(dst_c + col0);
+                    if (res) {
+                        const uint4 *rs = reinterpret_cast<const uint4 *>(res + col0);
+#pragma unroll
+                        for (int v = 0; v < 4; ++v) {
+                            const uint4 x = rs[v];
+                            const uint32_t xs[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                const float2 f = ptx::bf16x2_to_f2(xs[e]);
+                                r[v * 8 + 2 * e] = __float_as_uint(__uint_as_float(r[v * 8 + 2 * e]) + f.x);
+                                r[v * 8 + 2 * e + 1] = __float_as_uint(__uint_as_float(r[v * 8 + 2 * e + 1]) + f.y);
+                            }
+                        }
+                    }
+                } else {
+                    // columns [0, Hkv Dqk) are K heads, then V heads; 32 columns never straddle a head (D % 32 == 0)
+                    const int nk = g.hkv * g.dqk;
+                    if (col0 < nk) {
+                        const int head = col0 / g.dqk, dim = col0 - head * g.dqk;
+                        dst = reinterpret_cast<uint4 *>(dst_k + ((size_t)head * kPage * g.dqk + dim) * 2);
+                    } else {
+                        const int c2 = col0 - nk;
+                        const int head = c2 / g.dv, dim = c2 - head * g.dv;
+                        dst = reinterpret_cast<uint4 *>(dst_v + ((size_t)head * kPage * g.dv + dim) * 2);
+                    }
+                }
+#pragma unroll
+                for (int v = 0; v < 4; ++v) {
+                    uint4 w;
+                    w.x = ptx::pack_bf16x2(__uint_as_float(r[v * 8 + 0]), __uint_as_float(r[v * 8 + 1]));
+                    w.y = ptx::pack_bf16x2(__uint_as_float(r[v * 8 + 2]), __uint_as_float(r[v * 8 + 3]));
+                    w.z = ptx::pack_bf16x2(__uint_as_float(r[v * 8 + 4]), __uint_as_float(r[v * 8 + 5]));
+                    w.w = ptx::pack_bf16x2(__uint_as_float(r[v * 8 + 6]), __uint_as_float(r[v * 8 + 7]));
+                    if (EPI == kEpiPaged && zero_row) w = make_uint4(0u, 0u, 0u, 0u);
+                    dst[v] = w;
+                }
+                }
+                __syncwarp();  // the next tcgen05.ld is warp-collective
+            }
+            ptx::tc_fence_before();  // our TMEM reads precede the arrive that lets the next tile overwrite the buffer
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&acc_empty[acc]);
+            if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+        }
+    }
+
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    if (warp == 1) ptx::tmem_dealloc(tmem, 512);
+}
+
+template <int EPI>
+cudaError_t launch_t(const GemmArgs &g, const GemmMaps &maps, int num_sms, cudaStream_t st) {
+    auto kern = gemm_bf16_kernel<EPI>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM);
+    if (e != cudaSuccess) return e;
+    const int tiles = g.num_m_tiles * g.num_n_tiles;
+    if (tiles <= 0) return cudaSuccess;
+    const int grid = tiles < num_sms ? tiles : num_sms;
+    kern<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(g, maps);
+    return cudaGetLastError();
+}
+
+cudaError_t encode_maps(const GemmProblem &p, GemmMaps *maps) {
+    TensorMapBlob a, w;
+    cudaError_t e = encode_tma_2d_bf16(p.a, (uint64_t)p.K, (uint64_t)p.M, (uint64_t)p.K * 2, BK, BM, &a);
+    if (e != cudaSuccess) return e;
+    e = encode_tma_2d_bf16(p.w, (uint64_t)p.K, (uint64_t)p.N, (uint64_t)p.K * 2, BK, BN, &w);
+    if (e != cudaSuccess) return e;
+    static_assert(sizeof(CUtensorMap) == sizeof(TensorMapBlob), "CUtensorMap is 128 bytes");
+    memcpy(&maps->a, &a, sizeof(CUtensorMap));
+    memcpy(&maps->w, &w, sizeof(CUtensorMap));
+    return cudaSuccess;
+}
+
+}  // namespace
+
+// K and N: 16-byte row pitches for TMA (K % 8) and whole 64-byte epilogue stores (N % 32)
+bool gemm_shape_ok(int64_t M, int32_t N, int32_t K) { return M > 0 && M < (int64_t)INT32_MAX && N > 0 && K > 0 && K % 8 == 0 && N % 32 == 0; }
+
+cudaError_t launch_gemm_rowmajor(const GemmProblem &p, void *c, const void *residual, int num_sms, cudaStream_t stream) {
+    if (!gemm_shape_ok(p.M, p.N, p.K) || !p.a || !p.w || !c) return cudaErrorInvalidValue;
+    GemmMaps maps;
+    cudaError_t e = encode_maps(p, &maps);
+    if (e != cudaSuccess) return e;
+    GemmArgs g{};
+    g.M = p.M;
+    g.N = p.N;
+    g.K = p.K;
+    g.num_m_tiles = (int)((p.M + BM - 1) / BM);
+    g.num_n_tiles = (p.N + BN - 1) / BN;
+    g.c = (__nv_bfloat16 *)c;
+    g.residual = (const __nv_bfloat16 *)residual;
+    return launch_t<kEpiRowMajor>(g, maps, num_sms, stream);
+}
+
+cudaError_t launch_gemm_paged(const GemmProblem &p, const PoolGeom &pg, int layer, const GemmRowTile *tiles_dev,
+                              int num_tiles, int num_sms, cudaStream_t stream) {
+    if (!gemm_shape_ok(p.M, p.N, p.K) || !p.a || !p.w || !tiles_dev) return cudaErrorInvalidValue;
+    if (p.N != pg.num_kv_heads * (pg.head_dim_qk + pg.head_dim_v)) return cudaErrorInvalidValue;
+    GemmMaps maps;
+    cudaError_t e = encode_maps(p, &maps);
+    if (e != cudaSuccess) return e;
+    GemmArgs g{};
+    g.M = p.M;
+    g.N = p.N;
+    g.K = p.K;
+    g.num_m_tiles = num_tiles;
+    g.num_n_tiles = (p.N + BN - 1) / BN;
+    g.row_tiles = tiles_dev;
+    const size_t kb = (size_t)kPage * pg.head_dim_qk * 2, vb = (size_t)kPage * pg.head_dim_v * 2;
+    g.k_layer = (char *)pg.k_arena + (size_t)layer * pg.num_pages * pg.num_kv_heads * kb;
+    g.v_layer = (char *)pg.v_arena + (size_t)layer * pg.num_pages * pg.num_kv_heads * vb;
+    g.hkv = pg.num_kv_heads;
+    g.dqk = pg.head_dim_qk;
+    g.dv = pg.head_dim_v;
+    return launch_t<kEpiPaged>(g, maps, num_sms, stream);
+}
+
+}  // namespace comb

@@ -26,7 +26,7 @@ struct LaunchHook {
     void *ctx;
 };
 enum { kKernelStore = 0, kKernelDecodeSplit = 1, kKernelDecodeMerge = 2, kKernelPrefill = 3, kKernelDecodeCascade = 4,
-       kKernelCascadeMerge = 5, kKernelPrefillMerge = 6, kNumKernelIds = 7 };
+       kKernelCascadeMerge = 5, kKernelPrefillMerge = 6, kKernelGemm = 7, kNumKernelIds = 8 };
 
 struct PoolGeom {
     int32_t num_layers, num_kv_heads, head_dim_qk, head_dim_v, num_pages;
@@ -104,6 +104,10 @@ cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, con
                            float *lse, int64_t total_q, void *partials, int64_t part_rows, int tiles_per_cta,
                            int num_sms, cudaStream_t stream, int *launches, const LaunchHook *hook);
 
+// Dense row-major bf16 matrix [outer][inner] -> 2-D TMA map with SWIZZLE_128B boxes {box_inner (<= 64), box_outer}.
+cudaError_t encode_tma_2d_bf16(const void *base, uint64_t inner, uint64_t outer, uint64_t row_pitch_bytes,
+                               uint32_t box_inner, uint32_t box_outer, TensorMapBlob *out);
+
 // ---- (f1) chunk-major ("cascade") decode --------------------------------------------------------
 // One M tile of the chunk-major decode: `nrows` consecutive entries (query tokens) of chunk slot `slot`, starting at
 // position row0 of cas_row_req / cas_row_entry; each entry contributes G rows (the heads of one kv-head). A work
@@ -118,5 +122,28 @@ cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &
                                   const void *q, float scale, void *out, float *lse, int64_t total_entries,
                                   void *partials, int num_sms, cudaStream_t stream, int *launches,
                                   const LaunchHook *hook);
+
+// ---- (f2)/(f3) projections: C = A W^T on tcgen05 ---------------------------------------------------
+// A bf16 [M][K] row-major, W bf16 [N][K] row-major (the nn.Linear layout: row n holds the weights of output n),
+// fp32 accumulation in TMEM. Two epilogues:
+//   row-major : C bf16 [M][N] = bf16(acc (+ residual[M][N]))                                (Eq. 4; output projection)
+//   paged     : the columns are [K heads | V heads] of a chunk-KV pool layer; row t of a chunk goes straight into
+//               slot t % 16 of the chunk's page t / 16, tail slots of the last page are zero-filled   (Eq. 5-6 + store)
+// One M tile of the paged epilogue: 128 rows of A starting at a_row0; rows < rows_valid are tokens, rows in
+// [rows_valid, rows_zero_to) are the zero-filled tail of the chunk's last page, the rest is not written.
+struct GemmRowTile {
+    int32_t a_row0, rows_valid, rows_zero_to, pad;
+    int32_t pages[8];  // destination page of rows 16 i .. 16 i + 15 (-1: none)
+};
+struct GemmProblem {
+    const void *a;
+    const void *w;
+    int64_t M;
+    int32_t N, K;
+};
+cudaError_t launch_gemm_rowmajor(const GemmProblem &p, void *c, const void *residual, int num_sms, cudaStream_t stream);
+cudaError_t launch_gemm_paged(const GemmProblem &p, const PoolGeom &g, int layer, const GemmRowTile *tiles_dev,
+                              int num_tiles, int num_sms, cudaStream_t stream);
+bool gemm_shape_ok(int64_t M, int32_t N, int32_t K);
 
 }  // namespace comb

@@ -85,18 +85,28 @@ EncodeTiledFn encode_fn() {
 
 static_assert(sizeof(CUtensorMap) == sizeof(TensorMapBlob), "CUtensorMap is 128 bytes");
 
-// arena [L][pages][Hkv][16][D] seen as a dense bf16 matrix [rows][D]; box = {64 dims, 16 tokens}
-cudaError_t encode_arena_map(void *arena, int64_t rows, int d, TensorMapBlob *out) {
+}  // namespace
+
+// Dense row-major bf16 matrix [outer][inner] (row pitch given in bytes) -> 2-D tiled map, SWIZZLE_128B boxes.
+cudaError_t encode_tma_2d_bf16(const void *base, uint64_t inner, uint64_t outer, uint64_t row_pitch_bytes,
+                               uint32_t box_inner, uint32_t box_outer, TensorMapBlob *out) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return cudaErrorNotSupported;
-    const cuuint64_t dims[2] = {(cuuint64_t)d, (cuuint64_t)rows};
-    const cuuint64_t strides[1] = {(cuuint64_t)d * 2};
-    const cuuint32_t box[2] = {64, (cuuint32_t)kPage};
+    const cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)outer};
+    const cuuint64_t strides[1] = {(cuuint64_t)row_pitch_bytes};
+    const cuuint32_t box[2] = {box_inner, box_outer};
     const cuuint32_t estr[2] = {1, 1};
-    CUresult r = fn(reinterpret_cast<CUtensorMap *>(out), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, arena, dims, strides, box,
-                    estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r = fn(reinterpret_cast<CUtensorMap *>(out), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base),
+                    dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+namespace {
+
+// arena [L][pages][Hkv][16][D] seen as a dense bf16 matrix [rows][D]; box = {64 dims, 16 tokens}
+cudaError_t encode_arena_map(void *arena, int64_t rows, int d, TensorMapBlob *out) {
+    return encode_tma_2d_bf16(arena, (uint64_t)d, (uint64_t)rows, (uint64_t)d * 2, 64, (uint32_t)kPage, out);
 }
 
 template <int DQK, int DV, int NT>

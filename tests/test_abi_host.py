@@ -78,7 +78,7 @@ def check_tiles(indptr, ntok, tile_indptr, tile_ntok):
 def test_library_exports_every_declared_symbol():
     hdr = open(os.path.join(ROOT, "include", "comb.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(comb_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(comb_[a-z0-9_]+)\s*\(", hdr))
     assert {"comb_pool_create", "comb_store_chunk", "comb_link", "comb_cross_attn_prefill",
             "comb_cross_attn_decode"} <= declared
     lib = C.CDLL(_lib.LIB_PATH)
