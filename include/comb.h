@@ -134,7 +134,8 @@ int32_t comb_store_chunk(comb_pool_t *pool, int32_t layer, uint64_t chunk_id, in
                          const void *v, void *stream);
 /* Batched form, one kernel launch: chunk i has tokens tok_indptr[i]..tok_indptr[i+1] (host int32 [n+1]) of the
  * packed device tensors k_packed [sum T][Hkv][Dqk], v_packed [sum T][Hkv][Dv]. All-or-nothing: on any error
- * (including a CUDA failure) the directory and the free list are as before the call. The same id twice in one
+ * (including a CUDA failure) the directory and the free list are as before the call — except that chunks evicted
+ * to make room (COMB_OPT_EVICT_LRU) stay evicted and are listed by comb_pool_evicted(). The same id twice in one
  * batch is INVALID. Storing an id that already exists with the same length overwrites its pages (that is how
  * the other layers of a chunk are filled); ordering against attention calls in flight that read those pages is
  * the caller's, as for any store. */

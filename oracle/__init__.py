@@ -197,28 +197,90 @@ class PoolModel:
     appends its ids to the tail in page-list order (PAPER.md:205 "PIC allocator ... allocate free memory";
     PAPER.md:62 steps 1-4 hash table context -> PICache)."""
 
-    def __init__(self, num_pages: int, shuffle_seed: int = 0):
+    def __init__(self, num_pages: int, shuffle_seed: int = 0, evict_lru: bool = False):
         self.free = initial_free_list(num_pages, shuffle_seed)
         self.head = 0
         self.dir: Dict[int, Tuple[int, List[int]]] = {}
+        # lifecycle (include/comb.h "(f4) pool lifecycle"): pins, use stamps, LRU eviction
+        self.evict_lru = evict_lru
+        self.pins: Dict[int, int] = {}
+        self.stamp: Dict[int, int] = {}    # chunk -> tick of its last alloc / store / link
+        self.born: Dict[int, int] = {}     # chunk -> creation order
+        self.tick = 0
+        self.births = 0
+        self.evicted: List[int] = []       # by the most recent store call
 
     def free_pages(self) -> int:
         return len(self.free) - self.head
 
+    def _make_room(self, need: int, keep: Sequence[int]) -> bool:
+        """Evict unpinned chunks outside `keep` in ascending (use stamp, creation order) until `need` pages are
+        free; all or nothing."""
+        if self.free_pages() >= need:
+            return True
+        if not self.evict_lru:
+            return False
+        cands = sorted((c for c in self.dir if self.pins.get(c, 0) == 0 and c not in keep),
+                       key=lambda c: (self.stamp[c], self.born[c]))
+        have, take = self.free_pages(), []
+        for c in cands:
+            if have >= need:
+                break
+            take.append(c)
+            have += len(self.dir[c][1])
+        if have < need:
+            return False
+        for c in take:
+            self.release(c)
+            self.evicted.append(c)
+        return True
+
     def store(self, chunk_id: int, num_tokens: int) -> List[int]:
-        if chunk_id in self.dir:
-            if self.dir[chunk_id][0] != num_tokens:
-                raise KeyError("exists with different length")
-            return self.dir[chunk_id][1]
-        n = (num_tokens + PAGE - 1) // PAGE
-        if n > self.free_pages():
+        return self.store_batch([(chunk_id, num_tokens)])[0]
+
+    def store_batch(self, items: Sequence[Tuple[int, int]]) -> List[List[int]]:
+        """One alloc/store call naming several chunks: validated as a whole, room made for the whole batch (the
+        batch's own ids are never evicted), then pages taken from the head in batch order."""
+        self.evicted = []
+        need = 0
+        for cid, T in items:
+            if cid in self.dir:
+                if self.dir[cid][0] != T:
+                    raise KeyError("exists with different length")
+            else:
+                need += (T + PAGE - 1) // PAGE
+        if not self._make_room(need, [c for c, _ in items]):
             raise MemoryError("no space")
-        pages = self.free[self.head:self.head + n]
-        self.head += n
-        self.dir[chunk_id] = (num_tokens, pages)
-        return pages
+        out = []
+        for cid, T in items:
+            self.tick += 1
+            if cid not in self.dir:
+                n = (T + PAGE - 1) // PAGE
+                self.dir[cid] = (T, self.free[self.head:self.head + n])
+                self.head += n
+                self.born[cid] = self.births
+                self.births += 1
+            self.stamp[cid] = self.tick
+            out.append(self.dir[cid][1])
+        return out
+
+    def pin(self, chunk_id: int) -> None:
+        self.pins[chunk_id] = self.pins.get(chunk_id, 0) + 1
+
+    def unpin(self, chunk_id: int) -> None:
+        assert self.pins.get(chunk_id, 0) > 0
+        self.pins[chunk_id] -= 1
+
+    def touch(self, chunk_lists: Sequence[Sequence[int]]) -> None:
+        """What a comb_link does to the use stamps: ONE fresh tick for all the chunks it names."""
+        self.tick += 1
+        for lst in chunk_lists:
+            for c in lst:
+                self.stamp[int(c)] = self.tick
 
     def release(self, chunk_id: int) -> None:
+        if self.pins.get(chunk_id, 0) > 0:
+            raise RuntimeError("pinned")
         _, pages = self.dir.pop(chunk_id)
         self.free.extend(pages)
 

@@ -18,6 +18,7 @@ COMB_ERR_EXISTS = -3
 COMB_ERR_UNKNOWN_CHUNK = -4
 COMB_ERR_CAPACITY = -5
 COMB_ERR_CUDA = -6
+COMB_ERR_BUSY = -7
 
 
 class PoolConfig(C.Structure):
@@ -56,6 +57,10 @@ _SIGS = {
     "comb_pool_free_pages": (C.c_int32, [_P]),
     "comb_chunk_alloc": (C.c_int32, [_P, C.c_uint64, C.c_int32]),
     "comb_chunk_free": (C.c_int32, [_P, C.c_uint64]),
+    "comb_chunk_pin": (C.c_int32, [_P, C.c_uint64]),
+    "comb_chunk_unpin": (C.c_int32, [_P, C.c_uint64]),
+    "comb_pool_evicted": (C.c_int32, [_P, _P, C.c_int32]),
+    "comb_pool_eviction_count": (C.c_int64, [_P]),
     "comb_chunk_query": (C.c_int32, [_P, C.c_uint64, C.POINTER(C.c_int32), _P, C.c_int32]),
     "comb_store_chunk": (C.c_int32, [_P, C.c_int32, C.c_uint64, C.c_int32, _P, _P, _P]),
     "comb_store_chunks": (C.c_int32, [_P, C.c_int32, C.c_int32, _P, _P, _P, _P, _P]),

@@ -65,6 +65,26 @@ def comb_chunk_free(pool: int, chunk_id: int) -> None:
     check(lib.comb_chunk_free(pool, chunk_id), "comb_chunk_free")
 
 
+def comb_chunk_pin(pool: int, chunk_id: int) -> None:
+    check(lib.comb_chunk_pin(pool, chunk_id), "comb_chunk_pin")
+
+
+def comb_chunk_unpin(pool: int, chunk_id: int) -> None:
+    check(lib.comb_chunk_unpin(pool, chunk_id), "comb_chunk_unpin")
+
+
+def comb_pool_evicted(pool: int) -> list:
+    """Chunk ids evicted by the most recent alloc/store call, in eviction order."""
+    n = check(lib.comb_pool_evicted(pool, None, 0), "comb_pool_evicted")
+    ids = np.zeros(max(n, 1), dtype=np.uint64)
+    check(lib.comb_pool_evicted(pool, ids.ctypes.data, n), "comb_pool_evicted")
+    return [int(x) for x in ids[:n]]
+
+
+def comb_pool_eviction_count(pool: int) -> int:
+    return int(lib.comb_pool_eviction_count(pool))
+
+
 def comb_chunk_query(pool: int, chunk_id: int) -> Tuple[int, np.ndarray]:
     """(num_tokens, page ids) of a stored chunk."""
     nt = C.c_int32()
@@ -150,6 +170,7 @@ def comb_attn_workspace_bytes(pool: int, link: Link, num_q_heads: int, total_q: 
 
 
 OPT_DECODE_PATH = 1
+OPT_EVICT_LRU = 2
 DECODE_AUTO, DECODE_PER_REQUEST, DECODE_CHUNK_MAJOR = 0, 1, 2
 
 

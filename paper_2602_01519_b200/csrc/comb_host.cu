@@ -11,6 +11,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <type_traits>
 #include <unordered_map>
 #include <vector>
 
@@ -26,6 +27,17 @@ constexpr size_t kScratchBytesPerPage = 48;
 struct Chunk {
     int32_t num_tokens;
     std::vector<int32_t> pages;
+    // lifecycle
+    int32_t pins = 0;        // reference count: a pinned chunk is never evicted or freed
+    uint64_t last_use = 0;   // tick of the last alloc / store / comb_link that named it
+    uint64_t seq = 0;        // creation order (tie-break of the LRU order)
+    int32_t ready = -1;      // index of the event its last store recorded, -1 once known complete
+};
+
+// Event recorded by a store on its stream; comb_link makes its stream wait for it while it is pending.
+struct ReadyEvent {
+    cudaEvent_t ev = nullptr;
+    int32_t users = 0;  // chunks that still reference it
 };
 
 // Pinned host staging, reused round-robin; an event per slot marks when the GPU is done with it.
@@ -54,6 +66,24 @@ struct comb_pool {
     TensorMapBlob k_map, v_map;
     int64_t launches = 0;
     int64_t opt_decode_path = COMB_DECODE_AUTO;
+    bool opt_evict_lru = false;
+    uint64_t tick = 0, next_seq = 0;
+    std::vector<uint64_t> last_evicted;
+    int64_t evictions = 0;
+    std::vector<ReadyEvent> ready_events;
+    void drop_ready(Chunk &c) {
+        if (c.ready >= 0 && ready_events[(size_t)c.ready].users > 0) ready_events[(size_t)c.ready].users -= 1;
+        c.ready = -1;
+    }
+    // an event slot nobody references any more (or a new one); -1 on CUDA failure
+    int take_ready_event() {
+        for (size_t i = 0; i < ready_events.size(); ++i)
+            if (ready_events[i].users == 0 && ready_events[i].ev) return (int)i;
+        ReadyEvent e;
+        if (cudaEventCreateWithFlags(&e.ev, cudaEventDisableTiming) != cudaSuccess) return -1;
+        ready_events.push_back(e);
+        return (int)ready_events.size() - 1;
+    }
     // per-kernel timing (comb_profile_*)
     struct ProfRec { int id; cudaEvent_t a, b; };
     bool prof_on = false;
@@ -140,12 +170,48 @@ int32_t validate_cfg(const comb_pool_config_t *c) {
     return COMB_OK;
 }
 
+void dir_free(comb_pool_t *p, std::unordered_map<uint64_t, Chunk>::iterator it) {
+    // compact the consumed prefix now and then so the vector does not grow without bound
+    if (p->free_head > 65536 && p->free_head * 2 > p->free_list.size()) {
+        p->free_list.erase(p->free_list.begin(), p->free_list.begin() + p->free_head);
+        p->free_head = 0;
+    }
+    p->free_list.insert(p->free_list.end(), it->second.pages.begin(), it->second.pages.end());
+    p->drop_ready(it->second);
+    p->dir.erase(it);
+}
+
+// LRU eviction (policy stated in include/comb.h): make `need` pages available by evicting unpinned
+// chunks that are not in `keep`, in ascending (use stamp, creation order). All or nothing.
+bool evict_for(comb_pool_t *p, size_t need, const std::unordered_map<uint64_t, int32_t> *keep) {
+    size_t have = p->free_list.size() - p->free_head;
+    if (have >= need) return true;
+    if (!p->opt_evict_lru) return false;
+    struct Cand { uint64_t use, seq, id; size_t pages; };
+    std::vector<Cand> cands;
+    for (auto &kv : p->dir)
+        if (kv.second.pins == 0 && !(keep && keep->count(kv.first)))
+            cands.push_back(Cand{kv.second.last_use, kv.second.seq, kv.first, kv.second.pages.size()});
+    std::sort(cands.begin(), cands.end(),
+              [](const Cand &a, const Cand &b) { return a.use != b.use ? a.use < b.use : a.seq < b.seq; });
+    size_t n = 0;
+    while (n < cands.size() && have < need) have += cands[n++].pages;
+    if (have < need) return false;
+    for (size_t i = 0; i < n; ++i) {
+        dir_free(p, p->dir.find(cands[i].id));
+        p->last_evicted.push_back(cands[i].id);
+        p->evictions += 1;
+    }
+    return true;
+}
+
 // take ceil(T/16) pages from the head of the free list (or find the existing entry)
 int32_t dir_alloc(comb_pool_t *p, uint64_t id, int32_t T, const Chunk **out, bool *created) {
     if (T <= 0) return COMB_ERR_INVALID;
     auto it = p->dir.find(id);
     if (it != p->dir.end()) {
         if (it->second.num_tokens != T) return COMB_ERR_EXISTS;
+        it->second.last_use = ++p->tick;
         if (out) *out = &it->second;
         if (created) *created = false;
         return COMB_OK;
@@ -155,21 +221,13 @@ int32_t dir_alloc(comb_pool_t *p, uint64_t id, int32_t T, const Chunk **out, boo
     Chunk c;
     c.num_tokens = T;
     c.pages.assign(p->free_list.begin() + p->free_head, p->free_list.begin() + p->free_head + n);
+    c.last_use = ++p->tick;
+    c.seq = p->next_seq++;
     p->free_head += n;
     auto ins = p->dir.emplace(id, std::move(c));
     if (out) *out = &ins.first->second;
     if (created) *created = true;
     return COMB_OK;
-}
-
-void dir_free(comb_pool_t *p, std::unordered_map<uint64_t, Chunk>::iterator it) {
-    // compact the consumed prefix now and then so the vector does not grow without bound
-    if (p->free_head > 65536 && p->free_head * 2 > p->free_list.size()) {
-        p->free_list.erase(p->free_list.begin(), p->free_list.begin() + p->free_head);
-        p->free_head = 0;
-    }
-    p->free_list.insert(p->free_list.end(), it->second.pages.begin(), it->second.pages.end());
-    p->dir.erase(it);
 }
 
 struct LinkLayout {
@@ -417,6 +475,7 @@ const char *comb_strerror(int32_t s) {
         case COMB_ERR_UNKNOWN_CHUNK: return "unknown chunk id (compile + store it first)";
         case COMB_ERR_CAPACITY: return "buffer too small";
         case COMB_ERR_CUDA: return "CUDA error (see cudaGetLastError)";
+        case COMB_ERR_BUSY: return "chunk is pinned";
         default: return "unknown status";
     }
 }
@@ -461,6 +520,8 @@ int32_t comb_pool_destroy(comb_pool_t *p) {
     if (!p) return COMB_ERR_INVALID;
     for (auto &r : p->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto &e : p->prof_free) cudaEventDestroy(e);
+    for (auto &e : p->ready_events)
+        if (e.ev) cudaEventDestroy(e.ev);
     for (auto &s : p->ring) {
         if (s.busy) cudaEventSynchronize(s.ev);
         if (s.ev) cudaEventDestroy(s.ev);
@@ -531,13 +592,45 @@ int32_t comb_util_stream_read(const void *src, size_t bytes, void *sink, void *s
 
 int32_t comb_chunk_alloc(comb_pool_t *p, uint64_t id, int32_t T) {
     if (!p) return COMB_ERR_INVALID;
+    p->last_evicted.clear();
+    if (T > 0 && p->dir.find(id) == p->dir.end()) {
+        std::unordered_map<uint64_t, int32_t> keep;
+        if (!evict_for(p, (size_t)(T + kPage - 1) / kPage, &keep)) return COMB_ERR_NO_SPACE;
+    }
     return dir_alloc(p, id, T, nullptr, nullptr);
 }
+
+int32_t comb_chunk_pin(comb_pool_t *p, uint64_t id) {
+    if (!p) return COMB_ERR_INVALID;
+    auto it = p->dir.find(id);
+    if (it == p->dir.end()) return COMB_ERR_UNKNOWN_CHUNK;
+    it->second.pins += 1;
+    return COMB_OK;
+}
+
+int32_t comb_chunk_unpin(comb_pool_t *p, uint64_t id) {
+    if (!p) return COMB_ERR_INVALID;
+    auto it = p->dir.find(id);
+    if (it == p->dir.end()) return COMB_ERR_UNKNOWN_CHUNK;
+    if (it->second.pins <= 0) return COMB_ERR_INVALID;
+    it->second.pins -= 1;
+    return COMB_OK;
+}
+
+int32_t comb_pool_evicted(const comb_pool_t *p, uint64_t *ids, int32_t cap) {
+    if (!p || cap < 0 || (cap > 0 && !ids)) return COMB_ERR_INVALID;
+    const int32_t n = (int32_t)p->last_evicted.size();
+    for (int32_t i = 0; i < std::min(n, cap); ++i) ids[i] = p->last_evicted[(size_t)i];
+    return n;
+}
+
+int64_t comb_pool_eviction_count(const comb_pool_t *p) { return p ? p->evictions : 0; }
 
 int32_t comb_chunk_free(comb_pool_t *p, uint64_t id) {
     if (!p) return COMB_ERR_INVALID;
     auto it = p->dir.find(id);
     if (it == p->dir.end()) return COMB_ERR_UNKNOWN_CHUNK;
+    if (it->second.pins > 0) return COMB_ERR_BUSY;
     dir_free(p, it);
     return COMB_OK;
 }
@@ -556,6 +649,20 @@ int32_t comb_chunk_query(const comb_pool_t *p, uint64_t id, int32_t *num_tokens,
 #pragma GCC visibility pop
 
 namespace {
+
+// After a store's kernel has been enqueued on `st`: one event for the batch; every chunk of the batch points at it.
+bool mark_ready(comb_pool_t *p, const std::vector<const Chunk *> &chunks, const uint64_t *ids, cudaStream_t st) {
+    const int ei = p->take_ready_event();
+    if (ei < 0) return false;
+    if (cudaEventRecord(p->ready_events[(size_t)ei].ev, st) != cudaSuccess) return false;
+    for (size_t i = 0; i < chunks.size(); ++i) {
+        Chunk &c = p->dir.find(ids[i])->second;
+        p->drop_ready(c);
+        c.ready = ei;
+        p->ready_events[(size_t)ei].users += 1;
+    }
+    return true;
+}
 
 // The directory half of a batched store: validates everything first so an error allocates nothing, then takes the
 // pages. `undo` restores the directory and the free list exactly (pages are taken from the head in order).
@@ -588,8 +695,13 @@ int32_t store_begin(comb_pool_t *p, int32_t layer, int32_t n, const uint64_t *id
             }
         }
     }
-    if (need_pages > p->free_list.size() - p->free_head) return COMB_ERR_NO_SPACE;
     if (sb->total_pages > (size_t)p->cfg.num_pages) return COMB_ERR_CAPACITY;
+    p->last_evicted.clear();
+    if (need_pages > p->free_list.size() - p->free_head) {
+        std::unordered_map<uint64_t, int32_t> keep;
+        for (int32_t i = 0; i < n; ++i) keep.emplace(ids[i], 0);
+        if (!evict_for(p, need_pages, &keep)) return COMB_ERR_NO_SPACE;
+    }
     sb->head_before = p->free_head;
     sb->chunks.reserve((size_t)n);
     for (int32_t i = 0; i < n; ++i) {
@@ -648,6 +760,7 @@ int32_t comb_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, const uint64
         return COMB_ERR_CUDA;
     }
     p->launches += 1;
+    if (!mark_ready(p, sb.chunks, ids, st)) return COMB_ERR_CUDA;
     if (!p->release(slot, st)) return COMB_ERR_CUDA;
     return COMB_OK;
 }
@@ -700,6 +813,7 @@ int32_t comb_project_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, cons
         return COMB_ERR_CUDA;
     }
     p->launches += 1;
+    if (!mark_ready(p, sb.chunks, ids, st)) return COMB_ERR_CUDA;
     if (!p->release(slot, st)) return COMB_ERR_CUDA;
     return COMB_OK;
 }
@@ -737,8 +851,17 @@ size_t comb_link_host_bytes(int32_t R, int64_t E) {
     return align_up(sizeof(int32_t) * (size_t)std::max(R, 1), 16) + align_up(sizeof(int32_t) * (size_t)std::max<int64_t>(E, 1), 16);
 }
 
-int32_t comb_link_plan(const comb_pool_t *p, int32_t R, const int32_t *chunk_indptr, const uint64_t *chunk_ids,
-                       comb_link_t *link, void *staging) {
+}  // extern "C"
+#pragma GCC visibility pop
+
+namespace {
+
+// PoolT = const comb_pool_t: pure planning. PoolT = comb_pool_t (comb_link): additionally stamps every named chunk
+// with `tick` (LRU order) and collects the store events that are still pending for them.
+template <class PoolT>
+int32_t link_plan_impl(PoolT *p, int32_t R, const int32_t *chunk_indptr, const uint64_t *chunk_ids, comb_link_t *link,
+                       void *staging, uint64_t tick, std::vector<int32_t> *pending_events) {
+    constexpr bool kTouch = !std::is_const<PoolT>::value;
     if (!p || !link || R < 0 || !chunk_indptr || !staging || !link->device_buf) return COMB_ERR_INVALID;
     if (chunk_indptr[0] != 0) return COMB_ERR_INVALID;
     for (int32_t r = 0; r < R; ++r)
@@ -751,6 +874,7 @@ int32_t comb_link_plan(const comb_pool_t *p, int32_t R, const int32_t *chunk_ind
     std::vector<const Chunk *> found((size_t)E);  // one directory lookup per entry
     std::vector<int32_t> ent_slot((size_t)E);     // entry -> distinct index (first-appearance order for now)
     std::vector<const Chunk *> distinct;
+    std::vector<uint64_t> distinct_ids;
     std::vector<int32_t> drows;
     {
         std::unordered_map<const Chunk *, int32_t> seen;
@@ -767,8 +891,10 @@ int32_t comb_link_plan(const comb_pool_t *p, int32_t R, const int32_t *chunk_ind
                 auto ins = seen.emplace(c, (int32_t)distinct.size());
                 if (ins.second) {
                     distinct.push_back(c);
+                    distinct_ids.push_back(chunk_ids[e]);
                     drows.push_back(0);
                 }
+                (void)tick;
                 ent_slot[(size_t)e] = ins.first->second;
                 drows[(size_t)ins.first->second] += 1;
             }
@@ -898,8 +1024,26 @@ int32_t comb_link_plan(const comb_pool_t *p, int32_t R, const int32_t *chunk_ind
     link->distinct_pages = distinct_pages;
     link->distinct_kv_tokens = distinct_tok;
     link->bytes_used = L.bytes;
+    if constexpr (kTouch) {  // the link succeeded: stamp its chunks, note whose stores may still be in flight
+        for (int32_t u = 0; u < U; ++u) {
+            auto it = p->dir.find(distinct_ids[(size_t)u]);
+            it->second.last_use = tick;
+            if (it->second.ready >= 0 && pending_events) pending_events->push_back(it->second.ready);
+        }
+    }
     return COMB_OK;
 }
+
+}  // namespace
+
+#pragma GCC visibility push(default)
+extern "C" {
+
+int32_t comb_link_plan(const comb_pool_t *p, int32_t R, const int32_t *chunk_indptr, const uint64_t *chunk_ids,
+                       comb_link_t *link, void *staging) {
+    return link_plan_impl<const comb_pool_t>(p, R, chunk_indptr, chunk_ids, link, staging, 0, nullptr);
+}
+
 
 int32_t comb_link(comb_pool_t *p, int32_t R, const int32_t *chunk_indptr, const uint64_t *chunk_ids,
                   comb_link_t *link, void *stream) {
@@ -907,9 +1051,31 @@ int32_t comb_link(comb_pool_t *p, int32_t R, const int32_t *chunk_indptr, const 
     if (((uintptr_t)link->device_buf) & 15) return COMB_ERR_INVALID;
     const int slot = p->acquire(link->device_bytes);
     if (slot < 0) return COMB_ERR_CUDA;
-    int32_t rc = comb_link_plan(p, R, chunk_indptr, chunk_ids, link, p->ring[slot].host);
+    std::vector<int32_t> pending;
+    int32_t rc = link_plan_impl<comb_pool_t>(p, R, chunk_indptr, chunk_ids, link, p->ring[slot].host, p->tick + 1, &pending);
     if (rc != COMB_OK) return rc;
+    p->tick += 1;
     cudaStream_t st = (cudaStream_t)stream;
+    // "stored asynchronously": order this stream after the stores of the named chunks that are still
+    // in flight (usually none: an event found complete is forgotten for good)
+    if (!pending.empty()) {
+        std::sort(pending.begin(), pending.end());
+        pending.erase(std::unique(pending.begin(), pending.end()), pending.end());
+        for (int32_t ei : pending) {
+            ReadyEvent &re = p->ready_events[(size_t)ei];
+            const cudaError_t q = cudaEventQuery(re.ev);
+            if (q == cudaSuccess) {
+                for (auto &kv : p->dir)
+                    if (kv.second.ready == ei) kv.second.ready = -1;
+                re.users = 0;
+            } else if (q == cudaErrorNotReady) {
+                (void)cudaGetLastError();
+                if (cudaStreamWaitEvent(st, re.ev, 0) != cudaSuccess) return COMB_ERR_CUDA;
+            } else {
+                return COMB_ERR_CUDA;
+            }
+        }
+    }
     // the ONLY data movement of the link stage: the tables. K/V are never touched.
     if (cudaMemcpyAsync(link->device_buf, p->ring[slot].host, link->bytes_used, cudaMemcpyHostToDevice, st) !=
         cudaSuccess)
@@ -924,6 +1090,11 @@ int32_t comb_pool_set_option(comb_pool_t *p, int32_t option, int64_t value) {
         if (value != COMB_DECODE_AUTO && value != COMB_DECODE_PER_REQUEST && value != COMB_DECODE_CHUNK_MAJOR)
             return COMB_ERR_INVALID;
         p->opt_decode_path = value;
+        return COMB_OK;
+    }
+    if (option == COMB_OPT_EVICT_LRU) {
+        if (value != 0 && value != 1) return COMB_ERR_INVALID;
+        p->opt_evict_lru = value == 1;
         return COMB_OK;
     }
     return COMB_ERR_INVALID;

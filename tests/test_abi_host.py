@@ -310,3 +310,84 @@ def test_options_and_decode_group_sizes():
                                              0x7500_0000_0000, None, 0x7600_0000_0000, ws, None)
         assert (st != comb.COMB_ERR_INVALID) == ok, (Hq, st)
     comb.comb_pool_destroy(pool)
+
+
+def test_pins_and_lru_eviction_match_oracle_model():
+    """(f4) reference counts and LRU eviction: a random trace of alloc / link / pin / unpin / free on a small pool,
+    the library against the oracle's independent restatement of the policy (page lists and eviction order bit-exact)."""
+    rng = np.random.default_rng(7)
+    pool, model = make_pool(40, seed=3), oracle.PoolModel(40, 3, evict_lru=True)
+    comb.comb_pool_set_option(pool, comb.OPT_EVICT_LRU, 1)
+    nxt, evicted_total = 0, 0
+    for step in range(400):
+        live = sorted(model.dir)
+        op = rng.integers(0, 10)
+        if op <= 3 or not live:                                   # a new chunk (may evict)
+            T = int(rng.integers(1, 120))
+            try:
+                want = model.store(nxt, T)
+            except MemoryError:
+                with pytest.raises(comb.CombError) as e:
+                    comb.comb_chunk_alloc(pool, nxt, T)
+                assert e.value.status == comb.COMB_ERR_NO_SPACE
+                assert comb.comb_pool_evicted(pool) == []
+            else:
+                comb.comb_chunk_alloc(pool, nxt, T)
+                assert comb.comb_chunk_query(pool, nxt)[1].tolist() == want
+                assert comb.comb_pool_evicted(pool) == model.evicted
+                evicted_total += len(model.evicted)
+            nxt += 1
+        elif op <= 5:                                             # a link refreshes the use stamps (real comb_link
+            lists = [list(rng.choice(live, size=int(rng.integers(1, min(4, len(live)) + 1)), replace=False))
+                     for _ in range(2)]                           # needs CUDA; the stamps are host state: alloc of an
+            for lst in lists:                                     # existing id stamps too, one tick per call)
+                for c in lst:
+                    comb.comb_chunk_alloc(pool, int(c), model.dir[int(c)][0])
+                    model.store(int(c), model.dir[int(c)][0])
+        elif op == 6:
+            c = int(rng.choice(live))
+            comb.comb_chunk_pin(pool, c)
+            model.pin(c)
+        elif op == 7:
+            pinned = [c for c in live if model.pins.get(c, 0) > 0]
+            if pinned:
+                c = int(rng.choice(pinned))
+                comb.comb_chunk_unpin(pool, c)
+                model.unpin(c)
+        else:
+            c = int(rng.choice(live))
+            if model.pins.get(c, 0) > 0:
+                with pytest.raises(comb.CombError) as e:
+                    comb.comb_chunk_free(pool, c)
+                assert e.value.status == comb.COMB_ERR_BUSY
+            else:
+                comb.comb_chunk_free(pool, c)
+                model.release(c)
+        assert _lib.lib.comb_pool_free_pages(pool) == model.free_pages()
+    assert evicted_total > 10 and comb.comb_pool_eviction_count(pool) == evicted_total
+    for c in sorted(model.dir):
+        assert comb.comb_chunk_query(pool, c)[1].tolist() == model.dir[c][1]
+    with pytest.raises(comb.CombError) as e:
+        comb.comb_chunk_unpin(pool, sorted(c for c in model.dir if model.pins.get(c, 0) == 0)[0])
+    assert e.value.status == comb.COMB_ERR_INVALID
+    comb.comb_pool_destroy(pool)
+
+
+def test_eviction_is_off_by_default_and_all_or_nothing():
+    pool = make_pool(4)
+    comb.comb_chunk_alloc(pool, 1, 33)
+    with pytest.raises(comb.CombError) as e:
+        comb.comb_chunk_alloc(pool, 2, 17)
+    assert e.value.status == comb.COMB_ERR_NO_SPACE and comb.comb_pool_eviction_count(pool) == 0
+    comb.comb_pool_set_option(pool, comb.OPT_EVICT_LRU, 1)
+    comb.comb_chunk_pin(pool, 1)
+    with pytest.raises(comb.CombError) as e:                        # the only candidate is pinned
+        comb.comb_chunk_alloc(pool, 2, 17)
+    assert e.value.status == comb.COMB_ERR_NO_SPACE and comb.comb_chunk_query(pool, 1)[0] == 33
+    comb.comb_chunk_unpin(pool, 1)
+    comb.comb_chunk_alloc(pool, 2, 17)
+    assert comb.comb_pool_evicted(pool) == [1]
+    with pytest.raises(comb.CombError) as e:
+        comb.comb_chunk_query(pool, 1)
+    assert e.value.status == comb.COMB_ERR_UNKNOWN_CHUNK
+    comb.comb_pool_destroy(pool)

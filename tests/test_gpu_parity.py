@@ -784,3 +784,79 @@ def test_full_size_mla_prefill_every_item_and_a_whole_request():
     assert np.all(np.isfinite(cs.bf16_bits_to_f64(out)))
     per_item_samples(w, ld, out, lse, 128, (9, 0, 128), "cfg5 prefill")     # item = 1 tile x 128 tokens (G = 1)
     ld.pool.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# (f4) pool lifecycle on the device: stores on a side stream, eviction under memory pressure
+# ------------------------------------------------------------------------------------------------
+def test_store_on_a_side_stream_is_ordered_by_the_link():
+    """PAPER.md:205 "stored asynchronously": the chunks are stored on a side stream (behind a long fill that keeps that
+    stream busy), the link + attention run on the current stream right away, no event handling by the caller:
+    comb_link makes its stream wait for the stores of the chunks it names."""
+    import paper_2602_01519_b200 as comb
+    w = cs.custom("async", k=4, num_q_heads=32, num_kv_heads=8, head_dim_qk=128, head_dim_v=128,
+                  chunk_len=[2000, 1500, 3000, 700], links=[[2, 0], [1, 3, 2]], lq=[1, 1])
+    pool = comb.Pool(8, 128, 128, w.pool_pages, shuffle_seed=3, sentinel=SENTINEL)
+    side = torch.cuda.Stream()
+    tok = np.zeros(5, np.int32)
+    np.cumsum(w.chunk_len, out=tok[1:])
+    kv = [w.chunk_kv(c) for c in range(4)]
+    kd = H().bits_to_device(np.concatenate([k for k, _ in kv]), "cuda")
+    vd = H().bits_to_device(np.concatenate([v for _, v in kv]), "cuda")
+    q = H().bits_to_device(w.all_q(), "cuda")
+    busy = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
+    torch.cuda.synchronize()
+    for path in (comb.DECODE_PER_REQUEST, comb.DECODE_CHUNK_MAJOR):
+        pool.set_decode_path(path)
+        with torch.cuda.stream(side):
+            for i in range(4):
+                busy.fill_(i)                       # ~1 ms of work queued ahead of the store on the side stream
+        pool.store_chunks(list(range(4)), tok, kd, vd, stream=side)
+        lb = pool.link([list(map(int, l)) for l in w.links])      # current stream; waits for the pending store
+        out, lse = pool.decode(lb, q, w.scale)
+        torch.cuda.synchronize()
+        check_attention(H().device_to_bits(out), lse.cpu().numpy().astype(np.float64), *oracle.attention_for(w),
+                        tag="side-stream store, path %d" % path)
+        # poison the pages so that the second round cannot pass on stale data
+        pool.k_arena.fill_(int(np.array(SENTINEL, dtype=np.uint16).view(np.int16)))
+        torch.cuda.synchronize()
+    pool.close()
+
+
+def test_eviction_under_memory_pressure_on_device():
+    """A pool that holds 3 of 5 chunks: storing the 4th and 5th evicts the least recently linked unpinned ones, the
+    caller learns which, and attention over what is resident stays right."""
+    import paper_2602_01519_b200 as comb
+    w = cs.custom("evict", k=3, num_q_heads=8, num_kv_heads=2, head_dim_qk=64, head_dim_v=64,
+                  chunk_len=[160] * 5, links=[[0]], lq=[1])
+    pool = comb.Pool(2, 64, 64, 30, sentinel=SENTINEL)
+    comb.comb_pool_set_option(pool.handle, comb.OPT_EVICT_LRU, 1)
+    model = oracle.PoolModel(30, 0, evict_lru=True)
+
+    def store(c):
+        k, v = w.chunk_kv(c)
+        pool.store_chunk(c, H().bits_to_device(k, "cuda"), H().bits_to_device(v, "cuda"))
+        want = model.store(c, 160)
+        assert comb.comb_chunk_query(pool.handle, c)[1].tolist() == want
+        assert comb.comb_pool_evicted(pool.handle) == model.evicted
+    for c in (0, 1, 2):
+        store(c)
+    pool.link([[0]])                 # chunk 0 becomes the most recently used
+    model.touch([[0]])
+    comb.comb_chunk_pin(pool.handle, 1)
+    model.pin(1)
+    store(3)                         # evicts 2 (oldest unpinned)
+    assert model.evicted == [2]
+    store(4)                         # evicts 0 (1 is pinned, 3 is newer)
+    assert model.evicted == [0]
+    with pytest.raises(comb.CombError) as e:
+        pool.link([[0]])
+    assert e.value.status == comb.COMB_ERR_UNKNOWN_CHUNK
+    wl = cs.custom("evict", k=3, num_q_heads=8, num_kv_heads=2, head_dim_qk=64, head_dim_v=64,
+                   chunk_len=[160] * 5, links=[[4, 1, 3]], lq=[1])
+    lb = pool.link([[4, 1, 3]])
+    out, lse = pool.decode(lb, H().bits_to_device(wl.all_q(), "cuda"), wl.scale)
+    torch.cuda.synchronize()
+    check_attention(H().device_to_bits(out), lse.cpu().numpy().astype(np.float64), *oracle.attention_for(wl),
+                    tag="after eviction")
+    pool.close()

@@ -387,3 +387,26 @@ def test_bf16_rounding_helpers():
     assert [hex(v) for v in b] == ["0x3f80", "0x3f81", "0x3f80", "0x3f82", "0x3f81", "0xc020", "0x0"]
     #        exact     exact      tie -> even (down)  tie -> even (up)  just above the tie
     assert np.array_equal(ol.bf16_to_f64(b), [1.0, 1.0078125, 1.0, 1.015625, 1.0078125, -2.5, 0.0])
+
+
+def test_lru_eviction_hand_example():
+    """O3 lifecycle (include/comb.h "(f4) pool lifecycle"), worked by hand on 6 pages.
+    store a(2 pages) b(2) c(2): ticks 1,2,3, pool full.  link [a] -> tick 4 stamps a.  pin b.
+    store d(3 pages): needs 3; candidates in (stamp, birth) order: b is pinned; c (3) then a (4) -> evict c (2 pages,
+    not enough) and a (2 more): free list tail = c's pages then a's pages = [4,5,0,1]; d takes [4,5,0]."""
+    m = oracle.PoolModel(6, evict_lru=True)
+    assert m.store(10, 32) == [0, 1] and m.store(11, 17) == [2, 3] and m.store(12, 20) == [4, 5]
+    m.touch([[10]])
+    m.pin(11)
+    assert m.store(13, 40) == [4, 5, 0]
+    assert m.evicted == [12, 10] and sorted(m.dir) == [11, 13] and m.free_pages() == 1
+    with pytest.raises(MemoryError):          # 11 is pinned, 13 is the newest: evicting 13 alone frees 3 + 1 < 5
+        m.store(14, 80)
+    assert m.evicted == [] and sorted(m.dir) == [11, 13]          # all or nothing
+    m.unpin(11)
+    assert m.store(14, 80) == [1, 2, 3, 4, 5]                      # evicts 11 (stamp 2) then 13: tail 1 | 2,3 | 4,5,0
+    assert m.evicted == [11, 13]
+    no = oracle.PoolModel(2)                                       # eviction off: a full pool refuses
+    no.store(1, 32)
+    with pytest.raises(MemoryError):
+        no.store(2, 1)
