@@ -249,6 +249,8 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the other configs, store and CPU baseline")
     ap.add_argument("--only", default="", help="comma-separated extras to run (default: all)")
     ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--extra-launches", type=int, default=200,
+                    help="timed launches behind every median/min of the extras (lower it under a profiler)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -531,7 +533,7 @@ def main():
             return rr
 
         try:
-            N = 200  # launches behind every median / min below
+            N = max(3, args.extra_launches)  # launches behind every median / min below
             if not primary_prefill:
                 if want("rag_prefill"):
                     rp = prefill_extra("rag_prefill", cs.rag_prefill(seed=args.seed), N, "linked")
@@ -546,7 +548,7 @@ def main():
                     decode_extra("decode_link_per_request", cs.decode_link(seed=args.seed), N, "linked",
                                  path="per_request", wname="decode_link")
                 if want("decode_link_cold_l2"):
-                    decode_extra("decode_link_cold_l2", cs.decode_link(seed=args.seed), 50, "linked", flush=True,
+                    decode_extra("decode_link_cold_l2", cs.decode_link(seed=args.seed), min(N, 50), "linked", flush=True,
                                  wname="decode_link")
                 if want("decode_link_contiguous_pages"):  # ascending free list: chunks contiguous in the arena
                     decode_extra("decode_link_contiguous_pages", cs.decode_link(seed=args.seed), N, "linked", shuffle=0,
@@ -567,7 +569,7 @@ def main():
                 prefill_extra("rag_prefill_lq32_r4", cs.rag_prefill(seed=args.seed, lq=32, requests=4), N, "linked",
                               flush=True)
             if want("long_fewshot"):
-                prefill_extra("long_fewshot_prefill", cs.long_fewshot(seed=args.seed), 50, "all", flush=True,
+                prefill_extra("long_fewshot_prefill", cs.long_fewshot(seed=args.seed), min(N, 50), "all", flush=True,
                               wname="long_fewshot")
                 decode_extra("long_fewshot_decode", cs.long_fewshot(seed=args.seed), N, "all", flush=True,
                              wname="long_fewshot")
@@ -579,11 +581,26 @@ def main():
                 decode_extra("mla_shaped_decode_per_request", cs.mla_shaped(seed=args.seed), N, "linked",
                              path="per_request", wname="mla_shaped")
             if want("store"):
-                extras["store"] = bench_store(torch, comb, harness, cs.long_fewshot(seed=args.seed), pk)
+                extras["store"] = bench_store(torch, comb, harness, cs.long_fewshot(seed=args.seed), pk, N)
                 st = extras["store"]
                 summary.append("store k=%.4f/%.4f/%.4f GB=%.0f f=%.3f" % (
                     st["kernel_ms"], st["kernel_ms_median"], st["kernel_ms_min"], st["roofline"]["achieved"],
                     st["roofline"]["frac"]))
+            if want("project_store"):
+                extras["project_store"] = bench_project_store(torch, comb, cs.long_fewshot(seed=args.seed), pk, min(N, 50))
+                ps = extras["project_store"]
+                summary.append("project_store k=%.4f/%.4f/%.4f TF=%.0f f=%.3f two_step=%.4f" % (
+                    ps["kernel_ms"], ps["kernel_ms_median"], ps["kernel_ms_min"], ps["roofline"]["achieved"],
+                    ps["roofline"]["frac"], ps["two_step_ms"]))
+            if want("cross_layer"):
+                extras["cross_layer_prefill"] = bench_cross_layer(torch, comb, cs.rag_prefill(seed=args.seed), pk,
+                                                                 "prefill", max(3, min(N, 20)))
+                extras["cross_layer_decode"] = bench_cross_layer(torch, comb, cs.decode_link(seed=args.seed), pk,
+                                                                "decode", max(3, min(N, 50)))
+                for nm in ("cross_layer_prefill", "cross_layer_decode"):
+                    cl = extras[nm]
+                    summary.append("%s L=8 step=%.3f attn=%.3f gemm=%.3f TF=%.0f us/tok=%.2f" % (
+                        nm, cl["ms_per_step"], cl["attention_ms"], cl["gemm_ms"], cl["tflops"], cl["us_per_q_token"]))
             if want("link"):
                 extras["link"] = bench_link(torch, comb, harness, cs.decode_link(seed=args.seed))
                 summary.append("link host_p50=%.1fus resident_p50=%.1fus" % (
@@ -643,7 +660,7 @@ def main():
         dist.destroy_process_group()
 
 
-def bench_store(torch, comb, harness, w, pk):
+def bench_store(torch, comb, harness, w, pk, n=200):
     """(a2) batched paged store of configs[3]'s 64 variable-length chunks, 200 times over the same page lists (a store of
     an id that exists with the same length rewrites its pages), L2 flushed clean before every launch."""
     ld = harness.load_workload(w, fill="all", shuffle_seed=77, keep_host=False)
@@ -657,7 +674,6 @@ def bench_store(torch, comb, harness, w, pk):
     flush = L2Flush(torch)
     comb.comb_profile_enable(pool.handle, True)
     comb.comb_profile_read(pool.handle, comb.KERNEL_STORE)
-    n = 200
     for i in range(n + 3):
         flush(i)
         if i == 3:
@@ -678,6 +694,118 @@ def bench_store(torch, comb, harness, w, pk):
                          "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
                          "kernel": "store", "traffic": ncu_traffic("store", "long_fewshot")},
             "l2": L2Flush.HOW}
+
+
+def bench_project_store(torch, comb, w, pk, n=50, d_model=4096):
+    """(f2) K/V projection of configs[3]'s 64 chunks fused into the paged store (one tcgen05 GEMM launch whose epilogue
+    writes the pages), L2 flushed before every launch; beside it the unfused sequence on the same data: two row-major
+    GEMMs (K, V) + comb_store_chunks. Values are device-side N(0,1) (timing only; parity is tests/test_gpu_layer.py)."""
+    Hkv, Dqk, Dv = w.num_kv_heads, w.head_dim_qk, w.head_dim_v
+    pool = comb.Pool(Hkv, Dqk, Dv, w.pool_pages + 8, shuffle_seed=77)
+    ids = list(range(w.num_chunks))
+    tok = np.zeros(w.num_chunks + 1, np.int32)
+    np.cumsum(w.chunk_len, out=tok[1:])
+    T = int(tok[-1])
+    N = Hkv * (Dqk + Dv)
+    h = torch.randn((T, d_model), device="cuda").to(torch.bfloat16)
+    wkv = (torch.randn((N, d_model), device="cuda") / d_model ** 0.5).to(torch.bfloat16)
+    flush = L2Flush(torch)
+    comb.comb_profile_enable(pool.handle, True)
+    for i in range(n + 3):
+        flush(i)
+        if i == 3:
+            torch.cuda.synchronize()
+            comb.comb_profile_read(pool.handle, comb.KERNEL_GEMM)
+        pool.project_store_chunks(ids, tok, h, wkv)
+    st = stats(comb.comb_profile_read_samples(pool.handle, comb.KERNEL_GEMM, cap=n + 8))
+    # unfused: K = H W_K^T, V = H W_V^T row-major, then the paged store
+    kbuf = torch.empty((T, Hkv, Dqk), dtype=torch.bfloat16, device="cuda")
+    vbuf = torch.empty((T, Hkv, Dv), dtype=torch.bfloat16, device="cuda")
+    two = []
+    for i in range(min(n, 20) + 3):
+        flush(i)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        comb.comb_gemm_bf16(pool.handle, h, wkv[:Hkv * Dqk], kbuf, T, Hkv * Dqk, d_model)
+        comb.comb_gemm_bf16(pool.handle, h, wkv[Hkv * Dqk:], vbuf, T, Hkv * Dv, d_model)
+        pool.store_chunks(ids, tok, kbuf, vbuf)
+        b.record()
+        torch.cuda.synchronize()
+        if i >= 3:
+            two.append(a.elapsed_time(b))
+    comb.comb_profile_enable(pool.handle, False)
+    pool.close()
+    flops = 2.0 * T * N * d_model
+    nbytes = T * d_model * 2 + N * d_model * 2 + T * N * 2   # H and W read once, pages written once
+    achieved = flops / (st["mean"] * 1e-3) / 1e12
+    return {"workload": "K/V projection of long_fewshot's %d chunks (%d tokens) x d_model %d -> %d columns, written "
+                        "into pages by the GEMM epilogue" % (w.num_chunks, T, d_model, N),
+            "kernel_ms": st["mean"], "kernel_ms_median": st["median"], "kernel_ms_min": st["min"],
+            "launches_timed": st["n"], "two_step_ms": float(np.mean(two)),
+            "two_step": "2 x comb_gemm_bf16 (row-major K, V) + comb_store_chunks, CUDA events around the three launches",
+            "roofline": {"bound": "tensor", "achieved": achieved, "peak": pk["tf_burst"], "unit": "TFLOP/s",
+                         "frac": achieved / pk["tf_burst"], "frac_of_sustained": achieved / pk["tf_sustained"],
+                         "frac_of_nominal_2250": achieved / NOMINAL_BF16_TFLOPS, "algorithmic_flops": flops,
+                         "algorithmic_bytes": nbytes, "kernel": "gemm_paged",
+                         "traffic": ncu_traffic("gemm_paged", "long_fewshot")},
+            "l2": L2Flush.HOW}
+
+
+def bench_cross_layer(torch, comb, w, pk, phase, n, d_model=4096, L=8):
+    """(f3) the cross-attention sub-layer x + Attn(x W_Q) W_O over the paper's L = 8 cross layers on one
+    link: 8 x (Q-projection GEMM, attention, output-projection GEMM with the residual in its epilogue). The 8-layer pool
+    is filled with device-side N(0,1) (timing only); only the directory entries of the workload's chunks are made."""
+    Hq, Hkv, Dqk, Dv = w.num_q_heads, w.num_kv_heads, w.head_dim_qk, w.head_dim_v
+    pool = comb.Pool(Hkv, Dqk, Dv, w.pool_pages, num_layers=L, shuffle_seed=2024)
+    pool.k_arena.view(torch.bfloat16).normal_()
+    pool.v_arena.view(torch.bfloat16).normal_()
+    for c in range(w.num_chunks):
+        comb.comb_chunk_alloc(pool.handle, c, int(w.chunk_len[c]))
+    lb = pool.link_flat(w.chunk_indptr, w.chunk_ids_flat)
+    wq = w.decode_phase() if phase == "decode" and int(w.lq.max()) > 1 else w
+    rows = int(wq.total_q)
+    q_indptr = None if phase == "decode" else wq.q_indptr
+    x = torch.randn((rows, d_model), device="cuda").to(torch.bfloat16)
+    wqs = [(torch.randn((Hq * Dqk, d_model), device="cuda") / d_model ** 0.5).to(torch.bfloat16) for _ in range(L)]
+    wos = [(torch.randn((d_model, Hq * Dv), device="cuda") * (0.1 / (Hq * Dv) ** 0.5)).to(torch.bfloat16) for _ in range(L)]
+
+    bufs = [torch.empty_like(x), torch.empty_like(x)]
+
+    def step():  # ping-pong between two buffers; layer 0 reads x
+        src = x
+        for l in range(L):
+            dst = bufs[l & 1]
+            pool.layer_forward(lb, src, q_indptr, wqs[l], wos[l], w.scale, layer=l, out=dst)
+            src = dst
+
+    for _ in range(3):
+        step()
+    torch.cuda.synchronize()
+    comb.comb_profile_enable(pool.handle, True)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    with ClockSampler(torch.cuda.current_device()) as clk:
+        ev[0].record()
+        for _ in range(n):
+            step()
+        ev[1].record()
+        torch.cuda.synchronize()
+    ms = ev[0].elapsed_time(ev[1]) / n
+    gemm_ms = comb.comb_profile_read(pool.handle, comb.KERNEL_GEMM)[0] / n
+    attn_ms = sum(comb.comb_profile_read(pool.handle, k)[0] for k in (
+        comb.KERNEL_PREFILL, comb.KERNEL_PREFILL_MERGE, comb.KERNEL_DECODE_SPLIT, comb.KERNEL_DECODE_MERGE,
+        comb.KERNEL_DECODE_CASCADE, comb.KERNEL_CASCADE_MERGE)) / n
+    comb.comb_profile_enable(pool.handle, False)
+    pool.close()
+    torch.cuda.empty_cache()
+    gemm_flops = L * 2.0 * rows * d_model * (Hq * Dqk + Hq * Dv)
+    attn_flops = L * float(wq.attention_flops())
+    return {"workload": "%d cross layers (PAPER.md:78) of %s, %s phase: %d rows x d_model %d" % (
+                L, w.name, phase, rows, d_model),
+            "ms_per_step": ms, "gemm_ms": gemm_ms, "attention_ms": attn_ms,
+            "tflops": (gemm_flops + attn_flops) / (ms * 1e-3) / 1e12, "gemm_tflops": gemm_flops / (gemm_ms * 1e-3) / 1e12,
+            "us_per_q_token": ms * 1e3 / rows, "us_per_q_token_per_layer": ms * 1e3 / rows / L,
+            "weight_bytes": L * 2 * d_model * (Hq * Dqk + Hq * Dv), "clocks": clk.summary(),
+            "note": "Eq. 12: T_cross = O(L_cross l_query l_doc); per-layer cost = step / 8"}
 
 
 def bench_link(torch, comb, harness, w):
