@@ -184,9 +184,10 @@ int32_t comb_project_store_chunks(comb_pool_t *pool, int32_t layer, int32_t n, c
  *   cas_row_req     int32 [E]    request of the entry;   cas_row_entry int32 [E]   the entry's number
  *                                (inside a slot, entries are in ascending entry number)
  * Host mirror (only when host_buf != NULL; plain host memory the caller owns — a caller that builds its own
- * tables fills these two arrays itself):
+ * tables fills these three arrays itself):
  *   host_req_pages int32 [R]     page_indptr[r+1] - page_indptr[r]  (the prefill planner cuts KV ranges with it)
- *   host_cas_rows  int32 [U]     cas_row_indptr[u+1] - cas_row_indptr[u]  (the chunk-major decode tiles rows with it)
+ *   host_cas_rows  int32 [U]     cas_row_indptr[u+1] - cas_row_indptr[u]  (the chunk-major decode groups rows with it)
+ *   host_cas_pages int32 [U]     cas_page_indptr[u+1] - cas_page_indptr[u] (... and cuts long chunks into KV ranges)
  * Without a host mirror both attention calls still work: prefill does not cut KV ranges, decode runs per request.
  * A request with zero chunks is legal (kv_len 0). Duplicate ids inside a request are taken literally (two entries).
  * Errors: INVALID, UNKNOWN_CHUNK (nothing written), CAPACITY, CUDA. */
@@ -214,6 +215,7 @@ typedef struct {
     /* out: host pointers into host_buf (NULL without one) */
     int32_t *host_req_pages;
     int32_t *host_cas_rows;
+    int32_t *host_cas_pages;
     /* out: host-side summary */
     int32_t num_requests;
     int32_t max_pages_per_request;
@@ -266,9 +268,10 @@ int32_t comb_cross_attn_prefill(comb_pool_t *pool, int32_t layer, const comb_lin
  * Two paths compute it (same result up to fp32 summation order and, on the second, bf16 rounding of the softmax
  * weights fed to the tensor cores, as in prefill):
  *   per-request : split-KV kernel on CUDA cores (HBM-bound, GEMV-shaped) + LSE-merge kernel;
- *   chunk-major : every distinct chunk of the batch is streamed ONCE; the (entries x Hq/Hkv) query rows that link
- *                 it form the M tile of a tcgen05 contraction; per-entry fp32 partials are merged by LSE per
- *                 request (needs link->host_cas_rows).
+ *   chunk-major : every distinct chunk of the batch is streamed from HBM ONCE; the (entries x Hq/Hkv) query rows that
+ *                 link it are the N dimension (16 or 32 columns) of a tcgen05 contraction whose M dimension is the
+ *                 128 keys of a KV tile; per-(entry, KV range) fp32 partials are merged by LSE per request
+ *                 (needs link->host_cas_rows and host_cas_pages; Hq/Hkv <= 16).
  * COMB_OPT_DECODE_PATH picks one (default: chunk-major when the batch shares chunks, see comb_pool_set_option).
  * Errors as above. */
 int32_t comb_cross_attn_decode(comb_pool_t *pool, int32_t layer, const comb_link_t *link, int32_t num_requests,

@@ -39,7 +39,7 @@ class Link(C.Structure):
                 ("cas_page_indptr", C.c_void_p), ("cas_page_ids", C.c_void_p), ("cas_tile_indptr", C.c_void_p),
                 ("cas_tile_ntok", C.c_void_p), ("cas_row_indptr", C.c_void_p), ("cas_row_req", C.c_void_p),
                 ("cas_row_entry", C.c_void_p),
-                ("host_req_pages", C.c_void_p), ("host_cas_rows", C.c_void_p),
+                ("host_req_pages", C.c_void_p), ("host_cas_rows", C.c_void_p), ("host_cas_pages", C.c_void_p),
                 ("num_requests", C.c_int32), ("max_pages_per_request", C.c_int32),
                 ("total_pages", C.c_int64), ("total_tiles", C.c_int64), ("total_kv_tokens", C.c_int64),
                 ("total_entries", C.c_int64), ("num_distinct_chunks", C.c_int32), ("max_rows_per_chunk", C.c_int32),

@@ -270,11 +270,13 @@ class LinkedBatch:
         """The host arrays the attention planners read (None without a host buffer)."""
         L = self.link
         if not L.host_req_pages:
-            return {"req_pages": None, "cas_rows": None}
+            return {"req_pages": None, "cas_rows": None, "cas_pages": None}
         base = self.host.ctypes.data
-        o1, o2 = L.host_req_pages - base, L.host_cas_rows - base
+        o1, o2, o3 = L.host_req_pages - base, L.host_cas_rows - base, L.host_cas_pages - base
+        U = int(L.num_distinct_chunks)
         return {"req_pages": self.host[o1:o1 + 4 * L.num_requests].view(np.int32),
-                "cas_rows": self.host[o2:o2 + 4 * int(L.num_distinct_chunks)].view(np.int32)}
+                "cas_rows": self.host[o2:o2 + 4 * U].view(np.int32),
+                "cas_pages": self.host[o3:o3 + 4 * U].view(np.int32)}
 
 
 class Pool:

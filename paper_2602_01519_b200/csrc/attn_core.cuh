@@ -1,5 +1,6 @@
-// attn_core.cuh — the tcgen05 / TMEM / TMA flash-attention core shared by (a4) prefill cross-attention
-// (prefill_kernel.cu) and (f1) the chunk-major decode (cascade_kernel.cu).  PAPER.md:112-115 §4.2 Eq. 7-8:
+// attn_core.cuh — the tcgen05 / TMEM / TMA flash-attention core of (a4) prefill cross-attention
+// (prefill_kernel.cu; the chunk-major decode has its own swapped-operand kernel in cascade_kernel.cu).
+// PAPER.md:112-115 §4.2 Eq. 7-8:
 // A = softmax(QK^T/sqrt d) without mask, H = AV; PAPER.md:119 + 149: one joint softmax over the concatenation of the
 // linked chunks; Eq. 12 cost.
 //
@@ -14,8 +15,6 @@
 // MODE selects what an item is and where its rows go:
 //   kModeFinal   (request, kv-head, 1-2 Q tiles) over all of the request's KV  -> out / lse
 //   kModeRanges  the same over one KV range of the request                       -> fp32 partial rows (merged by LSE)
-//   kModeCascade (distinct chunk, kv-head, tile of the entries that link it): the Q rows are GATHERED from the
-//                requests that link the chunk, the KV is the chunk's own page list -> per-entry fp32 partials
 #pragma once
 #include "kernels.h"
 #include "ptx.cuh"
@@ -26,7 +25,7 @@
 namespace comb {
 namespace {
 
-enum { kModeFinal = 0, kModeRanges = 1, kModeCascade = 2 };
+enum { kModeFinal = 0, kModeRanges = 1 };
 
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
@@ -48,24 +47,12 @@ struct PrefillArgs {
     float *part_lse;     // [partial rows]       log2(sum_j 2^(s_j * scale_log2)) over the item's range
     int64_t total_q;
     int nsplit;
-    // chunk-major decode (kModeCascade): page_indptr / page_ids / tile_indptr / tile_ntok above are the link's cas_*
-    // tables (a "request" is a chunk slot); the Q rows of a tile are gathered through cas_row_req and its partial
-    // rows go to part_o / part_lse [entry][Hq]
-    const CascadeTile *cas_tiles;
-    const int32_t *cas_row_req, *cas_row_entry;
-    const char *q;       // bf16 [R][Hq][Dqk]
 };
 
 // Work item `idx` of the launch.
 template <int MODE>
 __device__ __forceinline__ PrefillItem fetch_item(const PrefillArgs &a, int idx) {
-    if constexpr (MODE == kModeCascade) {
-        const int tile = idx / a.num_kv_heads;
-        const CascadeTile ct = a.cas_tiles[tile];
-        return PrefillItem{ct.slot, idx - tile * a.num_kv_heads, ct.row0, ct.nrows, 0, INT32_MAX / kTilePages, 0, 0};
-    } else {
-        return a.items[idx];
-    }
+    return a.items[idx];
 }
 
 // The slice of a request's tables an item covers: first table entry, number of entries, first tile.
@@ -235,19 +222,11 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                 }
                 continue;
             }
-            // chunk-major tiles are mostly a few rows (entries x G): warps that own no valid row only keep the
-            // barrier protocol going (their P rows stay garbage, and so do the O rows nobody stores)
-            const bool warp_active = MODE != kModeCascade || (warp & 3) * 32 < tok_valid * G;
             float m_used = -INFINITY, l_run = 0.f;
             for (int j = 0; j < n_kv; ++j) {
                 const uint64_t ntok8 = a.tile_ntok[tile0 + j];
                 ptx::mbar_wait(&s_full[t], s_cnt & 1);
                 ++s_cnt;
-                if (!warp_active) {
-                    ptx::mbar_arrive(&p_full[t * 2]);
-                    ptx::mbar_arrive(&p_full[t * 2 + 1]);
-                    continue;
-                }
                 ptx::tc_fence_after();
                 uint32_t r[kTileN];
 #pragma unroll
@@ -268,7 +247,7 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                 const float m_new = fmaxf(fmax3(mx4[0], mx4[1], mx4[2]), fmaxf(mx4[3], m_used));
                 if (j == 0) {
                     m_used = m_new;
-                } else if (__any_sync(0xffffffffu, (MODE != kModeCascade || row_valid) && (m_new - m_used) * c > 8.f)) {
+                } else if (__any_sync(0xffffffffu, (m_new - m_used) * c > 8.f)) {
                     // rare: move the reference max and rescale this warp's rows of the accumulator
                     ptx::mbar_wait(&o_done[t], (o_cnt + j - 1) & 1);  // P V_{j-1} has landed
                     ptx::tc_fence_after();
@@ -308,19 +287,14 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                 l_run += (sA.x + sA.y) + (sB.x + sB.y);
             }
             // ---- epilogue: O / l -> bf16 (or an fp32 partial row) ----
-            if (!warp_active) {
-                o_cnt += n_kv;
-                continue;
-            }
             ptx::mbar_wait(&o_done[t], (o_cnt + n_kv - 1) & 1);
             o_cnt += n_kv;
             ptx::tc_fence_after();
             const float inv = 1.f / l_run;
-            // partial: one KV range of several, or one chunk of the request's several (compiled in only then)
-            const bool partial = (MODE == kModeRanges && tv.split >= 0) || MODE == kModeCascade;
+            // partial: one KV range of several (compiled in only then)
+            const bool partial = MODE == kModeRanges && tv.split >= 0;
             size_t prow = 0;
             if (MODE == kModeRanges && partial) prow = (size_t)it.part_base + (size_t)tv.split * (2 * kTileM) + t * kTileM + row;
-            if (MODE == kModeCascade && row_valid) prow = (size_t)a.cas_row_entry[tok] * Hq + head;
 #pragma unroll
             for (int q = 0; q < DV / 32; ++q) {
                 uint32_t o[32];
@@ -363,53 +337,16 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                 n_kv[t] = (t < NT && tv[t].tok_valid > 0) ? (tv[t].npages + kTilePages - 1) / kTilePages : 0;
             }
             if (n_kv[0] == 0) continue;
-            if constexpr (MODE == kModeCascade) {
-                // Q rows of a chunk-major tile come from different requests: gather them with plain 16-byte loads
-                // and lay them out as the SWIZZLE_128B tile TMA would have written (16-byte unit j of row r sits at
-                // unit j ^ (r & 7) of its 128-byte row). Loads are issued before the wait for the tile slot.
-                constexpr int UPR = DQK / 8;  // 16-byte units per row
-                const int units = tv[0].tok_valid * G * UPR;
-                bool waited = false;
-                for (int u0 = 0; u0 < units; u0 += 32 * 4) {
-                    uint4 val[4];
-                    uint32_t dst[4];
 #pragma unroll
-                    for (int x = 0; x < 4; ++x) {
-                        const int u = u0 + x * 32 + lane;
-                        dst[x] = 0xffffffffu;
-                        if (u < units) {
-                            const int row = u / UPR, j = u - row * UPR;
-                            const int slot = row / G, hh = row - slot * G;
-                            const int qrow = a.cas_row_req[tv[0].q_row0 + slot];
-                            val[x] = __ldg(reinterpret_cast<const uint4 *>(
-                                a.q + (((size_t)qrow * Hq + it.kv_head * G + hh) * DQK) * 2 + (size_t)j * 16));
-                            dst[x] = (uint32_t)((j >> 3) * C::HALF + row * 128 + (((j & 7) ^ (row & 7)) << 4));
-                        }
-                    }
-                    if (!waited) {
-                        ptx::mbar_wait(&q_empty[0], (qcnt[0] & 1) ^ 1);
-                        ++qcnt[0];
-                        waited = true;
-                    }
-#pragma unroll
-                    for (int x = 0; x < 4; ++x)
-                        if (dst[x] != 0xffffffffu) *reinterpret_cast<uint4 *>(sQ + dst[x]) = val[x];
-                }
-                ptx::fence_proxy_async_smem();  // generic-proxy stores -> visible to the tensor core's smem reads
-                __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(&q_full[0]);
-            } else {
-#pragma unroll
-                for (int t = 0; t < NT; ++t) {
-                    if (n_kv[t] == 0) continue;
-                    ptx::mbar_wait(&q_empty[t], (qcnt[t] & 1) ^ 1);
-                    ++qcnt[t];
-                    if (lane == 0) {
-                        ptx::mbar_expect_tx(&q_full[t], C::Q_BYTES);
-                        for (int h = 0; h < C::KH; ++h)
-                            ptx::tma_load_3d(sQ + t * C::Q_BYTES + h * C::HALF, &maps.q, h * 64, it.kv_head * G,
-                                             tv[t].q_row0, &q_full[t]);
-                    }
+            for (int t = 0; t < NT; ++t) {
+                if (n_kv[t] == 0) continue;
+                ptx::mbar_wait(&q_empty[t], (qcnt[t] & 1) ^ 1);
+                ++qcnt[t];
+                if (lane == 0) {
+                    ptx::mbar_expect_tx(&q_full[t], C::Q_BYTES);
+                    for (int h = 0; h < C::KH; ++h)
+                        ptx::tma_load_3d(sQ + t * C::Q_BYTES + h * C::HALF, &maps.q, h * 64, it.kv_head * G,
+                                         tv[t].q_row0, &q_full[t]);
                 }
             }
             // one K (is_v = false) or V tile of tile slot t's stream into the next ring slot

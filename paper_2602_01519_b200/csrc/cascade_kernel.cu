@@ -4,25 +4,503 @@
 // (§1 "in any order/position"), and retrieval workloads re-use a few hot chunks heavily
 // (PAPER.md:297).  So instead of streaming a chunk once per linking request (GEMV-shaped, CUDA cores, up to 99 reads
 // of the hottest chunk in BASELINE configs[1]), the batch is inverted at link time and every DISTINCT chunk is
-// streamed once: the (entries x G) query rows that link it form the M tile of the tcgen05 contraction of
-// attn_core.cuh (mode kModeCascade: Q rows gathered from the linking requests, KV = the chunk's own page list).  Each
-// (entry, head) gets a normalised fp32 partial row and a log2-domain LSE; cascade_merge_kernel combines a request's
-// entries by identity P8:  O = sum_e w_e O_e / sum_e w_e,  w_e = 2^(lse2_e - max),
+// streamed from HBM once; the query rows of all the requests that link it attend to it together.
+//
+// Decode has few query rows per chunk (entries x G, mostly 4..32) and many keys, so the contraction is issued with
+// the operands swapped: the 128 KEYS of a KV tile are the M dimension of the tcgen05 MMA and the query rows the N
+// dimension (16 or 32):
+//   S^T[key][row] = K_tile[128 x Dqk] . Q^T          A = K tile (smem, K-major, as TMA wrote the pages), B = Q rows
+//   O^T[d][row]  += V_tile^T[Dv x 128] . P^T         A = V tile (smem, MN-major, straight from its page layout), B = P
+// One softmax thread owns one KEY (TMEM lane) and the 16/32 rows are its columns: 8x fewer exponentials and TMEM reads
+// per tile than a 128-row tile needs, and the per-tile dependency chain is ~500 clk, so the kernel is bound by the
+// HBM stream alone.  The row maximum (over keys = across threads) is a CREDUX per row and warp plus one exchange
+// through shared memory; the reference maximum only moves when it grows by more than 2^8 (lazy rescale of O^T).
+// Work items (tile of entries, KV range of the chunk, kv-head) are handed out through an atomic counter (the tail of a
+// static assignment cost 16 % on configs[1]); long chunks are cut into KV ranges when the batch has too few items.
+// Each (entry, range, head) gets a normalised fp32 partial row and a log2-domain LSE; cascade_merge_kernel combines a
+// request's partials by identity P8:  O = sum_e w_e O_e / sum_e w_e,  w_e = 2^(lse2_e - max),
 // LSE = ln 2 (max + log2 sum_e w_e).  One joint softmax over the concatenation, as Eq. 7-8 with PAPER.md:149 demand.
-#include "attn_core.cuh"
+//
+// Warp roles (256 threads, one CTA per SM): 0-3 softmax + epilogue (thread = key / output column d), 4 K/V TMA loader,
+// 5 tcgen05.mma issuer, 6 scheduler (atomic item fetch) + gather of the items' Q rows, 7 idle.
+#include "kernels.h"
+#include "ptx.cuh"
 
+#include <cuda.h>
+#include <cuda_bf16.h>
 #include <cstring>
 
 namespace comb {
 namespace {
 
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kLn2 = 0.6931471805599453f;
+constexpr int kRowsMax = 32;       // query rows (N of the MMA) per item: 16 or 32
+constexpr int kItemRing = 3;       // items the scheduler may be ahead
+
+struct CascadeArgs {
+    const CascadeItem *items;
+    unsigned int *counter;
+    int num_items;  // units x kv-heads
+    const int32_t *cas_page_indptr, *cas_page_ids, *cas_tile_indptr;
+    const uint64_t *cas_tile_ntok;
+    const int32_t *cas_row_req, *cas_row_entry;
+    const char *q;  // bf16 [R][Hq][Dqk]
+    float *part_o, *part_lse;
+    int4 *ent_info;
+    int num_q_heads, num_kv_heads, group, group_shift;
+    int layer_row0;
+    float scale_log2;
+};
+
+struct KvMaps {
+    CUtensorMap k, v;
+};
+
+// what the scheduler hands to the other warps (shared memory)
+struct ItemEntry {
+    int32_t valid, kvh, nrows, ncols;
+    int32_t pbeg, npages, tile0, row0;
+    int32_t part0, stride, range_nr, pad;
+};
+
+template <int DQK, int DV>
+struct CasCfg {
+    static constexpr int KH = DQK / 64, VH = DV / 64;
+    static constexpr int HALF = 128 * 128;               // [128 keys][64 bf16] of a K or V tile
+    static constexpr int K_BYTES = KH * HALF, V_BYTES = VH * HALF;
+    static constexpr int SLOT = K_BYTES > V_BYTES ? K_BYTES : V_BYTES;
+    static constexpr int QH = kRowsMax * 128;             // [32 rows][64 bf16] of a Q or P tile
+    static constexpr int Q_BYTES = KH * QH;
+    static constexpr int P_BYTES = 2 * QH;                // 32 rows x 128 keys
+    static constexpr int MISC = 3072;
+    static constexpr int SMEM_MAX = 232448;
+    static constexpr int NSLOT_RAW = (SMEM_MAX - 1024 - MISC - 2 * Q_BYTES - P_BYTES) / SLOT;
+    static constexpr int NSLOT = NSLOT_RAW > 8 ? 8 : NSLOT_RAW;
+    static constexpr int SMEM = 1024 + 2 * Q_BYTES + P_BYTES + NSLOT * SLOT + MISC;
+    static constexpr int THREADS = 256;
+    static constexpr int TMEM_COLS = 128;                 // S^T x2 @0,32; O^T x2 @64,96
+};
+
+struct Misc {
+    uint64_t item_full[kItemRing], item_empty[kItemRing];
+    uint64_t q_full[2], q_empty[2], s_full[2], s_empty[2], o_full[2], o_empty[2];
+    uint64_t p_full, p_empty;
+    uint64_t kv_full[8], kv_empty[8];
+    float wmax[2][4][kRowsMax];
+    float wsum[4][kRowsMax];
+    int32_t srow[2][kRowsMax];
+    ItemEntry items[kItemRing];
+    uint32_t tmem_slot;
+};
+static_assert(sizeof(Misc) <= 3072, "Misc must fit its reservation");
+
+__device__ __forceinline__ float warp_max(float x) {
+    float y;
+    asm volatile("redux.sync.max.f32 %0, %1, 0xffffffff;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ void named_bar_sync(int id, int threads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+// kind::f16 instruction descriptor, bf16 x bf16 -> fp32, with either operand MN-major
+__host__ __device__ constexpr uint32_t idesc_bf16(int m, int n, bool a_mn, bool b_mn) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((a_mn ? 1u : 0u) << 15) | ((b_mn ? 1u : 0u) << 16) |
+           ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
+}
+
+// ---- softmax + epilogue of one item, NC = 16 or 32 query rows (columns of S^T / O^T) ----
+template <int DQK, int DV, int NC>
+__device__ __forceinline__ void softmax_item(const CascadeArgs &a, Misc *mi, unsigned char *sP, uint32_t tmem,
+                                             const ItemEntry &it, const int k, uint32_t &t) {
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+    const int ip = k & 1;
+    const int n_kv = (it.npages + kTilePages - 1) / kTilePages;
+    const int rows_valid = it.nrows * a.group;
+    const float c = a.scale_log2;
+    float m_used[NC], l_part[NC];
+#pragma unroll
+    for (int n = 0; n < NC; ++n) { m_used[n] = -INFINITY; l_part[n] = 0.f; }
+    // this thread's key inside a tile: page kp, slot ks; where its P goes (row n adds n * 128 and the swizzle)
+    const int kp = tid >> 4, ks = tid & 15;
+    const uint32_t p_key = (uint32_t)((tid >> 6) * CasCfg<DQK, DV>::QH + (tid & 7) * 2);
+    const uint32_t p_unit = (uint32_t)((tid & 63) >> 3);
+    for (int j = 0; j < n_kv; ++j, ++t) {
+        const uint64_t ntok8 = a.cas_tile_ntok[it.tile0 + j];
+        const bool key_valid = ks < (int)((ntok8 >> (8 * kp)) & 0xffu);
+        const int sb = t & 1;
+        ptx::mbar_wait(&mi->s_full[sb], (t >> 1) & 1);
+        ptx::tc_fence_after();
+        uint32_t r[NC];
+#pragma unroll
+        for (int q = 0; q < NC / 16; ++q)
+            ptx::tmem_ld16(tmem + lane_base + sb * kRowsMax + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&r[q * 16]));
+        ptx::tmem_wait_ld();
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&mi->s_empty[sb]);
+        // max over the keys of every row: in the warp by CREDUX, across the four warps through shared memory
+        float wm[NC];
+#pragma unroll
+        for (int n = 0; n < NC; ++n) {
+            if (!key_valid) r[n] = 0xff800000u;  // slots past a chunk's length / pages the tile does not have
+            wm[n] = warp_max(__uint_as_float(r[n]));
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int n = 0; n < NC; n += 4)
+                *reinterpret_cast<float4 *>(&mi->wmax[sb][warp][n]) = make_float4(wm[n], wm[n + 1], wm[n + 2], wm[n + 3]);
+        }
+        named_bar_sync(1, 128);
+        bool grow = false;
+#pragma unroll
+        for (int n = 0; n < NC; n += 4) {
+            const float4 w0 = *reinterpret_cast<const float4 *>(&mi->wmax[sb][0][n]);
+            const float4 w1 = *reinterpret_cast<const float4 *>(&mi->wmax[sb][1][n]);
+            const float4 w2 = *reinterpret_cast<const float4 *>(&mi->wmax[sb][2][n]);
+            const float4 w3 = *reinterpret_cast<const float4 *>(&mi->wmax[sb][3][n]);
+            wm[n] = fmaxf(fmaxf(w0.x, w1.x), fmaxf(w2.x, w3.x));
+            wm[n + 1] = fmaxf(fmaxf(w0.y, w1.y), fmaxf(w2.y, w3.y));
+            wm[n + 2] = fmaxf(fmaxf(w0.z, w1.z), fmaxf(w2.z, w3.z));
+            wm[n + 3] = fmaxf(fmaxf(w0.w, w1.w), fmaxf(w2.w, w3.w));
+        }
+#pragma unroll
+        for (int n = 0; n < NC; ++n) grow |= n < rows_valid && (wm[n] - m_used[n]) * c > 8.f;
+        // P V_{t-1} has completed: the P tile may be overwritten and O^T is up to date
+        ptx::mbar_wait(&mi->p_empty, (t & 1) ^ 1);
+        if (j == 0) {
+#pragma unroll
+            for (int n = 0; n < NC; ++n) m_used[n] = wm[n];
+        } else if (grow) {  // identical in all 128 threads (same shared data): move the reference, rescale O^T
+            ptx::tc_fence_after();
+            uint32_t o[NC];
+#pragma unroll
+            for (int q = 0; q < NC / 16; ++q)
+                ptx::tmem_ld16(tmem + lane_base + 64 + ip * kRowsMax + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
+            ptx::tmem_wait_ld();
+#pragma unroll
+            for (int n = 0; n < NC; ++n) {
+                const float m_new = fmaxf(m_used[n], wm[n]);
+                const float alpha = ptx::ex2((m_used[n] - m_new) * c);
+                o[n] = __float_as_uint(__uint_as_float(o[n]) * alpha);
+                l_part[n] *= alpha;
+                m_used[n] = m_new;
+            }
+#pragma unroll
+            for (int q = 0; q < NC / 16; ++q)
+                ptx::tmem_st16(tmem + lane_base + 64 + ip * kRowsMax + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
+            ptx::tmem_wait_st();
+            ptx::tc_fence_before();
+        }
+#pragma unroll
+        for (int n = 0; n < NC; ++n) {
+            const float p = ptx::ex2(fmaf(__uint_as_float(r[n]), c, -m_used[n] * c));
+            l_part[n] += p;
+            const __nv_bfloat16 pb = __float2bfloat16_rn(p);
+            *reinterpret_cast<__nv_bfloat16 *>(sP + p_key + n * 128 + ((p_unit ^ (uint32_t)(n & 7)) << 4)) = pb;
+        }
+        ptx::fence_proxy_async_smem();  // generic-proxy stores -> visible to the tensor core's shared-memory reads
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&mi->p_full);
+    }
+    // ---- epilogue: row sums across the 128 keys, then O^T / l -> fp32 partial rows ----
+#pragma unroll
+    for (int n = 0; n < NC; ++n) {
+        float v = l_part[n];
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+        l_part[n] = v;
+    }
+    if (lane == 0) {
+#pragma unroll
+        for (int n = 0; n < NC; n += 4)
+            *reinterpret_cast<float4 *>(&mi->wsum[warp][n]) = make_float4(l_part[n], l_part[n + 1], l_part[n + 2], l_part[n + 3]);
+    }
+    named_bar_sync(1, 128);
+    ptx::mbar_wait(&mi->o_full[ip], (k >> 1) & 1);
+    ptx::tc_fence_after();
+    uint32_t o[NC];
+#pragma unroll
+    for (int q = 0; q < NC / 16; ++q)
+        ptx::tmem_ld16(tmem + lane_base + 64 + ip * kRowsMax + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
+    ptx::tmem_wait_ld();
+    ptx::tc_fence_before();
+    __syncwarp();
+    if (lane == 0) ptx::mbar_arrive(&mi->o_empty[ip]);
+#pragma unroll
+    for (int n = 0; n < NC; ++n) {
+        const int prow = mi->srow[ip][n];
+        if (prow < 0) continue;  // padding row (uniform)
+        const float l = (mi->wsum[0][n] + mi->wsum[1][n]) + (mi->wsum[2][n] + mi->wsum[3][n]);
+        if (tid < DV) a.part_o[(size_t)prow * DV + tid] = __uint_as_float(o[n]) * (1.f / l);
+        if (tid == n) a.part_lse[prow] = m_used[n] * c + log2f(l);
+    }
+}
+
+template <int DQK, int DV>
+__global__ void __launch_bounds__(256, 1)
+cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) {
+    using C = CasCfg<DQK, DV>;
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    unsigned char *sQ = smem;                       // 2 x [KH][32 rows][64]
+    unsigned char *sP = sQ + 2 * C::Q_BYTES;        // [2][32 rows][64 keys]
+    unsigned char *sKV = sP + C::P_BYTES;           // ring of NSLOT K / V tiles
+    Misc *mi = reinterpret_cast<Misc *>(sKV + C::NSLOT * C::SLOT);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        for (int i = 0; i < kItemRing; ++i) {
+            ptx::mbar_init(&mi->item_full[i], 1);
+            ptx::mbar_init(&mi->item_empty[i], 6);  // loader, issuer, four softmax warps
+        }
+        for (int i = 0; i < 2; ++i) {
+            ptx::mbar_init(&mi->q_full[i], 1);
+            ptx::mbar_init(&mi->q_empty[i], 1);
+            ptx::mbar_init(&mi->s_full[i], 1);
+            ptx::mbar_init(&mi->s_empty[i], 4);
+            ptx::mbar_init(&mi->o_full[i], 1);
+            ptx::mbar_init(&mi->o_empty[i], 4);
+        }
+        ptx::mbar_init(&mi->p_full, 4);
+        ptx::mbar_init(&mi->p_empty, 1);
+        for (int s = 0; s < C::NSLOT; ++s) {
+            ptx::mbar_init(&mi->kv_full[s], 1);
+            ptx::mbar_init(&mi->kv_empty[s], 1);
+        }
+        ptx::fence_barrier_init();
+        ptx::tma_prefetch_desc(&maps.k);
+        ptx::tma_prefetch_desc(&maps.v);
+    }
+    if (warp == 5) {
+        ptx::tmem_alloc(&mi->tmem_slot, C::TMEM_COLS);
+        ptx::tmem_relinquish();
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem = mi->tmem_slot;
+    const int G = a.group, Hq = a.num_q_heads, Hkv = a.num_kv_heads;
+
+    if (warp < 4) {
+        // ===================== softmax + epilogue: thread = key of the tile / output column d =====================
+        uint32_t t = 0;
+        for (int k = 0;; ++k) {
+            const int ir = k % kItemRing;
+            ptx::mbar_wait(&mi->item_full[ir], (k / kItemRing) & 1);
+            const ItemEntry it = mi->items[ir];
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&mi->item_empty[ir]);
+            if (!it.valid) break;
+            if (tid < kRowsMax) {  // where the rows of this item go
+                const int e_pos = tid >> a.group_shift, head = tid & (G - 1);
+                const bool valid = e_pos < it.nrows;
+                mi->srow[k & 1][tid] = valid ? (it.part0 + e_pos) * Hq + it.kvh * G + head : -1;
+                if (valid && head == 0 && it.kvh == 0 && (it.range_nr & 0xff) == 0)
+                    a.ent_info[a.cas_row_entry[it.row0 + e_pos]] =
+                        make_int4(it.part0 + e_pos, it.stride, it.range_nr >> 8, 0);
+            }
+            // (srow is read after the barrier syncs of the tile loop below)
+            if (it.ncols == 16) softmax_item<DQK, DV, 16>(a, mi, sP, tmem, it, k, t);
+            else softmax_item<DQK, DV, 32>(a, mi, sP, tmem, it, k, t);
+        }
+    } else if (warp == 4) {
+        // ===================== K/V TMA loader: K_t, then V_{t-1}, through one ring =====================
+        uint32_t slot = 0, phase = 0;
+        bool have_prev = false;
+        int prev_row0 = 0, prev_pages = 0;
+        auto issue = [&](bool is_v, int row0, int pages_here) {
+            ptx::mbar_wait(&mi->kv_empty[slot], phase ^ 1);
+            unsigned char *dst = sKV + slot * C::SLOT;
+            if (lane == 0) ptx::mbar_expect_tx(&mi->kv_full[slot], (uint32_t)pages_here * kPage * (is_v ? DV : DQK) * 2);
+            __syncwarp();
+            if (lane < pages_here) {
+                if (!is_v) {
+#pragma unroll
+                    for (int h = 0; h < C::KH; ++h)
+                        ptx::tma_load_2d(dst + h * C::HALF + lane * 2048, &maps.k, h * 64, row0, &mi->kv_full[slot]);
+                } else {
+#pragma unroll
+                    for (int h = 0; h < C::VH; ++h)
+                        ptx::tma_load_2d(dst + h * C::HALF + lane * 2048, &maps.v, h * 64, row0, &mi->kv_full[slot]);
+                }
+            }
+            if (++slot == C::NSLOT) { slot = 0; phase ^= 1; }
+        };
+        for (int k = 0;; ++k) {
+            const int ir = k % kItemRing;
+            ptx::mbar_wait(&mi->item_full[ir], (k / kItemRing) & 1);
+            const ItemEntry it = mi->items[ir];
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&mi->item_empty[ir]);
+            if (!it.valid) break;
+            const int n_kv = (it.npages + kTilePages - 1) / kTilePages;
+            int ids = 0;
+            for (int j = 0; j < n_kv; ++j) {
+                if ((j & 3) == 0)  // page ids of the next four tiles, one load
+                    ids = (j * kTilePages + lane < it.npages) ? a.cas_page_ids[it.pbeg + j * kTilePages + lane] : 0;
+                const int pages_here = min(kTilePages, it.npages - j * kTilePages);
+                const int pid = __shfl_sync(0xffffffffu, ids, (j & 3) * kTilePages + (lane & 7));
+                const int row0 = a.layer_row0 + (pid * Hkv + it.kvh) * kPage;
+                issue(false, row0, pages_here);
+                if (have_prev) issue(true, prev_row0, prev_pages);
+                prev_row0 = row0;
+                prev_pages = pages_here;
+                have_prev = true;
+            }
+        }
+        if (have_prev) issue(true, prev_row0, prev_pages);
+    } else if (warp == 5) {
+        // ===================== MMA issuer: S^T_t is issued before P V_{t-1} =====================
+        const bool leader = ptx::elect_one();
+        const uint64_t dq0 = ptx::umma_desc_sw128(ptx::smem_u32(sQ), 16, 1024);
+        const uint64_t dp0 = ptx::umma_desc_sw128(ptx::smem_u32(sP), 16, 1024);
+        const uint64_t dk0 = ptx::umma_desc_sw128(ptx::smem_u32(sKV), 16, 1024);
+        const uint64_t dv0 = ptx::umma_desc_sw128(ptx::smem_u32(sKV), C::VH > 1 ? C::HALF : 0, 1024);
+        uint32_t slot = 0, phase = 0, t = 0;
+        struct Pend { bool on, first, last; int pages, ip, k; uint32_t t, idesc; } pd{false, false, false, 0, 0, 0, 0, 0};
+        auto do_pv = [&]() {
+            ptx::mbar_wait(&mi->kv_full[slot], phase);
+            ptx::mbar_wait(&mi->p_full, pd.t & 1);
+            if (pd.first) ptx::mbar_wait(&mi->o_empty[pd.ip], ((pd.k >> 1) & 1) ^ 1);
+            ptx::tc_fence_after();
+            for (int ks = 0; ks < pd.pages; ++ks)  // one k-step of 16 keys per page the tile has
+                if (leader)
+                    ptx::mma_ss(tmem + 64 + pd.ip * kRowsMax, dv0 + (uint64_t)((slot * C::SLOT + ks * 2048) >> 4),
+                                dp0 + (uint64_t)(((ks >> 2) * C::QH + (ks & 3) * 32) >> 4), pd.idesc,
+                                (pd.first && ks == 0) ? 0u : 1u);
+            if (leader) {
+                ptx::mma_commit(&mi->p_empty);
+                ptx::mma_commit(&mi->kv_empty[slot]);
+                if (pd.last) ptx::mma_commit(&mi->o_full[pd.ip]);
+            }
+            if (++slot == C::NSLOT) { slot = 0; phase ^= 1; }
+            pd.on = false;
+        };
+        for (int k = 0;; ++k) {
+            const int ir = k % kItemRing;
+            ptx::mbar_wait(&mi->item_full[ir], (k / kItemRing) & 1);
+            const ItemEntry it = mi->items[ir];
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&mi->item_empty[ir]);
+            if (!it.valid) break;
+            const int ip = k & 1;
+            const int n_kv = (it.npages + kTilePages - 1) / kTilePages;
+            const uint32_t idesc_s = idesc_bf16(128, it.ncols, false, false);
+            const uint32_t idesc_o = idesc_bf16(128, it.ncols, true, false);
+            ptx::mbar_wait(&mi->q_full[ip], (k >> 1) & 1);
+            for (int j = 0; j < n_kv; ++j, ++t) {
+                const int sb = t & 1;
+                ptx::mbar_wait(&mi->kv_full[slot], phase);
+                ptx::mbar_wait(&mi->s_empty[sb], ((t >> 1) & 1) ^ 1);
+                ptx::tc_fence_after();
+                const uint64_t dk = dk0 + (uint64_t)((slot * C::SLOT) >> 4), dq = dq0 + (uint64_t)((ip * C::Q_BYTES) >> 4);
+#pragma unroll
+                for (int kk = 0; kk < DQK / 16; ++kk)
+                    if (leader)
+                        ptx::mma_ss(tmem + sb * kRowsMax, dk + (uint64_t)(((kk / 4) * C::HALF + (kk % 4) * 32) >> 4),
+                                    dq + (uint64_t)(((kk / 4) * C::QH + (kk % 4) * 32) >> 4), idesc_s, kk > 0);
+                if (leader) {
+                    ptx::mma_commit(&mi->s_full[sb]);
+                    ptx::mma_commit(&mi->kv_empty[slot]);
+                    if (j + 1 == n_kv) ptx::mma_commit(&mi->q_empty[ip]);
+                }
+                if (++slot == C::NSLOT) { slot = 0; phase ^= 1; }
+                if (pd.on) do_pv();
+                pd = Pend{true, j == 0, j + 1 == n_kv, min(kTilePages, it.npages - j * kTilePages), ip, k, t, idesc_o};
+            }
+        }
+        if (pd.on) do_pv();
+    } else if (warp == 6) {
+        // ===================== scheduler + Q gather =====================
+        constexpr int UPR = DQK / 8;  // 16-byte units per Q row
+        for (int k = 0;; ++k) {
+            const int ir = k % kItemRing;
+            ptx::mbar_wait(&mi->item_empty[ir], ((k / kItemRing) & 1) ^ 1);
+            unsigned int idx = 0;
+            if (lane == 0) idx = atomicAdd(a.counter, 1u);
+            idx = __shfl_sync(0xffffffffu, idx, 0);
+            if (idx >= (unsigned int)a.num_items) {
+                if (lane == 0) {
+                    mi->items[ir].valid = 0;
+                    ptx::mbar_arrive(&mi->item_full[ir]);
+                }
+                break;
+            }
+            const int unit = (int)idx / Hkv, kvh = (int)idx - unit * Hkv;
+            const CascadeItem ci = a.items[unit];
+            const int pb = a.cas_page_indptr[ci.slot], np = a.cas_page_indptr[ci.slot + 1] - pb;
+            const int skip = min(np, ci.kv_tile0 * kTilePages);
+            const int rows_valid = ci.nrows * G;
+            const int ncols = rows_valid <= 16 ? 16 : 32;
+            if (lane == 0) {
+                ItemEntry e;
+                e.valid = 1;
+                e.kvh = kvh;
+                e.nrows = ci.nrows;
+                e.ncols = ncols;
+                e.pbeg = pb + skip;
+                e.npages = min(np - skip, ci.kv_tiles * kTilePages);
+                e.tile0 = a.cas_tile_indptr[ci.slot] + ci.kv_tile0;
+                e.row0 = ci.row0;
+                e.part0 = ci.part0;
+                e.stride = ci.part_stride;
+                e.range_nr = ci.range_nr;
+                e.pad = 0;
+                mi->items[ir] = e;
+                ptx::mbar_arrive(&mi->item_full[ir]);
+            }
+            // ---- Q rows of the item: entry e_pos of the tile, head hh of the kv-head -> row e_pos * G + hh, laid out
+            // as the SWIZZLE_128B K-major tile TMA would have written (unit j of row r at unit j ^ (r & 7)); rows up
+            // to ncols are zero-filled
+            const int req_lane = lane < ci.nrows ? a.cas_row_req[ci.row0 + lane] : 0;
+            const int qb = k & 1;
+            ptx::mbar_wait(&mi->q_empty[qb], ((k >> 1) & 1) ^ 1);
+            unsigned char *dstq = sQ + qb * C::Q_BYTES;
+            const int units = ncols * UPR;
+            for (int u0 = 0; u0 < units; u0 += 128) {
+                uint4 val[4];
+                uint32_t dst[4];
+#pragma unroll
+                for (int x = 0; x < 4; ++x) {
+                    const int u = u0 + x * 32 + lane;
+                    const int row = u / UPR, j = u - row * UPR;
+                    const int e_pos = row >> a.group_shift, hh = row & (G - 1);
+                    const int qrow = __shfl_sync(0xffffffffu, req_lane, e_pos & 31);
+                    val[x] = make_uint4(0u, 0u, 0u, 0u);
+                    dst[x] = 0xffffffffu;
+                    if (u < units) {
+                        if (row < rows_valid)
+                            val[x] = __ldg(reinterpret_cast<const uint4 *>(
+                                a.q + (((size_t)qrow * Hq + kvh * G + hh) * DQK) * 2 + (size_t)j * 16));
+                        dst[x] = (uint32_t)((j >> 3) * C::QH + row * 128 + (((j & 7) ^ (row & 7)) << 4));
+                    }
+                }
+#pragma unroll
+                for (int x = 0; x < 4; ++x)
+                    if (dst[x] != 0xffffffffu) *reinterpret_cast<uint4 *>(dstq + dst[x]) = val[x];
+            }
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&mi->q_full[qb]);
+        }
+    }
+
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    if (warp == 5) ptx::tmem_dealloc(tmem, C::TMEM_COLS);
+}
+
 // One CTA of 4 warps per (request, q head): the request's entries are dealt round-robin to the warps, a lane owns
 // DV/32 consecutive output columns, and the four warps' weighted sums meet in shared memory.  Every warp first reads
-// ALL of the request's LSEs (one per lane per pass; they are few) to agree on the maximum, then streams its share of
-// the partial rows with 4 independent loads in flight.
+// ALL of the request's LSEs to agree on the maximum, then streams its share of the partial rows.  An entry's partials
+// (one per KV range of its chunk) are found through ent_info = (first index, stride, count).
 template <int DV>
 __global__ void __launch_bounds__(128) cascade_merge_kernel(const float *__restrict__ part_o,
                                                             const float *__restrict__ part_lse,
+                                                            const int4 *__restrict__ ent_info,
                                                             const int32_t *__restrict__ entry_indptr,
                                                             __nv_bfloat16 *__restrict__ out, float *__restrict__ lse,
                                                             int Hq) {
@@ -40,34 +518,40 @@ __global__ void __launch_bounds__(128) cascade_merge_kernel(const float *__restr
         return;
     }
     float m = -INFINITY;
-    for (int e = e0 + lane; e < e1; e += 32) m = fmaxf(m, part_lse[(size_t)e * Hq + h]);
+    for (int e = e0 + lane; e < e1; e += 32) {
+        const int4 inf = ent_info[e];
+        for (int s = 0; s < inf.z; ++s) m = fmaxf(m, part_lse[(size_t)(inf.x + s * inf.y) * Hq + h]);
+    }
 #pragma unroll
     for (int off = 16; off >= 1; off >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, off));
     float acc[CPL];
 #pragma unroll
     for (int c = 0; c < CPL; ++c) acc[c] = 0.f;
     float wsum = 0.f;
-    for (int eb = e0 + warp; eb < e1; eb += 16) {  // this warp: entries eb, eb + 4, eb + 8, eb + 12
-        float w[4];
-        float4 v[4];
+    for (int e = e0 + warp; e < e1; e += 4) {
+        const int4 inf = ent_info[e];
+        for (int s0 = 0; s0 < inf.z; s0 += 4) {
+            float w[4];
+            float4 v[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int e = eb + 4 * u;
-            const bool ok = e < e1;
-            w[u] = ok ? ptx::ex2(part_lse[(size_t)e * Hq + h] - m) : 0.f;
-            v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (ok) {
-                const float *po = part_o + ((size_t)e * Hq + h) * DV + lane * CPL;
-                if constexpr (CPL == 4) v[u] = *reinterpret_cast<const float4 *>(po);
-                else { const float2 t = *reinterpret_cast<const float2 *>(po); v[u].x = t.x; v[u].y = t.y; }
+            for (int u = 0; u < 4; ++u) {
+                const bool ok = s0 + u < inf.z;
+                const size_t prow = (size_t)(inf.x + (s0 + u) * inf.y) * Hq + h;
+                w[u] = ok ? ptx::ex2(part_lse[ok ? prow : 0] - m) : 0.f;
+                v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (ok) {
+                    const float *po = part_o + prow * DV + lane * CPL;
+                    if constexpr (CPL == 4) v[u] = *reinterpret_cast<const float4 *>(po);
+                    else { const float2 t = *reinterpret_cast<const float2 *>(po); v[u].x = t.x; v[u].y = t.y; }
+                }
             }
-        }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            wsum += w[u];
-            acc[0] += w[u] * v[u].x;
-            acc[1] += w[u] * v[u].y;
-            if constexpr (CPL == 4) { acc[2] += w[u] * v[u].z; acc[3] += w[u] * v[u].w; }
+            for (int u = 0; u < 4; ++u) {
+                wsum += w[u];
+                acc[0] += w[u] * v[u].x;
+                acc[1] += w[u] * v[u].y;
+                if constexpr (CPL == 4) { acc[2] += w[u] * v[u].z; acc[3] += w[u] * v[u].w; }
+            }
         }
     }
 #pragma unroll
@@ -86,64 +570,70 @@ __global__ void __launch_bounds__(128) cascade_merge_kernel(const float *__restr
 }
 
 template <int DQK, int DV>
-cudaError_t launch_cascade_t(const PrefillArgs &a, const Maps &maps, int num_items, int num_sms, cudaStream_t st) {
-    using C = V1Cfg<DQK, DV, 1>;
-    if constexpr (!C::FITS) {
-        return cudaErrorInvalidValue;
-    } else {
-        auto kern = attn_core_kernel<DQK, DV, kModeCascade, 1>;
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
-        if (e != cudaSuccess) return e;
-        const int ctas = num_sms * C::CTAS_PER_SM;
-        const int grid = num_items < ctas ? num_items : ctas;
-        kern<<<grid, C::THREADS, C::SMEM, st>>>(a, maps, num_items);
-        return cudaGetLastError();
-    }
+cudaError_t launch_cascade_t(const CascadeArgs &a, const KvMaps &maps, int num_sms, cudaStream_t st) {
+    using C = CasCfg<DQK, DV>;
+    static_assert(C::NSLOT >= 3, "the ring needs at least K_t, V_{t-1} and one tile in flight");
+    auto kern = cascade_decode_kernel<DQK, DV>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
+    if (e != cudaSuccess) return e;
+    const int grid = a.num_items < num_sms ? a.num_items : num_sms;
+    kern<<<grid, C::THREADS, C::SMEM, st>>>(a, maps);
+    return cudaGetLastError();
 }
 
 }  // namespace
 
-size_t cascade_partial_bytes(int64_t total_entries, int num_q_heads, int dv) {
-    return (size_t)total_entries * (size_t)num_q_heads * (size_t)(dv + 1) * sizeof(float);
+bool cascade_supported(int group, int dqk, int dv) {
+    if (group < 1 || group > 16 || (group & (group - 1))) return false;
+    return (dqk == 64 || dqk == 128 || dqk == 192) && (dv == 64 || dv == 128);
+}
+
+CascadeLayout cascade_layout(size_t num_units, int64_t total_entries, int64_t num_partials, int num_q_heads, int dv) {
+    auto up = [](size_t x) { return (x + 255) / 256 * 256; };
+    CascadeLayout L;
+    L.off_items = kCascadeHeaderBytes;
+    L.off_ent = up(L.off_items + (num_units > 0 ? num_units : 1) * sizeof(CascadeItem));
+    L.off_part_o = up(L.off_ent + (size_t)(total_entries > 0 ? total_entries : 1) * sizeof(int4));
+    L.off_part_lse = up(L.off_part_o + (size_t)num_partials * (size_t)num_q_heads * (size_t)dv * sizeof(float));
+    L.bytes = up(L.off_part_lse + (size_t)num_partials * (size_t)num_q_heads * sizeof(float));
+    return L;
 }
 
 cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &pm,
-                                  const CascadeTile *tiles_dev, int num_tiles, int num_requests, int num_q_heads,
-                                  const void *q, float scale, void *out, float *lse, int64_t total_entries,
-                                  void *partials, int num_sms, cudaStream_t stream, int *launches,
-                                  const LaunchHook *hook) {
-    PrefillArgs a{};
-    a.items = nullptr;
-    a.page_indptr = lv.cas_page_indptr;  // a "request" of the core kernel is a chunk slot
-    a.page_ids = lv.cas_page_ids;
-    a.tile_indptr = lv.cas_tile_indptr;
-    a.tile_ntok = lv.cas_tile_ntok;
-    a.out = (__nv_bfloat16 *)out;
-    a.lse = lse;
-    a.num_q_heads = num_q_heads;
-    a.num_kv_heads = g.num_kv_heads;
-    a.group = num_q_heads / g.num_kv_heads;
-    a.layer_row0 = layer * g.num_pages * g.num_kv_heads * kPage;
-    a.scale_log2 = scale * kLog2e;
-    a.total_q = num_requests;
-    a.nsplit = 1;
-    a.part_o = (float *)partials;
-    a.part_lse = a.part_o + (size_t)total_entries * num_q_heads * g.head_dim_v;
-    a.cas_tiles = tiles_dev;
+                                  void *workspace, const CascadeLayout &lay, int num_units, int num_requests,
+                                  int num_q_heads, const void *q, float scale, void *out, float *lse, int num_sms,
+                                  cudaStream_t stream, int *launches, const LaunchHook *hook) {
+    if (!workspace) return cudaErrorInvalidValue;
+    char *ws = (char *)workspace;
+    CascadeArgs a{};
+    a.items = (const CascadeItem *)(ws + lay.off_items);
+    a.counter = (unsigned int *)ws;
+    a.num_items = num_units * g.num_kv_heads;
+    a.cas_page_indptr = lv.cas_page_indptr;
+    a.cas_page_ids = lv.cas_page_ids;
+    a.cas_tile_indptr = lv.cas_tile_indptr;
+    a.cas_tile_ntok = lv.cas_tile_ntok;
     a.cas_row_req = lv.cas_row_req;
     a.cas_row_entry = lv.cas_row_entry;
     a.q = (const char *)q;
-    if (!partials) return cudaErrorInvalidValue;
-    Maps maps;
-    memcpy(&maps.q, &pm.k, sizeof(CUtensorMap));  // unused in this mode (Q rows are gathered); any valid map
+    a.part_o = (float *)(ws + lay.off_part_o);
+    a.part_lse = (float *)(ws + lay.off_part_lse);
+    a.ent_info = (int4 *)(ws + lay.off_ent);
+    a.num_q_heads = num_q_heads;
+    a.num_kv_heads = g.num_kv_heads;
+    a.group = num_q_heads / g.num_kv_heads;
+    a.group_shift = 0;
+    while ((1 << a.group_shift) < a.group) ++a.group_shift;
+    a.layer_row0 = layer * g.num_pages * g.num_kv_heads * kPage;
+    a.scale_log2 = scale * kLog2e;
+    KvMaps maps;
     memcpy(&maps.k, &pm.k, sizeof(CUtensorMap));
     memcpy(&maps.v, &pm.v, sizeof(CUtensorMap));
-    const int num_items = num_tiles * g.num_kv_heads;
-    cudaError_t e = num_items > 0 ? cudaErrorInvalidValue : cudaSuccess;  // every request empty: only the merge runs
-    if (hook && num_items > 0) hook->begin(hook->ctx, kKernelDecodeCascade, stream);
-#define COMB_CASCADE_CASE(DQ, DVV)                                    \
-    if (num_items > 0 && g.head_dim_qk == DQ && g.head_dim_v == DVV) \
-        e = launch_cascade_t<DQ, DVV>(a, maps, num_items, num_sms, stream);
+    cudaError_t e = a.num_items > 0 ? cudaErrorInvalidValue : cudaSuccess;  // every request empty: only the merge runs
+    if (hook && a.num_items > 0) hook->begin(hook->ctx, kKernelDecodeCascade, stream);
+#define COMB_CASCADE_CASE(DQ, DVV)                                      \
+    if (a.num_items > 0 && g.head_dim_qk == DQ && g.head_dim_v == DVV) \
+        e = launch_cascade_t<DQ, DVV>(a, maps, num_sms, stream);
     COMB_CASCADE_CASE(128, 128)
     COMB_CASCADE_CASE(64, 64)
     COMB_CASCADE_CASE(192, 128)
@@ -151,15 +641,17 @@ cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &
     COMB_CASCADE_CASE(64, 128)
     COMB_CASCADE_CASE(192, 64)
 #undef COMB_CASCADE_CASE
-    if (hook && num_items > 0) hook->end(hook->ctx, stream);
+    if (hook && a.num_items > 0) hook->end(hook->ctx, stream);
     if (e != cudaSuccess) return e;
-    *launches += num_items > 0 ? 1 : 0;
+    *launches += a.num_items > 0 ? 1 : 0;
     const int rows = num_requests * num_q_heads;
     if (hook) hook->begin(hook->ctx, kKernelCascadeMerge, stream);
     if (g.head_dim_v == 128)
-        cascade_merge_kernel<128><<<rows, 128, 0, stream>>>(a.part_o, a.part_lse, lv.entry_indptr, a.out, lse, num_q_heads);
+        cascade_merge_kernel<128><<<rows, 128, 0, stream>>>(a.part_o, a.part_lse, a.ent_info, lv.entry_indptr,
+                                                           (__nv_bfloat16 *)out, lse, num_q_heads);
     else
-        cascade_merge_kernel<64><<<rows, 128, 0, stream>>>(a.part_o, a.part_lse, lv.entry_indptr, a.out, lse, num_q_heads);
+        cascade_merge_kernel<64><<<rows, 128, 0, stream>>>(a.part_o, a.part_lse, a.ent_info, lv.entry_indptr,
+                                                          (__nv_bfloat16 *)out, lse, num_q_heads);
     if (hook) hook->end(hook->ctx, stream);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     *launches += 1;

@@ -425,38 +425,71 @@ int32_t plan_prefill(comb_pool *p, const comb_link_t *link, int32_t R, const int
 }
 
 // ---------------------------------------------------------------- chunk-major decode planning
-// Tiles of the chunk-major decode: slot u's entries in groups of 128/G (each entry = G rows of the M tile).
-// Slots are already ordered by descending entry count (comb_link), so the hot chunks' tiles come first and run
-// at the same time (their shared K/V stream is an L2 hit for all but one of them).
-int32_t plan_cascade(const comb_link_t *link, int G, std::vector<CascadeTile> *tiles) {
+// Units of the chunk-major decode: slot u's entries in groups of 32/G (each entry = G query rows = G columns of the
+// swapped-operand MMA), times the KV ranges of the slot.  A long chunk is cut into ranges when the batch would
+// otherwise give an SM fewer than ~4 items' worth of work (few chunks, few requests): the item size aimed at is
+// a quarter of an SM's share of all KV tiles, never below 2 tiles.  Units are handed out by an atomic counter in the
+// order written here: longest first (stable, so the units that stream the same bytes stay adjacent and the second
+// and later readers hit L2; slots arrive ordered by descending entry count from comb_link).
+constexpr int kCascadeRows = 32;
+constexpr int kCascadeMaxRanges = 64;
+
+// units == nullptr: sizes only (what comb_attn_workspace_bytes needs).
+int32_t plan_cascade(const comb_link_t *link, int G, int Hkv, int num_sms, std::vector<CascadeItem> *units,
+                     size_t *num_units, int64_t *num_partials) {
     const int32_t U = link->num_distinct_chunks;
-    const int32_t *rows = link->host_cas_rows;
-    int64_t sum = 0;
+    const int32_t *rows = link->host_cas_rows, *pages = link->host_cas_pages;
+    if (!rows || !pages || G < 1 || G > kCascadeRows) return COMB_ERR_INVALID;
+    const int per_unit = kCascadeRows / G;
+    int64_t sum = 0, psum = 0, work = 0;
     int32_t mx = 0;
     for (int32_t u = 0; u < U; ++u) {
-        if (rows[u] <= 0) return COMB_ERR_INVALID;
+        if (rows[u] <= 0 || pages[u] <= 0) return COMB_ERR_INVALID;
         sum += rows[u];
+        psum += pages[u];
         mx = std::max(mx, rows[u]);
+        work += (int64_t)((rows[u] + per_unit - 1) / per_unit) * ((pages[u] + kTilePages - 1) / kTilePages);
     }
-    if (sum != link->total_entries || mx != link->max_rows_per_chunk) return COMB_ERR_INVALID;
-    const int per_tile = 128 / G;
-    tiles->clear();
+    if (sum != link->total_entries || mx != link->max_rows_per_chunk || psum != link->distinct_pages)
+        return COMB_ERR_INVALID;
+    work *= Hkv;
+    const int64_t share = (int64_t)std::max(num_sms, 1) * 4;
+    const int64_t aim = std::max<int64_t>(2, (work + share - 1) / share);
+    if (units) units->clear();
+    size_t n_units = 0;
+    int64_t partials = 0;
     int32_t row0 = 0;
     for (int32_t u = 0; u < U; ++u) {
-        for (int32_t t = 0; t < rows[u]; t += per_tile)
-            tiles->push_back(CascadeTile{u, row0 + t, std::min<int32_t>(per_tile, rows[u] - t), 0});
+        const int32_t tiles = (pages[u] + kTilePages - 1) / kTilePages;
+        int32_t nr = (int32_t)std::min<int64_t>((tiles + aim - 1) / aim, kCascadeMaxRanges);
+        const int32_t tps = (tiles + nr - 1) / nr;
+        nr = (tiles + tps - 1) / tps;
+        n_units += (size_t)((rows[u] + per_unit - 1) / per_unit) * (size_t)nr;
+        if (units) {
+            for (int32_t s = 0; s < nr; ++s)
+                for (int32_t t = 0; t < rows[u]; t += per_unit) {
+                    CascadeItem it;
+                    it.slot = u;
+                    it.row0 = row0 + t;
+                    it.nrows = std::min<int32_t>(per_unit, rows[u] - t);
+                    it.kv_tile0 = s * tps;
+                    it.kv_tiles = std::min(tps, tiles - s * tps);
+                    it.part0 = (int32_t)(partials + (int64_t)s * rows[u] + t);
+                    it.part_stride = rows[u];
+                    it.range_nr = (nr << 8) | s;
+                    units->push_back(it);
+                }
+        }
+        partials += (int64_t)rows[u] * nr;
         row0 += rows[u];
+        if (partials > INT32_MAX / 2 || n_units > (size_t)INT32_MAX / 64) return COMB_ERR_CAPACITY;
     }
+    if (units)
+        std::stable_sort(units->begin(), units->end(),
+                         [](const CascadeItem &a, const CascadeItem &b) { return a.kv_tiles > b.kv_tiles; });
+    *num_units = n_units;
+    *num_partials = partials;
     return COMB_OK;
-}
-size_t cascade_tiles_bytes(size_t n) { return align_up(std::max<size_t>(n, 1) * sizeof(CascadeTile), 256); }
-// tiles of a link at group size G without building them: sum_u ceil(rows_u / (128/G))
-size_t cascade_tile_count(const comb_link_t *link, int G) {
-    const int per_tile = 128 / G;
-    size_t n = 0;
-    for (int32_t u = 0; u < link->num_distinct_chunks; ++u)
-        n += (size_t)(std::max(link->host_cas_rows[u], 0) + per_tile - 1) / per_tile;
-    return n;
 }
 
 }  // namespace
@@ -848,7 +881,8 @@ size_t comb_link_bytes(int32_t R, int64_t E, int64_t total_pages) {
 
 size_t comb_link_host_bytes(int32_t R, int64_t E) {
     if (R < 0 || E < 0) return 0;
-    return align_up(sizeof(int32_t) * (size_t)std::max(R, 1), 16) + align_up(sizeof(int32_t) * (size_t)std::max<int64_t>(E, 1), 16);
+    return align_up(sizeof(int32_t) * (size_t)std::max(R, 1), 16) +
+           2 * align_up(sizeof(int32_t) * (size_t)std::max<int64_t>(E, 1), 16);
 }
 
 }  // extern "C"
@@ -1007,11 +1041,16 @@ int32_t link_plan_impl(PoolT *p, int32_t R, const int32_t *chunk_indptr, const u
     link->cas_row_entry = (int32_t *)(db + L.off_cas_row_entry);
     link->host_req_pages = nullptr;
     link->host_cas_rows = nullptr;
+    link->host_cas_pages = nullptr;
     if (link->host_buf) {  // the host mirror: what the planners of the two attention calls read
         link->host_req_pages = (int32_t *)link->host_buf;
         link->host_cas_rows = (int32_t *)((char *)link->host_buf + align_up(sizeof(int32_t) * (size_t)std::max(R, 1), 16));
         for (int32_t r = 0; r < R; ++r) link->host_req_pages[r] = page_indptr[r + 1] - page_indptr[r];
-        for (int32_t u = 0; u < U; ++u) link->host_cas_rows[u] = cas_row_indptr[u + 1] - cas_row_indptr[u];
+        link->host_cas_pages = (int32_t *)((char *)link->host_cas_rows + align_up(sizeof(int32_t) * (size_t)std::max(U, 1), 16));
+        for (int32_t u = 0; u < U; ++u) {
+            link->host_cas_rows[u] = cas_row_indptr[u + 1] - cas_row_indptr[u];
+            link->host_cas_pages[u] = cas_page_indptr[u + 1] - cas_page_indptr[u];
+        }
     }
     link->num_requests = R;
     link->max_pages_per_request = max_pages;
@@ -1118,10 +1157,11 @@ size_t comb_attn_workspace_bytes(const comb_pool_t *p, const comb_link_t *link, 
     if (!p || !link || Hq <= 0 || total_q < 0) return 0;
     size_t need = comb_workspace_bytes(p, link->num_requests, Hq, total_q, link->max_pages_per_request);
     const int G = std::max(1, Hq / p->cfg.num_kv_heads);
-    if (link->host_cas_rows && G <= 128) {
-        const size_t cas = cascade_tiles_bytes(cascade_tile_count(link, G)) +
-                           cascade_partial_bytes(link->total_entries, Hq, p->cfg.head_dim_v);
-        need = std::max(need, align_up(cas, 256) + 256);
+    if (link->host_cas_rows && link->host_cas_pages && cascade_supported(G, p->cfg.head_dim_qk, p->cfg.head_dim_v)) {
+        size_t units = 0;
+        int64_t partials = 0;
+        if (plan_cascade(link, G, p->cfg.num_kv_heads, p->num_sms, nullptr, &units, &partials) == COMB_OK)
+            need = std::max(need, cascade_layout(units, link->total_entries, partials, Hq, p->cfg.head_dim_v).bytes + 256);
     }
     return need;
 }
@@ -1141,8 +1181,8 @@ int32_t comb_cross_attn_decode(comb_pool_t *p, int32_t layer, const comb_link_t 
     p->probe_device();
     cudaStream_t st = (cudaStream_t)stream;
     // ---- which path: chunk-major when the batch shares chunks (or when told to), else per request
-    const bool can_cascade = link->host_cas_rows && link->cas_page_indptr && link->entry_indptr &&
-                             prefill_supported(G, p->cfg.head_dim_qk, p->cfg.head_dim_v);
+    const bool can_cascade = link->host_cas_rows && link->host_cas_pages && link->cas_page_indptr &&
+                             link->entry_indptr && cascade_supported(G, p->cfg.head_dim_qk, p->cfg.head_dim_v);
     bool cascade = false;
     if (p->opt_decode_path == COMB_DECODE_CHUNK_MAJOR) {
         if (!can_cascade) return COMB_ERR_INVALID;
@@ -1151,12 +1191,13 @@ int32_t comb_cross_attn_decode(comb_pool_t *p, int32_t layer, const comb_link_t 
         cascade = link->total_entries * 4 >= (int64_t)link->num_distinct_chunks * 5 && link->total_entries > 0;
     }
     if (cascade) {
-        std::vector<CascadeTile> tiles;
-        int32_t rc = plan_cascade(link, G, &tiles);
+        std::vector<CascadeItem> units;
+        size_t num_units = 0;
+        int64_t partials = 0;
+        int32_t rc = plan_cascade(link, G, p->cfg.num_kv_heads, p->num_sms, &units, &num_units, &partials);
         if (rc != COMB_OK) return rc;
-        const size_t tiles_bytes = cascade_tiles_bytes(tiles.size());
-        const size_t need = tiles_bytes + cascade_partial_bytes(link->total_entries, Hq, p->cfg.head_dim_v);
-        if (!ws || ws_bytes < need || (((uintptr_t)ws) & 15)) {
+        const CascadeLayout lay = cascade_layout(num_units, link->total_entries, partials, Hq, p->cfg.head_dim_v);
+        if (!ws || ws_bytes < lay.bytes || (((uintptr_t)ws) & 15)) {
             if (p->opt_decode_path == COMB_DECODE_CHUNK_MAJOR) return COMB_ERR_CAPACITY;
             cascade = false;  // a workspace sized by the link-independent bound: take the per-request path
         } else {
@@ -1168,19 +1209,18 @@ int32_t comb_cross_attn_decode(comb_pool_t *p, int32_t layer, const comb_link_t 
             maps.k = p->k_map;
             maps.v = p->v_map;
             maps.q = p->k_map;
-            if (!tiles.empty()) {
-                const int slot = p->acquire(tiles.size() * sizeof(CascadeTile));
-                if (slot < 0) return COMB_ERR_CUDA;
-                memcpy(p->ring[slot].host, tiles.data(), tiles.size() * sizeof(CascadeTile));
-                if (cudaMemcpyAsync(ws, p->ring[slot].host, tiles.size() * sizeof(CascadeTile), cudaMemcpyHostToDevice,
-                                    st) != cudaSuccess)
-                    return COMB_ERR_CUDA;
-                if (!p->release(slot, st)) return COMB_ERR_CUDA;
-            }
+            // header (the kernel's item counter, zero) + the units, one copy
+            const size_t head_bytes = kCascadeHeaderBytes + num_units * sizeof(CascadeItem);
+            const int slot = p->acquire(head_bytes);
+            if (slot < 0) return COMB_ERR_CUDA;
+            memset(p->ring[slot].host, 0, kCascadeHeaderBytes);
+            if (num_units) memcpy((char *)p->ring[slot].host + lay.off_items, units.data(), num_units * sizeof(CascadeItem));
+            if (cudaMemcpyAsync(ws, p->ring[slot].host, head_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
+                return COMB_ERR_CUDA;
+            if (!p->release(slot, st)) return COMB_ERR_CUDA;
             int launches = 0;
-            cudaError_t e = launch_decode_cascade(p->geom, layer, view_of(link), maps, (const CascadeTile *)ws,
-                                                  (int)tiles.size(), R, Hq, q, scale, out, lse, link->total_entries,
-                                                  (char *)ws + tiles_bytes, p->num_sms, st, &launches, p->active_hook());
+            cudaError_t e = launch_decode_cascade(p->geom, layer, view_of(link), maps, ws, lay, (int)num_units, R, Hq, q,
+                                                  scale, out, lse, p->num_sms, st, &launches, p->active_hook());
             p->launches += launches;
             return e == cudaSuccess ? COMB_OK : COMB_ERR_CUDA;
         }

@@ -109,19 +109,33 @@ cudaError_t encode_tma_2d_bf16(const void *base, uint64_t inner, uint64_t outer,
                                uint32_t box_inner, uint32_t box_outer, TensorMapBlob *out);
 
 // ---- (f1) chunk-major ("cascade") decode --------------------------------------------------------
-// One M tile of the chunk-major decode: `nrows` consecutive entries (query tokens) of chunk slot `slot`, starting at
-// position row0 of cas_row_req / cas_row_entry; each entry contributes G rows (the heads of one kv-head). A work
-// item of the kernel is (tile, kv-head).
-struct CascadeTile {
-    int32_t slot, row0, nrows, pad;
+// One work unit of the chunk-major decode: up to 32/G consecutive entries (query tokens) of chunk slot `slot`, starting
+// at position row0 of cas_row_req / cas_row_entry (each entry contributes the G rows of one kv-head), against KV tiles
+// [kv_tile0, kv_tile0 + kv_tiles) of the chunk. A work item of the kernel is (unit, kv-head).
+// Every (entry, KV range) pair owns one partial result; entry i of the slot at range s has partial index
+// part_base + s * part_stride + i, and `part0` is that index for the unit's first entry and its own range.
+struct CascadeItem {
+    int32_t slot, row0, nrows;
+    int32_t kv_tile0, kv_tiles;
+    int32_t part0;        // partial index of entry row0 at this unit's range
+    int32_t part_stride;  // entries of the slot (distance between the ranges of one entry)
+    int32_t range_nr;     // (number of ranges of the slot << 8) | this unit's range index
 };
-size_t cascade_partial_bytes(int64_t total_entries, int num_q_heads, int dv);
-// tcgen05 kernel over (tile, kv-head) items writing per-entry partials, then the per-request LSE merge.
+// device workspace of one chunk-major decode call:
+//   [0, 16)  header (uint32 item counter, zero)   [16, ..) CascadeItem[num_units]     -- one H2D copy
+//   then int4 ent_info[E] (written by the kernel: where the merge finds an entry's partials),
+//   then float part_o[P][Hq][Dv], float part_lse[P][Hq]        (P = partial indices in all)
+constexpr size_t kCascadeHeaderBytes = 16;
+struct CascadeLayout {
+    size_t off_items, off_ent, off_part_o, off_part_lse, bytes;
+};
+CascadeLayout cascade_layout(size_t num_units, int64_t total_entries, int64_t num_partials, int num_q_heads, int dv);
+bool cascade_supported(int group, int dqk, int dv);
+// tcgen05 kernel over (unit, kv-head) items writing per-(entry, range) partials, then the per-request LSE merge.
 cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &maps,
-                                  const CascadeTile *tiles_dev, int num_tiles, int num_requests, int num_q_heads,
-                                  const void *q, float scale, void *out, float *lse, int64_t total_entries,
-                                  void *partials, int num_sms, cudaStream_t stream, int *launches,
-                                  const LaunchHook *hook);
+                                  void *workspace, const CascadeLayout &lay, int num_units, int num_requests,
+                                  int num_q_heads, const void *q, float scale, void *out, float *lse, int num_sms,
+                                  cudaStream_t stream, int *launches, const LaunchHook *hook);
 
 // ---- (f2)/(f3) projections: C = A W^T on tcgen05 ---------------------------------------------------
 // A bf16 [M][K] row-major, W bf16 [N][K] row-major (the nn.Linear layout: row n holds the weights of output n),

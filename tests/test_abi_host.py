@@ -60,6 +60,8 @@ def plan(pool, lists, host_mirror=True):
         o1, o2 = link.host_req_pages - mirror.ctypes.data, link.host_cas_rows - mirror.ctypes.data
         tabs["host_req_pages"] = mirror[o1:o1 + 4 * R].view(np.int32).copy()
         tabs["host_cas_rows"] = mirror[o2:o2 + 4 * U].view(np.int32).copy()
+        o3 = link.host_cas_pages - mirror.ctypes.data
+        tabs["host_cas_pages"] = mirror[o3:o3 + 4 * U].view(np.int32).copy()
     link._keepalive = (host, mirror)
     return link, tabs
 
@@ -162,6 +164,7 @@ def test_allocator_and_tables_match_oracle_model(seed):
     # host mirror = what the planners read
     assert np.array_equal(got["host_req_pages"], np.diff(exp["page_indptr"]))
     assert np.array_equal(got["host_cas_rows"], np.diff(cm["cas_row_indptr"]))
+    assert np.array_equal(got["host_cas_pages"], np.diff(got["cas_page_indptr"]))
     assert link.total_kv_tokens == int(exp["kv_len"].sum())
     assert link.max_pages_per_request == int(np.diff(exp["page_indptr"]).max())
     comb.comb_pool_destroy(pool)
