@@ -57,7 +57,8 @@ typedef enum {
                                     must compile + store first, PAPER.md:62 step 2); nothing is written */
     COMB_ERR_CAPACITY = -5,      /* link buffer, scratch or workspace too small */
     COMB_ERR_CUDA = -6,          /* a CUDA call failed; cudaGetLastError() is preserved for the caller */
-    COMB_ERR_BUSY = -7           /* comb_chunk_free of a pinned chunk */
+    COMB_ERR_BUSY = -7,          /* comb_chunk_free of a pinned chunk */
+    COMB_ERR_READ_ONLY = -8      /* alloc / store / free on a pool opened with comb_pool_import */
 } comb_status_t;
 
 typedef struct comb_pool comb_pool_t; /* opaque */
@@ -112,6 +113,32 @@ int32_t comb_chunk_unpin(comb_pool_t *pool, uint64_t chunk_id);
 /* Writes up to `cap` ids evicted by the most recent alloc/store call (in eviction order); returns how many were. */
 int32_t comb_pool_evicted(const comb_pool_t *pool, uint64_t *chunk_ids, int32_t cap);
 int64_t comb_pool_eviction_count(const comb_pool_t *pool); /* chunks evicted since the pool was created */
+
+/* (f4) export to another process — PAPER.md:205 §5.3: the PIC manager is its own component that "reserves a portion
+ * ... of GPU memory" and hands PICaches to the inference engine; PAPER.md:229 (vLLM engine processes).  The manager
+ * process owns the arenas and the directory; an engine process opens them READ-ONLY through CUDA IPC and runs
+ * comb_link + the attention calls on the same bytes (zero copy, as the link itself).
+ *   comb_pool_export  writes a self-contained blob (host memory): geometry, the directory (every chunk's id, length
+ *       and page list, in creation order) and — unless COMB_EXPORT_DIRECTORY_ONLY — the cudaIpcMemHandle_t of the
+ *       allocations that hold the K and V arenas (plus the arenas' offsets inside them: the arenas may be
+ *       sub-allocations of a caching allocator) and the handle of an interprocess event recorded on `stream` after
+ *       every store enqueued so far (`stream` is first made to wait for the pending store events).  The arenas must
+ *       come from cudaMalloc (legacy IPC does not cover cuMemCreate / expandable segments).  *written = bytes used;
+ *       CAPACITY if cap < comb_pool_export_bytes().  A directory-only export needs no GPU.
+ *   comb_pool_import  (another process, same GPU) opens the handles, rebuilds the directory and makes `stream` wait
+ *       for the exporter's event.  The pool it returns is read-only: comb_link, comb_link_plan, comb_chunk_query/
+ *       pin/unpin, both attention calls and comb_cross_layer_forward work; comb_chunk_alloc/free and the stores
+ *       return COMB_ERR_READ_ONLY.  Its free list is empty.  comb_pool_destroy closes the handles.
+ *   comb_pool_refresh replaces an imported pool's directory by the one in a newer blob of the same exporter (full or
+ *       directory-only; geometry must match: INVALID otherwise) and, when the blob carries an event, orders `stream`
+ *       after it.  Chunks the exporter has evicted since disappear; what they were pinned for is the caller's
+ *       protocol (the exporter must not reuse pages an importer may still read: pin on the exporter side).
+ * Errors: INVALID (null, malformed or truncated blob, geometry mismatch), CAPACITY, CUDA. */
+enum { COMB_EXPORT_DIRECTORY_ONLY = 1 };
+size_t comb_pool_export_bytes(const comb_pool_t *pool);
+int32_t comb_pool_export(comb_pool_t *pool, uint32_t flags, void *stream, void *blob, size_t cap, size_t *written);
+int32_t comb_pool_import(const void *blob, size_t bytes, void *stream, comb_pool_t **out);
+int32_t comb_pool_refresh(comb_pool_t *pool, const void *blob, size_t bytes, void *stream);
 
 /* Directory-only half of a store: insert chunk_id with num_tokens and take ceil(T/16) pages from the head
  * of the free list; no data moves (a fused producer may write the pages itself). Idempotent for an

@@ -19,6 +19,7 @@ COMB_ERR_UNKNOWN_CHUNK = -4
 COMB_ERR_CAPACITY = -5
 COMB_ERR_CUDA = -6
 COMB_ERR_BUSY = -7
+COMB_ERR_READ_ONLY = -8
 
 
 class PoolConfig(C.Structure):
@@ -61,6 +62,10 @@ _SIGS = {
     "comb_chunk_unpin": (C.c_int32, [_P, C.c_uint64]),
     "comb_pool_evicted": (C.c_int32, [_P, _P, C.c_int32]),
     "comb_pool_eviction_count": (C.c_int64, [_P]),
+    "comb_pool_export_bytes": (C.c_size_t, [_P]),
+    "comb_pool_export": (C.c_int32, [_P, C.c_uint32, _P, _P, C.c_size_t, C.POINTER(C.c_size_t)]),
+    "comb_pool_import": (C.c_int32, [_P, C.c_size_t, _P, C.POINTER(_P)]),
+    "comb_pool_refresh": (C.c_int32, [_P, _P, C.c_size_t, _P]),
     "comb_chunk_query": (C.c_int32, [_P, C.c_uint64, C.POINTER(C.c_int32), _P, C.c_int32]),
     "comb_store_chunk": (C.c_int32, [_P, C.c_int32, C.c_uint64, C.c_int32, _P, _P, _P]),
     "comb_store_chunks": (C.c_int32, [_P, C.c_int32, C.c_int32, _P, _P, _P, _P, _P]),

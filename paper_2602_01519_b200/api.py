@@ -85,6 +85,42 @@ def comb_pool_eviction_count(pool: int) -> int:
     return int(lib.comb_pool_eviction_count(pool))
 
 
+EXPORT_DIRECTORY_ONLY = 1
+
+
+def comb_pool_export(pool: int, directory_only: bool = False, stream=None) -> np.ndarray:
+    """(f4) self-contained blob (uint8 array, 8-byte aligned) another process hands to comb_pool_import."""
+    cap = int(lib.comb_pool_export_bytes(pool))
+    blob = np.zeros((cap + 7) // 8, dtype=np.uint64).view(np.uint8)
+    n = C.c_size_t()
+    check(lib.comb_pool_export(pool, EXPORT_DIRECTORY_ONLY if directory_only else 0,
+                               None if directory_only else _stream_ptr(stream), blob.ctypes.data, blob.nbytes,
+                               C.byref(n)), "comb_pool_export")
+    return blob[:n.value]
+
+
+def _aligned_blob(blob) -> np.ndarray:
+    raw = np.frombuffer(bytes(blob), dtype=np.uint8) if not isinstance(blob, np.ndarray) else blob
+    out = np.zeros((raw.size + 7) // 8, dtype=np.uint64).view(np.uint8)
+    out[:raw.size] = raw
+    return out
+
+
+def comb_pool_import(blob, stream=None) -> int:
+    """Opens an exported pool read-only in this process (CUDA IPC); returns the pool handle."""
+    b = _aligned_blob(blob)
+    out = C.c_void_p()
+    check(lib.comb_pool_import(b.ctypes.data, len(bytes(blob)) if not isinstance(blob, np.ndarray) else blob.size,
+                               _stream_ptr(stream), C.byref(out)), "comb_pool_import")
+    return out.value
+
+
+def comb_pool_refresh(pool: int, blob, stream=None) -> None:
+    b = _aligned_blob(blob)
+    check(lib.comb_pool_refresh(pool, b.ctypes.data, len(bytes(blob)) if not isinstance(blob, np.ndarray) else blob.size,
+                                _stream_ptr(stream)), "comb_pool_refresh")
+
+
 def comb_chunk_query(pool: int, chunk_id: int) -> Tuple[int, np.ndarray]:
     """(num_tokens, page ids) of a stored chunk."""
     nt = C.c_int32()
@@ -303,6 +339,29 @@ class Pool:
         self.handle = comb_pool_create(self.cfg)
         self._ws: Optional[torch.Tensor] = None
         self._lws: Optional[torch.Tensor] = None
+
+    @classmethod
+    def from_export(cls, blob, device: str = "cuda", stream=None) -> "Pool":
+        """(f4) read-only view, in this process, of a pool another process exported (Pool.export); no arena is
+        allocated here: the exporter's bytes are mapped through CUDA IPC."""
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2602_01519_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+        self = cls.__new__(cls)
+        self.device = torch.device(device)
+        self.handle = comb_pool_import(blob, stream)
+        hdr = np.frombuffer(bytes(blob)[16:40], dtype=np.int32)  # geometry fields of the blob's header
+        self.num_layers, self.num_kv_heads, self.head_dim_qk, self.head_dim_v = (int(x) for x in hdr[:4])
+        self.num_pages = int(hdr[5])
+        self.k_arena = self.v_arena = self.scratch = None
+        self.cfg = None
+        self._ws = self._lws = None
+        return self
+
+    def export(self, directory_only: bool = False, stream=None) -> bytes:
+        return comb_pool_export(self.handle, directory_only, stream).tobytes()
+
+    def refresh(self, blob, stream=None) -> None:
+        comb_pool_refresh(self.handle, blob, stream)
 
     def _aligned_i16(self, nbytes: int, align: int = 1024) -> torch.Tensor:
         raw = torch.empty(nbytes // 2 + align // 2, dtype=torch.int16, device=self.device)

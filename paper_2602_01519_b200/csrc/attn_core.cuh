@@ -141,7 +141,7 @@ __global__ void __launch_bounds__(V1Cfg<DQK, DV, NT>::THREADS, 3 - NT)  // regis
 attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const int num_items) {
     using C = V1Cfg<DQK, DV, NT>;
     extern __shared__ unsigned char smem_raw[];
-    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    unsigned char *smem = ptx::align_smem_1024(smem_raw);
     unsigned char *sQ = smem;                    // [2 tiles][KH][128][64]
     unsigned char *sKV = smem + NT * C::Q_BYTES;  // ring of NSLOT tiles
     uint64_t *bars = reinterpret_cast<uint64_t *>(sKV + C::NSLOT * C::SLOT);

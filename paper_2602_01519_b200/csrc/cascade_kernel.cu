@@ -87,9 +87,10 @@ struct Misc {
     uint64_t q_full[2], q_empty[2], s_full[2], s_empty[2], o_full[2], o_empty[2];
     uint64_t p_full, p_empty;
     uint64_t kv_full[8], kv_empty[8];
-    float wmax[2][4][kRowsMax];
+    float wmax[4][kRowsMax];
     float wsum[4][kRowsMax];
-    int32_t srow[2][kRowsMax];
+    float mref[kRowsMax], inv_l[kRowsMax];
+    alignas(16) int32_t srow[2][kRowsMax];
     ItemEntry items[kItemRing];
     uint32_t tmem_slot;
 };
@@ -109,7 +110,51 @@ __host__ __device__ constexpr uint32_t idesc_bf16(int m, int n, bool a_mn, bool 
            ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
 
+// Named barrier over `threads` threads that also ORs a predicate across them (one instruction: no flag in shared
+// memory, no vote).
+__device__ __forceinline__ bool named_bar_or(int id, int threads, bool pred) {
+    uint32_t r;
+    asm volatile(
+        "{\n\t.reg .pred p, q;\n\tsetp.ne.u32 p, %1, 0;\n\t"
+        "bar.red.or.pred q, %2, %3, p;\n\tselp.u32 %0, 1, 0, q;\n\t}"
+        : "=r"(r)
+        : "r"((uint32_t)pred), "r"(id), "r"(threads)
+        : "memory");
+    return r != 0;
+}
+
+// One stage of a butterfly reduce-scatter over the lanes of a warp: every lane holds 2 CNT values, keeps CNT of them
+// (the upper half if its `OFF` bit is set) and adds the partner's copies of those.
+template <int CNT, int OFF>
+__device__ __forceinline__ void scatter_stage(float *v, int lane) {
+    const bool hi = (lane & OFF) != 0;
+#pragma unroll
+    for (int i = 0; i < CNT; ++i) {
+        const float a = v[i], b = v[i + CNT];
+        v[i] = (hi ? b : a) + __shfl_xor_sync(0xffffffffu, hi ? a : b, OFF);
+    }
+}
+// v[n] = this lane's value for row n.  Returns the sum over the 32 lanes for row (lane & (NC - 1)).
+template <int NC>
+__device__ __forceinline__ float warp_row_sums(float (&v)[NC], int lane) {
+    if constexpr (NC == 32) {
+        scatter_stage<16, 16>(v, lane);
+    } else {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) v[i] += __shfl_xor_sync(0xffffffffu, v[i], 16);
+    }
+    scatter_stage<8, 8>(v, lane);
+    scatter_stage<4, 4>(v, lane);
+    scatter_stage<2, 2>(v, lane);
+    scatter_stage<1, 1>(v, lane);
+    return v[0];
+}
+
 // ---- softmax + epilogue of one item, NC = 16 or 32 query rows (columns of S^T / O^T) ----
+// A thread owns one key of the tile.  mc[n] is the reference maximum of row n in the log2 domain (max * scale_log2),
+// identical in all 128 threads.  The exact row maxima (CREDUX per warp + an exchange through shared memory) are only
+// computed for an item's first tile and when some score exceeds its row's reference by more than 2^8 (one barrier
+// with an OR reduction decides that for all 128 threads); otherwise the reference stays and O^T needs no rescale.
 template <int DQK, int DV, int NC>
 __device__ __forceinline__ void softmax_item(const CascadeArgs &a, Misc *mi, unsigned char *sP, uint32_t tmem,
                                              const ItemEntry &it, const int k, uint32_t &t) {
@@ -117,14 +162,13 @@ __device__ __forceinline__ void softmax_item(const CascadeArgs &a, Misc *mi, uns
     const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
     const int ip = k & 1;
     const int n_kv = (it.npages + kTilePages - 1) / kTilePages;
-    const int rows_valid = it.nrows * a.group;
     const float c = a.scale_log2;
-    float m_used[NC], l_part[NC];
+    float mc[NC], l_part[NC];
 #pragma unroll
-    for (int n = 0; n < NC; ++n) { m_used[n] = -INFINITY; l_part[n] = 0.f; }
+    for (int n = 0; n < NC; ++n) { mc[n] = -INFINITY; l_part[n] = 0.f; }
     // this thread's key inside a tile: page kp, slot ks; where its P goes (row n adds n * 128 and the swizzle)
     const int kp = tid >> 4, ks = tid & 15;
-    const uint32_t p_key = (uint32_t)((tid >> 6) * CasCfg<DQK, DV>::QH + (tid & 7) * 2);
+    unsigned char *p_dst = sP + (tid >> 6) * CasCfg<DQK, DV>::QH + (tid & 7) * 2;
     const uint32_t p_unit = (uint32_t)((tid & 63) >> 3);
     for (int j = 0; j < n_kv; ++j, ++t) {
         const uint64_t ntok8 = a.cas_tile_ntok[it.tile0 + j];
@@ -140,84 +184,91 @@ __device__ __forceinline__ void softmax_item(const CascadeArgs &a, Misc *mi, uns
         ptx::tc_fence_before();
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(&mi->s_empty[sb]);
-        // max over the keys of every row: in the warp by CREDUX, across the four warps through shared memory
-        float wm[NC];
+        if (!key_valid) {  // slots past a chunk's length / pages the tile does not have
 #pragma unroll
-        for (int n = 0; n < NC; ++n) {
-            if (!key_valid) r[n] = 0xff800000u;  // slots past a chunk's length / pages the tile does not have
-            wm[n] = warp_max(__uint_as_float(r[n]));
+            for (int n = 0; n < NC; ++n) r[n] = 0xff800000u;
         }
-        if (lane == 0) {
-#pragma unroll
-            for (int n = 0; n < NC; n += 4)
-                *reinterpret_cast<float4 *>(&mi->wmax[sb][warp][n]) = make_float4(wm[n], wm[n + 1], wm[n + 2], wm[n + 3]);
-        }
-        named_bar_sync(1, 128);
-        bool grow = false;
-#pragma unroll
-        for (int n = 0; n < NC; n += 4) {
-            const float4 w0 = *reinterpret_cast<const float4 *>(&mi->wmax[sb][0][n]);
-            const float4 w1 = *reinterpret_cast<const float4 *>(&mi->wmax[sb][1][n]);
-            const float4 w2 = *reinterpret_cast<const float4 *>(&mi->wmax[sb][2][n]);
-            const float4 w3 = *reinterpret_cast<const float4 *>(&mi->wmax[sb][3][n]);
-            wm[n] = fmaxf(fmaxf(w0.x, w1.x), fmaxf(w2.x, w3.x));
-            wm[n + 1] = fmaxf(fmaxf(w0.y, w1.y), fmaxf(w2.y, w3.y));
-            wm[n + 2] = fmaxf(fmaxf(w0.z, w1.z), fmaxf(w2.z, w3.z));
-            wm[n + 3] = fmaxf(fmaxf(w0.w, w1.w), fmaxf(w2.w, w3.w));
-        }
-#pragma unroll
-        for (int n = 0; n < NC; ++n) grow |= n < rows_valid && (wm[n] - m_used[n]) * c > 8.f;
-        // P V_{t-1} has completed: the P tile may be overwritten and O^T is up to date
-        ptx::mbar_wait(&mi->p_empty, (t & 1) ^ 1);
-        if (j == 0) {
-#pragma unroll
-            for (int n = 0; n < NC; ++n) m_used[n] = wm[n];
-        } else if (grow) {  // identical in all 128 threads (same shared data): move the reference, rescale O^T
-            ptx::tc_fence_after();
-            uint32_t o[NC];
-#pragma unroll
-            for (int q = 0; q < NC / 16; ++q)
-                ptx::tmem_ld16(tmem + lane_base + 64 + ip * kRowsMax + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
-            ptx::tmem_wait_ld();
+        float x[NC];  // exponent of every weight: s * c - mc
+        bool exact = j == 0;
+        if (j > 0) {
+            float over = -INFINITY;
 #pragma unroll
             for (int n = 0; n < NC; ++n) {
-                const float m_new = fmaxf(m_used[n], wm[n]);
-                const float alpha = ptx::ex2((m_used[n] - m_new) * c);
-                o[n] = __float_as_uint(__uint_as_float(o[n]) * alpha);
-                l_part[n] *= alpha;
-                m_used[n] = m_new;
+                x[n] = fmaf(__uint_as_float(r[n]), c, -mc[n]);
+                over = fmaxf(over, x[n]);
+            }
+            exact = named_bar_or(1, 128, over > 8.f);
+        }
+        if (exact) {  // the same decision in all 128 threads
+            float wm[NC];
+#pragma unroll
+            for (int n = 0; n < NC; ++n) wm[n] = warp_max(__uint_as_float(r[n]));
+            if (lane == 0) {
+#pragma unroll
+                for (int n = 0; n < NC; n += 4)
+                    *reinterpret_cast<float4 *>(&mi->wmax[warp][n]) = make_float4(wm[n], wm[n + 1], wm[n + 2], wm[n + 3]);
+            }
+            named_bar_sync(1, 128);
+#pragma unroll
+            for (int n = 0; n < NC; n += 4) {
+                const float4 w0 = *reinterpret_cast<const float4 *>(&mi->wmax[0][n]);
+                const float4 w1 = *reinterpret_cast<const float4 *>(&mi->wmax[1][n]);
+                const float4 w2 = *reinterpret_cast<const float4 *>(&mi->wmax[2][n]);
+                const float4 w3 = *reinterpret_cast<const float4 *>(&mi->wmax[3][n]);
+                wm[n] = fmaxf(fmaxf(w0.x, w1.x), fmaxf(w2.x, w3.x)) * c;
+                wm[n + 1] = fmaxf(fmaxf(w0.y, w1.y), fmaxf(w2.y, w3.y)) * c;
+                wm[n + 2] = fmaxf(fmaxf(w0.z, w1.z), fmaxf(w2.z, w3.z)) * c;
+                wm[n + 3] = fmaxf(fmaxf(w0.w, w1.w), fmaxf(w2.w, w3.w)) * c;
+            }
+            // P V_{t-1} has completed: the P tile may be overwritten and O^T is up to date
+            ptx::mbar_wait(&mi->p_empty, (t & 1) ^ 1);
+            if (j > 0) {  // move the reference of every row that grew, rescale O^T and the partial row sums
+                ptx::tc_fence_after();
+                uint32_t o[NC];
+#pragma unroll
+                for (int q = 0; q < NC / 16; ++q)
+                    ptx::tmem_ld16(tmem + lane_base + 64 + ip * kRowsMax + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
+                ptx::tmem_wait_ld();
+#pragma unroll
+                for (int n = 0; n < NC; ++n) {
+                    const float m_new = fmaxf(mc[n], wm[n]);
+                    const float alpha = ptx::ex2(mc[n] - m_new);
+                    o[n] = __float_as_uint(__uint_as_float(o[n]) * alpha);
+                    l_part[n] *= alpha;
+                    mc[n] = m_new;
+                }
+#pragma unroll
+                for (int q = 0; q < NC / 16; ++q)
+                    ptx::tmem_st16(tmem + lane_base + 64 + ip * kRowsMax + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
+                ptx::tmem_wait_st();
+                ptx::tc_fence_before();
+            } else {
+#pragma unroll
+                for (int n = 0; n < NC; ++n) mc[n] = wm[n];
             }
 #pragma unroll
-            for (int q = 0; q < NC / 16; ++q)
-                ptx::tmem_st16(tmem + lane_base + 64 + ip * kRowsMax + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
-            ptx::tmem_wait_st();
-            ptx::tc_fence_before();
+            for (int n = 0; n < NC; ++n) x[n] = fmaf(__uint_as_float(r[n]), c, -mc[n]);
+        } else {
+            ptx::mbar_wait(&mi->p_empty, (t & 1) ^ 1);
         }
 #pragma unroll
         for (int n = 0; n < NC; ++n) {
-            const float p = ptx::ex2(fmaf(__uint_as_float(r[n]), c, -m_used[n] * c));
+            const float p = ptx::ex2(x[n]);
             l_part[n] += p;
-            const __nv_bfloat16 pb = __float2bfloat16_rn(p);
-            *reinterpret_cast<__nv_bfloat16 *>(sP + p_key + n * 128 + ((p_unit ^ (uint32_t)(n & 7)) << 4)) = pb;
+            *reinterpret_cast<__nv_bfloat16 *>(p_dst + n * 128 + ((p_unit ^ (uint32_t)(n & 7)) << 4)) = __float2bfloat16_rn(p);
         }
         ptx::fence_proxy_async_smem();  // generic-proxy stores -> visible to the tensor core's shared-memory reads
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(&mi->p_full);
     }
     // ---- epilogue: row sums across the 128 keys, then O^T / l -> fp32 partial rows ----
-#pragma unroll
-    for (int n = 0; n < NC; ++n) {
-        float v = l_part[n];
-#pragma unroll
-        for (int off = 16; off >= 1; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
-        l_part[n] = v;
-    }
-    if (lane == 0) {
+    const float lsum = warp_row_sums<NC>(l_part, lane);
+    if (lane < NC) mi->wsum[warp][lane] = lsum;
+    if (tid == 0) {
 #pragma unroll
         for (int n = 0; n < NC; n += 4)
-            *reinterpret_cast<float4 *>(&mi->wsum[warp][n]) = make_float4(l_part[n], l_part[n + 1], l_part[n + 2], l_part[n + 3]);
+            *reinterpret_cast<float4 *>(&mi->mref[n]) = make_float4(mc[n], mc[n + 1], mc[n + 2], mc[n + 3]);
     }
-    named_bar_sync(1, 128);
     ptx::mbar_wait(&mi->o_full[ip], (k >> 1) & 1);
     ptx::tc_fence_after();
     uint32_t o[NC];
@@ -228,13 +279,24 @@ __device__ __forceinline__ void softmax_item(const CascadeArgs &a, Misc *mi, uns
     ptx::tc_fence_before();
     __syncwarp();
     if (lane == 0) ptx::mbar_arrive(&mi->o_empty[ip]);
+    named_bar_sync(1, 128);
+    if (tid < NC) {  // thread n finishes row n: 1 / l for the scaling below, and the row's log2-domain LSE
+        const float l = (mi->wsum[0][tid] + mi->wsum[1][tid]) + (mi->wsum[2][tid] + mi->wsum[3][tid]);
+        mi->inv_l[tid] = 1.f / l;
+        const int prow = mi->srow[ip][tid];
+        if (prow >= 0) a.part_lse[prow] = mi->mref[tid] + log2f(l);
+    }
+    named_bar_sync(1, 128);
+    if (tid < DV) {
 #pragma unroll
-    for (int n = 0; n < NC; ++n) {
-        const int prow = mi->srow[ip][n];
-        if (prow < 0) continue;  // padding row (uniform)
-        const float l = (mi->wsum[0][n] + mi->wsum[1][n]) + (mi->wsum[2][n] + mi->wsum[3][n]);
-        if (tid < DV) a.part_o[(size_t)prow * DV + tid] = __uint_as_float(o[n]) * (1.f / l);
-        if (tid == n) a.part_lse[prow] = m_used[n] * c + log2f(l);
+        for (int n = 0; n < NC; n += 4) {
+            const int4 pr = *reinterpret_cast<const int4 *>(&mi->srow[ip][n]);
+            const float4 iv = *reinterpret_cast<const float4 *>(&mi->inv_l[n]);
+            if (pr.x >= 0) a.part_o[(size_t)pr.x * DV + tid] = __uint_as_float(o[n]) * iv.x;
+            if (pr.y >= 0) a.part_o[(size_t)pr.y * DV + tid] = __uint_as_float(o[n + 1]) * iv.y;
+            if (pr.z >= 0) a.part_o[(size_t)pr.z * DV + tid] = __uint_as_float(o[n + 2]) * iv.z;
+            if (pr.w >= 0) a.part_o[(size_t)pr.w * DV + tid] = __uint_as_float(o[n + 3]) * iv.w;
+        }
     }
 }
 
@@ -243,7 +305,7 @@ __global__ void __launch_bounds__(256, 1)
 cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) {
     using C = CasCfg<DQK, DV>;
     extern __shared__ unsigned char smem_raw[];
-    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    unsigned char *smem = ptx::align_smem_1024(smem_raw);
     unsigned char *sQ = smem;                       // 2 x [KH][32 rows][64]
     unsigned char *sP = sQ + 2 * C::Q_BYTES;        // [2][32 rows][64 keys]
     unsigned char *sKV = sP + C::P_BYTES;           // ring of NSLOT K / V tiles

@@ -71,6 +71,11 @@ struct comb_pool {
     std::vector<uint64_t> last_evicted;
     int64_t evictions = 0;
     std::vector<ReadyEvent> ready_events;
+    // (f4) CUDA IPC: an imported pool is read-only and owns the mappings it opened; an exporting pool owns one
+    // interprocess event
+    bool imported = false;
+    void *ipc_k_base = nullptr, *ipc_v_base = nullptr;
+    cudaEvent_t ipc_event = nullptr;
     void drop_ready(Chunk &c) {
         if (c.ready >= 0 && ready_events[(size_t)c.ready].users > 0) ready_events[(size_t)c.ready].users -= 1;
         c.ready = -1;
@@ -509,6 +514,7 @@ const char *comb_strerror(int32_t s) {
         case COMB_ERR_CAPACITY: return "buffer too small";
         case COMB_ERR_CUDA: return "CUDA error (see cudaGetLastError)";
         case COMB_ERR_BUSY: return "chunk is pinned";
+        case COMB_ERR_READ_ONLY: return "pool was imported read-only";
         default: return "unknown status";
     }
 }
@@ -555,6 +561,9 @@ int32_t comb_pool_destroy(comb_pool_t *p) {
     for (auto &e : p->prof_free) cudaEventDestroy(e);
     for (auto &e : p->ready_events)
         if (e.ev) cudaEventDestroy(e.ev);
+    if (p->ipc_event) cudaEventDestroy(p->ipc_event);
+    if (p->ipc_k_base) cudaIpcCloseMemHandle(p->ipc_k_base);
+    if (p->ipc_v_base && p->ipc_v_base != p->ipc_k_base) cudaIpcCloseMemHandle(p->ipc_v_base);
     for (auto &s : p->ring) {
         if (s.busy) cudaEventSynchronize(s.ev);
         if (s.ev) cudaEventDestroy(s.ev);
@@ -625,6 +634,7 @@ int32_t comb_util_stream_read(const void *src, size_t bytes, void *sink, void *s
 
 int32_t comb_chunk_alloc(comb_pool_t *p, uint64_t id, int32_t T) {
     if (!p) return COMB_ERR_INVALID;
+    if (p->imported) return COMB_ERR_READ_ONLY;
     p->last_evicted.clear();
     if (T > 0 && p->dir.find(id) == p->dir.end()) {
         std::unordered_map<uint64_t, int32_t> keep;
@@ -661,6 +671,7 @@ int64_t comb_pool_eviction_count(const comb_pool_t *p) { return p ? p->evictions
 
 int32_t comb_chunk_free(comb_pool_t *p, uint64_t id) {
     if (!p) return COMB_ERR_INVALID;
+    if (p->imported) return COMB_ERR_READ_ONLY;
     auto it = p->dir.find(id);
     if (it == p->dir.end()) return COMB_ERR_UNKNOWN_CHUNK;
     if (it->second.pins > 0) return COMB_ERR_BUSY;
@@ -708,6 +719,7 @@ struct StoreBatch {
 int32_t store_begin(comb_pool_t *p, int32_t layer, int32_t n, const uint64_t *ids, const int32_t *tok_indptr,
                     StoreBatch *sb) {
     if (!p || n < 0 || (n > 0 && (!ids || !tok_indptr))) return COMB_ERR_INVALID;
+    if (p->imported) return COMB_ERR_READ_ONLY;
     if (layer < 0 || layer >= p->cfg.num_layers) return COMB_ERR_INVALID;
     if (n == 0) return COMB_OK;
     if (tok_indptr[0] != 0) return COMB_ERR_INVALID;
@@ -1320,6 +1332,263 @@ int32_t comb_cross_layer_forward(comb_pool_t *p, int32_t layer, const comb_link_
     if (rc != COMB_OK) return rc;
     // output projection, residual added in the epilogue
     return comb_gemm_bf16(p, obuf, w_o, x, x_out, rows, d_model, Hq * Dv, stream);
+}
+
+}  // extern "C"
+#pragma GCC visibility pop
+
+// ---------------------------------------------------------------- (f4) export / import over CUDA IPC
+namespace {
+
+constexpr uint64_t kExportMagic = 0x31435049424d4f43ull;  // "COMBIPC1"
+constexpr uint32_t kExportHasDevice = 1u;
+
+// Fixed-size head of an export blob (little-endian, natural alignment, no pointers); the directory follows:
+// per chunk {uint64 id; int32 num_tokens; int32 num_pages; int32 pages[num_pages]} padded to 8 bytes, creation order.
+struct ExportHeader {
+    uint64_t magic;
+    uint32_t version, flags;
+    int32_t num_layers, num_kv_heads, head_dim_qk, head_dim_v, page_size, num_pages;
+    uint64_t k_bytes, v_bytes, k_offset, v_offset;
+    unsigned char k_handle[64], v_handle[64], ev_handle[64];
+    uint64_t num_chunks, dir_bytes;
+};
+static_assert(sizeof(cudaIpcMemHandle_t) == 64 && sizeof(cudaIpcEventHandle_t) == 64, "CUDA IPC handles are 64 bytes");
+
+size_t export_dir_bytes(const comb_pool_t *p) {
+    size_t b = 0;
+    for (auto &kv : p->dir) b += 16 + align_up(kv.second.pages.size() * sizeof(int32_t), 8);
+    return b;
+}
+
+// base address of the allocation that contains ptr (cuMemGetAddressRange through the runtime's driver entry point)
+bool allocation_base(const void *ptr, void **base) {
+    typedef int (*Fn)(unsigned long long *, size_t *, unsigned long long);
+    static Fn fn = nullptr;
+    if (!fn) {
+        void *f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuMemGetAddressRange", &f, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            return false;
+        fn = reinterpret_cast<Fn>(f);
+    }
+    unsigned long long b = 0;
+    size_t sz = 0;
+    if (fn(&b, &sz, (unsigned long long)(uintptr_t)ptr) != 0) return false;
+    *base = (void *)(uintptr_t)b;
+    return true;
+}
+
+// Parses and checks a blob; on success *h points into it and *dir at the first directory record.
+int32_t parse_blob(const void *blob, size_t bytes, const ExportHeader **h, const unsigned char **dir) {
+    if (!blob || bytes < sizeof(ExportHeader) || (((uintptr_t)blob) & 7)) return COMB_ERR_INVALID;
+    const ExportHeader *x = (const ExportHeader *)blob;
+    if (x->magic != kExportMagic || x->version != 1) return COMB_ERR_INVALID;
+    if (x->dir_bytes > bytes - sizeof(ExportHeader)) return COMB_ERR_INVALID;
+    comb_pool_config_t c{};
+    c.num_layers = x->num_layers;
+    c.num_kv_heads = x->num_kv_heads;
+    c.head_dim_qk = x->head_dim_qk;
+    c.head_dim_v = x->head_dim_v;
+    c.page_size = x->page_size;
+    c.num_pages = x->num_pages;
+    if (validate_cfg(&c) != COMB_OK) return COMB_ERR_INVALID;
+    *h = x;
+    *dir = (const unsigned char *)blob + sizeof(ExportHeader);
+    return COMB_OK;
+}
+
+// Rebuilds a directory from the records of a blob (validating every page id); `out` replaces the pool's on success.
+int32_t read_directory(const ExportHeader *h, const unsigned char *dir, std::unordered_map<uint64_t, Chunk> *out) {
+    size_t at = 0;
+    std::vector<unsigned char> used((size_t)h->num_pages, 0);
+    for (uint64_t i = 0; i < h->num_chunks; ++i) {
+        if (at + 16 > h->dir_bytes) return COMB_ERR_INVALID;
+        uint64_t id;
+        int32_t T, np;
+        memcpy(&id, dir + at, 8);
+        memcpy(&T, dir + at + 8, 4);
+        memcpy(&np, dir + at + 12, 4);
+        at += 16;
+        if (T <= 0 || np != (T + kPage - 1) / kPage) return COMB_ERR_INVALID;
+        const size_t pb = align_up((size_t)np * sizeof(int32_t), 8);
+        if (at + pb > h->dir_bytes) return COMB_ERR_INVALID;
+        Chunk c;
+        c.num_tokens = T;
+        c.pages.resize((size_t)np);
+        memcpy(c.pages.data(), dir + at, (size_t)np * sizeof(int32_t));
+        at += pb;
+        for (int32_t pg : c.pages) {
+            if (pg < 0 || pg >= h->num_pages || used[(size_t)pg]) return COMB_ERR_INVALID;  // out of range / shared
+            used[(size_t)pg] = 1;
+        }
+        c.seq = i;
+        if (!out->emplace(id, std::move(c)).second) return COMB_ERR_INVALID;  // the same id twice
+    }
+    return COMB_OK;
+}
+
+int32_t wait_remote_event(const ExportHeader *h, cudaStream_t st) {
+    cudaIpcEventHandle_t eh;
+    memcpy(&eh, h->ev_handle, sizeof(eh));
+    cudaEvent_t ev = nullptr;
+    if (cudaIpcOpenEventHandle(&ev, eh) != cudaSuccess) return COMB_ERR_CUDA;
+    const cudaError_t e = cudaStreamWaitEvent(st, ev, 0);
+    cudaEventDestroy(ev);
+    return e == cudaSuccess ? COMB_OK : COMB_ERR_CUDA;
+}
+
+}  // namespace
+
+#pragma GCC visibility push(default)
+extern "C" {
+
+size_t comb_pool_export_bytes(const comb_pool_t *p) {
+    if (!p) return 0;
+    return sizeof(ExportHeader) + export_dir_bytes(p);
+}
+
+int32_t comb_pool_export(comb_pool_t *p, uint32_t flags, void *stream, void *blob, size_t cap, size_t *written) {
+    if (!p || !blob || (flags & ~(uint32_t)COMB_EXPORT_DIRECTORY_ONLY) || (((uintptr_t)blob) & 7)) return COMB_ERR_INVALID;
+    const size_t dir_bytes = export_dir_bytes(p);
+    if (cap < sizeof(ExportHeader) + dir_bytes) return COMB_ERR_CAPACITY;
+    ExportHeader h;
+    memset(&h, 0, sizeof(h));
+    h.magic = kExportMagic;
+    h.version = 1;
+    h.num_layers = p->cfg.num_layers;
+    h.num_kv_heads = p->cfg.num_kv_heads;
+    h.head_dim_qk = p->cfg.head_dim_qk;
+    h.head_dim_v = p->cfg.head_dim_v;
+    h.page_size = p->cfg.page_size;
+    h.num_pages = p->cfg.num_pages;
+    size_t kb = 0, vb = 0;
+    comb_pool_bytes(&p->cfg, &kb, &vb, nullptr);
+    h.k_bytes = kb;
+    h.v_bytes = vb;
+    h.num_chunks = p->dir.size();
+    h.dir_bytes = dir_bytes;
+    if (!(flags & COMB_EXPORT_DIRECTORY_ONLY)) {
+        if (p->imported) return COMB_ERR_READ_ONLY;  // only the owner of the arenas hands them out
+        cudaStream_t st = (cudaStream_t)stream;
+        void *kbase = nullptr, *vbase = nullptr;
+        if (!allocation_base(p->cfg.k_arena, &kbase) || !allocation_base(p->cfg.v_arena, &vbase)) return COMB_ERR_CUDA;
+        cudaIpcMemHandle_t kh, vh;
+        if (cudaIpcGetMemHandle(&kh, kbase) != cudaSuccess || cudaIpcGetMemHandle(&vh, vbase) != cudaSuccess)
+            return COMB_ERR_CUDA;
+        memcpy(h.k_handle, &kh, 64);
+        memcpy(h.v_handle, &vh, 64);
+        h.k_offset = (uint64_t)((char *)p->cfg.k_arena - (char *)kbase);
+        h.v_offset = (uint64_t)((char *)p->cfg.v_arena - (char *)vbase);
+        // every store enqueued so far precedes the event the importer waits for
+        for (auto &re : p->ready_events)
+            if (re.ev && re.users > 0 && cudaStreamWaitEvent(st, re.ev, 0) != cudaSuccess) return COMB_ERR_CUDA;
+        if (!p->ipc_event &&
+            cudaEventCreateWithFlags(&p->ipc_event, cudaEventDisableTiming | cudaEventInterprocess) != cudaSuccess)
+            return COMB_ERR_CUDA;
+        if (cudaEventRecord(p->ipc_event, st) != cudaSuccess) return COMB_ERR_CUDA;
+        cudaIpcEventHandle_t eh;
+        if (cudaIpcGetEventHandle(&eh, p->ipc_event) != cudaSuccess) return COMB_ERR_CUDA;
+        memcpy(h.ev_handle, &eh, 64);
+        h.flags |= kExportHasDevice;
+    }
+    memcpy(blob, &h, sizeof(h));
+    // directory in creation order (deterministic blobs; the importer keeps the order as its own creation order)
+    std::vector<std::pair<uint64_t, uint64_t>> order;  // (seq, id)
+    order.reserve(p->dir.size());
+    for (auto &kv : p->dir) order.emplace_back(kv.second.seq, kv.first);
+    std::sort(order.begin(), order.end());
+    unsigned char *d = (unsigned char *)blob + sizeof(ExportHeader);
+    size_t at = 0;
+    for (auto &o : order) {
+        const Chunk &c = p->dir.find(o.second)->second;
+        const int32_t np = (int32_t)c.pages.size();
+        memcpy(d + at, &o.second, 8);
+        memcpy(d + at + 8, &c.num_tokens, 4);
+        memcpy(d + at + 12, &np, 4);
+        at += 16;
+        const size_t pb = align_up((size_t)np * sizeof(int32_t), 8);
+        memset(d + at, 0, pb);
+        memcpy(d + at, c.pages.data(), (size_t)np * sizeof(int32_t));
+        at += pb;
+    }
+    if (written) *written = sizeof(ExportHeader) + at;
+    return COMB_OK;
+}
+
+int32_t comb_pool_import(const void *blob, size_t bytes, void *stream, comb_pool_t **out) {
+    if (!out) return COMB_ERR_INVALID;
+    *out = nullptr;
+    const ExportHeader *h = nullptr;
+    const unsigned char *dir = nullptr;
+    int32_t rc = parse_blob(blob, bytes, &h, &dir);
+    if (rc != COMB_OK) return rc;
+    if (!(h->flags & kExportHasDevice)) return COMB_ERR_INVALID;  // a directory-only blob cannot open the arenas
+    std::unordered_map<uint64_t, Chunk> d;
+    if ((rc = read_directory(h, dir, &d)) != COMB_OK) return rc;
+    comb_pool_t *p = new (std::nothrow) comb_pool();
+    if (!p) return COMB_ERR_INVALID;
+    cudaIpcMemHandle_t kh, vh;
+    memcpy(&kh, h->k_handle, 64);
+    memcpy(&vh, h->v_handle, 64);
+    const bool same = memcmp(h->k_handle, h->v_handle, 64) == 0;  // both arenas inside one allocation
+    if (cudaIpcOpenMemHandle(&p->ipc_k_base, kh, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
+        delete p;
+        return COMB_ERR_CUDA;
+    }
+    if (same) {
+        p->ipc_v_base = p->ipc_k_base;
+    } else if (cudaIpcOpenMemHandle(&p->ipc_v_base, vh, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
+        cudaIpcCloseMemHandle(p->ipc_k_base);
+        delete p;
+        return COMB_ERR_CUDA;
+    }
+    p->imported = true;
+    p->cfg.num_layers = h->num_layers;
+    p->cfg.num_kv_heads = h->num_kv_heads;
+    p->cfg.head_dim_qk = h->head_dim_qk;
+    p->cfg.head_dim_v = h->head_dim_v;
+    p->cfg.page_size = h->page_size;
+    p->cfg.num_pages = h->num_pages;
+    p->cfg.k_arena = (char *)p->ipc_k_base + h->k_offset;
+    p->cfg.v_arena = (char *)p->ipc_v_base + h->v_offset;
+    p->cfg.scratch = nullptr;
+    p->cfg.free_list_shuffle_seed = 0;
+    p->geom = PoolGeom{h->num_layers, h->num_kv_heads, h->head_dim_qk, h->head_dim_v, h->num_pages, p->cfg.k_arena,
+                       p->cfg.v_arena};
+    p->dir.swap(d);
+    p->next_seq = h->num_chunks;
+    if ((rc = wait_remote_event(h, (cudaStream_t)stream)) != COMB_OK) {
+        comb_pool_destroy(p);
+        return rc;
+    }
+    *out = p;
+    return COMB_OK;
+}
+
+int32_t comb_pool_refresh(comb_pool_t *p, const void *blob, size_t bytes, void *stream) {
+    if (!p || !p->imported) return COMB_ERR_INVALID;
+    const ExportHeader *h = nullptr;
+    const unsigned char *dir = nullptr;
+    int32_t rc = parse_blob(blob, bytes, &h, &dir);
+    if (rc != COMB_OK) return rc;
+    if (h->num_layers != p->cfg.num_layers || h->num_kv_heads != p->cfg.num_kv_heads ||
+        h->head_dim_qk != p->cfg.head_dim_qk || h->head_dim_v != p->cfg.head_dim_v || h->num_pages != p->cfg.num_pages)
+        return COMB_ERR_INVALID;
+    std::unordered_map<uint64_t, Chunk> d;
+    if ((rc = read_directory(h, dir, &d)) != COMB_OK) return rc;
+    for (auto &kv : d) {  // local pins and use stamps survive for the chunks that are still there
+        auto old = p->dir.find(kv.first);
+        if (old != p->dir.end() && old->second.num_tokens == kv.second.num_tokens) {
+            kv.second.pins = old->second.pins;
+            kv.second.last_use = old->second.last_use;
+        }
+    }
+    if ((h->flags & kExportHasDevice) && (rc = wait_remote_event(h, (cudaStream_t)stream)) != COMB_OK) return rc;
+    p->dir.swap(d);
+    p->next_seq = h->num_chunks;
+    return COMB_OK;
 }
 
 }  // extern "C"

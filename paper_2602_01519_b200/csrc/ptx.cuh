@@ -9,6 +9,12 @@ namespace ptx {
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ int lane_id() { return (int)(threadIdx.x & 31); }
+// First 1024-byte-aligned byte of the dynamic shared memory array (SWIZZLE_128B tiles need it).  Plain pointer
+// arithmetic on the __shared__ array: a round trip through uintptr_t would make every later access a generic
+// LD/ST instead of LDS/STS.
+__device__ __forceinline__ unsigned char *align_smem_1024(unsigned char *raw) {
+    return raw + ((1024u - (smem_u32(raw) & 1023u)) & 1023u);
+}
 
 __device__ __forceinline__ bool elect_one() {
     uint32_t pred;

@@ -394,3 +394,61 @@ def test_eviction_is_off_by_default_and_all_or_nothing():
         comb.comb_chunk_query(pool, 1)
     assert e.value.status == comb.COMB_ERR_UNKNOWN_CHUNK
     comb.comb_pool_destroy(pool)
+
+
+def parse_export(blob: bytes):
+    """Independent reader of the export blob format documented in include/comb.h / comb_host.cu."""
+    magic, version, flags = np.frombuffer(blob[:16], dtype=[("m", "<u8"), ("v", "<u4"), ("f", "<u4")])[0]
+    geom = np.frombuffer(blob[16:40], dtype="<i4")
+    n_chunks, dir_bytes = np.frombuffer(blob[264:280], dtype="<u8")
+    at, chunks = 280, []
+    for _ in range(int(n_chunks)):
+        cid = int(np.frombuffer(blob[at:at + 8], "<u8")[0])
+        T, npg = (int(x) for x in np.frombuffer(blob[at + 8:at + 16], "<i4"))
+        pages = np.frombuffer(blob[at + 16:at + 16 + 4 * npg], "<i4").copy()
+        at += 16 + (4 * npg + 7) // 8 * 8
+        chunks.append((cid, T, pages))
+    assert at == 280 + int(dir_bytes) == len(blob)
+    return {"magic": int(magic), "version": int(version), "flags": int(flags), "geom": geom, "chunks": chunks}
+
+
+def test_directory_export_matches_oracle_model_and_rejects_bad_blobs():
+    """(f4) the host half of the CUDA-IPC export: the blob carries the geometry and every chunk's id, length and page
+    list in creation order, equal to the oracle's independent PoolModel after a trace of stores and frees."""
+    pool = make_pool(num_pages=40, Hkv=2, Dqk=64, Dv=128, seed=9, layers=3)
+    model = oracle.PoolModel(40, shuffle_seed=9)
+    rng = np.random.default_rng(3)
+    live = []
+    for step in range(60):
+        if live and rng.random() < 0.35:
+            cid = live.pop(int(rng.integers(len(live))))
+            comb.comb_chunk_free(pool, cid)
+            model.release(cid)
+        else:
+            cid, T = 1000 + step, int(rng.integers(1, 70))
+            if model.free_pages() < (T + 15) // 16:
+                continue
+            comb.comb_chunk_alloc(pool, cid, T)
+            model.store(cid, T)
+            live.append(cid)
+    blob = comb.comb_pool_export(pool, directory_only=True).tobytes()
+    ex = parse_export(blob)
+    assert ex["magic"] == int.from_bytes(b"COMBIPC1", "little") and ex["version"] == 1 and ex["flags"] == 0
+    assert list(ex["geom"]) == [3, 2, 64, 128, 16, 40]
+    assert [c[0] for c in ex["chunks"]] == sorted(live, key=lambda c: c)  # ids grow with creation order in this trace
+    for cid, T, pages in ex["chunks"]:
+        assert (T, list(pages)) == (model.dir[cid][0], list(model.dir[cid][1]))
+    # a directory-only blob cannot open arenas; malformed blobs are INVALID; nothing here needs a GPU
+    aligned = np.zeros((len(blob) + 7) // 8, np.uint64).view(np.uint8)
+    aligned[:len(blob)] = np.frombuffer(blob, np.uint8)
+    out = C.c_void_p()
+    assert _lib.lib.comb_pool_import(aligned.ctypes.data, len(blob), None, C.byref(out)) == comb.COMB_ERR_INVALID
+    assert _lib.lib.comb_pool_import(aligned.ctypes.data, 100, None, C.byref(out)) == comb.COMB_ERR_INVALID
+    bad = aligned.copy()
+    bad[0] ^= 0xff
+    assert _lib.lib.comb_pool_import(bad.ctypes.data, len(blob), None, C.byref(out)) == comb.COMB_ERR_INVALID
+    n = C.c_size_t()
+    assert _lib.lib.comb_pool_export(pool, 1, None, aligned.ctypes.data, 64, C.byref(n)) == comb.COMB_ERR_CAPACITY
+    assert _lib.lib.comb_pool_export(pool, 2, None, aligned.ctypes.data, len(blob), C.byref(n)) == comb.COMB_ERR_INVALID
+    assert _lib.lib.comb_pool_refresh(pool, aligned.ctypes.data, len(blob), None) == comb.COMB_ERR_INVALID  # not imported
+    comb.comb_pool_destroy(pool)

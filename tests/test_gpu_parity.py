@@ -860,3 +860,52 @@ def test_eviction_under_memory_pressure_on_device():
     check_attention(H().device_to_bits(out), lse.cpu().numpy().astype(np.float64), *oracle.attention_for(wl),
                     tag="after eviction")
     pool.close()
+
+
+def test_pool_export_import_across_processes(tmp_path):
+    """(f4) PAPER.md:205: the PIC manager process owns the reserved memory, the engine process attends over it.  This
+    process stores chunks and exports the pool; a child process imports it read-only over CUDA IPC, links and runs
+    decode (both paths) and prefill on the exporter's bytes; a chunk stored later on a side stream becomes visible
+    through comb_pool_refresh, ordered by the interprocess event of the second blob."""
+    import subprocess
+    import sys
+    import paper_2602_01519_b200 as comb
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import ipc_child
+    spec = ipc_child.SPEC
+    w = cs.custom("ipc", links=ipc_child.LINKS_A, lq=[1, 1, 1], **spec)
+    pool = comb.Pool(8, 128, 128, w.pool_pages + 4, shuffle_seed=11, sentinel=SENTINEL)
+    kv = [w.chunk_kv(c) for c in range(4)]
+    dev = [(H().bits_to_device(k, "cuda"), H().bits_to_device(v, "cuda")) for k, v in kv]
+    for c in range(3):
+        pool.store_chunk(c, *dev[c])
+    blob1 = pool.export()
+    side = torch.cuda.Stream()
+    busy = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
+    with torch.cuda.stream(side):
+        for i in range(8):
+            busy.fill_(i)                       # the store of chunk 3 sits behind ~2 ms of queued work
+    pool.store_chunk(3, *dev[3], stream=side)
+    blob2 = pool.export(stream=side)
+    assert comb.comb_pool_export(pool.handle, directory_only=True).size == len(blob2)
+    f1, f2, fo = (str(tmp_path / n) for n in ("b1.bin", "b2.bin", "out.npz"))
+    open(f1, "wb").write(blob1)
+    open(f2, "wb").write(blob2)
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "tests", "ipc_child.py"), f1, f2, fo], capture_output=True,
+                       text=True, timeout=600)
+    assert p.returncode == 0, p.stderr[-2000:]
+    res = np.load(fo)
+    assert res["geom"].tolist() == [1, 8, 128, 128, w.pool_pages + 4]
+    assert res["pages0"].tolist() == comb.comb_chunk_query(pool.handle, 0)[1].tolist()
+    assert res["status"].tolist() == [comb.COMB_ERR_READ_ONLY, comb.COMB_ERR_READ_ONLY, comb.COMB_ERR_UNKNOWN_CHUNK]
+    f64 = lambda a: a.astype(np.float64)  # noqa: E731
+    O, L = oracle.attention_for(w)
+    check_attention(res["dec_pr_o"], f64(res["dec_pr_l"]), O, L, tag="ipc decode per request")
+    check_attention(res["dec_cm_o"], f64(res["dec_cm_l"]), O, L, tag="ipc decode chunk major")
+    wp = cs.custom("ipc", links=ipc_child.LINKS_A, lq=[40, 130, 7], **spec)
+    check_attention(res["pre_o"], f64(res["pre_l"]), *oracle.attention_for(wp), tag="ipc prefill")
+    wd2 = cs.custom("ipc", links=ipc_child.LINKS_B, lq=[1, 1, 1], **spec)
+    check_attention(res["dec2_o"], f64(res["dec2_l"]), *oracle.attention_for(wd2), tag="ipc decode after refresh")
+    wp2 = cs.custom("ipc", links=ipc_child.LINKS_B, lq=[9, 200, 33], **spec)
+    check_attention(res["pre2_o"], f64(res["pre2_l"]), *oracle.attention_for(wp2), tag="ipc prefill after refresh")
+    pool.close()
