@@ -32,6 +32,10 @@ struct Chunk {
     uint64_t last_use = 0;   // tick of the last alloc / store / comb_link that named it
     uint64_t seq = 0;        // creation order (tie-break of the LRU order)
     int32_t ready = -1;      // index of the event its last store recorded, -1 once known complete
+    // scratch of the link planner: which link call saw this chunk last, and its distinct index there (so that
+    // finding the distinct chunks of a batch needs no second hash map)
+    mutable uint64_t link_mark = 0;
+    mutable int32_t link_index = 0;
 };
 
 // Event recorded by a store on its stream; comb_link makes its stream wait for it while it is pending.
@@ -71,6 +75,7 @@ struct comb_pool {
     std::vector<uint64_t> last_evicted;
     int64_t evictions = 0;
     std::vector<ReadyEvent> ready_events;
+    mutable uint64_t link_calls = 0;  // stamps Chunk::link_mark
     // (f4) CUDA IPC: an imported pool is read-only and owns the mappings it opened; an exporting pool owns one
     // interprocess event
     bool imported = false;
@@ -923,8 +928,7 @@ int32_t link_plan_impl(PoolT *p, int32_t R, const int32_t *chunk_indptr, const u
     std::vector<uint64_t> distinct_ids;
     std::vector<int32_t> drows;
     {
-        std::unordered_map<const Chunk *, int32_t> seen;
-        seen.reserve((size_t)E * 2 + 8);
+        const uint64_t mark = ++p->link_calls;
         for (int32_t r = 0; r < R; ++r) {
             int64_t pr = 0;
             for (int32_t e = chunk_indptr[r]; e < chunk_indptr[r + 1]; ++e) {
@@ -934,15 +938,16 @@ int32_t link_plan_impl(PoolT *p, int32_t R, const int32_t *chunk_indptr, const u
                 found[(size_t)e] = c;
                 pr += (int64_t)c->pages.size();
                 total_tok += c->num_tokens;
-                auto ins = seen.emplace(c, (int32_t)distinct.size());
-                if (ins.second) {
+                if (c->link_mark != mark) {  // first appearance in this batch
+                    c->link_mark = mark;
+                    c->link_index = (int32_t)distinct.size();
                     distinct.push_back(c);
                     distinct_ids.push_back(chunk_ids[e]);
                     drows.push_back(0);
                 }
                 (void)tick;
-                ent_slot[(size_t)e] = ins.first->second;
-                drows[(size_t)ins.first->second] += 1;
+                ent_slot[(size_t)e] = c->link_index;
+                drows[(size_t)c->link_index] += 1;
             }
             if (pr > INT32_MAX / kPage) return COMB_ERR_CAPACITY;
             total_pages += pr;
