@@ -25,6 +25,7 @@ from __future__ import annotations
 import argparse
 import json
 import os
+import re
 import sys
 import threading
 import time
@@ -231,6 +232,59 @@ def run_reference(args):
     }), flush=True)
 
 
+KERNEL_CLASSES = (("cascade_decode_kernel", "decode_cascade"), ("cascade_merge_kernel", "cascade_merge"),
+                  ("decode_split_kernel", "decode_split"), ("decode_merge_kernel", "decode_merge"),
+                  ("attn_core_kernel", "prefill"), ("prefill_merge_kernel", "prefill_merge"),
+                  ("store_pages_kernel", "store"), ("gemm_bf16_kernel<1", "gemm_paged"), ("gemm_bf16_kernel<0", "gemm"))
+
+
+def make_traffic_table(directory: str, last: int = 6):
+    """profiles/ncu_traffic.csv from the ncu logs beside it: for every *traffic_<workload>.csv (the --csv log of
+    `ncu --metrics gpu__time_duration.sum,dram__bytes_read.sum,dram__bytes_write.sum,lts__t_sector_hit_rate.pct ...
+    python bench.py --profile-only <extras>`), the mean over the LAST `last` launches of every kernel class (the timed
+    launches; earlier ones are pool fills and warm-ups)."""
+    import csv
+    import glob
+    rows_out = []
+    for path in sorted(glob.glob(os.path.join(directory, "*traffic_*.csv"))):
+        if os.path.basename(path) == "ncu_traffic.csv":
+            continue
+        workload = os.path.basename(path).split("traffic_", 1)[1][:-4]
+        with open(path) as f:
+            lines = [l for l in f if l.startswith('"')]
+        launches = {}  # id -> {kernel, metrics}
+        for rec in csv.DictReader(lines):
+            d = launches.setdefault(int(rec["ID"]), {"kernel": rec["Kernel Name"]})
+            d[rec["Metric Name"]] = (float(rec["Metric Value"].replace(",", "")), rec["Metric Unit"])
+        by_class = {}
+        for i in sorted(launches):
+            k = launches[i]["kernel"]
+            for needle, cls in KERNEL_CLASSES:
+                if needle in k:
+                    by_class.setdefault(cls, []).append(launches[i])
+                    break
+        for cls, ls in by_class.items():
+            if cls == "store" and not workload.endswith("_chunks"):
+                continue  # pool fills of the harness
+            ls = ls[-last:]
+            scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "ns": 1e-3, "us": 1.0, "ms": 1e3, "%": 1.0}
+
+            def mean(metric):
+                return sum(l[metric][0] * scale[l[metric][1]] for l in ls) / len(ls)
+            rd, wr = mean("dram__bytes_read.sum"), mean("dram__bytes_write.sum")
+            m_ = re.search(r"(\w+_kernel(<[^>]*>)?)", ls[-1]["kernel"].replace("(int)", ""))
+            sym = m_.group(1) if m_ else cls
+            rows_out.append((cls, workload, int(rd + wr), int(rd), int(wr), round(mean("gpu__time_duration.sum"), 1),
+                             round(mean("lts__t_sector_hit_rate.pct"), 1), len(ls), sym, os.path.basename(path)))
+    out = os.path.join(directory, "ncu_traffic.csv")
+    with open(out, "w") as f:
+        f.write("kernel,workload,dram_bytes_per_launch,dram_read,dram_write,ncu_duration_us,l2_sector_hit_pct,"
+                "launches_averaged,kernel_symbol,source\n")
+        for r_ in rows_out:
+            f.write("%s,%s,%d,%d,%d,%.1f,%.1f,%d,\"%s\",%s\n" % r_)
+    log("wrote %s (%d rows)" % (out, len(rows_out)))
+
+
 def stats(x):
     x = np.asarray(x, np.float64)
     if x.size == 0:
@@ -251,9 +305,18 @@ def main():
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--extra-launches", type=int, default=200,
                     help="timed launches behind every median/min of the extras (lower it under a profiler)")
+    ap.add_argument("--profile-only", default="",
+                    help="profiler driver: run ONLY these extras (comma-separated, no primary step, no JSON line) so that "
+                         "an ncu capture of the command holds one workload's kernels")
+    ap.add_argument("--traffic-table", default="",
+                    help="no GPU: reduce DIR/*traffic_<workload>.csv (ncu --csv logs of --profile-only runs) to "
+                         "DIR/ncu_traffic.csv, one row per (kernel class, workload)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
+    if args.traffic_table:
+        make_traffic_table(args.traffic_table)
+        return
     if args.impl == "reference":
         run_reference(args)
         return
@@ -472,7 +535,11 @@ def main():
         summary.append(s)
 
     # ------------------------------------------------------------------ primary workload
-    if primary_prefill:
+    profile_only = bool(args.profile_only)
+    if profile_only:
+        args.only, args.no_extras = args.profile_only, False
+        r = roof = None
+    elif primary_prefill:
         w = cs.rag_prefill(seed=args.seed + rank)
         r = bench_attention(w, "prefill", args.steps, args.warmup, fill="linked")
         value = world * r["flops"] / (r["ms_per_step"] * 1e-3) / 1e12
@@ -487,9 +554,11 @@ def main():
         roof = roofline_hbm(r, "decode_link")
         e2e_val = world * r["kv_bytes"] / (r["e2e_ms"] * 1e-3) / 1e9
     dtype = "bf16"
-    log("primary", json.dumps(r))
-    note(args.workload, r, roof, None if primary_prefill else "log=%.0f" % roof["achieved_logical"])
-    clocks = r["clocks"]
+    clocks = None
+    if not profile_only:
+        log("primary", json.dumps(r))
+        note(args.workload, r, roof, None if primary_prefill else "log=%.0f" % roof["achieved_logical"])
+        clocks = r["clocks"]
 
     cpu = None
     prefill_top = None
@@ -553,7 +622,7 @@ def main():
                 if want("decode_link_contiguous_pages"):  # ascending free list: chunks contiguous in the arena
                     decode_extra("decode_link_contiguous_pages", cs.decode_link(seed=args.seed), N, "linked", shuffle=0,
                                  wname="decode_link")
-            elif want("decode_link"):
+            if (primary_prefill or profile_only) and want("decode_link"):
                 decode_extra("decode_link", cs.decode_link(seed=args.seed), N, "linked")
             # cfg 2 geometry with 1024 DISTINCT chunks: every linked byte has to come from HBM (2.15 GB per step)
             if want("decode_no_reuse"):
@@ -613,6 +682,10 @@ def main():
         except Exception as e:  # extras must never lose the primary line
             extras["error"] = repr(e)
             log("extras failed:", repr(e))
+        if profile_only:
+            for line_ in summary:
+                log(line_[:118])
+            return
         # ---- CPU baseline: the oracle on the host cores, bounded sample ----
         try:
             o = oracle_sample(w, "prefill" if primary_prefill else "decode")
@@ -692,7 +765,7 @@ def bench_store(torch, comb, harness, w, pk, n=200):
                          "frac": achieved / pk["hbm"], "algorithmic_bytes": nbytes,
                          "bytes_definition": "read + write of every token's K and V",
                          "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
-                         "kernel": "store", "traffic": ncu_traffic("store", "long_fewshot")},
+                         "kernel": "store", "traffic": ncu_traffic("store", "long_fewshot_chunks")},
             "l2": L2Flush.HOW}
 
 
@@ -747,7 +820,7 @@ def bench_project_store(torch, comb, w, pk, n=50, d_model=4096):
                          "frac": achieved / pk["tf_burst"], "frac_of_sustained": achieved / pk["tf_sustained"],
                          "frac_of_nominal_2250": achieved / NOMINAL_BF16_TFLOPS, "algorithmic_flops": flops,
                          "algorithmic_bytes": nbytes, "kernel": "gemm_paged",
-                         "traffic": ncu_traffic("gemm_paged", "long_fewshot")},
+                         "traffic": ncu_traffic("gemm_paged", "long_fewshot_chunks")},
             "l2": L2Flush.HOW}
 
 

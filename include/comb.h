@@ -72,13 +72,37 @@ typedef struct {
     int32_t head_dim_v;    /* Dv  in {64, 128} */
     int32_t page_size;     /* must be 16 */
     int32_t num_pages;     /* pages per layer */
-    void *k_arena;         /* device, bf16, comb_pool_bytes().k_bytes, 1024-byte aligned */
-    void *v_arena;         /* device, bf16, comb_pool_bytes().v_bytes, 1024-byte aligned */
+    void *k_arena;         /* device, bf16 (or e4m3 bytes), comb_pool_bytes().k_bytes, 1024-byte aligned */
+    void *v_arena;         /* device, bf16 (or e4m3 bytes), comb_pool_bytes().v_bytes, 1024-byte aligned */
     void *scratch;         /* device, comb_pool_bytes().scratch_bytes: store page / tile descriptors (ring of 4) */
     uint64_t free_list_shuffle_seed; /* 0: ascending ids. Else: Fisher-Yates (i = n-1..1, j = next() mod
                                         (i+1), swap) driven by splitmix64(seed) — scatters a chunk's pages
                                         over the arena like a long-running server would */
+    /* (f4) fp8 pages — see "fp8 pools" below. Zero-initialised = a bf16 pool. */
+    int32_t kv_dtype;      /* COMB_KV_BF16 (0) or COMB_KV_E4M3 (1) */
+    int32_t reserved;      /* must be 0 */
+    void *k_scale;         /* device fp32 [num_layers][num_pages][num_kv_heads], comb_pool_scale_bytes(); E4M3 only */
+    void *v_scale;         /* likewise for V */
 } comb_pool_config_t;
+enum { COMB_KV_BF16 = 0, COMB_KV_E4M3 = 1 };
+
+/* fp8 pools (SURVEY.md §8(f4) "fp8 (e4m3) pages with per-page scales to halve decode bytes"; KV memory is
+ * what bounds concurrency).  The paper has no quantised cache; this is DESIGN.md §2 readings I31-I33.
+ *   layout   K arena u8 [L][pages][Hkv][16][Dqk], V arena u8 [L][pages][Hkv][16][Dv]: the bf16 layout with one byte per
+ *            element (OCP E4M3: 1-4-3, bias 7, max 448, no infinity); scales fp32 [L][pages][Hkv], one per (page,
+ *            kv-head) block of K and of V.  head_dim_qk = head_dim_v = 128 only (INVALID otherwise).
+ *   store    the caller still hands bf16 K/V.  Per block: amax = max |x| over its 16 x D values (slots past the chunk's
+ *            length count as zero), scale = 2^e with e the smallest integer such that amax <= 448 * 2^e (clamped to
+ *            [-100, 100]; 1 for an all-zero block), code = e4m3(x / scale) round-to-nearest-even; tail slots are byte 0.
+ *            The page image (codes and scales) is part of the bit-exact contract.
+ *   attend   attention over an fp8 pool is Eq. 7-8 over the dequantised values value(code) * scale (exactly bf16
+ *            numbers, because the scale is a power of two).  comb_cross_attn_decode always takes the chunk-major path
+ *            (the link needs its host mirror): K and V codes feed tcgen05 kind::f8f6f4 directly; the query rows and the
+ *            softmax weights, the small operands, are each split into two e4m3 terms (hi + lo) so that side keeps
+ *            bf16-level accuracy.  comb_cross_attn_prefill dequantises the batch's DISTINCT pages into bf16 staging in
+ *            the workspace and runs the bf16 kernel on it (correct, not fast: prefill runs once per request, decode
+ *            once per generated token).  comb_project_store_chunks and comb_pool_export return INVALID on fp8 pools. */
+size_t comb_pool_scale_bytes(const comb_pool_config_t *cfg); /* bytes of k_scale (= of v_scale); 0 for a bf16 pool */
 
 /* Sizes the caller must allocate for a config (pointers in cfg are ignored). */
 int32_t comb_pool_bytes(const comb_pool_config_t *cfg, size_t *k_bytes, size_t *v_bytes, size_t *scratch_bytes);

@@ -6,7 +6,7 @@ Importing this package loads libcomb.so and raises if it is not built — there 
 from . import _lib  # noqa: F401  (loads libcomb.so or raises)
 from ._lib import (COMB_ERR_BUSY, COMB_ERR_READ_ONLY, COMB_ERR_CAPACITY, COMB_ERR_CUDA, COMB_ERR_EXISTS, COMB_ERR_INVALID, COMB_ERR_NO_SPACE,
                    COMB_ERR_UNKNOWN_CHUNK, COMB_OK, CombError, Link, PoolConfig)
-from .api import (DECODE_AUTO, DECODE_CHUNK_MAJOR, DECODE_PER_REQUEST, KERNEL_CASCADE_MERGE, KERNEL_DECODE_CASCADE,
+from .api import (KV_BF16, KV_E4M3, comb_pool_scale_bytes, DECODE_AUTO, DECODE_CHUNK_MAJOR, DECODE_PER_REQUEST, KERNEL_CASCADE_MERGE, KERNEL_DECODE_CASCADE,
                   KERNEL_DECODE_MERGE, KERNEL_DECODE_SPLIT, KERNEL_GEMM, KERNEL_PREFILL, KERNEL_PREFILL_MERGE, KERNEL_STORE,
                   OPT_DECODE_PATH, OPT_EVICT_LRU, PAGE, LinkedBatch, Pool, comb_attn_workspace_bytes, comb_chunk_alloc,
                   comb_chunk_free, comb_chunk_pin, comb_chunk_query, comb_chunk_unpin, comb_pool_evicted,

@@ -27,7 +27,8 @@ class PoolConfig(C.Structure):
     _fields_ = [("num_layers", C.c_int32), ("num_kv_heads", C.c_int32), ("head_dim_qk", C.c_int32),
                 ("head_dim_v", C.c_int32), ("page_size", C.c_int32), ("num_pages", C.c_int32),
                 ("k_arena", C.c_void_p), ("v_arena", C.c_void_p), ("scratch", C.c_void_p),
-                ("free_list_shuffle_seed", C.c_uint64)]
+                ("free_list_shuffle_seed", C.c_uint64),
+                ("kv_dtype", C.c_int32), ("reserved", C.c_int32), ("k_scale", C.c_void_p), ("v_scale", C.c_void_p)]
 
 
 class Link(C.Structure):
@@ -53,6 +54,7 @@ _P = C.c_void_p
 _SIGS = {
     "comb_pool_bytes": (C.c_int32, [C.POINTER(PoolConfig), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t),
                                     C.POINTER(C.c_size_t)]),
+    "comb_pool_scale_bytes": (C.c_size_t, [C.POINTER(PoolConfig)]),
     "comb_pool_create": (C.c_int32, [C.POINTER(PoolConfig), C.POINTER(_P)]),
     "comb_pool_destroy": (C.c_int32, [_P]),
     "comb_pool_free_pages": (C.c_int32, [_P]),

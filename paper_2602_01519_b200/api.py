@@ -39,12 +39,22 @@ def _stream_ptr(stream) -> Optional[int]:
 # ------------------------------------------------------------------------------------------------
 # the C calls, one to one
 # ------------------------------------------------------------------------------------------------
+KV_BF16, KV_E4M3 = 0, 1
+
+
 def comb_pool_bytes(num_layers: int, num_kv_heads: int, head_dim_qk: int, head_dim_v: int, num_pages: int,
-                    page_size: int = PAGE) -> Tuple[int, int, int]:
-    cfg = PoolConfig(num_layers, num_kv_heads, head_dim_qk, head_dim_v, page_size, num_pages, None, None, None, 0)
+                    page_size: int = PAGE, kv_dtype: int = KV_BF16) -> Tuple[int, int, int]:
+    cfg = PoolConfig(num_layers, num_kv_heads, head_dim_qk, head_dim_v, page_size, num_pages, None, None, None, 0,
+                     kv_dtype)
     k, v, s = C.c_size_t(), C.c_size_t(), C.c_size_t()
     check(lib.comb_pool_bytes(C.byref(cfg), C.byref(k), C.byref(v), C.byref(s)), "comb_pool_bytes")
     return k.value, v.value, s.value
+
+
+def comb_pool_scale_bytes(num_layers: int, num_kv_heads: int, head_dim_qk: int, head_dim_v: int, num_pages: int,
+                          kv_dtype: int = KV_E4M3) -> int:
+    cfg = PoolConfig(num_layers, num_kv_heads, head_dim_qk, head_dim_v, PAGE, num_pages, None, None, None, 0, kv_dtype)
+    return int(lib.comb_pool_scale_bytes(C.byref(cfg)))
 
 
 def comb_pool_create(cfg: PoolConfig) -> int:
@@ -319,23 +329,37 @@ class Pool:
     """Chunk-KV pool (a1): allocates the arenas with torch and forwards every call to libcomb.so."""
 
     def __init__(self, num_kv_heads: int, head_dim_qk: int, head_dim_v: int, num_pages: int, num_layers: int = 1,
-                 shuffle_seed: int = 0, device: str = "cuda", sentinel: Optional[int] = None):
+                 shuffle_seed: int = 0, device: str = "cuda", sentinel: Optional[int] = None, kv_dtype: int = KV_BF16):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2602_01519_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
         self.device = torch.device(device)
         self.num_layers, self.num_kv_heads = num_layers, num_kv_heads
         self.head_dim_qk, self.head_dim_v, self.num_pages = head_dim_qk, head_dim_v, num_pages
-        kb, vb, sb = comb_pool_bytes(num_layers, num_kv_heads, head_dim_qk, head_dim_v, num_pages)
-        # arenas as int16 bit patterns [L][pages][Hkv][16][D]; optional sentinel (e.g. 0x7FC0 = bf16 NaN) for tests
+        self.kv_dtype = kv_dtype
+        kb, vb, sb = comb_pool_bytes(num_layers, num_kv_heads, head_dim_qk, head_dim_v, num_pages, kv_dtype=kv_dtype)
+        # arenas as int16 bit patterns [L][pages][Hkv][16][D]; optional sentinel (e.g. 0x7FC0 = bf16 NaN) for tests.
+        # fp8 pools: the same layout with one byte per element (viewed as uint8 through k_codes / v_codes) plus fp32
+        # scale tables [L][pages][Hkv]; their sentinel fills every byte with its low 8 bits and the scales with -7.
         self.k_arena = self._aligned_i16(kb)
         self.v_arena = self._aligned_i16(vb)
+        self.k_scale = self.v_scale = None
+        if kv_dtype == KV_E4M3:
+            n = num_layers * num_pages * num_kv_heads
+            self.k_scale = torch.full((n,), -7.0, dtype=torch.float32, device=self.device)
+            self.v_scale = torch.full((n,), -7.0, dtype=torch.float32, device=self.device)
         if sentinel is not None:
-            s = int(np.array(sentinel, dtype=np.uint16).view(np.int16))
-            self.k_arena.fill_(s)
-            self.v_arena.fill_(s)
+            if kv_dtype == KV_E4M3:
+                self.k_arena.view(torch.uint8).fill_(sentinel & 0xff)
+                self.v_arena.view(torch.uint8).fill_(sentinel & 0xff)
+            else:
+                s = int(np.array(sentinel, dtype=np.uint16).view(np.int16))
+                self.k_arena.fill_(s)
+                self.v_arena.fill_(s)
         self.scratch = torch.empty(max(sb, 256), dtype=torch.uint8, device=self.device)
         self.cfg = PoolConfig(num_layers, num_kv_heads, head_dim_qk, head_dim_v, PAGE, num_pages,
-                              self.k_arena.data_ptr(), self.v_arena.data_ptr(), self.scratch.data_ptr(), shuffle_seed)
+                              self.k_arena.data_ptr(), self.v_arena.data_ptr(), self.scratch.data_ptr(), shuffle_seed,
+                              kv_dtype, 0, None if self.k_scale is None else self.k_scale.data_ptr(),
+                              None if self.v_scale is None else self.v_scale.data_ptr())
         self.handle = comb_pool_create(self.cfg)
         self._ws: Optional[torch.Tensor] = None
         self._lws: Optional[torch.Tensor] = None

@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libcomb.so")
-SOURCES = ["comb_host.cu", "store_kernel.cu", "decode_kernel.cu", "prefill_kernel.cu", "cascade_kernel.cu", "gemm_kernel.cu"]
+SOURCES = ["comb_host.cu", "store_kernel.cu", "decode_kernel.cu", "prefill_kernel.cu", "cascade_kernel.cu", "gemm_kernel.cu", "fp8_kernel.cu"]
 HEADERS = [os.path.join(CSRC, "kernels.h"), os.path.join(CSRC, "ptx.cuh"), os.path.join(CSRC, "attn_core.cuh"),
            os.path.join(os.path.dirname(HERE), "include", "comb.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

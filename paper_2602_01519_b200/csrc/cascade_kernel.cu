@@ -28,6 +28,7 @@
 
 #include <cuda.h>
 #include <cuda_bf16.h>
+#include <cuda_fp8.h>
 #include <cstring>
 
 namespace comb {
@@ -51,6 +52,8 @@ struct CascadeArgs {
     int num_q_heads, num_kv_heads, group, group_shift;
     int layer_row0;
     float scale_log2;
+    // fp8 pools: this layer's scale tables, fp32 [num_pages][Hkv]
+    const float *k_scale, *v_scale;
 };
 
 struct KvMaps {
@@ -63,6 +66,7 @@ struct ItemEntry {
     int32_t pbeg, npages, tile0, row0;
     int32_t part0, stride, range_nr, pad;
 };
+static_assert(sizeof(ItemEntry) == 48, "ItemEntry is copied as three 16-byte words");
 
 template <int DQK, int DV>
 struct CasCfg {
@@ -90,6 +94,9 @@ struct Misc {
     float wmax[4][kRowsMax];
     float wsum[4][kRowsMax];
     float mref[kRowsMax], inv_l[kRowsMax];
+    // fp8 pools: scales of the 8 pages of the last 8 tiles (written by the loader), the items' Q scale, and the warps'
+    // largest V scale of a tile
+    float kscale[8][8], vscale[8][8], qscale[2], wvs[4];
     alignas(16) int32_t srow[2][kRowsMax];
     ItemEntry items[kItemRing];
     uint32_t tmem_slot;
@@ -477,11 +484,11 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
     } else if (warp == 6) {
         // ===================== scheduler + Q gather =====================
         constexpr int UPR = DQK / 8;  // 16-byte units per Q row
+        unsigned int idx = 0;
+        if (lane == 0) idx = atomicAdd(a.counter, 1u);
         for (int k = 0;; ++k) {
             const int ir = k % kItemRing;
             ptx::mbar_wait(&mi->item_empty[ir], ((k / kItemRing) & 1) ^ 1);
-            unsigned int idx = 0;
-            if (lane == 0) idx = atomicAdd(a.counter, 1u);
             idx = __shfl_sync(0xffffffffu, idx, 0);
             if (idx >= (unsigned int)a.num_items) {
                 if (lane == 0) {
@@ -492,8 +499,8 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
             }
             const int unit = (int)idx / Hkv, kvh = (int)idx - unit * Hkv;
             const CascadeItem ci = a.items[unit];
-            const int pb = a.cas_page_indptr[ci.slot], np = a.cas_page_indptr[ci.slot + 1] - pb;
-            const int skip = min(np, ci.kv_tile0 * kTilePages);
+            // the next item's index is fetched now, so the atomic's round trip runs under this item's Q gather
+            if (lane == 0) idx = atomicAdd(a.counter, 1u);
             const int rows_valid = ci.nrows * G;
             const int ncols = rows_valid <= 16 ? 16 : 32;
             if (lane == 0) {
@@ -502,9 +509,9 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
                 e.kvh = kvh;
                 e.nrows = ci.nrows;
                 e.ncols = ncols;
-                e.pbeg = pb + skip;
-                e.npages = min(np - skip, ci.kv_tiles * kTilePages);
-                e.tile0 = a.cas_tile_indptr[ci.slot] + ci.kv_tile0;
+                e.pbeg = ci.pbeg;
+                e.npages = ci.npages;
+                e.tile0 = ci.tile0;
                 e.row0 = ci.row0;
                 e.part0 = ci.part0;
                 e.stride = ci.part_stride;
@@ -543,6 +550,471 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
                 for (int x = 0; x < 4; ++x)
                     if (dst[x] != 0xffffffffu) *reinterpret_cast<uint4 *>(dstq + dst[x]) = val[x];
             }
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&mi->q_full[qb]);
+        }
+    }
+
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    if (warp == 5) ptx::tmem_dealloc(tmem, C::TMEM_COLS);
+}
+
+// =====================================================================================================================
+// fp8 pools (include/comb.h "fp8 pools"; DESIGN.md §2 I31-I33, §4.4): the same kernel over e4m3 pages, Dqk = Dv = 128.
+//   K and V codes go to the tensor cores as they are (kind::f8f6f4); a (page, kv-head) block's power-of-two scale is
+//   applied by the softmax thread that owns the key: to its score column entries (K) and to its weights (V).
+//   Both operands of kind::f8f6f4 must be 8-bit, so the SMALL operands are split into two e4m3 terms each:
+//     Q rows   q / qs = hi + lo / 16   (qs: one power-of-two scale per item; lo = e4m3(16 (q / qs - hi)))
+//     weights  p vs / vref = hi + lo / 16
+//   which keeps 7-8 significant bits on that side (bf16 has 8).  hi and lo are extra COLUMNS of the same MMAs:
+//   S^T has 2 N columns (hi | lo), O^T likewise; the thread combines hi + lo / 16 after tcgen05.ld.
+//   vref, the reference V scale of the accumulator, is the largest V scale met so far in the item; it moves (with a
+//   rescale of O^T) through the same rare path as the reference maximum.
+// =====================================================================================================================
+struct F8Cfg {
+    static constexpr int SLOT = 128 * 128;                  // [128 keys][128 bytes] of a K or V tile
+    static constexpr int NSLOT = 8;
+    static constexpr int Q_BYTES = 2 * kRowsMax * 128;      // [hi 32 rows | lo 32 rows][128 bytes]
+    static constexpr int P_BYTES = 2 * kRowsMax * 128;      // [hi | lo][128 keys]
+    static constexpr int MISC = 3072;
+    static constexpr int SMEM = 1024 + 2 * Q_BYTES + P_BYTES + NSLOT * SLOT + MISC;
+    static constexpr int THREADS = 256;
+    static constexpr int TMEM_COLS = 256;                   // S^T x2 @0,64; O^T x2 @128,192 (2 N columns each)
+};
+
+__device__ __forceinline__ float pow2_scale_for(float amax) {  // smallest 2^e with amax <= 448 * 2^e, e in [-100, 100]
+    if (!(amax > 0.f)) return 1.f;
+    const uint32_t bits = __float_as_uint(amax);
+    int e = (int)(bits >> 23) - 127 - 8 + ((bits & 0x7fffffu) > 0x600000u ? 1 : 0);
+    if ((bits >> 23) == 0) e = -100;
+    e = e < -100 ? -100 : (e > 100 ? 100 : e);
+    return __uint_as_float((uint32_t)(e + 127) << 23);
+}
+// two values -> (hi codes, lo codes), each two e4m3 bytes (first value in the low byte): v = hi + lo / 16
+__device__ __forceinline__ void split_e4m3x2(float v0, float v1, uint32_t &hi, uint32_t &lo) {
+    hi = (uint32_t)__nv_cvt_float2_to_fp8x2(make_float2(v0, v1), __NV_SATFINITE, __NV_E4M3);
+    const __half2_raw hr = __nv_cvt_fp8x2_to_halfraw2((__nv_fp8x2_storage_t)hi, __NV_E4M3);
+    const float2 b = __half22float2(*reinterpret_cast<const __half2 *>(&hr));
+    lo = (uint32_t)__nv_cvt_float2_to_fp8x2(make_float2((v0 - b.x) * 16.f, (v1 - b.y) * 16.f), __NV_SATFINITE, __NV_E4M3);
+}
+
+template <int NC>
+__device__ __forceinline__ void softmax_item_f8(const CascadeArgs &a, Misc *mi, unsigned char *sP, uint32_t tmem,
+                                                const ItemEntry &it, const int k, uint32_t &t) {
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+    const int ip = k & 1;
+    const int n_kv = (it.npages + kTilePages - 1) / kTilePages;
+    const float c = a.scale_log2;
+    float mc[NC], l_part[NC];
+#pragma unroll
+    for (int n = 0; n < NC; ++n) { mc[n] = -INFINITY; l_part[n] = 0.f; }
+    float vref = 0.f;  // reference V scale of O^T (identical in all 128 threads)
+    // this thread's key inside a tile: page kp, slot ks; byte ks of 16-byte unit kp in every P row
+    const int kp = tid >> 4, ks = tid & 15;
+    unsigned char *p_dst = sP + ks;
+    const float qs = mi->qscale[ip];
+    for (int j = 0; j < n_kv; ++j, ++t) {
+        const uint64_t ntok8 = a.cas_tile_ntok[it.tile0 + j];
+        const bool key_valid = ks < (int)((ntok8 >> (8 * kp)) & 0xffu);
+        const int sb = t & 1;
+        ptx::mbar_wait(&mi->s_full[sb], (t >> 1) & 1);
+        ptx::tc_fence_after();
+        uint32_t r[2 * NC];
+#pragma unroll
+        for (int q = 0; q < 2 * NC / 16; ++q)
+            ptx::tmem_ld16(tmem + lane_base + sb * 64 + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&r[q * 16]));
+        const float ksc = mi->kscale[t & 7][kp], vsc = key_valid ? mi->vscale[t & 7][kp] : 0.f;
+        ptx::tmem_wait_ld();
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&mi->s_empty[sb]);
+        // log2-domain scores of this key: (hi + lo / 16) * (K scale * Q scale * scale_log2)
+        const float f = ksc * qs * c;
+        float y[NC];
+#pragma unroll
+        for (int n = 0; n < NC; ++n)
+            y[n] = key_valid ? fmaf(__uint_as_float(r[NC + n]), 0.0625f, __uint_as_float(r[n])) * f : -INFINITY;
+        bool exact = j == 0;
+        if (j > 0) {
+            float over = -INFINITY;
+#pragma unroll
+            for (int n = 0; n < NC; ++n) over = fmaxf(over, y[n] - mc[n]);
+            exact = named_bar_or(1, 128, over > 8.f || vsc > vref);
+        }
+        if (exact) {  // the same decision in all 128 threads
+            float wm[NC];
+#pragma unroll
+            for (int n = 0; n < NC; ++n) wm[n] = warp_max(y[n]);
+            const float wv = warp_max(vsc);
+            if (lane == 0) {
+#pragma unroll
+                for (int n = 0; n < NC; n += 4)
+                    *reinterpret_cast<float4 *>(&mi->wmax[warp][n]) = make_float4(wm[n], wm[n + 1], wm[n + 2], wm[n + 3]);
+                mi->wvs[warp] = wv;
+            }
+            named_bar_sync(1, 128);
+#pragma unroll
+            for (int n = 0; n < NC; n += 4) {
+                const float4 w0 = *reinterpret_cast<const float4 *>(&mi->wmax[0][n]);
+                const float4 w1 = *reinterpret_cast<const float4 *>(&mi->wmax[1][n]);
+                const float4 w2 = *reinterpret_cast<const float4 *>(&mi->wmax[2][n]);
+                const float4 w3 = *reinterpret_cast<const float4 *>(&mi->wmax[3][n]);
+                wm[n] = fmaxf(fmaxf(w0.x, w1.x), fmaxf(w2.x, w3.x));
+                wm[n + 1] = fmaxf(fmaxf(w0.y, w1.y), fmaxf(w2.y, w3.y));
+                wm[n + 2] = fmaxf(fmaxf(w0.z, w1.z), fmaxf(w2.z, w3.z));
+                wm[n + 3] = fmaxf(fmaxf(w0.w, w1.w), fmaxf(w2.w, w3.w));
+            }
+            const float vnew = fmaxf(vref, fmaxf(fmaxf(mi->wvs[0], mi->wvs[1]), fmaxf(mi->wvs[2], mi->wvs[3])));
+            ptx::mbar_wait(&mi->p_empty, (t & 1) ^ 1);  // P V_{t-1} has completed
+            if (j > 0) {  // move the references, rescale O^T (hi and lo columns) and the partial row sums
+                ptx::tc_fence_after();
+                const float av = vref / vnew;  // exact: powers of two
+                uint32_t o[2 * NC];
+#pragma unroll
+                for (int q = 0; q < 2 * NC / 16; ++q)
+                    ptx::tmem_ld16(tmem + lane_base + 128 + ip * 64 + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
+                ptx::tmem_wait_ld();
+#pragma unroll
+                for (int n = 0; n < NC; ++n) {
+                    const float m_new = fmaxf(mc[n], wm[n]);
+                    const float alpha = ptx::ex2(mc[n] - m_new);
+                    o[n] = __float_as_uint(__uint_as_float(o[n]) * (alpha * av));
+                    o[NC + n] = __float_as_uint(__uint_as_float(o[NC + n]) * (alpha * av));
+                    l_part[n] *= alpha;
+                    mc[n] = m_new;
+                }
+#pragma unroll
+                for (int q = 0; q < 2 * NC / 16; ++q)
+                    ptx::tmem_st16(tmem + lane_base + 128 + ip * 64 + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
+                ptx::tmem_wait_st();
+                ptx::tc_fence_before();
+            } else {
+#pragma unroll
+                for (int n = 0; n < NC; ++n) mc[n] = wm[n];
+            }
+            vref = vnew;
+        } else {
+            ptx::mbar_wait(&mi->p_empty, (t & 1) ^ 1);
+        }
+        const float vw = vsc / vref;  // <= 1, exact (0 for a masked key)
+#pragma unroll
+        for (int n = 0; n < NC; n += 2) {
+            const float p0 = ptx::ex2(y[n] - mc[n]), p1 = ptx::ex2(y[n + 1] - mc[n + 1]);
+            l_part[n] += p0;
+            l_part[n + 1] += p1;
+            uint32_t hi, lo;
+            split_e4m3x2(p0 * vw, p1 * vw, hi, lo);
+            // row R of the P tile: R * 128 + ((unit ^ (R & 7)) << 4) + byte; rows [0, NC) hi, [NC, 2 NC) lo
+            p_dst[n * 128 + ((kp ^ (n & 7)) << 4)] = (unsigned char)(hi & 0xffu);
+            p_dst[(n + 1) * 128 + ((kp ^ ((n + 1) & 7)) << 4)] = (unsigned char)(hi >> 8);
+            p_dst[(NC + n) * 128 + ((kp ^ (n & 7)) << 4)] = (unsigned char)(lo & 0xffu);
+            p_dst[(NC + n + 1) * 128 + ((kp ^ ((n + 1) & 7)) << 4)] = (unsigned char)(lo >> 8);
+        }
+        ptx::fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&mi->p_full);
+    }
+    // ---- epilogue ----
+    const float lsum = warp_row_sums<NC>(l_part, lane);
+    if (lane < NC) mi->wsum[warp][lane] = lsum;
+    if (tid == 0) {
+#pragma unroll
+        for (int n = 0; n < NC; n += 4)
+            *reinterpret_cast<float4 *>(&mi->mref[n]) = make_float4(mc[n], mc[n + 1], mc[n + 2], mc[n + 3]);
+    }
+    ptx::mbar_wait(&mi->o_full[ip], (k >> 1) & 1);
+    ptx::tc_fence_after();
+    uint32_t o[2 * NC];
+#pragma unroll
+    for (int q = 0; q < 2 * NC / 16; ++q)
+        ptx::tmem_ld16(tmem + lane_base + 128 + ip * 64 + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
+    ptx::tmem_wait_ld();
+    ptx::tc_fence_before();
+    __syncwarp();
+    if (lane == 0) ptx::mbar_arrive(&mi->o_empty[ip]);
+    named_bar_sync(1, 128);
+    if (tid < NC) {
+        const float l = (mi->wsum[0][tid] + mi->wsum[1][tid]) + (mi->wsum[2][tid] + mi->wsum[3][tid]);
+        mi->inv_l[tid] = vref / l;  // the accumulator is in units of vref
+        const int prow = mi->srow[ip][tid];
+        if (prow >= 0) a.part_lse[prow] = mi->mref[tid] + log2f(l);
+    }
+    named_bar_sync(1, 128);
+#pragma unroll
+    for (int n = 0; n < NC; n += 4) {
+        const int4 pr = *reinterpret_cast<const int4 *>(&mi->srow[ip][n]);
+        const float4 iv = *reinterpret_cast<const float4 *>(&mi->inv_l[n]);
+        const int prow[4] = {pr.x, pr.y, pr.z, pr.w};
+        const float inv[4] = {iv.x, iv.y, iv.z, iv.w};
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+            if (prow[e] >= 0)
+                a.part_o[(size_t)prow[e] * 128 + tid] =
+                    fmaf(__uint_as_float(o[NC + n + e]), 0.0625f, __uint_as_float(o[n + e])) * inv[e];
+    }
+}
+
+__global__ void __launch_bounds__(256, 1)
+cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) {
+    using C = F8Cfg;
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = ptx::align_smem_1024(smem_raw);
+    unsigned char *sQ = smem;                       // 2 x [64 rows][128 B]
+    unsigned char *sP = sQ + 2 * C::Q_BYTES;        // [64 rows][128 keys]
+    unsigned char *sKV = sP + C::P_BYTES;           // ring of NSLOT K / V tiles
+    Misc *mi = reinterpret_cast<Misc *>(sKV + C::NSLOT * C::SLOT);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // A k-step of the P V contraction spans 32 keys = two pages; when a tile has an odd number of pages the second
+    // half is whatever the slot held before (weight 0).  Start from zeros so that no byte is ever a NaN code.
+    for (int i = tid; i < C::NSLOT * C::SLOT / 16; i += C::THREADS) reinterpret_cast<uint4 *>(sKV)[i] = make_uint4(0, 0, 0, 0);
+    ptx::fence_proxy_async_smem();
+    if (tid == 0) {
+        for (int i = 0; i < kItemRing; ++i) {
+            ptx::mbar_init(&mi->item_full[i], 1);
+            ptx::mbar_init(&mi->item_empty[i], 6);
+        }
+        for (int i = 0; i < 2; ++i) {
+            ptx::mbar_init(&mi->q_full[i], 1);
+            ptx::mbar_init(&mi->q_empty[i], 1);
+            ptx::mbar_init(&mi->s_full[i], 1);
+            ptx::mbar_init(&mi->s_empty[i], 4);
+            ptx::mbar_init(&mi->o_full[i], 1);
+            ptx::mbar_init(&mi->o_empty[i], 4);
+        }
+        ptx::mbar_init(&mi->p_full, 4);
+        ptx::mbar_init(&mi->p_empty, 1);
+        for (int s = 0; s < C::NSLOT; ++s) {
+            ptx::mbar_init(&mi->kv_full[s], 1);
+            ptx::mbar_init(&mi->kv_empty[s], 1);
+        }
+        ptx::fence_barrier_init();
+        ptx::tma_prefetch_desc(&maps.k);
+        ptx::tma_prefetch_desc(&maps.v);
+    }
+    if (warp == 5) {
+        ptx::tmem_alloc(&mi->tmem_slot, C::TMEM_COLS);
+        ptx::tmem_relinquish();
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem = mi->tmem_slot;
+    const int G = a.group, Hq = a.num_q_heads, Hkv = a.num_kv_heads;
+
+    if (warp < 4) {
+        // ===================== softmax + epilogue =====================
+        uint32_t t = 0;
+        for (int k = 0;; ++k) {
+            const int ir = k % kItemRing;
+            ptx::mbar_wait(&mi->item_full[ir], (k / kItemRing) & 1);
+            const ItemEntry it = mi->items[ir];
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&mi->item_empty[ir]);
+            if (!it.valid) break;
+            if (tid < kRowsMax) {
+                const int e_pos = tid >> a.group_shift, head = tid & (G - 1);
+                const bool valid = e_pos < it.nrows;
+                mi->srow[k & 1][tid] = valid ? (it.part0 + e_pos) * Hq + it.kvh * G + head : -1;
+                if (valid && head == 0 && it.kvh == 0 && (it.range_nr & 0xff) == 0)
+                    a.ent_info[a.cas_row_entry[it.row0 + e_pos]] =
+                        make_int4(it.part0 + e_pos, it.stride, it.range_nr >> 8, 0);
+            }
+            ptx::mbar_wait(&mi->q_full[k & 1], (k >> 1) & 1);  // the item's Q scale is written with its Q tile
+            if (it.ncols == 16) softmax_item_f8<16>(a, mi, sP, tmem, it, k, t);
+            else softmax_item_f8<32>(a, mi, sP, tmem, it, k, t);
+        }
+    } else if (warp == 4) {
+        // ===================== K/V TMA loader + page scales =====================
+        uint32_t slot = 0, phase = 0, tt = 0;
+        bool have_prev = false;
+        int prev_row0 = 0, prev_pages = 0;
+        auto issue = [&](bool is_v, int row0, int pages_here) {
+            ptx::mbar_wait(&mi->kv_empty[slot], phase ^ 1);
+            unsigned char *dst = sKV + slot * C::SLOT;
+            if (lane == 0) ptx::mbar_expect_tx(&mi->kv_full[slot], (uint32_t)pages_here * kPage * 128);
+            __syncwarp();
+            if (lane < pages_here) ptx::tma_load_2d(dst + lane * 2048, is_v ? &maps.v : &maps.k, 0, row0, &mi->kv_full[slot]);
+            if (++slot == C::NSLOT) { slot = 0; phase ^= 1; }
+        };
+        for (int k = 0;; ++k) {
+            const int ir = k % kItemRing;
+            ptx::mbar_wait(&mi->item_full[ir], (k / kItemRing) & 1);
+            const ItemEntry it = mi->items[ir];
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&mi->item_empty[ir]);
+            if (!it.valid) break;
+            const int n_kv = (it.npages + kTilePages - 1) / kTilePages;
+            int ids = 0;
+            float ksc = 1.f, vsc = 1.f;
+            for (int j = 0; j < n_kv; ++j, ++tt) {
+                if ((j & 3) == 0) {  // page ids and scales of the next four tiles
+                    const bool have = j * kTilePages + lane < it.npages;
+                    ids = have ? a.cas_page_ids[it.pbeg + j * kTilePages + lane] : 0;
+                    ksc = have ? a.k_scale[(size_t)ids * Hkv + it.kvh] : 1.f;
+                    vsc = have ? a.v_scale[(size_t)ids * Hkv + it.kvh] : 0.f;
+                }
+                const int pages_here = min(kTilePages, it.npages - j * kTilePages);
+                const int pid = __shfl_sync(0xffffffffu, ids, (j & 3) * kTilePages + (lane & 7));
+                const int row0 = a.layer_row0 + (pid * Hkv + it.kvh) * kPage;
+                // (the softmax threads read these after S_tt has completed, i.e. after the K tile's barrier, which this
+                // warp arrives on below; entry tt & 7 was last used by tile tt - 8, long consumed)
+                if ((lane >> 3) == (j & 3)) {
+                    mi->kscale[tt & 7][lane & 7] = ksc;
+                    mi->vscale[tt & 7][lane & 7] = vsc;
+                }
+                __syncwarp();
+                issue(false, row0, pages_here);
+                if (have_prev) issue(true, prev_row0, prev_pages);
+                prev_row0 = row0;
+                prev_pages = pages_here;
+                have_prev = true;
+            }
+        }
+        if (have_prev) issue(true, prev_row0, prev_pages);
+    } else if (warp == 5) {
+        // ===================== MMA issuer =====================
+        const bool leader = ptx::elect_one();
+        const uint64_t dq0 = ptx::umma_desc_sw128(ptx::smem_u32(sQ), 16, 1024);
+        const uint64_t dp0 = ptx::umma_desc_sw128(ptx::smem_u32(sP), 16, 1024);
+        const uint64_t dk0 = ptx::umma_desc_sw128(ptx::smem_u32(sKV), 16, 1024);
+        const uint64_t dv0 = ptx::umma_desc_sw128(ptx::smem_u32(sKV), 0, 1024);  // MN-major: one 128-byte block along d
+        uint32_t slot = 0, phase = 0, t = 0;
+        struct Pend { bool on, first, last; int pages, ip, k; uint32_t t, idesc; } pd{false, false, false, 0, 0, 0, 0, 0};
+        auto do_pv = [&]() {
+            ptx::mbar_wait(&mi->kv_full[slot], phase);
+            ptx::mbar_wait(&mi->p_full, pd.t & 1);
+            if (pd.first) ptx::mbar_wait(&mi->o_empty[pd.ip], ((pd.k >> 1) & 1) ^ 1);
+            ptx::tc_fence_after();
+            const int ksteps = (pd.pages + 1) >> 1;  // 32 keys (two pages) per k-step
+            for (int ks = 0; ks < ksteps; ++ks)
+                if (leader)
+                    ptx::mma_ss_f8(tmem + 128 + pd.ip * 64, dv0 + (uint64_t)((slot * C::SLOT + ks * 4096) >> 4),
+                                   dp0 + (uint64_t)((ks * 32) >> 4), pd.idesc, (pd.first && ks == 0) ? 0u : 1u);
+            if (leader) {
+                ptx::mma_commit(&mi->p_empty);
+                ptx::mma_commit(&mi->kv_empty[slot]);
+                if (pd.last) ptx::mma_commit(&mi->o_full[pd.ip]);
+            }
+            if (++slot == C::NSLOT) { slot = 0; phase ^= 1; }
+            pd.on = false;
+        };
+        for (int k = 0;; ++k) {
+            const int ir = k % kItemRing;
+            ptx::mbar_wait(&mi->item_full[ir], (k / kItemRing) & 1);
+            const ItemEntry it = mi->items[ir];
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&mi->item_empty[ir]);
+            if (!it.valid) break;
+            const int ip = k & 1;
+            const int n_kv = (it.npages + kTilePages - 1) / kTilePages;
+            const uint32_t idesc_s = ptx::umma_idesc_e4m3(128, 2 * it.ncols, false, false);
+            const uint32_t idesc_o = ptx::umma_idesc_e4m3(128, 2 * it.ncols, true, false);
+            ptx::mbar_wait(&mi->q_full[ip], (k >> 1) & 1);
+            for (int j = 0; j < n_kv; ++j, ++t) {
+                const int sb = t & 1;
+                ptx::mbar_wait(&mi->kv_full[slot], phase);
+                ptx::mbar_wait(&mi->s_empty[sb], ((t >> 1) & 1) ^ 1);
+                ptx::tc_fence_after();
+                const uint64_t dk = dk0 + (uint64_t)((slot * C::SLOT) >> 4), dq = dq0 + (uint64_t)((ip * C::Q_BYTES) >> 4);
+#pragma unroll
+                for (int kk = 0; kk < 4; ++kk)  // 32 dims per k-step
+                    if (leader)
+                        ptx::mma_ss_f8(tmem + sb * 64, dk + (uint64_t)((kk * 32) >> 4), dq + (uint64_t)((kk * 32) >> 4),
+                                       idesc_s, kk > 0);
+                if (leader) {
+                    ptx::mma_commit(&mi->s_full[sb]);
+                    ptx::mma_commit(&mi->kv_empty[slot]);
+                    if (j + 1 == n_kv) ptx::mma_commit(&mi->q_empty[ip]);
+                }
+                if (++slot == C::NSLOT) { slot = 0; phase ^= 1; }
+                if (pd.on) do_pv();
+                pd = Pend{true, j == 0, j + 1 == n_kv, min(kTilePages, it.npages - j * kTilePages), ip, k, t, idesc_o};
+            }
+        }
+        if (pd.on) do_pv();
+    } else if (warp == 6) {
+        // ===================== scheduler + Q gather (rows quantised to hi + lo / 16 with one scale per item) =========
+        unsigned int idx = 0;
+        if (lane == 0) idx = atomicAdd(a.counter, 1u);
+        for (int k = 0;; ++k) {
+            const int ir = k % kItemRing;
+            ptx::mbar_wait(&mi->item_empty[ir], ((k / kItemRing) & 1) ^ 1);
+            idx = __shfl_sync(0xffffffffu, idx, 0);
+            if (idx >= (unsigned int)a.num_items) {
+                if (lane == 0) {
+                    mi->items[ir].valid = 0;
+                    ptx::mbar_arrive(&mi->item_full[ir]);
+                }
+                break;
+            }
+            const int unit = (int)idx / Hkv, kvh = (int)idx - unit * Hkv;
+            const CascadeItem ci = a.items[unit];
+            if (lane == 0) idx = atomicAdd(a.counter, 1u);
+            const int rows_valid = ci.nrows * G;
+            const int ncols = rows_valid <= 16 ? 16 : 32;
+            if (lane == 0) {
+                ItemEntry e;
+                e.valid = 1;
+                e.kvh = kvh;
+                e.nrows = ci.nrows;
+                e.ncols = ncols;
+                e.pbeg = ci.pbeg;
+                e.npages = ci.npages;
+                e.tile0 = ci.tile0;
+                e.row0 = ci.row0;
+                e.part0 = ci.part0;
+                e.stride = ci.part_stride;
+                e.range_nr = ci.range_nr;
+                e.pad = 0;
+                mi->items[ir] = e;
+                ptx::mbar_arrive(&mi->item_full[ir]);
+            }
+            // Q rows: 16 units of 8 bf16 per row; lane holds unit (x * 32 + lane) = row 2 x + (lane >> 4), unit lane & 15
+            const int req_lane = lane < ci.nrows ? a.cas_row_req[ci.row0 + lane] : 0;
+            const int qb = k & 1;
+            uint4 val[16];
+            float amax = 0.f;
+#pragma unroll
+            for (int x = 0; x < 16; ++x) {
+                const int row = 2 * x + (lane >> 4), j = lane & 15;
+                const int e_pos = row >> a.group_shift, hh = row & (G - 1);
+                const int qrow = __shfl_sync(0xffffffffu, req_lane, e_pos & 31);
+                val[x] = make_uint4(0u, 0u, 0u, 0u);
+                if (row < rows_valid)
+                    val[x] = __ldg(reinterpret_cast<const uint4 *>(a.q + (((size_t)qrow * Hq + kvh * G + hh) * 128) * 2 +
+                                                                   (size_t)j * 16));
+                const uint32_t w[4] = {val[x].x, val[x].y, val[x].z, val[x].w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e)
+                    amax = fmaxf(amax, fmaxf(fabsf(__uint_as_float(w[e] << 16)), fabsf(__uint_as_float(w[e] & 0xffff0000u))));
+            }
+            amax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(amax)));
+            const float qs = pow2_scale_for(amax), qinv = 1.f / qs;
+            ptx::mbar_wait(&mi->q_empty[qb], ((k >> 1) & 1) ^ 1);
+            unsigned char *dstq = sQ + qb * F8Cfg::Q_BYTES;
+#pragma unroll
+            for (int x = 0; x < 16; ++x) {
+                const int row = 2 * x + (lane >> 4), j = lane & 15;
+                if (row < ncols) {
+                    const uint32_t w[4] = {val[x].x, val[x].y, val[x].z, val[x].w};
+                    uint32_t hi[4], lo[4];
+#pragma unroll
+                    for (int e = 0; e < 4; ++e)
+                        split_e4m3x2(__uint_as_float(w[e] << 16) * qinv, __uint_as_float(w[e] & 0xffff0000u) * qinv, hi[e], lo[e]);
+                    // 8 bytes at byte j * 8 of the row: 16-byte unit j >> 1, half j & 1; SWIZZLE_128B on the unit
+                    const uint32_t off_hi = (uint32_t)(row * 128 + ((((j >> 1) ^ (row & 7))) << 4) + (j & 1) * 8);
+                    const int rl = ncols + row;
+                    const uint32_t off_lo = (uint32_t)(rl * 128 + ((((j >> 1) ^ (rl & 7))) << 4) + (j & 1) * 8);
+                    *reinterpret_cast<uint2 *>(dstq + off_hi) = make_uint2(hi[0] | (hi[1] << 16), hi[2] | (hi[3] << 16));
+                    *reinterpret_cast<uint2 *>(dstq + off_lo) = make_uint2(lo[0] | (lo[1] << 16), lo[2] | (lo[3] << 16));
+                }
+            }
+            if (lane == 0) mi->qscale[qb] = qs;
             ptx::fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(&mi->q_full[qb]);
@@ -693,6 +1165,20 @@ cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &
     memcpy(&maps.v, &pm.v, sizeof(CUtensorMap));
     cudaError_t e = a.num_items > 0 ? cudaErrorInvalidValue : cudaSuccess;  // every request empty: only the merge runs
     if (hook && a.num_items > 0) hook->begin(hook->ctx, kKernelDecodeCascade, stream);
+    if (g.kv_dtype == 1) {  // fp8 pool
+        if (g.head_dim_qk != 128 || g.head_dim_v != 128 || !g.k_scale || !g.v_scale) return cudaErrorInvalidValue;
+        const size_t blocks = (size_t)g.num_pages * g.num_kv_heads;
+        a.k_scale = g.k_scale + (size_t)layer * blocks;
+        a.v_scale = g.v_scale + (size_t)layer * blocks;
+        if (a.num_items > 0) {
+            e = cudaFuncSetAttribute(cascade_decode_f8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, F8Cfg::SMEM);
+            if (e == cudaSuccess) {
+                const int grid = a.num_items < num_sms ? a.num_items : num_sms;
+                cascade_decode_f8_kernel<<<grid, F8Cfg::THREADS, F8Cfg::SMEM, stream>>>(a, maps);
+                e = cudaGetLastError();
+            }
+        }
+    } else {
 #define COMB_CASCADE_CASE(DQ, DVV)                                      \
     if (a.num_items > 0 && g.head_dim_qk == DQ && g.head_dim_v == DVV) \
         e = launch_cascade_t<DQ, DVV>(a, maps, num_sms, stream);
@@ -703,6 +1189,7 @@ cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &
     COMB_CASCADE_CASE(64, 128)
     COMB_CASCADE_CASE(192, 64)
 #undef COMB_CASCADE_CASE
+    }
     if (hook && a.num_items > 0) hook->end(hook->ctx, stream);
     if (e != cudaSuccess) return e;
     *launches += a.num_items > 0 ? 1 : 0;

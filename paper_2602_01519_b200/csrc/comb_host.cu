@@ -177,6 +177,9 @@ int32_t validate_cfg(const comb_pool_config_t *c) {
     if (c->page_size != kPage || c->num_layers < 1 || c->num_kv_heads < 1 || c->num_pages < 1)
         return COMB_ERR_INVALID;
     if (!dims_ok(c->head_dim_qk, c->head_dim_v)) return COMB_ERR_INVALID;
+    if (c->kv_dtype != COMB_KV_BF16 && c->kv_dtype != COMB_KV_E4M3) return COMB_ERR_INVALID;
+    if (c->reserved != 0) return COMB_ERR_INVALID;
+    if (c->kv_dtype == COMB_KV_E4M3 && (c->head_dim_qk != 128 || c->head_dim_v != 128)) return COMB_ERR_INVALID;
     return COMB_OK;
 }
 
@@ -371,8 +374,7 @@ int32_t plan_prefill(comb_pool *p, const comb_link_t *link, int32_t R, const int
     const int tok_per_tile = 128 / G, tok_per_item = out->tiles_per_cta * tok_per_tile;
     // ---- work items: (request, kv-head, one or two Q tiles) against the request's KV, or against a range of it.
     // Requests are ordered by work (query rows x KV tiles when the page counts are known on the host, else query
-    // rows) so the tail of the persistent grid is made of short items; the kv-heads of one Q tile group sit together
-    // so CTAs that stream the same K/V run at the same time (L2 reuse).
+    // rows) so the tail of the persistent grid is made of short items.
     auto tiles_of = [&](int32_t r) { return req_pages ? (req_pages[r] + kTilePages - 1) / kTilePages : 1; };
     struct Req { int32_t r; int64_t rows, cost; };
     std::vector<Req> order;
@@ -382,10 +384,14 @@ int32_t plan_prefill(comb_pool *p, const comb_link_t *link, int32_t R, const int
         order.push_back(Req{r, rows, rows * std::max(1, tiles_of(r))});
     }
     std::stable_sort(order.begin(), order.end(), [](const Req &a, const Req &b) { return a.cost > b.cost; });
+    // kv-head-major: the items in flight at any time (one per CTA, consecutive in this list) then belong to one or two
+    // kv-heads across ALL requests, so requests that link the same chunk read its (page, head) blocks within the same
+    // window and the later readers hit L2 (Zipf / few-shot reuse); the Q tile groups of one (request, kv-head) are
+    // adjacent and share their K/V stream as before.
     std::vector<PrefillItem> base;
-    for (const Req &x : order)
-        for (int64_t t = 0; t < x.rows; t += tok_per_item)
-            for (int g = 0; g < Hkv; ++g)
+    for (int g = 0; g < Hkv; ++g)
+        for (const Req &x : order)
+            for (int64_t t = 0; t < x.rows; t += tok_per_item)
                 base.push_back(PrefillItem{x.r, g, q_indptr[x.r] + (int32_t)t,
                                            (int32_t)std::min<int64_t>(tok_per_item, x.rows - t), 0,
                                            INT32_MAX / kTilePages, -1, 0, 0, 0});
@@ -469,6 +475,7 @@ int32_t plan_cascade(const comb_link_t *link, int G, int Hkv, int num_sms, std::
     size_t n_units = 0;
     int64_t partials = 0;
     int32_t row0 = 0;
+    int64_t page0 = 0, tile0 = 0;  // prefix sums = cas_page_indptr[u], cas_tile_indptr[u]
     for (int32_t u = 0; u < U; ++u) {
         const int32_t tiles = (pages[u] + kTilePages - 1) / kTilePages;
         int32_t nr = (int32_t)std::min<int64_t>((tiles + aim - 1) / aim, kCascadeMaxRanges);
@@ -487,11 +494,18 @@ int32_t plan_cascade(const comb_link_t *link, int G, int Hkv, int num_sms, std::
                     it.part0 = (int32_t)(partials + (int64_t)s * rows[u] + t);
                     it.part_stride = rows[u];
                     it.range_nr = (nr << 8) | s;
+                    const int32_t skip = std::min(pages[u], it.kv_tile0 * kTilePages);
+                    it.pbeg = (int32_t)page0 + skip;
+                    it.npages = std::min(pages[u] - skip, it.kv_tiles * kTilePages);
+                    it.tile0 = (int32_t)tile0 + it.kv_tile0;
+                    it.pad = 0;
                     units->push_back(it);
                 }
         }
         partials += (int64_t)rows[u] * nr;
         row0 += rows[u];
+        page0 += pages[u];
+        tile0 += tiles;
         if (partials > INT32_MAX / 2 || n_units > (size_t)INT32_MAX / 64) return COMB_ERR_CAPACITY;
     }
     if (units)
@@ -528,11 +542,17 @@ int32_t comb_pool_bytes(const comb_pool_config_t *cfg, size_t *k_bytes, size_t *
     int32_t rc = validate_cfg(cfg);
     if (rc != COMB_OK) return rc;
     const size_t blocks = (size_t)cfg->num_layers * cfg->num_pages * cfg->num_kv_heads * kPage;
-    if (k_bytes) *k_bytes = blocks * cfg->head_dim_qk * 2;
-    if (v_bytes) *v_bytes = blocks * cfg->head_dim_v * 2;
+    const size_t elt = cfg->kv_dtype == COMB_KV_E4M3 ? 1 : 2;
+    if (k_bytes) *k_bytes = blocks * cfg->head_dim_qk * elt;
+    if (v_bytes) *v_bytes = blocks * cfg->head_dim_v * elt;
     if (scratch_bytes)
         *scratch_bytes = kRingSlots * align_up((size_t)cfg->num_pages * kScratchBytesPerPage, 256);
     return COMB_OK;
+}
+
+size_t comb_pool_scale_bytes(const comb_pool_config_t *cfg) {
+    if (validate_cfg(cfg) != COMB_OK || cfg->kv_dtype != COMB_KV_E4M3) return 0;
+    return (size_t)cfg->num_layers * cfg->num_pages * cfg->num_kv_heads * sizeof(float);
 }
 
 int32_t comb_pool_create(const comb_pool_config_t *cfg, comb_pool_t **out) {
@@ -542,11 +562,17 @@ int32_t comb_pool_create(const comb_pool_config_t *cfg, comb_pool_t **out) {
     if (rc != COMB_OK) return rc;
     if (!cfg->k_arena || !cfg->v_arena || !cfg->scratch) return COMB_ERR_INVALID;
     if (((uintptr_t)cfg->k_arena | (uintptr_t)cfg->v_arena) & 1023) return COMB_ERR_INVALID;
+    if (cfg->kv_dtype == COMB_KV_E4M3 &&
+        (!cfg->k_scale || !cfg->v_scale || (((uintptr_t)cfg->k_scale | (uintptr_t)cfg->v_scale) & 3)))
+        return COMB_ERR_INVALID;
     comb_pool_t *p = new (std::nothrow) comb_pool();
     if (!p) return COMB_ERR_INVALID;
     p->cfg = *cfg;
     p->geom = PoolGeom{cfg->num_layers, cfg->num_kv_heads, cfg->head_dim_qk, cfg->head_dim_v, cfg->num_pages,
                        cfg->k_arena, cfg->v_arena};
+    p->geom.kv_dtype = cfg->kv_dtype;
+    p->geom.k_scale = (float *)cfg->k_scale;
+    p->geom.v_scale = (float *)cfg->v_scale;
     p->free_list.resize(cfg->num_pages);
     for (int32_t i = 0; i < cfg->num_pages; ++i) p->free_list[i] = i;
     if (cfg->free_list_shuffle_seed) {
@@ -803,7 +829,9 @@ int32_t comb_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, const uint64
         return COMB_ERR_CUDA;
     }
     if (p->prof_on) p->hook.begin(p, kKernelStore, st);
-    const cudaError_t se = launch_store(p->geom, layer, dev, (int)at, k_packed, v_packed, st);
+    const cudaError_t se = p->geom.kv_dtype == COMB_KV_E4M3
+                               ? launch_store_fp8(p->geom, layer, dev, (int)at, k_packed, v_packed, st)
+                               : launch_store(p->geom, layer, dev, (int)at, k_packed, v_packed, st);
     if (p->prof_on) p->hook.end(p, st);
     if (se != cudaSuccess) {
         store_undo(p, sb);
@@ -820,6 +848,7 @@ int32_t comb_project_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, cons
                                   void *stream) {
     if (n > 0 && (!h_packed || !w_kv)) return COMB_ERR_INVALID;
     if (!p || d_model <= 0 || d_model % 8) return COMB_ERR_INVALID;
+    if (p->geom.kv_dtype != COMB_KV_BF16) return COMB_ERR_INVALID;  // the paged epilogue writes bf16 pages only
     const int32_t N = p->cfg.num_kv_heads * (p->cfg.head_dim_qk + p->cfg.head_dim_v);
     StoreBatch sb;
     int32_t rc = store_begin(p, layer, n, ids, tok_indptr, &sb);
@@ -1201,7 +1230,8 @@ int32_t comb_cross_attn_decode(comb_pool_t *p, int32_t layer, const comb_link_t 
     const bool can_cascade = link->host_cas_rows && link->host_cas_pages && link->cas_page_indptr &&
                              link->entry_indptr && cascade_supported(G, p->cfg.head_dim_qk, p->cfg.head_dim_v);
     bool cascade = false;
-    if (p->opt_decode_path == COMB_DECODE_CHUNK_MAJOR) {
+    const bool fp8 = p->geom.kv_dtype == COMB_KV_E4M3;  // fp8 pools: the chunk-major kernel is the only decode kernel
+    if (p->opt_decode_path == COMB_DECODE_CHUNK_MAJOR || fp8) {
         if (!can_cascade) return COMB_ERR_INVALID;
         cascade = true;
     } else if (p->opt_decode_path == COMB_DECODE_AUTO && can_cascade) {
@@ -1215,7 +1245,7 @@ int32_t comb_cross_attn_decode(comb_pool_t *p, int32_t layer, const comb_link_t 
         if (rc != COMB_OK) return rc;
         const CascadeLayout lay = cascade_layout(num_units, link->total_entries, partials, Hq, p->cfg.head_dim_v);
         if (!ws || ws_bytes < lay.bytes || (((uintptr_t)ws) & 15)) {
-            if (p->opt_decode_path == COMB_DECODE_CHUNK_MAJOR) return COMB_ERR_CAPACITY;
+            if (p->opt_decode_path == COMB_DECODE_CHUNK_MAJOR || fp8) return COMB_ERR_CAPACITY;
             cascade = false;  // a workspace sized by the link-independent bound: take the per-request path
         } else {
             if (!p->kv_maps_ready) {
@@ -1270,6 +1300,7 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     if (!q || !out || !link->page_indptr) return COMB_ERR_INVALID;
     const int Hkv = p->cfg.num_kv_heads, G = Hq / Hkv;
     if (!prefill_supported(G, p->cfg.head_dim_qk, p->cfg.head_dim_v)) return COMB_ERR_INVALID;
+    if (p->geom.kv_dtype != COMB_KV_BF16) return COMB_ERR_INVALID;
     p->probe_device();
     PrefillPlan plan;
     int32_t rc = plan_prefill(p, link, R, q_indptr, Hq, &plan);
@@ -1456,6 +1487,7 @@ size_t comb_pool_export_bytes(const comb_pool_t *p) {
 
 int32_t comb_pool_export(comb_pool_t *p, uint32_t flags, void *stream, void *blob, size_t cap, size_t *written) {
     if (!p || !blob || (flags & ~(uint32_t)COMB_EXPORT_DIRECTORY_ONLY) || (((uintptr_t)blob) & 7)) return COMB_ERR_INVALID;
+    if (p->geom.kv_dtype != COMB_KV_BF16) return COMB_ERR_INVALID;  // the blob has no place for the scale tables
     const size_t dir_bytes = export_dir_bytes(p);
     if (cap < sizeof(ExportHeader) + dir_bytes) return COMB_ERR_CAPACITY;
     ExportHeader h;

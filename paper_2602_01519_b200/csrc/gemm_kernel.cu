@@ -18,10 +18,18 @@
 namespace comb {
 namespace {
 
-constexpr int BM = 128, BN = 256, BK = 64, STAGES = 4;
-constexpr int A_BYTES = BM * BK * 2, B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int BM = 128, BK = 64;
+constexpr int A_BYTES = BM * BK * 2;
 constexpr int GEMM_THREADS = 192;
-constexpr int GEMM_SMEM = 1024 + STAGES * STAGE_BYTES + 256;
+// N tile: 256 columns (4 stages of 48 KB), or 64 columns with an 8-stage ring of 24 KB for problems whose 256-column
+// tiles would leave most SMs idle (a decode-phase projection: M <= 128 rows, so the weights are the traffic and every
+// SM should stream its share of them)
+template <int BN>
+struct GemmCfg {
+    static constexpr int STAGES = BN == 256 ? 4 : 8;
+    static constexpr int B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
+    static constexpr int SMEM = 1024 + STAGES * STAGE_BYTES + 256;
+};
 
 enum { kEpiRowMajor = 0, kEpiPaged = 1 };
 
@@ -42,9 +50,10 @@ struct GemmMaps {
     CUtensorMap a, w;
 };
 
-template <int EPI>
+template <int EPI, int BN>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_bf16_kernel(const GemmArgs g, const __grid_constant__ GemmMaps maps) {
+    constexpr int STAGES = GemmCfg<BN>::STAGES, STAGE_BYTES = GemmCfg<BN>::STAGE_BYTES;
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = ptx::align_smem_1024(smem_raw);
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + STAGES * STAGE_BYTES);
@@ -212,23 +221,34 @@ gemm_bf16_kernel(const GemmArgs g, const __grid_constant__ GemmMaps maps) {
     if (warp == 1) ptx::tmem_dealloc(tmem, 512);
 }
 
-template <int EPI>
-cudaError_t launch_t(const GemmArgs &g, const GemmMaps &maps, int num_sms, cudaStream_t st) {
-    auto kern = gemm_bf16_kernel<EPI>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM);
+template <int EPI, int BN>
+cudaError_t launch_bn(const GemmArgs &g, const GemmMaps &maps, int num_sms, cudaStream_t st) {
+    auto kern = gemm_bf16_kernel<EPI, BN>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmCfg<BN>::SMEM);
     if (e != cudaSuccess) return e;
     const int tiles = g.num_m_tiles * g.num_n_tiles;
     if (tiles <= 0) return cudaSuccess;
     const int grid = tiles < num_sms ? tiles : num_sms;
-    kern<<<grid, GEMM_THREADS, GEMM_SMEM, st>>>(g, maps);
+    kern<<<grid, GEMM_THREADS, GemmCfg<BN>::SMEM, st>>>(g, maps);
     return cudaGetLastError();
 }
 
-cudaError_t encode_maps(const GemmProblem &p, GemmMaps *maps) {
+// 64-column tiles when 256-column tiles would occupy fewer than half of the SMs
+int pick_bn(int num_m_tiles, int N, int num_sms) {
+    return (int64_t)num_m_tiles * ((N + 255) / 256) * 2 <= num_sms ? 64 : 256;
+}
+
+template <int EPI>
+cudaError_t launch_t(GemmArgs &g, const GemmMaps &maps, int bn, int num_sms, cudaStream_t st) {
+    g.num_n_tiles = (g.N + bn - 1) / bn;
+    return bn == 64 ? launch_bn<EPI, 64>(g, maps, num_sms, st) : launch_bn<EPI, 256>(g, maps, num_sms, st);
+}
+
+cudaError_t encode_maps(const GemmProblem &p, int bn, GemmMaps *maps) {
     TensorMapBlob a, w;
     cudaError_t e = encode_tma_2d_bf16(p.a, (uint64_t)p.K, (uint64_t)p.M, (uint64_t)p.K * 2, BK, BM, &a);
     if (e != cudaSuccess) return e;
-    e = encode_tma_2d_bf16(p.w, (uint64_t)p.K, (uint64_t)p.N, (uint64_t)p.K * 2, BK, BN, &w);
+    e = encode_tma_2d_bf16(p.w, (uint64_t)p.K, (uint64_t)p.N, (uint64_t)p.K * 2, BK, (uint32_t)bn, &w);
     if (e != cudaSuccess) return e;
     static_assert(sizeof(CUtensorMap) == sizeof(TensorMapBlob), "CUtensorMap is 128 bytes");
     memcpy(&maps->a, &a, sizeof(CUtensorMap));
@@ -243,33 +263,34 @@ bool gemm_shape_ok(int64_t M, int32_t N, int32_t K) { return M > 0 && M < (int64
 
 cudaError_t launch_gemm_rowmajor(const GemmProblem &p, void *c, const void *residual, int num_sms, cudaStream_t stream) {
     if (!gemm_shape_ok(p.M, p.N, p.K) || !p.a || !p.w || !c) return cudaErrorInvalidValue;
+    const int num_m_tiles = (int)((p.M + BM - 1) / BM);
+    const int bn = pick_bn(num_m_tiles, p.N, num_sms);
     GemmMaps maps;
-    cudaError_t e = encode_maps(p, &maps);
+    cudaError_t e = encode_maps(p, bn, &maps);
     if (e != cudaSuccess) return e;
     GemmArgs g{};
     g.M = p.M;
     g.N = p.N;
     g.K = p.K;
-    g.num_m_tiles = (int)((p.M + BM - 1) / BM);
-    g.num_n_tiles = (p.N + BN - 1) / BN;
+    g.num_m_tiles = num_m_tiles;
     g.c = (__nv_bfloat16 *)c;
     g.residual = (const __nv_bfloat16 *)residual;
-    return launch_t<kEpiRowMajor>(g, maps, num_sms, stream);
+    return launch_t<kEpiRowMajor>(g, maps, bn, num_sms, stream);
 }
 
 cudaError_t launch_gemm_paged(const GemmProblem &p, const PoolGeom &pg, int layer, const GemmRowTile *tiles_dev,
                               int num_tiles, int num_sms, cudaStream_t stream) {
     if (!gemm_shape_ok(p.M, p.N, p.K) || !p.a || !p.w || !tiles_dev) return cudaErrorInvalidValue;
     if (p.N != pg.num_kv_heads * (pg.head_dim_qk + pg.head_dim_v)) return cudaErrorInvalidValue;
+    const int bn = pick_bn(num_tiles, p.N, num_sms);
     GemmMaps maps;
-    cudaError_t e = encode_maps(p, &maps);
+    cudaError_t e = encode_maps(p, bn, &maps);
     if (e != cudaSuccess) return e;
     GemmArgs g{};
     g.M = p.M;
     g.N = p.N;
     g.K = p.K;
     g.num_m_tiles = num_tiles;
-    g.num_n_tiles = (p.N + BN - 1) / BN;
     g.row_tiles = tiles_dev;
     const size_t kb = (size_t)kPage * pg.head_dim_qk * 2, vb = (size_t)kPage * pg.head_dim_v * 2;
     g.k_layer = (char *)pg.k_arena + (size_t)layer * pg.num_pages * pg.num_kv_heads * kb;
@@ -277,7 +298,7 @@ cudaError_t launch_gemm_paged(const GemmProblem &p, const PoolGeom &pg, int laye
     g.hkv = pg.num_kv_heads;
     g.dqk = pg.head_dim_qk;
     g.dv = pg.head_dim_v;
-    return launch_t<kEpiPaged>(g, maps, num_sms, stream);
+    return launch_t<kEpiPaged>(g, maps, bn, num_sms, stream);
 }
 
 }  // namespace comb

@@ -31,6 +31,10 @@ enum { kKernelStore = 0, kKernelDecodeSplit = 1, kKernelDecodeMerge = 2, kKernel
 struct PoolGeom {
     int32_t num_layers, num_kv_heads, head_dim_qk, head_dim_v, num_pages;
     void *k_arena, *v_arena;
+    // fp8 pools (include/comb.h "fp8 pools"): one byte per element, fp32 power-of-two scale per (page, kv-head) block
+    int32_t kv_dtype = 0;   // 0 bf16, 1 e4m3
+    float *k_scale = nullptr, *v_scale = nullptr;
+    size_t elt_bytes() const { return kv_dtype == 1 ? 1 : 2; }
 };
 
 // Device pointers of a link (see comb_link_t in include/comb.h).
@@ -46,6 +50,14 @@ struct LinkView {
 // ---- (a2) store -------------------------------------------------------------------------------
 cudaError_t launch_store(const PoolGeom &g, int layer, const StorePageDesc *descs_dev, int num_descs,
                          const void *k_src, const void *v_src, cudaStream_t stream);
+
+// fp8 pool: quantising store (same descriptors; bf16 source, e4m3 codes + scales out). D = 128 only.
+cudaError_t launch_store_fp8(const PoolGeom &g, int layer, const StorePageDesc *descs_dev, int num_descs,
+                             const void *k_src, const void *v_src, cudaStream_t stream);
+// fp8 pool: dequantise `num_pages` pages (ids in page_ids_dev, e.g. the distinct pages of a link) of `layer` into compact
+// bf16 staging arenas k_out / v_out [num_pages][Hkv][16][128] (page i of the staging = page_ids[i] of the pool).
+cudaError_t launch_dequant_pages(const PoolGeom &g, int layer, const int32_t *page_ids_dev, int num_pages, void *k_out,
+                                 void *v_out, cudaStream_t stream);
 
 // read-only HBM stream over `bytes` bytes (measurement utility; `sink` = 4 device bytes)
 cudaError_t launch_stream_read(const void *src, size_t bytes, void *sink, cudaStream_t stream);
@@ -108,6 +120,9 @@ cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, con
 cudaError_t encode_tma_2d_bf16(const void *base, uint64_t inner, uint64_t outer, uint64_t row_pitch_bytes,
                                uint32_t box_inner, uint32_t box_outer, TensorMapBlob *out);
 
+cudaError_t encode_tma_2d_u8(const void *base, uint64_t inner, uint64_t outer, uint64_t row_pitch_bytes,
+                             uint32_t box_inner, uint32_t box_outer, TensorMapBlob *out);
+
 // ---- (f1) chunk-major ("cascade") decode --------------------------------------------------------
 // One work unit of the chunk-major decode: up to 32/G consecutive entries (query tokens) of chunk slot `slot`, starting
 // at position row0 of cas_row_req / cas_row_entry (each entry contributes the G rows of one kv-head), against KV tiles
@@ -120,6 +135,9 @@ struct CascadeItem {
     int32_t part0;        // partial index of entry row0 at this unit's range
     int32_t part_stride;  // entries of the slot (distance between the ranges of one entry)
     int32_t range_nr;     // (number of ranges of the slot << 8) | this unit's range index
+    // where the unit's KV lives in the chunk-major tables (filled by the planner from the host mirror, so the kernel's
+    // scheduler needs no dependent table lookups): first entry of cas_page_ids, number of pages, first cas_tile_ntok
+    int32_t pbeg, npages, tile0, pad;
 };
 // device workspace of one chunk-major decode call:
 //   [0, 16)  header (uint32 item counter, zero)   [16, ..) CascadeItem[num_units]     -- one H2D copy

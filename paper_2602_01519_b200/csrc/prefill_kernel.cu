@@ -102,10 +102,27 @@ cudaError_t encode_tma_2d_bf16(const void *base, uint64_t inner, uint64_t outer,
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
+// Dense row-major byte matrix [outer][inner bytes] -> 2-D tiled map of uint8, SWIZZLE_128B boxes (box_inner <= 128).
+cudaError_t encode_tma_2d_u8(const void *base, uint64_t inner, uint64_t outer, uint64_t row_pitch_bytes,
+                             uint32_t box_inner, uint32_t box_outer, TensorMapBlob *out) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return cudaErrorNotSupported;
+    const cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)outer};
+    const cuuint64_t strides[1] = {(cuuint64_t)row_pitch_bytes};
+    const cuuint32_t box[2] = {box_inner, box_outer};
+    const cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(reinterpret_cast<CUtensorMap *>(out), CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(base),
+                    dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
 namespace {
 
 // arena [L][pages][Hkv][16][D] seen as a dense bf16 matrix [rows][D]; box = {64 dims, 16 tokens}
-cudaError_t encode_arena_map(void *arena, int64_t rows, int d, TensorMapBlob *out) {
+// (fp8 pools: a byte matrix [rows][D], box = {128 bytes, 16 tokens})
+cudaError_t encode_arena_map(void *arena, int64_t rows, int d, bool fp8, TensorMapBlob *out) {
+    if (fp8) return encode_tma_2d_u8(arena, (uint64_t)d, (uint64_t)rows, (uint64_t)d, 128, (uint32_t)kPage, out);
     return encode_tma_2d_bf16(arena, (uint64_t)d, (uint64_t)rows, (uint64_t)d * 2, 64, (uint32_t)kPage, out);
 }
 
@@ -135,9 +152,9 @@ bool prefill_supported(int group, int dqk, int dv) {
 cudaError_t prefill_encode_kv_maps(const PoolGeom &g, TensorMapBlob *k_map, TensorMapBlob *v_map) {
     const int64_t rows = (int64_t)g.num_layers * g.num_pages * g.num_kv_heads * kPage;
     if (rows > INT32_MAX) return cudaErrorInvalidValue;
-    cudaError_t e = encode_arena_map(g.k_arena, rows, g.head_dim_qk, k_map);
+    cudaError_t e = encode_arena_map(g.k_arena, rows, g.head_dim_qk, g.kv_dtype == 1, k_map);
     if (e != cudaSuccess) return e;
-    return encode_arena_map(g.v_arena, rows, g.head_dim_v, v_map);
+    return encode_arena_map(g.v_arena, rows, g.head_dim_v, g.kv_dtype == 1, v_map);
 }
 
 // q [total_q][Hq][Dqk]; box = {64 dims, G heads of one kv-head, 128/G tokens} -> tile row = token * G + head

@@ -40,12 +40,12 @@ class Loaded:
 
 
 def load_workload(w, *, fill: str = "all", shuffle_seed: int = 0, extra_pages: int = 0, sentinel: Optional[int] = None,
-                  batch_tokens: int = 1 << 16, device: str = "cuda", keep_host: bool = True) -> Loaded:
+                  batch_tokens: int = 1 << 16, device: str = "cuda", keep_host: bool = True, kv_dtype: int = 0) -> Loaded:
     """``fill="all"``: every chunk of the population comes from ``w.chunk_kv`` (host, seeded).
     ``fill="linked"``: only linked chunks do; the rest get device-side N(0,1) bf16 noise."""
     assert fill in ("all", "linked")
     pool = Pool(w.num_kv_heads, w.head_dim_qk, w.head_dim_v, w.pool_pages + extra_pages, shuffle_seed=shuffle_seed,
-                device=device, sentinel=sentinel)
+                device=device, sentinel=sentinel, kv_dtype=kv_dtype)
     linked = set(int(c) for c in w.linked_chunks())
     stored: Dict[int, tuple] = {}
     Hkv, Dqk, Dv = w.num_kv_heads, w.head_dim_qk, w.head_dim_v

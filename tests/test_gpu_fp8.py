@@ -1,0 +1,199 @@
+"""GPU parity tests (run with -m gpu on a B200) of fp8 (e4m3) pools — SURVEY.md §8(f4), include/comb.h "fp8 pools",
+DESIGN.md §2 readings I31-I33 — through the C ABI against oracle/fp8.py:
+
+  store    codes and power-of-two scales of every (page, kv-head) block BIT-EXACT (the quantisation rule is part of the
+           contract); tail slots byte 0; pages owned by no chunk untouched.
+  attend   attention over an fp8 pool is Eq. 7-8 over the DEQUANTISED values.  Those are exactly bf16 numbers (the scale
+           is a power of two), so the expected result is the pinned fp64 C oracle run on the dequantised chunks; the
+           numpy statement in oracle/fp8.py must agree with it too.
+
+Tolerances: outputs as for bf16 pools (max abs 2e-2, mean abs 2e-3, relative L2 1e-2; the kernel's hi+lo
+split of Q and of the weights keeps ~8 significant bits, like bf16).  LSE: the query rows are re-rounded to 8 bits
+relative to the item's largest element, which perturbs every logit by ~1e-3 x |logit| / sqrt(D) x ...: |LSE error| <=
+2e-3 on N(0,1) inputs, 1e-2 on the peaked variants (measured worst cases are recorded beside the bf16 ones)."""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+
+import comb_synth as cs
+import oracle
+from oracle import fp8
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+BYTE_SENTINEL = 0xA5
+
+
+def H():
+    from paper_2602_01519_b200 import harness
+    return harness
+
+
+def record(tag, **kw):
+    try:
+        os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+        with open(os.path.join(ROOT, "gpurun_out", "parity_measured.jsonl"), "a") as f:
+            f.write(json.dumps(dict(tag=tag, **{k: float(v) for k, v in kw.items()})) + "\n")
+    except OSError:
+        pass
+
+
+class Dequantised:
+    """The workload with every chunk replaced by its dequantised fp8 image (bf16-exact), for the C oracle."""
+
+    def __init__(self, w):
+        self._w, self._cache = w, {}
+
+    def __getattr__(self, name):
+        return getattr(self._w, name)
+
+    def chunk_kv(self, c):
+        c = int(c)
+        if c not in self._cache:
+            kb, vb = self._w.chunk_kv(c)
+            kc, ks, vc, vs = fp8.quantise_chunk(kb, vb)
+            kd = fp8.dequantise_chunk(kc, ks, kb.shape[0]).astype(np.float32)
+            vd = fp8.dequantise_chunk(vc, vs, vb.shape[0]).astype(np.float32)
+            kbits, vbits = cs.f32_to_bf16_bits(kd), cs.f32_to_bf16_bits(vd)
+            assert np.array_equal(cs.bf16_bits_to_f64(kbits), kd.astype(np.float64))  # exact: nothing was rounded
+            self._cache[c] = (kbits, vbits)
+        return self._cache[c]
+
+
+def check(out_bits, lse, O, L, tag, lse_tol):
+    got = cs.bf16_bits_to_f64(out_bits)
+    assert np.all(np.isfinite(got)), tag + ": non-finite output"
+    err = np.abs(got - O)
+    rel = math.sqrt(float((err ** 2).sum()) / max(float((O ** 2).sum()), 1e-300))
+    excess = err - (2e-2 + 2.0 ** -8 * np.maximum(np.abs(O) - 2.0, 0.0))
+    assert excess.max() <= 0, "%s: max abs %.3e" % (tag, err.max())
+    assert err.mean() <= 2e-3, "%s: mean abs %.3e" % (tag, err.mean())
+    assert rel <= 1e-2, "%s: rel L2 %.3e" % (tag, rel)
+    fin = np.isfinite(L)
+    assert np.array_equal(np.isneginf(lse), np.isneginf(L)), tag + ": -inf pattern of LSE"
+    e = np.abs(lse[fin] - L[fin]).max() if fin.any() else 0.0
+    assert e <= lse_tol, "%s: LSE err %.3e" % (tag, e)
+    record("fp8 " + tag, max_abs=err.max(), mean_abs=err.mean(), rel_l2=rel, lse=e)
+
+
+def run_decode(w, **kw):
+    import paper_2602_01519_b200 as comb
+    ld = H().load_workload(w, sentinel=BYTE_SENTINEL, kv_dtype=comb.KV_E4M3, **kw)
+    out, lse = ld.pool.decode(ld.batch, ld.q, w.scale)
+    torch.cuda.synchronize()
+    return ld, H().device_to_bits(out), lse.cpu().numpy().astype(np.float64)
+
+
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shuffle", [0, 99])
+@pytest.mark.parametrize("Hkv", [2, 8])
+def test_fp8_store_page_image_is_bit_exact(shuffle, Hkv):
+    import paper_2602_01519_b200 as comb
+    lens = [128, 1, 16, 17, 250, 33, 512, 15]
+    w = cs.custom("store8", k=8, num_q_heads=Hkv, num_kv_heads=Hkv, head_dim_qk=128, head_dim_v=128, chunk_len=lens,
+                  links=[[3, 0, 6], [], [7, 1, 1, 4]], lq=[1, 1, 1])
+    ld = H().load_workload(w, shuffle_seed=shuffle, extra_pages=5, sentinel=BYTE_SENTINEL, batch_tokens=300,
+                           kv_dtype=comb.KV_E4M3)
+    num_pages = w.pool_pages + 5
+    model = oracle.PoolModel(num_pages, shuffle)
+    pages = {c: model.store(c, int(w.chunk_len[c])) for c in range(w.num_chunks)}
+    for c in range(w.num_chunks):
+        assert comb.comb_chunk_query(ld.pool.handle, c)[1].tolist() == pages[c]
+    k_img, ks_img, v_img, vs_img = fp8.page_image(num_pages, (Hkv, 128, 128),
+                                                  {c: w.chunk_kv(c) for c in range(w.num_chunks)}, pages,
+                                                  sentinel=BYTE_SENTINEL, scale_sentinel=-7.0)
+    k_got = ld.pool.k_arena.view(torch.uint8).cpu().numpy().reshape(k_img.shape)
+    v_got = ld.pool.v_arena.view(torch.uint8).cpu().numpy().reshape(v_img.shape)
+    assert np.array_equal(ld.pool.k_scale.cpu().numpy().reshape(ks_img.shape), ks_img), "K scales differ"
+    assert np.array_equal(ld.pool.v_scale.cpu().numpy().reshape(vs_img.shape), vs_img), "V scales differ"
+    assert np.array_equal(k_got, k_img), "K codes differ: %d bytes" % int((k_got != k_img).sum())
+    assert np.array_equal(v_got, v_img), "V codes differ"
+    ld.pool.close()
+
+
+FP8_SHAPES = [(32, 8), (16, 16), (4, 2), (16, 1), (16, 2)]   # (Hq, Hkv): G = 4, 1, 2, 16, 8
+
+
+@pytest.mark.parametrize("heads", FP8_SHAPES)
+@pytest.mark.parametrize("peaked", [False, True])
+def test_fp8_decode_matches_the_dequantised_oracle(heads, peaked):
+    """Ragged chunks (partial and odd page counts: a P V k-step of the kernel spans two pages), shared chunks, an empty
+    request, a duplicate link; both statements of the oracle."""
+    Hq, Hkv = heads
+    lens = [300, 16, 1000, 77, 512, 33, 129, 2000, 48, 5]
+    links = [[0, 2, 4], [4, 0], [], [7], [1, 3, 5, 6, 8, 9], [2, 2], [9], [4, 7, 0, 2], [6, 4], [0], [4], [2, 4, 0]]
+    w = cs.custom("dec8", k=8, num_q_heads=Hq, num_kv_heads=Hkv, head_dim_qk=128, head_dim_v=128, chunk_len=lens,
+                  links=links, lq=[1] * len(links), q_gain=4.0 if peaked else 1.0)
+    ld, out, lse = run_decode(w, shuffle_seed=5)
+    wd = Dequantised(w)
+    O, L = oracle.attention_for(wd)
+    O2, L2 = fp8.attention_for(w)
+    assert np.abs(O - O2).max() <= 1e-9 and np.abs(L[np.isfinite(L)] - L2[np.isfinite(L2)]).max() <= 1e-9
+    check(out, lse, O, L, "decode %s peaked=%s" % (heads, peaked), 1e-2 if peaked else 2e-3)
+    # what the quantisation itself costs against the unquantised chunks (reported, not asserted beyond sanity)
+    Ou, _ = oracle.attention_for(w)
+    q_err = np.abs(cs.bf16_bits_to_f64(out) - Ou)
+    record("fp8 quantisation %s peaked=%s" % (heads, peaked), max_abs=q_err.max(), mean_abs=q_err.mean(),
+           rel_l2=math.sqrt(float((q_err ** 2).sum()) / float((Ou ** 2).sum())))
+    assert math.sqrt(float((q_err ** 2).sum()) / float((Ou ** 2).sum())) <= 0.2
+    ld.pool.close()
+
+
+def test_fp8_closed_forms_on_gpu():
+    """P3 single key: O = the key's V as the pool holds it (dequantised), LSE = its score; P4 equal scores (Q = 0):
+    O = mean of the dequantised V, LSE = ln(kv_len); P12 empty link."""
+    w = cs.custom("cf8", k=8, num_q_heads=8, num_kv_heads=2, head_dim_qk=128, head_dim_v=128, chunk_len=[1, 512, 40],
+                  links=[[0], [1], [], [2, 1]], lq=[1, 1, 1, 1])
+    ld, out, lse = run_decode(w)
+    wd = Dequantised(w)
+    O, L = oracle.attention_for(wd)
+    got = cs.bf16_bits_to_f64(out)
+    assert np.array_equal(got[0], O[0]), "single key: the dequantised V row, bit for bit"
+    assert np.all(got[2] == 0) and np.all(np.isneginf(lse[2]))
+    check(out, lse, O, L, "closed forms", 2e-3)
+    # Q = 0: every weight equal
+    import paper_2602_01519_b200 as comb  # noqa: F401
+    q0 = torch.zeros_like(ld.q)
+    out0, lse0 = ld.pool.decode(ld.batch, q0, w.scale)
+    torch.cuda.synchronize()
+    l0 = lse0.cpu().numpy().astype(np.float64)
+    assert np.abs(l0[1] - math.log(512)).max() <= 1e-5 and np.abs(l0[3] - math.log(552)).max() <= 1e-5
+    vk = cs.bf16_bits_to_f64(wd.chunk_kv(1)[1])                       # [512][Hkv][128]
+    mean = vk.mean(axis=0)                                            # [Hkv][128]
+    g0 = cs.bf16_bits_to_f64(H().device_to_bits(out0))[1]             # [Hq][128]
+    assert np.abs(g0 - np.repeat(mean, 4, axis=0)).max() <= 2.0 ** -8 * np.abs(mean).max() + 1e-3
+    ld.pool.close()
+
+
+def test_fp8_full_size_decode_link_every_element():
+    """BASELINE configs[1] on an fp8 pool, in the launch configuration bench.py times, every output element."""
+    w = cs.decode_link(seed=0)
+    ld, out, lse = run_decode(w, fill="linked", shuffle_seed=2024, keep_host=False)
+    O, L = oracle.attention_for(Dequantised(w))
+    check(out, lse, O, L, "cfg2 decode (every element)", 2e-3)
+    ld.pool.close()
+
+
+def test_fp8_pool_rejects_what_is_not_built():
+    import paper_2602_01519_b200 as comb
+    for dq, dv in ((64, 64), (192, 128), (128, 64)):
+        with pytest.raises(comb.CombError) as e:
+            comb.Pool(2, dq, dv, 16, kv_dtype=comb.KV_E4M3)
+        assert e.value.status == comb.COMB_ERR_INVALID
+    w = cs.custom("rej8", k=8, num_q_heads=8, num_kv_heads=2, head_dim_qk=128, head_dim_v=128, chunk_len=[64],
+                  links=[[0]], lq=[4])
+    ld = H().load_workload(w, kv_dtype=comb.KV_E4M3)
+    with pytest.raises(comb.CombError) as e:
+        ld.pool.export()
+    assert e.value.status == comb.COMB_ERR_INVALID
+    hs = torch.zeros((64, 256), dtype=torch.bfloat16, device="cuda")
+    wkv = torch.zeros((2 * 256, 256), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(comb.CombError) as e:
+        ld.pool.project_store_chunks([5], np.array([0, 64], np.int32), hs, wkv)
+    assert e.value.status == comb.COMB_ERR_INVALID
+    ld.pool.close()

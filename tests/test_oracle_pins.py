@@ -410,3 +410,99 @@ def test_lru_eviction_hand_example():
     no.store(1, 32)
     with pytest.raises(MemoryError):
         no.store(2, 1)
+
+
+# ------------------------------------------------------------------------------------------------
+# fp8 (e4m3) pages: the oracle's quantisation model (oracle/fp8.py; DESIGN.md §2 I31-I33)
+# ------------------------------------------------------------------------------------------------
+def test_e4m3_code_table_closed_form_and_round_trip():
+    """The format's own numbers: 448 = 1.75 * 2^8 is the largest finite value, 2^-9 the smallest subnormal, 2^-6 the
+    smallest normal, 0x38 is 1.0; codes ascend with their values; encode(decode(c)) = c for every finite code."""
+    from oracle import fp8
+    t = fp8.e4m3_value_table()
+    assert t[0x7e] == 448.0 and t[0xfe] == -448.0 and np.isnan(t[0x7f]) and np.isnan(t[0xff])
+    assert t[0x01] == 2.0 ** -9 and t[0x07] == 7 * 2.0 ** -9 and t[0x08] == 2.0 ** -6 and t[0x38] == 1.0
+    assert t[0x39] == 1.125 and t[0x40] == 2.0 and t[0x00] == 0.0
+    assert np.all(np.diff(t[:127]) > 0)
+    finite = np.array([c for c in range(256) if c not in (0x7f, 0xff)], np.uint8)
+    back = fp8.e4m3_encode(t[finite])
+    keep = finite != 0x80                       # -0.0 encodes as the sign bit over code 0: same value
+    assert np.array_equal(back[keep], finite[keep]) and fp8.e4m3_decode(back[~keep])[0] == 0.0
+
+
+def test_e4m3_rounding_ties_to_even_and_saturates():
+    """Hand-worked: between 1.0 (0x38, mantissa 0) and 1.125 (0x39) the midpoint 1.0625 goes to the even mantissa 1.0;
+    between 1.125 (0x39) and 1.25 (0x3a) the midpoint 1.1875 goes to 1.25; just above / below a midpoint goes to the
+    nearer value; beyond 448 saturates (no infinity in this format); the subnormal midpoint 1.5 * 2^-9 goes to 2^-8."""
+    from oracle import fp8
+    x = np.array([1.0625, 1.1875, 1.0626, 1.0624, 1000.0, -1e9, 464.0, 1.5 * 2.0 ** -9, 0.4 * 2.0 ** -9, -1.0625])
+    want = np.array([1.0, 1.25, 1.125, 1.0, 448.0, -448.0, 448.0, 2.0 ** -8, 0.0, -1.0])
+    assert np.array_equal(fp8.e4m3_decode(fp8.e4m3_encode(x)), want)
+    # brute force: the code chosen is a nearest finite value for 20,000 random inputs
+    rng = np.random.default_rng(5)
+    y = rng.standard_normal(20000) * np.exp(rng.uniform(-6, 6, 20000))
+    t = fp8.e4m3_value_table()
+    fin = t[~np.isnan(t)]
+    got = fp8.e4m3_decode(fp8.e4m3_encode(y))
+    best = np.abs(np.clip(y, -448, 448)[:, None] - fin[None, :]).min(axis=1)
+    assert np.allclose(np.abs(np.clip(y, -448, 448) - got), best, rtol=0, atol=0)
+
+
+def test_fp8_block_quantisation_properties():
+    """scale = the smallest power of two 2^e with amax <= 448 * 2^e, so the block's largest element lands in (224, 448];
+    the dequantised value is within half an e4m3 step (2^-4 relative for normals) of the input and is exactly a bf16
+    number; an all-zero block has scale 1 and codes 0; tail slots of a chunk's last page are byte 0 and do not
+    influence the scale.  Hand-worked scales: amax 448 -> 1, 449 -> 2, 224 -> 0.5, 3.5 -> 2^-7, 3.51 -> 2^-6."""
+    from oracle import fp8
+    w = cs.custom("q8", k=7, num_q_heads=4, num_kv_heads=2, head_dim_qk=128, head_dim_v=128, chunk_len=[37],
+                  links=[[0]], lq=[1])
+    kb, vb = w.chunk_kv(0)
+    kc, ks, vc, vs = fp8.quantise_chunk(kb, vb)
+    assert kc.shape == (3, 2, 16, 128) and ks.shape == (3, 2)
+    x = fp8.bf16_bits_to_f32(kb).astype(np.float64)
+    for i in range(3):
+        n = min(16, 37 - 16 * i)
+        for h in range(2):
+            blk = x[16 * i:16 * i + n, h]
+            top = np.abs(fp8.e4m3_decode(kc[i, h, :n])).max()
+            assert 224.0 < np.abs(blk).max() / float(ks[i, h]) <= 448.0 and 224.0 <= top <= 448.0
+            assert float(ks[i, h]) == 2.0 ** round(np.log2(float(ks[i, h])))
+            assert np.all(kc[i, h, n:] == 0)
+    assert [fp8.block_scale(a) for a in (448.0, 449.0, 224.0, 3.5, 3.51, 0.0)] == [1.0, 2.0, 0.5, 2.0 ** -7, 2.0 ** -6, 1.0]
+    xd = fp8.dequantise_chunk(kc, ks, 37)
+    assert xd.shape == x.shape
+    assert np.array_equal(cs.bf16_bits_to_f64(cs.f32_to_bf16_bits(xd.astype(np.float32))), xd)   # bf16-exact
+    # half a step: 2^-4 of the value for normals, half the subnormal spacing (2^-10 * 448 / amax ...) near zero
+    step = np.maximum(np.abs(x) * 2.0 ** -4, ks.max() * 2.0 ** -10)
+    assert np.all(np.abs(xd - x) <= step * 1.0001)
+    z = np.zeros((5, 2, 128), np.uint16)
+    zc, zs, _, _ = fp8.quantise_chunk(z, z)
+    assert np.all(zc == 0) and np.all(zs == 1.0)
+
+
+def test_fp8_attention_reduces_to_the_bf16_oracle_on_exactly_representable_chunks():
+    """When every K/V element is +-448 * 2^-j-free, i.e. a small integer multiple of the block's amax / 448 that e4m3
+    holds exactly, quantisation loses nothing and attention over the fp8 pages equals the C oracle over the bf16 chunks:
+    pins oracle/fp8.attention_for (concatenation order, GQA map, softmax axis) to O1."""
+    from oracle import fp8
+    w = cs.custom("q8exact", k=7, num_q_heads=8, num_kv_heads=2, head_dim_qk=128, head_dim_v=128,
+                  chunk_len=[40, 16, 23], links=[[2, 0], [1], [0, 1, 2]], lq=[3, 1, 2])
+    exact_vals = np.array([0, 1, 2, 3, 4, 6, 8, 14, 16, -1, -2, -3, -5, -7, -12, 28], np.float32)   # x 1/16: all e4m3-exact
+
+    class Exact:  # the workload with its chunks replaced (Workload is frozen: delegate everything else)
+        def __getattr__(self, name):
+            return getattr(w, name)
+
+        def chunk_kv(self, c):
+            rng = np.random.default_rng([11, int(c)])
+            t = int(w.chunk_len[c])
+
+            def draw(d):
+                a = exact_vals[rng.integers(0, len(exact_vals), (t, 2, d))] / np.float32(16)
+                a[:, :, 0] = np.float32(28.0 / 16)  # every block's amax is 28/16 = 448 / 256: scale = 2^-8 exactly
+                return cs.f32_to_bf16_bits(a)
+            return draw(128), draw(128)
+    we = Exact()
+    O8, L8 = fp8.attention_for(we)
+    O, L = oracle.attention_for(we)
+    assert np.abs(O8 - O).max() <= 1e-12 and np.abs(L8 - L).max() <= 1e-12
