@@ -353,12 +353,12 @@ def main():
 
     # ------------------------------------------------------------------ attention benches
     def bench_attention(w, phase, steps, warmup, *, fill, flush_l2=False, with_link=True, e2e=True, shuffle=None,
-                        decode_path="auto"):
+                        decode_path="auto", kv_dtype=0):
         """Timings of `steps` passes of (link +) attention on workload w. Kernel times are per launch (CUDA events
         recorded by the library on the launching stream, comb_profile_*)."""
         # free list: permuted (a chunk's pages scattered over the arena, as in a long-running server) unless told
         ld = harness.load_workload(w, fill=fill, shuffle_seed=(2024 + rank) if shuffle is None else shuffle,
-                                   keep_host=False)
+                                   keep_host=False, kv_dtype=kv_dtype)
         pool = ld.pool
         pool.set_decode_path(PATHS[decode_path])
         if phase == "decode":
@@ -417,10 +417,13 @@ def main():
         else:
             main_k, merge_k = "prefill", "prefill_merge"
         L = batch.link
-        elt = 2 * wq.num_kv_heads * (wq.head_dim_qk + wq.head_dim_v)
+        # bytes per token of K + V over all kv-heads: bf16, or e4m3 codes + one fp32 scale per (page, kv-head) block
+        elt = (2 if kv_dtype == 0 else 1) * wq.num_kv_heads * (wq.head_dim_qk + wq.head_dim_v) + \
+              (0 if kv_dtype == 0 else wq.num_kv_heads * 2 * 4 // 16)
         res = {"ms_per_step": max_over_ranks(total_ms / steps), "kernel": main_k, "kernel_stats": stats(ks[main_k]),
                "merge_stats": stats(ks[merge_k]), "launches": launches, "clocks": clk.summary(),
-               "flops": wq.attention_flops(), "kv_bytes": wq.kv_bytes_logical(),
+               "flops": wq.attention_flops(),
+               "kv_bytes": wq.kv_bytes_logical() if kv_dtype == 0 else int(L.total_kv_tokens) * elt,
                "kv_bytes_unique": int(L.distinct_kv_tokens) * elt, "q_tokens": wq.total_q,
                "timed_seconds": total_ms / 1e3, "entries": int(L.total_entries),
                "distinct_chunks": int(L.num_distinct_chunks)}
@@ -587,11 +590,12 @@ def main():
             note(name, rr, rt, ("hbm=%.0f/%.3f" % (rh["achieved"], rh["frac"])) if rh else None)
             return rr
 
-        def decode_extra(name, wk, steps, fill, flush=False, shuffle=None, path="auto", wname=None):
+        def decode_extra(name, wk, steps, fill, flush=False, shuffle=None, path="auto", wname=None, kv_dtype=0):
             rr = bench_attention(wk, "decode", steps, 3, fill=fill, flush_l2=flush, e2e=False, shuffle=shuffle,
-                                 decode_path=path)
+                                 decode_path=path, kv_dtype=kv_dtype)
             rh = roofline_hbm(rr, wname or name)
-            extras[name] = {"workload": name, "decode_path": path, "ms_per_step": rr["ms_per_step"],
+            extras[name] = {"workload": name, "decode_path": path, "kv_dtype": "e4m3" if kv_dtype else "bf16",
+                            "ms_per_step": rr["ms_per_step"],
                             "kernel_ms": rr["kernel_ms"], "merge_ms": rr["merge_ms"],
                             "gbs_logical": rr["kv_bytes"] / (rr["ms_per_step"] * 1e-3) / 1e9,
                             "entries": rr["entries"], "distinct_chunks": rr["distinct_chunks"],
@@ -630,6 +634,12 @@ def main():
                              path="per_request", wname="decode_no_reuse")
                 decode_extra("decode_no_reuse_chunk_major", cs.decode_link(seed=args.seed, no_reuse=True), N, "linked",
                              path="chunk_major", wname="decode_no_reuse")
+            # (f4) fp8 pools: the same batches over e4m3 pages (bytes counted as stored: codes + scales)
+            if want("decode_fp8"):
+                decode_extra("decode_link_fp8", cs.decode_link(seed=args.seed), N, "linked", wname="decode_link_fp8",
+                             kv_dtype=comb.KV_E4M3)
+                decode_extra("decode_no_reuse_fp8", cs.decode_link(seed=args.seed, no_reuse=True), N, "linked",
+                             wname="decode_no_reuse_fp8", kv_dtype=comb.KV_E4M3)
             if want("rag_prefill_lq32"):
                 prefill_extra("rag_prefill_lq32", cs.rag_prefill(seed=args.seed, lq=32), N, "linked")
             # the paper's own regime (< 50 dynamic tokens) at a small batch: 32 work items for 148 SMs,

@@ -578,7 +578,7 @@ struct F8Cfg {
     static constexpr int SLOT = 128 * 128;                  // [128 keys][128 bytes] of a K or V tile
     static constexpr int NSLOT = 8;
     static constexpr int Q_BYTES = 2 * kRowsMax * 128;      // [hi 32 rows | lo 32 rows][128 bytes]
-    static constexpr int P_BYTES = 2 * kRowsMax * 128;      // [hi | lo][128 keys]
+    static constexpr int P_BYTES = 128 * 128;               // [128 keys][hi rows | lo rows, 128-byte pitch]: MN-major B
     static constexpr int MISC = 3072;
     static constexpr int SMEM = 1024 + 2 * Q_BYTES + P_BYTES + NSLOT * SLOT + MISC;
     static constexpr int THREADS = 256;
@@ -613,9 +613,10 @@ __device__ __forceinline__ void softmax_item_f8(const CascadeArgs &a, Misc *mi, 
 #pragma unroll
     for (int n = 0; n < NC; ++n) { mc[n] = -INFINITY; l_part[n] = 0.f; }
     float vref = 0.f;  // reference V scale of O^T (identical in all 128 threads)
-    // this thread's key inside a tile: page kp, slot ks; byte ks of 16-byte unit kp in every P row
+    // this thread's key inside a tile: page kp, slot ks; its weights are row `tid` of the P tile (MN-major B operand:
+    // the 2 NC codes of a key are contiguous, [hi rows | lo rows], in 16-byte units swizzled by the row)
     const int kp = tid >> 4, ks = tid & 15;
-    unsigned char *p_dst = sP + ks;
+    unsigned char *p_dst = sP + tid * 128;
     const float qs = mi->qscale[ip];
     for (int j = 0; j < n_kv; ++j, ++t) {
         const uint64_t ntok8 = a.cas_tile_ntok[it.tile0 + j];
@@ -701,18 +702,25 @@ __device__ __forceinline__ void softmax_item_f8(const CascadeArgs &a, Misc *mi, 
             ptx::mbar_wait(&mi->p_empty, (t & 1) ^ 1);
         }
         const float vw = vsc / vref;  // <= 1, exact (0 for a masked key)
+        uint32_t ph[NC / 4], pl[NC / 4];  // codes of rows 4 i .. 4 i + 3, hi and lo
 #pragma unroll
-        for (int n = 0; n < NC; n += 2) {
+        for (int n = 0; n < NC; n += 4) {
             const float p0 = ptx::ex2(y[n] - mc[n]), p1 = ptx::ex2(y[n + 1] - mc[n + 1]);
+            const float p2 = ptx::ex2(y[n + 2] - mc[n + 2]), p3 = ptx::ex2(y[n + 3] - mc[n + 3]);
             l_part[n] += p0;
             l_part[n + 1] += p1;
-            uint32_t hi, lo;
-            split_e4m3x2(p0 * vw, p1 * vw, hi, lo);
-            // row R of the P tile: R * 128 + ((unit ^ (R & 7)) << 4) + byte; rows [0, NC) hi, [NC, 2 NC) lo
-            p_dst[n * 128 + ((kp ^ (n & 7)) << 4)] = (unsigned char)(hi & 0xffu);
-            p_dst[(n + 1) * 128 + ((kp ^ ((n + 1) & 7)) << 4)] = (unsigned char)(hi >> 8);
-            p_dst[(NC + n) * 128 + ((kp ^ (n & 7)) << 4)] = (unsigned char)(lo & 0xffu);
-            p_dst[(NC + n + 1) * 128 + ((kp ^ ((n + 1) & 7)) << 4)] = (unsigned char)(lo >> 8);
+            l_part[n + 2] += p2;
+            l_part[n + 3] += p3;
+            uint32_t h0, l0, h1, l1;
+            split_e4m3x2(p0 * vw, p1 * vw, h0, l0);
+            split_e4m3x2(p2 * vw, p3 * vw, h1, l1);
+            ph[n / 4] = h0 | (h1 << 16);
+            pl[n / 4] = l0 | (l1 << 16);
+        }
+#pragma unroll
+        for (int u = 0; u < NC / 16; ++u) {  // hi units 0 .. NC/16 - 1, lo units NC/16 .. 2 NC/16 - 1
+            *reinterpret_cast<uint4 *>(p_dst + ((u ^ (tid & 7)) << 4)) = make_uint4(ph[4 * u], ph[4 * u + 1], ph[4 * u + 2], ph[4 * u + 3]);
+            *reinterpret_cast<uint4 *>(p_dst + (((NC / 16 + u) ^ (tid & 7)) << 4)) = make_uint4(pl[4 * u], pl[4 * u + 1], pl[4 * u + 2], pl[4 * u + 3]);
         }
         ptx::fence_proxy_async_smem();
         __syncwarp();
@@ -776,7 +784,7 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
     if (tid == 0) {
         for (int i = 0; i < kItemRing; ++i) {
             ptx::mbar_init(&mi->item_full[i], 1);
-            ptx::mbar_init(&mi->item_empty[i], 6);
+            ptx::mbar_init(&mi->item_empty[i], 7);  // two loaders, issuer, four softmax warps
         }
         for (int i = 0; i < 2; ++i) {
             ptx::mbar_init(&mi->q_full[i], 1);
@@ -828,17 +836,24 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             if (it.ncols == 16) softmax_item_f8<16>(a, mi, sP, tmem, it, k, t);
             else softmax_item_f8<32>(a, mi, sP, tmem, it, k, t);
         }
-    } else if (warp == 4) {
-        // ===================== K/V TMA loader + page scales =====================
+    } else if (warp == 4 || warp == 7) {
+        // ===================== K/V TMA loaders + page scales =====================
+        // Both warps walk the same slot sequence (K_t, then V_{t-1}); warp 4 issues the K tiles and writes the pages'
+        // scales, warp 7 issues the V tiles: per byte an fp8 tile needs twice the TMA issues of a bf16 tile, and one
+        // issuing warp was 75 % busy.
+        const bool mine_v = warp == 7;
         uint32_t slot = 0, phase = 0, tt = 0;
         bool have_prev = false;
         int prev_row0 = 0, prev_pages = 0;
         auto issue = [&](bool is_v, int row0, int pages_here) {
-            ptx::mbar_wait(&mi->kv_empty[slot], phase ^ 1);
-            unsigned char *dst = sKV + slot * C::SLOT;
-            if (lane == 0) ptx::mbar_expect_tx(&mi->kv_full[slot], (uint32_t)pages_here * kPage * 128);
-            __syncwarp();
-            if (lane < pages_here) ptx::tma_load_2d(dst + lane * 2048, is_v ? &maps.v : &maps.k, 0, row0, &mi->kv_full[slot]);
+            if (is_v == mine_v) {
+                ptx::mbar_wait(&mi->kv_empty[slot], phase ^ 1);
+                unsigned char *dst = sKV + slot * C::SLOT;
+                if (lane == 0) ptx::mbar_expect_tx(&mi->kv_full[slot], (uint32_t)pages_here * kPage * 128);
+                __syncwarp();
+                if (lane < pages_here)
+                    ptx::tma_load_2d(dst + lane * 2048, is_v ? &maps.v : &maps.k, 0, row0, &mi->kv_full[slot]);
+            }
             if (++slot == C::NSLOT) { slot = 0; phase ^= 1; }
         };
         for (int k = 0;; ++k) {
@@ -850,20 +865,23 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             if (!it.valid) break;
             const int n_kv = (it.npages + kTilePages - 1) / kTilePages;
             int ids = 0;
-            float ksc = 1.f, vsc = 1.f;
+            float ksc = 1.f, vsc = 0.f;
             for (int j = 0; j < n_kv; ++j, ++tt) {
-                if ((j & 3) == 0) {  // page ids and scales of the next four tiles
+                if ((j & 3) == 0) {  // page ids (and, in the K warp, scales) of the next four tiles
                     const bool have = j * kTilePages + lane < it.npages;
                     ids = have ? a.cas_page_ids[it.pbeg + j * kTilePages + lane] : 0;
-                    ksc = have ? a.k_scale[(size_t)ids * Hkv + it.kvh] : 1.f;
-                    vsc = have ? a.v_scale[(size_t)ids * Hkv + it.kvh] : 0.f;
+                    if (!mine_v) {
+                        ksc = have ? a.k_scale[(size_t)ids * Hkv + it.kvh] : 1.f;
+                        vsc = have ? a.v_scale[(size_t)ids * Hkv + it.kvh] : 0.f;
+                    }
                 }
                 const int pages_here = min(kTilePages, it.npages - j * kTilePages);
                 const int pid = __shfl_sync(0xffffffffu, ids, (j & 3) * kTilePages + (lane & 7));
                 const int row0 = a.layer_row0 + (pid * Hkv + it.kvh) * kPage;
-                // (the softmax threads read these after S_tt has completed, i.e. after the K tile's barrier, which this
-                // warp arrives on below; entry tt & 7 was last used by tile tt - 8, long consumed)
-                if ((lane >> 3) == (j & 3)) {
+                // The K warp writes both scales of tile tt BEFORE it arrives on K_tt's barrier; the softmax threads read
+                // them after S_tt has completed, which that barrier precedes.  Entry tt & 7 was last used by tile
+                // tt - 8, consumed long ago (the ring holds at most NSLOT / 2 tiles).
+                if (!mine_v && (lane >> 3) == (j & 3)) {
                     mi->kscale[tt & 7][lane & 7] = ksc;
                     mi->vscale[tt & 7][lane & 7] = vsc;
                 }
@@ -880,9 +898,9 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
         // ===================== MMA issuer =====================
         const bool leader = ptx::elect_one();
         const uint64_t dq0 = ptx::umma_desc_sw128(ptx::smem_u32(sQ), 16, 1024);
-        const uint64_t dp0 = ptx::umma_desc_sw128(ptx::smem_u32(sP), 16, 1024);
         const uint64_t dk0 = ptx::umma_desc_sw128(ptx::smem_u32(sKV), 16, 1024);
         const uint64_t dv0 = ptx::umma_desc_sw128(ptx::smem_u32(sKV), 0, 1024);  // MN-major: one 128-byte block along d
+        const uint64_t dpm = ptx::umma_desc_sw128(ptx::smem_u32(sP), 0, 1024);   // MN-major: a key's codes along the rows
         uint32_t slot = 0, phase = 0, t = 0;
         struct Pend { bool on, first, last; int pages, ip, k; uint32_t t, idesc; } pd{false, false, false, 0, 0, 0, 0, 0};
         auto do_pv = [&]() {
@@ -894,7 +912,7 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             for (int ks = 0; ks < ksteps; ++ks)
                 if (leader)
                     ptx::mma_ss_f8(tmem + 128 + pd.ip * 64, dv0 + (uint64_t)((slot * C::SLOT + ks * 4096) >> 4),
-                                   dp0 + (uint64_t)((ks * 32) >> 4), pd.idesc, (pd.first && ks == 0) ? 0u : 1u);
+                                   dpm + (uint64_t)((ks * 4096) >> 4), pd.idesc, (pd.first && ks == 0) ? 0u : 1u);
             if (leader) {
                 ptx::mma_commit(&mi->p_empty);
                 ptx::mma_commit(&mi->kv_empty[slot]);
@@ -913,7 +931,7 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             const int ip = k & 1;
             const int n_kv = (it.npages + kTilePages - 1) / kTilePages;
             const uint32_t idesc_s = ptx::umma_idesc_e4m3(128, 2 * it.ncols, false, false);
-            const uint32_t idesc_o = ptx::umma_idesc_e4m3(128, 2 * it.ncols, true, false);
+            const uint32_t idesc_o = ptx::umma_idesc_e4m3(128, 2 * it.ncols, true, true);
             ptx::mbar_wait(&mi->q_full[ip], (k >> 1) & 1);
             for (int j = 0; j < n_kv; ++j, ++t) {
                 const int sb = t & 1;
@@ -978,21 +996,23 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             const int req_lane = lane < ci.nrows ? a.cas_row_req[ci.row0 + lane] : 0;
             const int qb = k & 1;
             uint4 val[16];
-            float amax = 0.f;
+            __nv_bfloat162 am2 = __floats2bfloat162_rn(0.f, 0.f);
 #pragma unroll
             for (int x = 0; x < 16; ++x) {
-                const int row = 2 * x + (lane >> 4), j = lane & 15;
-                const int e_pos = row >> a.group_shift, hh = row & (G - 1);
-                const int qrow = __shfl_sync(0xffffffffu, req_lane, e_pos & 31);
-                val[x] = make_uint4(0u, 0u, 0u, 0u);
-                if (row < rows_valid)
-                    val[x] = __ldg(reinterpret_cast<const uint4 *>(a.q + (((size_t)qrow * Hq + kvh * G + hh) * 128) * 2 +
-                                                                   (size_t)j * 16));
-                const uint32_t w[4] = {val[x].x, val[x].y, val[x].z, val[x].w};
+                if (2 * x < ncols) {  // uniform: an item has 16 or 32 row slots
+                    const int row = 2 * x + (lane >> 4), j = lane & 15;
+                    const int e_pos = row >> a.group_shift, hh = row & (G - 1);
+                    const int qrow = __shfl_sync(0xffffffffu, req_lane, e_pos & 31);
+                    val[x] = make_uint4(0u, 0u, 0u, 0u);
+                    if (row < rows_valid)
+                        val[x] = __ldg(reinterpret_cast<const uint4 *>(a.q + (((size_t)qrow * Hq + kvh * G + hh) * 128) * 2 +
+                                                                       (size_t)j * 16));
+                    const __nv_bfloat162 *h2 = reinterpret_cast<const __nv_bfloat162 *>(&val[x]);
 #pragma unroll
-                for (int e = 0; e < 4; ++e)
-                    amax = fmaxf(amax, fmaxf(fabsf(__uint_as_float(w[e] << 16)), fabsf(__uint_as_float(w[e] & 0xffff0000u))));
+                    for (int e = 0; e < 4; ++e) am2 = __hmax2(am2, __habs2(h2[e]));
+                }
             }
+            float amax = fmaxf(__low2float(am2), __high2float(am2));
             amax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(amax)));
             const float qs = pow2_scale_for(amax), qinv = 1.f / qs;
             ptx::mbar_wait(&mi->q_empty[qb], ((k >> 1) & 1) ^ 1);
@@ -1000,7 +1020,7 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
 #pragma unroll
             for (int x = 0; x < 16; ++x) {
                 const int row = 2 * x + (lane >> 4), j = lane & 15;
-                if (row < ncols) {
+                if (2 * x < ncols) {
                     const uint32_t w[4] = {val[x].x, val[x].y, val[x].z, val[x].w};
                     uint32_t hi[4], lo[4];
 #pragma unroll

@@ -7,10 +7,10 @@ DESIGN.md §2 readings I31-I33 — through the C ABI against oracle/fp8.py:
            is a power of two), so the expected result is the pinned fp64 C oracle run on the dequantised chunks; the
            numpy statement in oracle/fp8.py must agree with it too.
 
-Tolerances: outputs as for bf16 pools (max abs 2e-2, mean abs 2e-3, relative L2 1e-2; the kernel's hi+lo
-split of Q and of the weights keeps ~8 significant bits, like bf16).  LSE: the query rows are re-rounded to 8 bits
-relative to the item's largest element, which perturbs every logit by ~1e-3 x |logit| / sqrt(D) x ...: |LSE error| <=
-2e-3 on N(0,1) inputs, 1e-2 on the peaked variants (measured worst cases are recorded beside the bf16 ones)."""
+Tolerances: exactly those of bf16 pools (max abs 2e-2, mean abs 2e-3, relative L2 1e-2, |LSE error|
+<= 2e-4): the kernel's hi + lo split of Q and of the weights keeps 7-8 significant bits per element, like bf16.
+Measured: relative L2 1.7e-3, |LSE error| 2e-6.  What the quantisation ITSELF costs against the unquantised chunks is
+recorded beside it (relative L2 3.3e-2 on N(0,1) inputs, 6.5e-2 on the peaked variants) and only sanity-checked."""
 import json
 import math
 import os
@@ -134,7 +134,7 @@ def test_fp8_decode_matches_the_dequantised_oracle(heads, peaked):
     O, L = oracle.attention_for(wd)
     O2, L2 = fp8.attention_for(w)
     assert np.abs(O - O2).max() <= 1e-9 and np.abs(L[np.isfinite(L)] - L2[np.isfinite(L2)]).max() <= 1e-9
-    check(out, lse, O, L, "decode %s peaked=%s" % (heads, peaked), 1e-2 if peaked else 2e-3)
+    check(out, lse, O, L, "decode %s peaked=%s" % (heads, peaked), 2e-4)
     # what the quantisation itself costs against the unquantised chunks (reported, not asserted beyond sanity)
     Ou, _ = oracle.attention_for(w)
     q_err = np.abs(cs.bf16_bits_to_f64(out) - Ou)
@@ -155,7 +155,7 @@ def test_fp8_closed_forms_on_gpu():
     got = cs.bf16_bits_to_f64(out)
     assert np.array_equal(got[0], O[0]), "single key: the dequantised V row, bit for bit"
     assert np.all(got[2] == 0) and np.all(np.isneginf(lse[2]))
-    check(out, lse, O, L, "closed forms", 2e-3)
+    check(out, lse, O, L, "closed forms", 2e-4)
     # Q = 0: every weight equal
     import paper_2602_01519_b200 as comb  # noqa: F401
     q0 = torch.zeros_like(ld.q)
@@ -175,7 +175,7 @@ def test_fp8_full_size_decode_link_every_element():
     w = cs.decode_link(seed=0)
     ld, out, lse = run_decode(w, fill="linked", shuffle_seed=2024, keep_host=False)
     O, L = oracle.attention_for(Dequantised(w))
-    check(out, lse, O, L, "cfg2 decode (every element)", 2e-3)
+    check(out, lse, O, L, "cfg2 decode (every element)", 2e-4)
     ld.pool.close()
 
 
