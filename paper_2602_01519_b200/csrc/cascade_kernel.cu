@@ -91,12 +91,14 @@ struct Misc {
     uint64_t q_full[2], q_empty[2], s_full[2], s_empty[2], o_full[2], o_empty[2];
     uint64_t p_full, p_empty;
     uint64_t kv_full[8], kv_empty[8];
+    uint64_t sc_full[8];  // fp8 kernel: the scales / tile mask of ring entry t & 7 are written
     float wmax[4][kRowsMax];
     float wsum[4][kRowsMax];
     float mref[kRowsMax], inv_l[kRowsMax];
     // fp8 pools: scales of the 8 pages of the last 8 tiles (written by the loader), the items' Q scale, and the warps'
     // largest V scale of a tile
     float kscale[8][8], vscale[8][8], qscale[2], wvs[4];
+    unsigned long long tntok[8];  // fp8 kernel: tile_ntok of the last 8 tiles (written by the K loader)
     alignas(16) int32_t srow[2][kRowsMax];
     ItemEntry items[kItemRing];
     uint32_t tmem_slot;
@@ -148,9 +150,14 @@ __device__ __forceinline__ float warp_row_sums(float (&v)[NC], int lane) {
         scatter_stage<16, 16>(v, lane);
     } else {
 #pragma unroll
-        for (int i = 0; i < 16; ++i) v[i] += __shfl_xor_sync(0xffffffffu, v[i], 16);
+        for (int i = 0; i < NC; ++i) v[i] += __shfl_xor_sync(0xffffffffu, v[i], 16);
     }
-    scatter_stage<8, 8>(v, lane);
+    if constexpr (NC >= 16) {
+        scatter_stage<8, 8>(v, lane);
+    } else {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) v[i] += __shfl_xor_sync(0xffffffffu, v[i], 8);
+    }
     scatter_stage<4, 4>(v, lane);
     scatter_stage<2, 2>(v, lane);
     scatter_stage<1, 1>(v, lane);
@@ -612,18 +619,19 @@ __device__ __forceinline__ void softmax_item_f8(const CascadeArgs &a, Misc *mi, 
     float mc[NC], l_part[NC];
 #pragma unroll
     for (int n = 0; n < NC; ++n) { mc[n] = -INFINITY; l_part[n] = 0.f; }
-    float vref = 0.f;  // reference V scale of O^T (identical in all 128 threads)
+    float vref = 0.f, inv_vref = 0.f;  // reference V scale of O^T (identical in all 128 threads) and 1 / vref
     // this thread's key inside a tile: page kp, slot ks; its weights are row `tid` of the P tile (MN-major B operand:
     // the 2 NC codes of a key are contiguous, [hi rows | lo rows], in 16-byte units swizzled by the row)
     const int kp = tid >> 4, ks = tid & 15;
     unsigned char *p_dst = sP + tid * 128;
     const float qs = mi->qscale[ip];
     for (int j = 0; j < n_kv; ++j, ++t) {
-        const uint64_t ntok8 = a.cas_tile_ntok[it.tile0 + j];
-        const bool key_valid = ks < (int)((ntok8 >> (8 * kp)) & 0xffu);
         const int sb = t & 1;
         ptx::mbar_wait(&mi->s_full[sb], (t >> 1) & 1);
         ptx::tc_fence_after();
+        ptx::mbar_wait(&mi->sc_full[t & 7], (t >> 3) & 1);  // the K loader has written this tile's mask and scales
+        const uint64_t ntok8 = mi->tntok[t & 7];
+        const bool key_valid = ks < (int)((ntok8 >> (8 * kp)) & 0xffu);
         uint32_t r[2 * NC];
 #pragma unroll
         for (int q = 0; q < 2 * NC / 16; ++q)
@@ -698,10 +706,11 @@ __device__ __forceinline__ void softmax_item_f8(const CascadeArgs &a, Misc *mi, 
                 for (int n = 0; n < NC; ++n) mc[n] = wm[n];
             }
             vref = vnew;
+            inv_vref = 1.f / vnew;
         } else {
             ptx::mbar_wait(&mi->p_empty, (t & 1) ^ 1);
         }
-        const float vw = vsc / vref;  // <= 1, exact (0 for a masked key)
+        const float vw = vsc * inv_vref;  // <= 1, exact (0 for a masked key)
         uint32_t ph[NC / 4], pl[NC / 4];  // codes of rows 4 i .. 4 i + 3, hi and lo
 #pragma unroll
         for (int n = 0; n < NC; n += 4) {
@@ -717,11 +726,12 @@ __device__ __forceinline__ void softmax_item_f8(const CascadeArgs &a, Misc *mi, 
             ph[n / 4] = h0 | (h1 << 16);
             pl[n / 4] = l0 | (l1 << 16);
         }
+        uint32_t pc[NC / 2];  // the key's 2 NC codes: [hi rows | lo rows]
 #pragma unroll
-        for (int u = 0; u < NC / 16; ++u) {  // hi units 0 .. NC/16 - 1, lo units NC/16 .. 2 NC/16 - 1
-            *reinterpret_cast<uint4 *>(p_dst + ((u ^ (tid & 7)) << 4)) = make_uint4(ph[4 * u], ph[4 * u + 1], ph[4 * u + 2], ph[4 * u + 3]);
-            *reinterpret_cast<uint4 *>(p_dst + (((NC / 16 + u) ^ (tid & 7)) << 4)) = make_uint4(pl[4 * u], pl[4 * u + 1], pl[4 * u + 2], pl[4 * u + 3]);
-        }
+        for (int i = 0; i < NC / 4; ++i) { pc[i] = ph[i]; pc[NC / 4 + i] = pl[i]; }
+#pragma unroll
+        for (int u = 0; u < NC / 8; ++u)  // 16-byte units, swizzled by the row (= key)
+            *reinterpret_cast<uint4 *>(p_dst + ((u ^ (tid & 7)) << 4)) = make_uint4(pc[4 * u], pc[4 * u + 1], pc[4 * u + 2], pc[4 * u + 3]);
         ptx::fence_proxy_async_smem();
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(&mi->p_full);
@@ -799,6 +809,7 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
         for (int s = 0; s < C::NSLOT; ++s) {
             ptx::mbar_init(&mi->kv_full[s], 1);
             ptx::mbar_init(&mi->kv_empty[s], 1);
+            ptx::mbar_init(&mi->sc_full[s], 1);
         }
         ptx::fence_barrier_init();
         ptx::tma_prefetch_desc(&maps.k);
@@ -828,12 +839,10 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
                 const int e_pos = tid >> a.group_shift, head = tid & (G - 1);
                 const bool valid = e_pos < it.nrows;
                 mi->srow[k & 1][tid] = valid ? (it.part0 + e_pos) * Hq + it.kvh * G + head : -1;
-                if (valid && head == 0 && it.kvh == 0 && (it.range_nr & 0xff) == 0)
-                    a.ent_info[a.cas_row_entry[it.row0 + e_pos]] =
-                        make_int4(it.part0 + e_pos, it.stride, it.range_nr >> 8, 0);
             }
             ptx::mbar_wait(&mi->q_full[k & 1], (k >> 1) & 1);  // the item's Q scale is written with its Q tile
-            if (it.ncols == 16) softmax_item_f8<16>(a, mi, sP, tmem, it, k, t);
+            if (it.ncols == 8) softmax_item_f8<8>(a, mi, sP, tmem, it, k, t);
+            else if (it.ncols == 16) softmax_item_f8<16>(a, mi, sP, tmem, it, k, t);
             else softmax_item_f8<32>(a, mi, sP, tmem, it, k, t);
         }
     } else if (warp == 4 || warp == 7) {
@@ -866,11 +875,13 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             const int n_kv = (it.npages + kTilePages - 1) / kTilePages;
             int ids = 0;
             float ksc = 1.f, vsc = 0.f;
+            unsigned long long nt4 = 0;
             for (int j = 0; j < n_kv; ++j, ++tt) {
-                if ((j & 3) == 0) {  // page ids (and, in the K warp, scales) of the next four tiles
+                if ((j & 3) == 0) {  // page ids (and, in the K warp, scales and tile masks) of the next four tiles
                     const bool have = j * kTilePages + lane < it.npages;
                     ids = have ? a.cas_page_ids[it.pbeg + j * kTilePages + lane] : 0;
                     if (!mine_v) {
+                        if (lane < 4 && j + lane < n_kv) nt4 = a.cas_tile_ntok[it.tile0 + j + lane];
                         ksc = have ? a.k_scale[(size_t)ids * Hkv + it.kvh] : 1.f;
                         vsc = have ? a.v_scale[(size_t)ids * Hkv + it.kvh] : 0.f;
                     }
@@ -878,15 +889,20 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
                 const int pages_here = min(kTilePages, it.npages - j * kTilePages);
                 const int pid = __shfl_sync(0xffffffffu, ids, (j & 3) * kTilePages + (lane & 7));
                 const int row0 = a.layer_row0 + (pid * Hkv + it.kvh) * kPage;
-                // The K warp writes both scales of tile tt BEFORE it arrives on K_tt's barrier; the softmax threads read
-                // them after S_tt has completed, which that barrier precedes.  Entry tt & 7 was last used by tile
-                // tt - 8, consumed long ago (the ring holds at most NSLOT / 2 tiles).
-                if (!mine_v && (lane >> 3) == (j & 3)) {
-                    mi->kscale[tt & 7][lane & 7] = ksc;
-                    mi->vscale[tt & 7][lane & 7] = vsc;
-                }
-                __syncwarp();
                 issue(false, row0, pages_here);
+                // The K warp publishes the tile's mask and scales AFTER it has issued the tile's loads (the scale loads
+                // depend on the page ids: waiting for them first would put a memory round trip in front of every
+                // item's first TMA).  Ring entry tt & 7 was last used by tile tt - 8, consumed long ago (the K/V ring
+                // holds at most NSLOT / 2 tiles); the softmax threads wait on sc_full before they read.
+                if (!mine_v) {
+                    if ((lane >> 3) == (j & 3)) {
+                        mi->kscale[tt & 7][lane & 7] = ksc;
+                        mi->vscale[tt & 7][lane & 7] = vsc;
+                    }
+                    if (lane == (j & 3)) mi->tntok[tt & 7] = nt4;
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(&mi->sc_full[tt & 7]);
+                }
                 if (have_prev) issue(true, prev_row0, prev_pages);
                 prev_row0 = row0;
                 prev_pages = pages_here;
@@ -974,7 +990,7 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             const CascadeItem ci = a.items[unit];
             if (lane == 0) idx = atomicAdd(a.counter, 1u);
             const int rows_valid = ci.nrows * G;
-            const int ncols = rows_valid <= 16 ? 16 : 32;
+            const int ncols = rows_valid <= 8 ? 8 : (rows_valid <= 16 ? 16 : 32);
             if (lane == 0) {
                 ItemEntry e;
                 e.valid = 1;
@@ -994,6 +1010,9 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             }
             // Q rows: 16 units of 8 bf16 per row; lane holds unit (x * 32 + lane) = row 2 x + (lane >> 4), unit lane & 15
             const int req_lane = lane < ci.nrows ? a.cas_row_req[ci.row0 + lane] : 0;
+            // where the merge finds an entry's partials (once per entry: first kv-head, first range)
+            if (lane < ci.nrows && kvh == 0 && (ci.range_nr & 0xff) == 0)
+                a.ent_info[a.cas_row_entry[ci.row0 + lane]] = make_int4(ci.part0 + lane, ci.part_stride, ci.range_nr >> 8, 0);
             const int qb = k & 1;
             uint4 val[16];
             __nv_bfloat162 am2 = __floats2bfloat162_rn(0.f, 0.f);
