@@ -572,8 +572,8 @@ def main():
             return not only or name in only
 
         # ---- the other configs (not bench lines; context for the BASELINE metric's prefill half) ----
-        def prefill_extra(name, wk, steps, fill, flush=False, wname=None):
-            rr = bench_attention(wk, "prefill", steps, 3, fill=fill, flush_l2=flush, e2e=False)
+        def prefill_extra(name, wk, steps, fill, flush=False, wname=None, kv_dtype=0):
+            rr = bench_attention(wk, "prefill", steps, 3, fill=fill, flush_l2=flush, e2e=False, kv_dtype=kv_dtype)
             # a prefill whose flops per logical KV byte sit under the ridge of the measured peaks is HBM-bound
             # (no GQA or few query tokens: SURVEY.md 8(d)); it is then reported against the HBM roof first
             ridge = pk["tf_burst"] * 1e12 / (pk["hbm"] * 1e9)
@@ -640,6 +640,9 @@ def main():
                              kv_dtype=comb.KV_E4M3)
                 decode_extra("decode_no_reuse_fp8", cs.decode_link(seed=args.seed, no_reuse=True), N, "linked",
                              wname="decode_no_reuse_fp8", kv_dtype=comb.KV_E4M3)
+            if want("prefill_fp8"):  # fp8 pool: dequantise the batch's distinct pages into bf16 staging, then the bf16 kernel
+                prefill_extra("rag_prefill_lq32_fp8", cs.rag_prefill(seed=args.seed, lq=32), min(N, 50), "linked",
+                              wname="rag_prefill_lq32_fp8", kv_dtype=comb.KV_E4M3)
             if want("rag_prefill_lq32"):
                 prefill_extra("rag_prefill_lq32", cs.rag_prefill(seed=args.seed, lq=32), N, "linked")
             # the paper's own regime (< 50 dynamic tokens) at a small batch: 32 work items for 148 SMs,

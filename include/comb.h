@@ -101,7 +101,8 @@ enum { COMB_KV_BF16 = 0, COMB_KV_E4M3 = 1 };
  *            softmax weights, the small operands, are each split into two e4m3 terms (hi + lo) so that side keeps
  *            bf16-level accuracy.  comb_cross_attn_prefill dequantises the batch's DISTINCT pages into bf16 staging in
  *            the workspace and runs the bf16 kernel on it (correct, not fast: prefill runs once per request, decode
- *            once per generated token).  comb_project_store_chunks and comb_pool_export return INVALID on fp8 pools. */
+ *            once per generated token); its workspace must be sized with comb_attn_workspace_bytes (the staging holds
+ *            link->distinct_pages pages).  comb_project_store_chunks and comb_pool_export return INVALID on fp8 pools. */
 size_t comb_pool_scale_bytes(const comb_pool_config_t *cfg); /* bytes of k_scale (= of v_scale); 0 for a bf16 pool */
 
 /* Sizes the caller must allocate for a config (pointers in cfg are ignored). */
@@ -263,6 +264,9 @@ typedef struct {
     int32_t *cas_row_indptr;
     int32_t *cas_row_req;
     int32_t *cas_row_entry;
+    int32_t *page_ids_compact;   /* fp8 pools only (NULL otherwise): int32 [total], entry i of page_ids as an index into
+                                    cas_page_ids (the batch's distinct pages) — the page table of the bf16 staging
+                                    that comb_cross_attn_prefill dequantises those pages into */
     /* out: host pointers into host_buf (NULL without one) */
     int32_t *host_req_pages;
     int32_t *host_cas_rows;

@@ -40,7 +40,7 @@ class Link(C.Structure):
                 ("entry_indptr", C.c_void_p),
                 ("cas_page_indptr", C.c_void_p), ("cas_page_ids", C.c_void_p), ("cas_tile_indptr", C.c_void_p),
                 ("cas_tile_ntok", C.c_void_p), ("cas_row_indptr", C.c_void_p), ("cas_row_req", C.c_void_p),
-                ("cas_row_entry", C.c_void_p),
+                ("cas_row_entry", C.c_void_p), ("page_ids_compact", C.c_void_p),
                 ("host_req_pages", C.c_void_p), ("host_cas_rows", C.c_void_p), ("host_cas_pages", C.c_void_p),
                 ("num_requests", C.c_int32), ("max_pages_per_request", C.c_int32),
                 ("total_pages", C.c_int64), ("total_tiles", C.c_int64), ("total_kv_tokens", C.c_int64),

@@ -246,11 +246,12 @@ int32_t dir_alloc(comb_pool_t *p, uint64_t id, int32_t T, const Chunk **out, boo
 struct LinkLayout {
     size_t off_page_indptr, off_kv_len, off_tile_indptr, off_entry_indptr, off_cas_page_indptr, off_cas_tile_indptr,
         off_cas_row_indptr, off_tile_ntok, off_cas_tile_ntok, off_page_ids, off_page_ntok, off_cas_page_ids,
-        off_cas_row_req, off_cas_row_entry, bytes;
+        off_cas_row_req, off_cas_row_entry, off_page_ids_compact, bytes;
 };
 
 // R requests, E entries, U distinct chunks with Pd pages and Tc tiles in all, P table entries, T tiles
-LinkLayout link_layout(int32_t R, int64_t E, int64_t U, int64_t P, int64_t T, int64_t Pd, int64_t Tc) {
+LinkLayout link_layout(int32_t R, int64_t E, int64_t U, int64_t P, int64_t T, int64_t Pd, int64_t Tc,
+                       bool compact = false) {
     LinkLayout L;
     size_t o = 0;
     auto take = [&](size_t elem, int64_t n) {
@@ -272,6 +273,8 @@ LinkLayout link_layout(int32_t R, int64_t E, int64_t U, int64_t P, int64_t T, in
     L.off_cas_page_ids = take(4, Pd);
     L.off_cas_row_req = take(4, E);
     L.off_cas_row_entry = take(4, E);
+    L.off_page_ids_compact = o;
+    if (compact) L.off_page_ids_compact = take(4, P);  // fp8 pools: the page table of the dequantised staging
     L.bytes = o;
     return L;
 }
@@ -438,6 +441,13 @@ int32_t plan_prefill(comb_pool *p, const comb_link_t *link, int32_t R, const int
         out->part_rows += (int64_t)eff * kPartRowsPerRange;
     }
     return COMB_OK;
+}
+
+// fp8 pools: bytes of the bf16 staging (K then V) that prefill dequantises `pages` distinct pages into
+size_t fp8_staging_bytes(const comb_pool *p, int64_t pages) {
+    const size_t per_page = (size_t)p->cfg.num_kv_heads * kPage * 2;
+    return align_up((size_t)std::max<int64_t>(pages, 1) * per_page * p->cfg.head_dim_qk, 1024) +
+           align_up((size_t)std::max<int64_t>(pages, 1) * per_page * p->cfg.head_dim_v, 1024);
 }
 
 // ---------------------------------------------------------------- chunk-major decode planning
@@ -922,7 +932,7 @@ size_t comb_link_bytes(int32_t R, int64_t E, int64_t total_pages) {
     if (R < 0 || E < 0 || total_pages < 0) return 0;
     // U <= E distinct chunks; their pages <= total_pages; a chunk's / request's last tile may be partly filled
     return link_layout(R, E, E, total_pages, total_pages / kTilePages + R + 1, total_pages,
-                       total_pages / kTilePages + E + 1).bytes;
+                       total_pages / kTilePages + E + 1, true).bytes;
 }
 
 size_t comb_link_host_bytes(int32_t R, int64_t E) {
@@ -999,7 +1009,8 @@ int32_t link_plan_impl(PoolT *p, int32_t R, const int32_t *chunk_indptr, const u
         distinct_tiles += ((int64_t)c->pages.size() + kTilePages - 1) / kTilePages;
         distinct_tok += c->num_tokens;
     }
-    const LinkLayout L = link_layout(R, E, U, total_pages, total_tiles, distinct_pages, distinct_tiles);
+    const bool compact = p->geom.kv_dtype == COMB_KV_E4M3;
+    const LinkLayout L = link_layout(R, E, U, total_pages, total_tiles, distinct_pages, distinct_tiles, compact);
     if (L.bytes > link->device_bytes) return COMB_ERR_CAPACITY;
     const size_t host_need = comb_link_host_bytes(R, U);
     if (link->host_buf && link->host_bytes < host_need) return COMB_ERR_CAPACITY;
@@ -1070,7 +1081,17 @@ int32_t link_plan_impl(PoolT *p, int32_t R, const int32_t *chunk_indptr, const u
                 fill[(size_t)u] += 1;
             }
     }
+    if (compact) {  // entry e's pages are pages cas_page_indptr[slot(e)] .. of the distinct-page list, in order
+        int32_t *pc = (int32_t *)(hb + L.off_page_ids_compact);
+        int64_t w = 0;
+        for (int64_t e = 0; e < E; ++e) {
+            const int32_t u = slot_of[(size_t)ent_slot[(size_t)e]];
+            const int32_t base = cas_page_indptr[u], np = cas_page_indptr[u + 1] - base;
+            for (int32_t j = 0; j < np; ++j) pc[w++] = base + j;
+        }
+    }
     char *db = (char *)link->device_buf;
+    link->page_ids_compact = compact ? (int32_t *)(db + L.off_page_ids_compact) : nullptr;
     link->page_indptr = (int32_t *)(db + L.off_page_indptr);
     link->kv_len = (int32_t *)(db + L.off_kv_len);
     link->tile_indptr = (int32_t *)(db + L.off_tile_indptr);
@@ -1202,6 +1223,8 @@ size_t comb_workspace_bytes(const comb_pool_t *p, int32_t R, int32_t Hq, int64_t
 size_t comb_attn_workspace_bytes(const comb_pool_t *p, const comb_link_t *link, int32_t Hq, int64_t total_q) {
     if (!p || !link || Hq <= 0 || total_q < 0) return 0;
     size_t need = comb_workspace_bytes(p, link->num_requests, Hq, total_q, link->max_pages_per_request);
+    if (p->geom.kv_dtype == COMB_KV_E4M3)  // prefill: bf16 staging of the batch's distinct pages behind the rest
+        need = align_up(need, 1024) + fp8_staging_bytes(p, link->distinct_pages);
     const int G = std::max(1, Hq / p->cfg.num_kv_heads);
     if (link->host_cas_rows && link->host_cas_pages && cascade_supported(G, p->cfg.head_dim_qk, p->cfg.head_dim_v)) {
         size_t units = 0;
@@ -1300,7 +1323,8 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     if (!q || !out || !link->page_indptr) return COMB_ERR_INVALID;
     const int Hkv = p->cfg.num_kv_heads, G = Hq / Hkv;
     if (!prefill_supported(G, p->cfg.head_dim_qk, p->cfg.head_dim_v)) return COMB_ERR_INVALID;
-    if (p->geom.kv_dtype != COMB_KV_BF16) return COMB_ERR_INVALID;
+    const bool fp8 = p->geom.kv_dtype == COMB_KV_E4M3;
+    if (fp8 && (!link->page_ids_compact || !link->cas_page_ids)) return COMB_ERR_INVALID;
     p->probe_device();
     PrefillPlan plan;
     int32_t rc = plan_prefill(p, link, R, q_indptr, Hq, &plan);
@@ -1309,16 +1333,41 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     if (num_items == 0) return COMB_OK;
     if (num_items > (size_t)INT32_MAX) return COMB_ERR_CAPACITY;
     const size_t items_bytes = prefill_items_bytes(num_items);
-    const size_t need = items_bytes + prefill_part_bytes(plan.part_rows, p->cfg.head_dim_v);
+    size_t need = items_bytes + prefill_part_bytes(plan.part_rows, p->cfg.head_dim_v);
+    const size_t stage_off = align_up(need, 1024);
+    if (fp8) need = stage_off + fp8_staging_bytes(p, link->distinct_pages);
     if (!ws || ws_bytes < need || (((uintptr_t)ws) & 15)) return COMB_ERR_CAPACITY;
     cudaStream_t st = (cudaStream_t)stream;
-    if (!p->kv_maps_ready) {
-        if (prefill_encode_kv_maps(p->geom, &p->k_map, &p->v_map) != cudaSuccess) return COMB_ERR_CUDA;
-        p->kv_maps_ready = true;
-    }
     PrefillMaps maps;
-    maps.k = p->k_map;
-    maps.v = p->v_map;
+    PoolGeom geom = p->geom;
+    LinkView lv = view_of(link);
+    int run_layer = layer;
+    if (fp8) {
+        // fp8 pool: dequantise the batch's distinct pages (exactly: the scales are powers of two) into a compact bf16
+        // pool in the workspace and attend over that through the link's compact page table
+        char *kst = (char *)ws + stage_off;
+        char *vst = kst + align_up((size_t)std::max<int64_t>(link->distinct_pages, 1) * p->cfg.num_kv_heads * kPage * 2 *
+                                   p->cfg.head_dim_qk, 1024);
+        if (launch_dequant_pages(p->geom, layer, link->cas_page_ids, (int)link->distinct_pages, kst, vst, st) != cudaSuccess)
+            return COMB_ERR_CUDA;
+        p->launches += 1;
+        geom.kv_dtype = 0;
+        geom.k_scale = geom.v_scale = nullptr;
+        geom.num_layers = 1;
+        geom.num_pages = (int32_t)std::max<int64_t>(link->distinct_pages, 1);
+        geom.k_arena = kst;
+        geom.v_arena = vst;
+        run_layer = 0;
+        lv.page_ids = link->page_ids_compact;
+        if (prefill_encode_kv_maps(geom, &maps.k, &maps.v) != cudaSuccess) return COMB_ERR_CUDA;
+    } else {
+        if (!p->kv_maps_ready) {
+            if (prefill_encode_kv_maps(p->geom, &p->k_map, &p->v_map) != cudaSuccess) return COMB_ERR_CUDA;
+            p->kv_maps_ready = true;
+        }
+        maps.k = p->k_map;
+        maps.v = p->v_map;
+    }
     if (prefill_encode_q_map(q, total_q, Hq, G, p->cfg.head_dim_qk, &maps.q) != cudaSuccess) return COMB_ERR_CUDA;
     const int slot = p->acquire(num_items * sizeof(PrefillItem));
     if (slot < 0) return COMB_ERR_CUDA;
@@ -1327,7 +1376,7 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     if (cudaMemcpyAsync(ws, h, num_items * sizeof(PrefillItem), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return COMB_ERR_CUDA;
     int launches = 0;
-    cudaError_t e = launch_prefill(p->geom, layer, view_of(link), maps, (const PrefillItem *)ws, (int)num_items, Hq,
+    cudaError_t e = launch_prefill(geom, run_layer, lv, maps, (const PrefillItem *)ws, (int)num_items, Hq,
                                    scale, out, lse, total_q, (char *)ws + items_bytes, plan.part_rows,
                                    plan.tiles_per_cta, p->num_sms, st, &launches, p->active_hook());
     if (e != cudaSuccess) return COMB_ERR_CUDA;

@@ -197,3 +197,60 @@ def test_fp8_pool_rejects_what_is_not_built():
         ld.pool.project_store_chunks([5], np.array([0, 64], np.int32), hs, wkv)
     assert e.value.status == comb.COMB_ERR_INVALID
     ld.pool.close()
+
+
+@pytest.mark.parametrize("heads", [(32, 8), (16, 16), (8, 1)])
+def test_fp8_prefill_over_dequantised_staging(heads):
+    """comb_cross_attn_prefill on an fp8 pool: the batch's distinct pages are dequantised (exactly) into bf16 staging
+    in the workspace and the bf16 kernel attends over it through the link's compact page table.  Ragged chunks, shared
+    chunks, an empty request, a duplicate link, query blocks of 1 .. 300 tokens (single-tile, two-tile and KV-range
+    plans); and row i of the prefill equals a decode of that row on the same pool (P11)."""
+    import paper_2602_01519_b200 as comb
+    Hq, Hkv = heads
+    lens = [300, 16, 1000, 77, 512, 33, 129, 2000]
+    links = [[0, 2, 4], [4, 0], [], [7], [1, 3, 5, 6], [2, 2], [4, 7, 0, 2]]
+    lq = [40, 1, 5, 300, 17, 130, 64]
+    w = cs.custom("pre8", k=8, num_q_heads=Hq, num_kv_heads=Hkv, head_dim_qk=128, head_dim_v=128, chunk_len=lens,
+                  links=links, lq=lq)
+    ld = H().load_workload(w, sentinel=BYTE_SENTINEL, kv_dtype=comb.KV_E4M3, shuffle_seed=7)
+    out, lse = ld.pool.prefill(ld.batch, ld.q, ld.q_indptr, w.scale)
+    torch.cuda.synchronize()
+    O, L = oracle.attention_for(Dequantised(w))
+    check(H().device_to_bits(out), lse.cpu().numpy().astype(np.float64), O, L, "prefill %s" % (heads,), 2e-4)
+    # the table the staging is read through: entry i of page_ids as an index into the distinct-page list
+    t = ld.batch.tables()
+    L_ = ld.batch.link
+    off = L_.page_ids_compact - ld.batch.buf.data_ptr()
+    compact = ld.batch.buf[off:off + 4 * int(L_.total_pages)].view(torch.int32).cpu().numpy()
+    assert np.array_equal(t["cas_page_ids"][compact], t["page_ids"])
+    # P11: the last row of request 3 as a decode over the same link list
+    r = 3
+    row = int(w.q_indptr[r + 1]) - 1
+    wd1 = cs.custom("pre8d", k=8, num_q_heads=Hq, num_kv_heads=Hkv, head_dim_qk=128, head_dim_v=128, chunk_len=lens,
+                    links=[links[r]], lq=[1])
+    lb = ld.pool.link([list(map(int, links[r]))])
+    o1, l1 = ld.pool.decode(lb, ld.q[row:row + 1].contiguous(), wd1.scale)
+    torch.cuda.synchronize()
+    a = cs.bf16_bits_to_f64(H().device_to_bits(out))[row]
+    b = cs.bf16_bits_to_f64(H().device_to_bits(o1))[0]
+    assert np.abs(a - b).max() <= 2.0 ** -7 * np.abs(a).max() + 1.5e-3
+    assert abs(float(lse[row].max()) - float(l1.max())) <= 2e-4
+    ld.pool.close()
+
+
+def test_fp8_full_size_rag_prefill_lq32_whole_requests():
+    """BASELINE configs[2] at lq = 32 (the paper's regime) on an fp8 pool, in bench.py's launch configuration: four
+    whole requests, every element."""
+    import paper_2602_01519_b200 as comb
+    w = cs.rag_prefill(seed=0, lq=32)
+    ld = H().load_workload(w, fill="linked", shuffle_seed=2024, keep_host=False, kv_dtype=comb.KV_E4M3)
+    out, lse = ld.pool.prefill(ld.batch, ld.q, ld.q_indptr, w.scale)
+    torch.cuda.synchronize()
+    got_o = H().device_to_bits(out)
+    got_l = lse.cpu().numpy().astype(np.float64)
+    wd = Dequantised(w)
+    for r in (0, 5, 17, w.num_requests - 1):
+        O, L = oracle.attention_for(wd, [r])
+        a, b = int(w.q_indptr[r]), int(w.q_indptr[r + 1])
+        check(got_o[a:b], got_l[a:b], O, L, "rag lq32 prefill, request %d" % r, 2e-4)
+    ld.pool.close()
