@@ -232,10 +232,10 @@ def run_reference(args):
     }), flush=True)
 
 
-KERNEL_CLASSES = (("cascade_decode_kernel", "decode_cascade"), ("cascade_merge_kernel", "cascade_merge"),
+KERNEL_CLASSES = (("cascade_decode_f8_kernel", "decode_cascade"), ("cascade_decode_kernel", "decode_cascade"), ("cascade_merge_kernel", "cascade_merge"),
                   ("decode_split_kernel", "decode_split"), ("decode_merge_kernel", "decode_merge"),
                   ("attn_core_kernel", "prefill"), ("prefill_merge_kernel", "prefill_merge"),
-                  ("store_pages_kernel", "store"), ("gemm_bf16_kernel<1", "gemm_paged"), ("gemm_bf16_kernel<0", "gemm"))
+                  ("store_pages_fp8_kernel", "store_fp8"), ("dequant_pages_kernel", "dequant"), ("store_pages_kernel", "store"), ("gemm_bf16_kernel<1", "gemm_paged"), ("gemm_bf16_kernel<0", "gemm"))
 
 
 def make_traffic_table(directory: str, last: int = 6):
@@ -264,7 +264,7 @@ def make_traffic_table(directory: str, last: int = 6):
                     by_class.setdefault(cls, []).append(launches[i])
                     break
         for cls, ls in by_class.items():
-            if cls == "store" and not workload.endswith("_chunks"):
+            if cls in ("store", "store_fp8") and not workload.endswith("_chunks"):
                 continue  # pool fills of the harness
             ls = ls[-last:]
             scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "ns": 1e-3, "us": 1.0, "ms": 1e3, "%": 1.0}

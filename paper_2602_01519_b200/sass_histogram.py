@@ -2,7 +2,7 @@
 
     python paper_2602_01519_b200/sass_histogram.py [path/to/libcomb.so]
 
-Build check for the Blackwell-only instructions: UTCHMMA (tcgen05.mma), UTCBAR (tcgen05.commit), LDTM / STTM
+Build check for the Blackwell-only instructions: UTCHMMA (tcgen05.mma kind::f16), UTCQMMA (kind::f8f6f4), UTCBAR (tcgen05.commit), LDTM / STTM
 (tcgen05.ld / st), UTMALDG (TMA tensor load), UBLKCP (1-D bulk copy), SYNCS (mbarrier), plus the arithmetic that
 dominates the CUDA-core paths. Needs cuobjdump and c++filt on PATH (CUDA toolkit, binutils); no GPU.
 """
@@ -14,7 +14,7 @@ import re
 import subprocess
 import sys
 
-COLS = ["UTCHMMA", "UTCBAR", "LDTM", "STTM", "UTMALDG", "UBLKCP", "SYNCS", "MUFU", "REDUX", "FFMA2", "FFMA", "F2FP",
+COLS = ["UTCHMMA", "UTCQMMA", "UTCBAR", "LDTM", "STTM", "UTMALDG", "UBLKCP", "SYNCS", "MUFU", "REDUX", "FFMA2", "FFMA", "F2FP",
         "LDS", "STS", "LDG", "STG", "ATOMG", "SHFL", "BAR"]
 
 
