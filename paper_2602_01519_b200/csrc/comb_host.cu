@@ -79,7 +79,7 @@ struct comb_pool {
     // (f4) CUDA IPC: an imported pool is read-only and owns the mappings it opened; an exporting pool owns one
     // interprocess event
     bool imported = false;
-    void *ipc_k_base = nullptr, *ipc_v_base = nullptr;
+    std::vector<std::pair<cudaIpcMemHandle_t, void *>> ipc_maps;  // allocations opened by comb_pool_import
     cudaEvent_t ipc_event = nullptr;
     void drop_ready(Chunk &c) {
         if (c.ready >= 0 && ready_events[(size_t)c.ready].users > 0) ready_events[(size_t)c.ready].users -= 1;
@@ -603,8 +603,7 @@ int32_t comb_pool_destroy(comb_pool_t *p) {
     for (auto &e : p->ready_events)
         if (e.ev) cudaEventDestroy(e.ev);
     if (p->ipc_event) cudaEventDestroy(p->ipc_event);
-    if (p->ipc_k_base) cudaIpcCloseMemHandle(p->ipc_k_base);
-    if (p->ipc_v_base && p->ipc_v_base != p->ipc_k_base) cudaIpcCloseMemHandle(p->ipc_v_base);
+    for (auto &m : p->ipc_maps) cudaIpcCloseMemHandle(m.second);
     for (auto &s : p->ring) {
         if (s.busy) cudaEventSynchronize(s.ev);
         if (s.ev) cudaEventDestroy(s.ev);
@@ -1437,6 +1436,10 @@ struct ExportHeader {
     uint64_t k_bytes, v_bytes, k_offset, v_offset;
     unsigned char k_handle[64], v_handle[64], ev_handle[64];
     uint64_t num_chunks, dir_bytes;
+    // fp8 pools: element type and the scale tables
+    int32_t kv_dtype, pad;
+    uint64_t ks_offset, vs_offset;
+    unsigned char ks_handle[64], vs_handle[64];
 };
 static_assert(sizeof(cudaIpcMemHandle_t) == 64 && sizeof(cudaIpcEventHandle_t) == 64, "CUDA IPC handles are 64 bytes");
 
@@ -1478,6 +1481,7 @@ int32_t parse_blob(const void *blob, size_t bytes, const ExportHeader **h, const
     c.head_dim_v = x->head_dim_v;
     c.page_size = x->page_size;
     c.num_pages = x->num_pages;
+    c.kv_dtype = x->kv_dtype;
     if (validate_cfg(&c) != COMB_OK) return COMB_ERR_INVALID;
     *h = x;
     *dir = (const unsigned char *)blob + sizeof(ExportHeader);
@@ -1536,7 +1540,6 @@ size_t comb_pool_export_bytes(const comb_pool_t *p) {
 
 int32_t comb_pool_export(comb_pool_t *p, uint32_t flags, void *stream, void *blob, size_t cap, size_t *written) {
     if (!p || !blob || (flags & ~(uint32_t)COMB_EXPORT_DIRECTORY_ONLY) || (((uintptr_t)blob) & 7)) return COMB_ERR_INVALID;
-    if (p->geom.kv_dtype != COMB_KV_BF16) return COMB_ERR_INVALID;  // the blob has no place for the scale tables
     const size_t dir_bytes = export_dir_bytes(p);
     if (cap < sizeof(ExportHeader) + dir_bytes) return COMB_ERR_CAPACITY;
     ExportHeader h;
@@ -1555,6 +1558,7 @@ int32_t comb_pool_export(comb_pool_t *p, uint32_t flags, void *stream, void *blo
     h.v_bytes = vb;
     h.num_chunks = p->dir.size();
     h.dir_bytes = dir_bytes;
+    h.kv_dtype = p->cfg.kv_dtype;
     if (!(flags & COMB_EXPORT_DIRECTORY_ONLY)) {
         if (p->imported) return COMB_ERR_READ_ONLY;  // only the owner of the arenas hands them out
         cudaStream_t st = (cudaStream_t)stream;
@@ -1567,6 +1571,17 @@ int32_t comb_pool_export(comb_pool_t *p, uint32_t flags, void *stream, void *blo
         memcpy(h.v_handle, &vh, 64);
         h.k_offset = (uint64_t)((char *)p->cfg.k_arena - (char *)kbase);
         h.v_offset = (uint64_t)((char *)p->cfg.v_arena - (char *)vbase);
+        if (p->cfg.kv_dtype == COMB_KV_E4M3) {
+            void *ksb = nullptr, *vsb = nullptr;
+            if (!allocation_base(p->cfg.k_scale, &ksb) || !allocation_base(p->cfg.v_scale, &vsb)) return COMB_ERR_CUDA;
+            cudaIpcMemHandle_t ksh, vsh;
+            if (cudaIpcGetMemHandle(&ksh, ksb) != cudaSuccess || cudaIpcGetMemHandle(&vsh, vsb) != cudaSuccess)
+                return COMB_ERR_CUDA;
+            memcpy(h.ks_handle, &ksh, 64);
+            memcpy(h.vs_handle, &vsh, 64);
+            h.ks_offset = (uint64_t)((char *)p->cfg.k_scale - (char *)ksb);
+            h.vs_offset = (uint64_t)((char *)p->cfg.v_scale - (char *)vsb);
+        }
         // every store enqueued so far precedes the event the importer waits for
         for (auto &re : p->ready_events)
             if (re.ev && re.users > 0 && cudaStreamWaitEvent(st, re.ev, 0) != cudaSuccess) return COMB_ERR_CUDA;
@@ -1615,19 +1630,24 @@ int32_t comb_pool_import(const void *blob, size_t bytes, void *stream, comb_pool
     if ((rc = read_directory(h, dir, &d)) != COMB_OK) return rc;
     comb_pool_t *p = new (std::nothrow) comb_pool();
     if (!p) return COMB_ERR_INVALID;
-    cudaIpcMemHandle_t kh, vh;
-    memcpy(&kh, h->k_handle, 64);
-    memcpy(&vh, h->v_handle, 64);
-    const bool same = memcmp(h->k_handle, h->v_handle, 64) == 0;  // both arenas inside one allocation
-    if (cudaIpcOpenMemHandle(&p->ipc_k_base, kh, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
-        delete p;
-        return COMB_ERR_CUDA;
-    }
-    if (same) {
-        p->ipc_v_base = p->ipc_k_base;
-    } else if (cudaIpcOpenMemHandle(&p->ipc_v_base, vh, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
-        cudaIpcCloseMemHandle(p->ipc_k_base);
-        delete p;
+    // open every distinct allocation once (several tables may live in one allocation of a caching allocator)
+    auto open = [&](const unsigned char *handle, uint64_t offset, void **out_ptr) -> bool {
+        for (auto &m : p->ipc_maps)
+            if (memcmp(&m.first, handle, 64) == 0) { *out_ptr = (char *)m.second + offset; return true; }
+        cudaIpcMemHandle_t mh;
+        memcpy(&mh, handle, 64);
+        void *base = nullptr;
+        if (cudaIpcOpenMemHandle(&base, mh, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) return false;
+        p->ipc_maps.emplace_back(mh, base);
+        *out_ptr = (char *)base + offset;
+        return true;
+    };
+    void *ka = nullptr, *va = nullptr, *ksa = nullptr, *vsa = nullptr;
+    bool ok = open(h->k_handle, h->k_offset, &ka) && open(h->v_handle, h->v_offset, &va);
+    if (ok && h->kv_dtype == COMB_KV_E4M3)
+        ok = open(h->ks_handle, h->ks_offset, &ksa) && open(h->vs_handle, h->vs_offset, &vsa);
+    if (!ok) {
+        comb_pool_destroy(p);
         return COMB_ERR_CUDA;
     }
     p->imported = true;
@@ -1637,12 +1657,19 @@ int32_t comb_pool_import(const void *blob, size_t bytes, void *stream, comb_pool
     p->cfg.head_dim_v = h->head_dim_v;
     p->cfg.page_size = h->page_size;
     p->cfg.num_pages = h->num_pages;
-    p->cfg.k_arena = (char *)p->ipc_k_base + h->k_offset;
-    p->cfg.v_arena = (char *)p->ipc_v_base + h->v_offset;
+    p->cfg.k_arena = ka;
+    p->cfg.v_arena = va;
     p->cfg.scratch = nullptr;
     p->cfg.free_list_shuffle_seed = 0;
+    p->cfg.kv_dtype = h->kv_dtype;
+    p->cfg.reserved = 0;
+    p->cfg.k_scale = ksa;
+    p->cfg.v_scale = vsa;
     p->geom = PoolGeom{h->num_layers, h->num_kv_heads, h->head_dim_qk, h->head_dim_v, h->num_pages, p->cfg.k_arena,
                        p->cfg.v_arena};
+    p->geom.kv_dtype = h->kv_dtype;
+    p->geom.k_scale = (float *)ksa;
+    p->geom.v_scale = (float *)vsa;
     p->dir.swap(d);
     p->next_seq = h->num_chunks;
     if ((rc = wait_remote_event(h, (cudaStream_t)stream)) != COMB_OK) {
@@ -1660,7 +1687,8 @@ int32_t comb_pool_refresh(comb_pool_t *p, const void *blob, size_t bytes, void *
     int32_t rc = parse_blob(blob, bytes, &h, &dir);
     if (rc != COMB_OK) return rc;
     if (h->num_layers != p->cfg.num_layers || h->num_kv_heads != p->cfg.num_kv_heads ||
-        h->head_dim_qk != p->cfg.head_dim_qk || h->head_dim_v != p->cfg.head_dim_v || h->num_pages != p->cfg.num_pages)
+        h->head_dim_qk != p->cfg.head_dim_qk || h->head_dim_v != p->cfg.head_dim_v || h->num_pages != p->cfg.num_pages ||
+        h->kv_dtype != p->cfg.kv_dtype)
         return COMB_ERR_INVALID;
     std::unordered_map<uint64_t, Chunk> d;
     if ((rc = read_directory(h, dir, &d)) != COMB_OK) return rc;

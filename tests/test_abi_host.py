@@ -401,14 +401,15 @@ def parse_export(blob: bytes):
     magic, version, flags = np.frombuffer(blob[:16], dtype=[("m", "<u8"), ("v", "<u4"), ("f", "<u4")])[0]
     geom = np.frombuffer(blob[16:40], dtype="<i4")
     n_chunks, dir_bytes = np.frombuffer(blob[264:280], dtype="<u8")
-    at, chunks = 280, []
+    HEAD = 280 + 8 + 16 + 128    # + kv_dtype, pad, two scale-table offsets and handles (fp8 pools)
+    at, chunks = HEAD, []
     for _ in range(int(n_chunks)):
         cid = int(np.frombuffer(blob[at:at + 8], "<u8")[0])
         T, npg = (int(x) for x in np.frombuffer(blob[at + 8:at + 16], "<i4"))
         pages = np.frombuffer(blob[at + 16:at + 16 + 4 * npg], "<i4").copy()
         at += 16 + (4 * npg + 7) // 8 * 8
         chunks.append((cid, T, pages))
-    assert at == 280 + int(dir_bytes) == len(blob)
+    assert at == HEAD + int(dir_bytes) == len(blob)
     return {"magic": int(magic), "version": int(version), "flags": int(flags), "geom": geom, "chunks": chunks}
 
 

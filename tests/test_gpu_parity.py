@@ -862,7 +862,8 @@ def test_eviction_under_memory_pressure_on_device():
     pool.close()
 
 
-def test_pool_export_import_across_processes(tmp_path):
+@pytest.mark.parametrize("kv_dtype", [0, 1])
+def test_pool_export_import_across_processes(tmp_path, kv_dtype):
     """(f4) PAPER.md:205: the PIC manager process owns the reserved memory, the engine process attends over it.  This
     process stores chunks and exports the pool; a child process imports it read-only over CUDA IPC, links and runs
     decode (both paths) and prefill on the exporter's bytes; a chunk stored later on a side stream becomes visible
@@ -874,7 +875,12 @@ def test_pool_export_import_across_processes(tmp_path):
     import ipc_child
     spec = ipc_child.SPEC
     w = cs.custom("ipc", links=ipc_child.LINKS_A, lq=[1, 1, 1], **spec)
-    pool = comb.Pool(8, 128, 128, w.pool_pages + 4, shuffle_seed=11, sentinel=SENTINEL)
+    pool = comb.Pool(8, 128, 128, w.pool_pages + 4, shuffle_seed=11, sentinel=SENTINEL, kv_dtype=kv_dtype)
+    if kv_dtype:   # fp8 pool (the blob carries the scale tables): the expectation is over the dequantised chunks
+        from test_gpu_fp8 import Dequantised
+        expect = lambda wl: oracle.attention_for(Dequantised(wl))  # noqa: E731
+    else:
+        expect = oracle.attention_for
     kv = [w.chunk_kv(c) for c in range(4)]
     dev = [(H().bits_to_device(k, "cuda"), H().bits_to_device(v, "cuda")) for k, v in kv]
     for c in range(3):
@@ -899,13 +905,13 @@ def test_pool_export_import_across_processes(tmp_path):
     assert res["pages0"].tolist() == comb.comb_chunk_query(pool.handle, 0)[1].tolist()
     assert res["status"].tolist() == [comb.COMB_ERR_READ_ONLY, comb.COMB_ERR_READ_ONLY, comb.COMB_ERR_UNKNOWN_CHUNK]
     f64 = lambda a: a.astype(np.float64)  # noqa: E731
-    O, L = oracle.attention_for(w)
+    O, L = expect(w)
     check_attention(res["dec_pr_o"], f64(res["dec_pr_l"]), O, L, tag="ipc decode per request")
     check_attention(res["dec_cm_o"], f64(res["dec_cm_l"]), O, L, tag="ipc decode chunk major")
     wp = cs.custom("ipc", links=ipc_child.LINKS_A, lq=[40, 130, 7], **spec)
-    check_attention(res["pre_o"], f64(res["pre_l"]), *oracle.attention_for(wp), tag="ipc prefill")
+    check_attention(res["pre_o"], f64(res["pre_l"]), *expect(wp), tag="ipc prefill")
     wd2 = cs.custom("ipc", links=ipc_child.LINKS_B, lq=[1, 1, 1], **spec)
-    check_attention(res["dec2_o"], f64(res["dec2_l"]), *oracle.attention_for(wd2), tag="ipc decode after refresh")
+    check_attention(res["dec2_o"], f64(res["dec2_l"]), *expect(wd2), tag="ipc decode after refresh")
     wp2 = cs.custom("ipc", links=ipc_child.LINKS_B, lq=[9, 200, 33], **spec)
-    check_attention(res["pre2_o"], f64(res["pre2_l"]), *oracle.attention_for(wp2), tag="ipc prefill after refresh")
+    check_attention(res["pre2_o"], f64(res["pre2_l"]), *expect(wp2), tag="ipc prefill after refresh")
     pool.close()
