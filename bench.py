@@ -635,9 +635,10 @@ def main():
                 decode_extra("decode_no_reuse_chunk_major", cs.decode_link(seed=args.seed, no_reuse=True), N, "linked",
                              path="chunk_major", wname="decode_no_reuse")
             # (f4) fp8 pools: the same batches over e4m3 pages (bytes counted as stored: codes + scales)
-            if want("decode_fp8"):
+            if want("decode_link_fp8"):
                 decode_extra("decode_link_fp8", cs.decode_link(seed=args.seed), N, "linked", wname="decode_link_fp8",
                              kv_dtype=comb.KV_E4M3)
+            if want("decode_no_reuse_fp8"):
                 decode_extra("decode_no_reuse_fp8", cs.decode_link(seed=args.seed, no_reuse=True), N, "linked",
                              wname="decode_no_reuse_fp8", kv_dtype=comb.KV_E4M3)
             if want("prefill_fp8"):  # fp8 pool: dequantise the batch's distinct pages into bf16 staging, then the bf16 kernel
