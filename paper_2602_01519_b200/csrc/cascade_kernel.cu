@@ -583,13 +583,17 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
 // =====================================================================================================================
 struct F8Cfg {
     static constexpr int SLOT = 128 * 128;                  // [128 keys][128 bytes] of a K or V tile
-    static constexpr int NSLOT = 8;
-    static constexpr int Q_BYTES = 2 * kRowsMax * 128;      // [hi 32 rows | lo 32 rows][128 bytes]
+    static constexpr int ROWS = 16;                         // query rows per item (8 or 16): N = 16 / 32 MMA columns
+    static constexpr int NSLOT = 4;                         // per CTA; two CTAs share an SM
+    static constexpr int Q_BYTES = 2 * ROWS * 128;          // [hi 16 rows | lo 16 rows][128 bytes]
     static constexpr int P_BYTES = 128 * 128;               // [128 keys][hi rows | lo rows, 128-byte pitch]: MN-major B
     static constexpr int MISC = 3072;
     static constexpr int SMEM = 1024 + 2 * Q_BYTES + P_BYTES + NSLOT * SLOT + MISC;
     static constexpr int THREADS = 256;
-    static constexpr int TMEM_COLS = 256;                   // S^T x2 @0,64; O^T x2 @128,192 (2 N columns each)
+    static constexpr int TMEM_COLS = 128;                   // S^T x2 @0,32; O^T x2 @64,96 (2 N columns each)
+    // Two CTAs per SM (their per-item bubbles — Q split, first loads, epilogue — hide under each other's tiles):
+    // 128 registers per thread on average, moved by setmaxnreg: 128 x 168 (softmax) + 128 x 88 (the rest) = 256 x 128
+    static constexpr int REG_SOFTMAX = 168, REG_OTHER = 88;
 };
 
 __device__ __forceinline__ float pow2_scale_for(float amax) {  // smallest 2^e with amax <= 448 * 2^e, e in [-100, 100]
@@ -635,7 +639,7 @@ __device__ __forceinline__ void softmax_item_f8(const CascadeArgs &a, Misc *mi, 
         uint32_t r[2 * NC];
 #pragma unroll
         for (int q = 0; q < 2 * NC / 16; ++q)
-            ptx::tmem_ld16(tmem + lane_base + sb * 64 + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&r[q * 16]));
+            ptx::tmem_ld16(tmem + lane_base + sb * 32 + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&r[q * 16]));
         const float ksc = mi->kscale[t & 7][kp], vsc = key_valid ? mi->vscale[t & 7][kp] : 0.f;
         ptx::tmem_wait_ld();
         ptx::tc_fence_before();
@@ -685,7 +689,7 @@ __device__ __forceinline__ void softmax_item_f8(const CascadeArgs &a, Misc *mi, 
                 uint32_t o[2 * NC];
 #pragma unroll
                 for (int q = 0; q < 2 * NC / 16; ++q)
-                    ptx::tmem_ld16(tmem + lane_base + 128 + ip * 64 + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
+                    ptx::tmem_ld16(tmem + lane_base + 64 + ip * 32 + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
                 ptx::tmem_wait_ld();
 #pragma unroll
                 for (int n = 0; n < NC; ++n) {
@@ -698,7 +702,7 @@ __device__ __forceinline__ void softmax_item_f8(const CascadeArgs &a, Misc *mi, 
                 }
 #pragma unroll
                 for (int q = 0; q < 2 * NC / 16; ++q)
-                    ptx::tmem_st16(tmem + lane_base + 128 + ip * 64 + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
+                    ptx::tmem_st16(tmem + lane_base + 64 + ip * 32 + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
                 ptx::tmem_wait_st();
                 ptx::tc_fence_before();
             } else {
@@ -749,7 +753,7 @@ __device__ __forceinline__ void softmax_item_f8(const CascadeArgs &a, Misc *mi, 
     uint32_t o[2 * NC];
 #pragma unroll
     for (int q = 0; q < 2 * NC / 16; ++q)
-        ptx::tmem_ld16(tmem + lane_base + 128 + ip * 64 + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
+        ptx::tmem_ld16(tmem + lane_base + 64 + ip * 32 + q * 16, *reinterpret_cast<uint32_t(*)[16]>(&o[q * 16]));
     ptx::tmem_wait_ld();
     ptx::tc_fence_before();
     __syncwarp();
@@ -776,7 +780,7 @@ __device__ __forceinline__ void softmax_item_f8(const CascadeArgs &a, Misc *mi, 
     }
 }
 
-__global__ void __launch_bounds__(256, 1)
+__global__ void __launch_bounds__(256, 2)
 cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) {
     using C = F8Cfg;
     extern __shared__ unsigned char smem_raw[];
@@ -809,8 +813,8 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
         for (int s = 0; s < C::NSLOT; ++s) {
             ptx::mbar_init(&mi->kv_full[s], 1);
             ptx::mbar_init(&mi->kv_empty[s], 1);
-            ptx::mbar_init(&mi->sc_full[s], 1);
         }
+        for (int s = 0; s < 8; ++s) ptx::mbar_init(&mi->sc_full[s], 1);
         ptx::fence_barrier_init();
         ptx::tma_prefetch_desc(&maps.k);
         ptx::tma_prefetch_desc(&maps.v);
@@ -824,6 +828,11 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
     ptx::tc_fence_after();
     const uint32_t tmem = mi->tmem_slot;
     const int G = a.group, Hq = a.num_q_heads, Hkv = a.num_kv_heads;
+    if (warp < 4) {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::REG_SOFTMAX));
+    } else {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::REG_OTHER));
+    }
 
     if (warp < 4) {
         // ===================== softmax + epilogue =====================
@@ -842,8 +851,7 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             }
             ptx::mbar_wait(&mi->q_full[k & 1], (k >> 1) & 1);  // the item's Q scale is written with its Q tile
             if (it.ncols == 8) softmax_item_f8<8>(a, mi, sP, tmem, it, k, t);
-            else if (it.ncols == 16) softmax_item_f8<16>(a, mi, sP, tmem, it, k, t);
-            else softmax_item_f8<32>(a, mi, sP, tmem, it, k, t);
+            else softmax_item_f8<16>(a, mi, sP, tmem, it, k, t);
         }
     } else if (warp == 4 || warp == 7) {
         // ===================== K/V TMA loaders + page scales =====================
@@ -927,7 +935,7 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             const int ksteps = (pd.pages + 1) >> 1;  // 32 keys (two pages) per k-step
             for (int ks = 0; ks < ksteps; ++ks)
                 if (leader)
-                    ptx::mma_ss_f8(tmem + 128 + pd.ip * 64, dv0 + (uint64_t)((slot * C::SLOT + ks * 4096) >> 4),
+                    ptx::mma_ss_f8(tmem + 64 + pd.ip * 32, dv0 + (uint64_t)((slot * C::SLOT + ks * 4096) >> 4),
                                    dpm + (uint64_t)((ks * 4096) >> 4), pd.idesc, (pd.first && ks == 0) ? 0u : 1u);
             if (leader) {
                 ptx::mma_commit(&mi->p_empty);
@@ -958,7 +966,7 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
 #pragma unroll
                 for (int kk = 0; kk < 4; ++kk)  // 32 dims per k-step
                     if (leader)
-                        ptx::mma_ss_f8(tmem + sb * 64, dk + (uint64_t)((kk * 32) >> 4), dq + (uint64_t)((kk * 32) >> 4),
+                        ptx::mma_ss_f8(tmem + sb * 32, dk + (uint64_t)((kk * 32) >> 4), dq + (uint64_t)((kk * 32) >> 4),
                                        idesc_s, kk > 0);
                 if (leader) {
                     ptx::mma_commit(&mi->s_full[sb]);
@@ -990,7 +998,7 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             const CascadeItem ci = a.items[unit];
             if (lane == 0) idx = atomicAdd(a.counter, 1u);
             const int rows_valid = ci.nrows * G;
-            const int ncols = rows_valid <= 8 ? 8 : (rows_valid <= 16 ? 16 : 32);
+            const int ncols = rows_valid <= 8 ? 8 : 16;
             if (lane == 0) {
                 ItemEntry e;
                 e.valid = 1;
@@ -1014,11 +1022,11 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             if (lane < ci.nrows && kvh == 0 && (ci.range_nr & 0xff) == 0)
                 a.ent_info[a.cas_row_entry[ci.row0 + lane]] = make_int4(ci.part0 + lane, ci.part_stride, ci.range_nr >> 8, 0);
             const int qb = k & 1;
-            uint4 val[16];
+            uint4 val[8];
             __nv_bfloat162 am2 = __floats2bfloat162_rn(0.f, 0.f);
 #pragma unroll
-            for (int x = 0; x < 16; ++x) {
-                if (2 * x < ncols) {  // uniform: an item has 16 or 32 row slots
+            for (int x = 0; x < 8; ++x) {
+                if (2 * x < ncols) {  // uniform: an item has 8 or 16 row slots
                     const int row = 2 * x + (lane >> 4), j = lane & 15;
                     const int e_pos = row >> a.group_shift, hh = row & (G - 1);
                     const int qrow = __shfl_sync(0xffffffffu, req_lane, e_pos & 31);
@@ -1037,7 +1045,7 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
             ptx::mbar_wait(&mi->q_empty[qb], ((k >> 1) & 1) ^ 1);
             unsigned char *dstq = sQ + qb * F8Cfg::Q_BYTES;
 #pragma unroll
-            for (int x = 0; x < 16; ++x) {
+            for (int x = 0; x < 8; ++x) {
                 const int row = 2 * x + (lane >> 4), j = lane & 15;
                 if (2 * x < ncols) {
                     const uint32_t w[4] = {val[x].x, val[x].y, val[x].z, val[x].w};
@@ -1212,7 +1220,7 @@ cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &
         if (a.num_items > 0) {
             e = cudaFuncSetAttribute(cascade_decode_f8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, F8Cfg::SMEM);
             if (e == cudaSuccess) {
-                const int grid = a.num_items < num_sms ? a.num_items : num_sms;
+                const int grid = a.num_items < 2 * num_sms ? a.num_items : 2 * num_sms;  // two CTAs per SM
                 cascade_decode_f8_kernel<<<grid, F8Cfg::THREADS, F8Cfg::SMEM, stream>>>(a, maps);
                 e = cudaGetLastError();
             }

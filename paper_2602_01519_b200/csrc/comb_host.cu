@@ -462,11 +462,11 @@ constexpr int kCascadeMaxRanges = 64;
 
 // units == nullptr: sizes only (what comb_attn_workspace_bytes needs).
 int32_t plan_cascade(const comb_link_t *link, int G, int Hkv, int num_sms, std::vector<CascadeItem> *units,
-                     size_t *num_units, int64_t *num_partials) {
+                     size_t *num_units, int64_t *num_partials, int rows_per_item = kCascadeRows) {
     const int32_t U = link->num_distinct_chunks;
     const int32_t *rows = link->host_cas_rows, *pages = link->host_cas_pages;
-    if (!rows || !pages || G < 1 || G > kCascadeRows) return COMB_ERR_INVALID;
-    const int per_unit = kCascadeRows / G;
+    if (!rows || !pages || G < 1 || G > rows_per_item) return COMB_ERR_INVALID;
+    const int per_unit = rows_per_item / G;  // 32 query rows per item (16 in the fp8 kernel)
     int64_t sum = 0, psum = 0, work = 0;
     int32_t mx = 0;
     for (int32_t u = 0; u < U; ++u) {
@@ -1228,7 +1228,8 @@ size_t comb_attn_workspace_bytes(const comb_pool_t *p, const comb_link_t *link, 
     if (link->host_cas_rows && link->host_cas_pages && cascade_supported(G, p->cfg.head_dim_qk, p->cfg.head_dim_v)) {
         size_t units = 0;
         int64_t partials = 0;
-        if (plan_cascade(link, G, p->cfg.num_kv_heads, p->num_sms, nullptr, &units, &partials) == COMB_OK)
+        if (plan_cascade(link, G, p->cfg.num_kv_heads, p->num_sms, nullptr, &units, &partials,
+                         p->geom.kv_dtype == COMB_KV_E4M3 ? 16 : kCascadeRows) == COMB_OK)
             need = std::max(need, cascade_layout(units, link->total_entries, partials, Hq, p->cfg.head_dim_v).bytes + 256);
     }
     return need;
@@ -1263,7 +1264,8 @@ int32_t comb_cross_attn_decode(comb_pool_t *p, int32_t layer, const comb_link_t 
         std::vector<CascadeItem> units;
         size_t num_units = 0;
         int64_t partials = 0;
-        int32_t rc = plan_cascade(link, G, p->cfg.num_kv_heads, p->num_sms, &units, &num_units, &partials);
+        int32_t rc = plan_cascade(link, G, p->cfg.num_kv_heads, p->num_sms, &units, &num_units, &partials,
+                                  fp8 ? 16 : kCascadeRows);
         if (rc != COMB_OK) return rc;
         const CascadeLayout lay = cascade_layout(num_units, link->total_entries, partials, Hq, p->cfg.head_dim_v);
         if (!ws || ws_bytes < lay.bytes || (((uintptr_t)ws) & 15)) {
