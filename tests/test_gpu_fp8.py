@@ -251,3 +251,57 @@ def test_fp8_full_size_rag_prefill_lq32_whole_requests():
         a, b = int(w.q_indptr[r]), int(w.q_indptr[r + 1])
         check(got_o[a:b], got_l[a:b], O, L, "rag lq32 prefill, request %d" % r, 2e-4)
     ld.pool.close()
+
+
+def test_fp8_layers_and_the_sublayer():
+    """L = 3 layers over one page-id space on an fp8 pool (codes AND scale tables are per layer), each layer's prefill
+    and decode against the oracle over that layer's dequantised chunks; then comb_cross_layer_forward (Eq. 4, 7-8,
+    PAPER.md:117) on layer 1 against the fp64 sub-layer oracle fed the dequantised K/V."""
+    from dataclasses import replace
+    import paper_2602_01519_b200 as comb
+    from oracle import layer as ol
+    base = cs.custom("lay8", k=8, num_q_heads=8, num_kv_heads=2, head_dim_qk=128, head_dim_v=128,
+                     chunk_len=[130, 17, 512, 64], links=[[2, 0, 1], [3, 1], [], [1, 2]], lq=[40, 7, 3, 9])
+    ws = [replace(base, seed=200 + l) for l in range(3)]
+    pool = comb.Pool(2, 128, 128, base.pool_pages, num_layers=3, shuffle_seed=21, sentinel=BYTE_SENTINEL,
+                     kv_dtype=comb.KV_E4M3)
+    ids = list(range(base.num_chunks))
+    tok = np.zeros(base.num_chunks + 1, np.int32)
+    np.cumsum(base.chunk_len, out=tok[1:])
+    for l in (2, 0, 1):
+        kv = [ws[l].chunk_kv(c) for c in ids]
+        pool.store_chunks(ids, tok, H().bits_to_device(np.concatenate([k for k, _ in kv]), "cuda"),
+                          H().bits_to_device(np.concatenate([v for _, v in kv]), "cuda"), layer=l)
+    batch = pool.link([list(map(int, x)) for x in base.links])
+    for l in range(3):
+        q = H().bits_to_device(ws[l].all_q(), "cuda")
+        out, lse = pool.prefill(batch, q, base.q_indptr, base.scale, layer=l)
+        torch.cuda.synchronize()
+        check(H().device_to_bits(out), lse.cpu().numpy().astype(np.float64), *oracle.attention_for(Dequantised(ws[l])),
+              "prefill layer %d" % l, 2e-4)
+        wd = ws[l].decode_phase()
+        outd, lsed = pool.decode(batch, H().bits_to_device(wd.all_q(), "cuda"), wd.scale, layer=l)
+        torch.cuda.synchronize()
+        check(H().device_to_bits(outd), lsed.cpu().numpy().astype(np.float64), *oracle.attention_for(Dequantised(wd)),
+              "decode layer %d" % l, 2e-4)
+    # the sub-layer on layer 1, prefill and decode rows
+    d_model, Hq, Hkv, D = 256, 8, 2, 128
+    wq = cs.projection_weight(5, 1, 1, Hq * D, d_model)
+    wo = cs.projection_weight(5, 2, 1, d_model, Hq * D, gain=0.1)
+    wl = Dequantised(ws[1])
+    kd = [cs.bf16_bits_to_f64(wl.chunk_kv(c)[0]) for c in ids]
+    vd = [cs.bf16_bits_to_f64(wl.chunk_kv(c)[1]) for c in ids]
+    for q_indptr, rows in ((base.q_indptr, int(base.total_q)), (None, base.num_requests)):
+        x = cs.hidden_states(9, 0 if q_indptr is not None else 1, rows, d_model)
+        xd = H().bits_to_device(x, "cuda")
+        y = pool.layer_forward(batch, xd, q_indptr, H().bits_to_device(wq, "cuda"), H().bits_to_device(wo, "cuda"),
+                               base.scale, layer=1)
+        torch.cuda.synchronize()
+        ind = q_indptr if q_indptr is not None else np.arange(base.num_requests + 1, dtype=np.int32)
+        want = ol.cross_layer(cs.bf16_bits_to_f64(x), ind, cs.bf16_bits_to_f64(wq), cs.bf16_bits_to_f64(wo), Hq, kd, vd,
+                              [list(map(int, l)) for l in base.links], base.scale)
+        got = cs.bf16_bits_to_f64(H().device_to_bits(y))
+        rel = math.sqrt(float(((got - want) ** 2).sum()) / float((want ** 2).sum()))
+        assert rel <= 1e-2, "sub-layer on an fp8 pool: rel L2 %.3e" % rel
+        assert np.abs(got - want).max() <= 2.0 ** -6 * np.abs(want).max()
+    pool.close()
