@@ -102,8 +102,10 @@ enum { COMB_KV_BF16 = 0, COMB_KV_E4M3 = 1 };
  *            bf16-level accuracy.  comb_cross_attn_prefill dequantises the batch's DISTINCT pages into bf16 staging in
  *            the workspace and runs the bf16 kernel on it (correct, not fast: prefill runs once per request, decode
  *            once per generated token); its workspace must be sized with comb_attn_workspace_bytes (the staging holds
- *            link->distinct_pages pages).  comb_project_store_chunks returns INVALID on fp8 pools (the paged GEMM epilogue
- *            writes bf16 pages only); comb_pool_export carries the scale tables along. */
+ *            link->distinct_pages pages).  comb_project_store_chunks quantises in the GEMM's epilogue (the values a bf16
+ *            pool would hold, bf16_rne of the fp32 accumulators, go through the store's rule; 256-column tiles so that
+ *            a head's 128 columns and a page's 16 rows meet in one half-warp); comb_pool_export carries the scale
+ *            tables along. */
 size_t comb_pool_scale_bytes(const comb_pool_config_t *cfg); /* bytes of k_scale (= of v_scale); 0 for a bf16 pool */
 
 /* Sizes the caller must allocate for a config (pointers in cfg are ignored). */

@@ -857,7 +857,6 @@ int32_t comb_project_store_chunks(comb_pool_t *p, int32_t layer, int32_t n, cons
                                   void *stream) {
     if (n > 0 && (!h_packed || !w_kv)) return COMB_ERR_INVALID;
     if (!p || d_model <= 0 || d_model % 8) return COMB_ERR_INVALID;
-    if (p->geom.kv_dtype != COMB_KV_BF16) return COMB_ERR_INVALID;  // the paged epilogue writes bf16 pages only
     const int32_t N = p->cfg.num_kv_heads * (p->cfg.head_dim_qk + p->cfg.head_dim_v);
     StoreBatch sb;
     int32_t rc = store_begin(p, layer, n, ids, tok_indptr, &sb);

@@ -13,6 +13,7 @@
 
 #include <cuda.h>
 #include <cuda_bf16.h>
+#include <cuda_fp8.h>
 #include <cstring>
 
 namespace comb {
@@ -31,7 +32,7 @@ struct GemmCfg {
     static constexpr int SMEM = 1024 + STAGES * STAGE_BYTES + 256;
 };
 
-enum { kEpiRowMajor = 0, kEpiPaged = 1 };
+enum { kEpiRowMajor = 0, kEpiPaged = 1, kEpiPagedF8 = 2 };
 
 struct GemmArgs {
     int64_t M;
@@ -42,7 +43,8 @@ struct GemmArgs {
     const __nv_bfloat16 *residual;
     // paged epilogue
     const GemmRowTile *row_tiles;
-    char *k_layer, *v_layer;   // this layer's arenas: bf16 [num_pages][Hkv][16][D]
+    char *k_layer, *v_layer;   // this layer's arenas: bf16 (or e4m3 bytes) [num_pages][Hkv][16][D]
+    float *k_scale, *v_scale;  // fp8 pools: this layer's scale tables [num_pages][Hkv]
     int hkv, dqk, dv;
 };
 
@@ -92,7 +94,7 @@ gemm_bf16_kernel(const GemmArgs g, const __grid_constant__ GemmMaps maps) {
         for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
             const int mt = tile / g.num_n_tiles, nt = tile - mt * g.num_n_tiles;
             int a_row0 = mt * BM;
-            if constexpr (EPI == kEpiPaged) a_row0 = g.row_tiles[mt].a_row0;
+            if constexpr (EPI != kEpiRowMajor) a_row0 = g.row_tiles[mt].a_row0;
             for (int kb = 0; kb < num_kb; ++kb) {
                 ptx::mbar_wait(&empty[stage], phase ^ 1);
                 if (lane == 0) {
@@ -139,6 +141,7 @@ gemm_bf16_kernel(const GemmArgs g, const __grid_constant__ GemmMaps maps) {
             const int mt = tile / g.num_n_tiles, nt = tile - mt * g.num_n_tiles;
             // ---- where this thread's row goes ----
             bool store_row = false, zero_row = false;
+            int page = -1;
             char *dst_k = nullptr, *dst_v = nullptr;           // paged: (page, head 0, slot) of the row in each arena
             __nv_bfloat16 *dst_c = nullptr;
             const __nv_bfloat16 *res = nullptr;
@@ -149,16 +152,73 @@ gemm_bf16_kernel(const GemmArgs g, const __grid_constant__ GemmMaps maps) {
                 res = g.residual ? g.residual + grow * g.N : nullptr;
             } else {
                 const GemmRowTile rt = g.row_tiles[mt];
-                const int page = rt.pages[row >> 4];
+                page = rt.pages[row >> 4];
                 zero_row = row >= rt.rows_valid && row < rt.rows_zero_to;
                 store_row = (row < rt.rows_valid || zero_row) && page >= 0;
                 const int slot = row & 15;
-                dst_k = g.k_layer + (((size_t)page * g.hkv) * kPage + slot) * (size_t)g.dqk * 2;
-                dst_v = g.v_layer + (((size_t)page * g.hkv) * kPage + slot) * (size_t)g.dv * 2;
+                constexpr size_t ELT = EPI == kEpiPagedF8 ? 1 : 2;
+                dst_k = g.k_layer + (((size_t)page * g.hkv) * kPage + slot) * (size_t)g.dqk * ELT;
+                dst_v = g.v_layer + (((size_t)page * g.hkv) * kPage + slot) * (size_t)g.dv * ELT;
             }
             ptx::mbar_wait(&acc_full[acc], acc_phase);
             ptx::tc_fence_after();
             const uint32_t tacc = tmem + lane_base + acc * BN;
+            if constexpr (EPI == kEpiPagedF8) {
+                // fp8 pool (include/comb.h "fp8 pools"): a 128-column group is one head; the 16 rows of a page sit in
+                // one half-warp.  Per (page, head) block: the values the bf16 pool would hold (bf16_rne of the
+                // accumulators; rows past the chunk's length count as zero), their amax over the half-warp, the
+                // power-of-two scale, e4m3 codes, 128-byte rows.
+#pragma unroll 1
+                for (int hb = 0; hb < BN / 128; ++hb) {
+                    uint32_t r[128];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        ptx::tmem_ld32(tacc + hb * 128 + q * 32, *reinterpret_cast<uint32_t(*)[32]>(&r[q * 32]));
+                    ptx::tmem_wait_ld();
+                    const int col0 = nt * BN + hb * 128;
+                    const bool live = store_row && !zero_row && col0 < g.N;
+                    float amax = 0.f;
+#pragma unroll
+                    for (int e = 0; e < 128; ++e) {
+                        const float x = live ? __bfloat162float(__float2bfloat16_rn(__uint_as_float(r[e]))) : 0.f;
+                        r[e] = __float_as_uint(x);
+                        amax = fmaxf(amax, fabsf(x));
+                    }
+#pragma unroll
+                    for (int off = 8; off >= 1; off >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, off));
+                    float scale = 1.f;
+                    if (amax > 0.f) {  // smallest 2^e with amax <= 448 * 2^e, e in [-100, 100]
+                        const uint32_t bits = __float_as_uint(amax);
+                        int e = (int)(bits >> 23) - 127 - 8 + ((bits & 0x7fffffu) > 0x600000u ? 1 : 0);
+                        if ((bits >> 23) == 0) e = -100;
+                        e = e < -100 ? -100 : (e > 100 ? 100 : e);
+                        scale = __uint_as_float((uint32_t)(e + 127) << 23);
+                    }
+                    const float inv = 1.f / scale;
+                    if (store_row && col0 < g.N) {
+                        const int nk = g.hkv * g.dqk;
+                        const bool is_k = col0 < nk;
+                        const int head = is_k ? col0 / g.dqk : (col0 - nk) / g.dv;
+                        uint4 *dst = reinterpret_cast<uint4 *>((is_k ? dst_k : dst_v) + (size_t)head * kPage * 128);
+#pragma unroll
+                        for (int v = 0; v < 8; ++v) {
+                            uint32_t w[4];
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) {
+                                const int e = v * 16 + j * 4;
+                                const uint32_t a = (uint32_t)__nv_cvt_float2_to_fp8x2(
+                                    make_float2(__uint_as_float(r[e]) * inv, __uint_as_float(r[e + 1]) * inv), __NV_SATFINITE, __NV_E4M3);
+                                const uint32_t b = (uint32_t)__nv_cvt_float2_to_fp8x2(
+                                    make_float2(__uint_as_float(r[e + 2]) * inv, __uint_as_float(r[e + 3]) * inv), __NV_SATFINITE, __NV_E4M3);
+                                w[j] = a | (b << 16);
+                            }
+                            dst[v] = make_uint4(w[0], w[1], w[2], w[3]);
+                        }
+                        if ((lane & 15) == 0) (is_k ? g.k_scale : g.v_scale)[(size_t)page * g.hkv + head] = scale;
+                    }
+                    __syncwarp();
+                }
+            } else {
 #pragma unroll 1
             for (int cb = 0; cb < BN / 32; ++cb) {
                 uint32_t r[32];
@@ -207,6 +267,7 @@ gemm_bf16_kernel(const GemmArgs g, const __grid_constant__ GemmMaps maps) {
                 }
                 }
                 __syncwarp();  // the next tcgen05.ld is warp-collective
+            }
             }
             ptx::tc_fence_before();  // our TMEM reads precede the arrive that lets the next tile overwrite the buffer
             __syncwarp();
@@ -282,7 +343,9 @@ cudaError_t launch_gemm_paged(const GemmProblem &p, const PoolGeom &pg, int laye
                               int num_tiles, int num_sms, cudaStream_t stream) {
     if (!gemm_shape_ok(p.M, p.N, p.K) || !p.a || !p.w || !tiles_dev) return cudaErrorInvalidValue;
     if (p.N != pg.num_kv_heads * (pg.head_dim_qk + pg.head_dim_v)) return cudaErrorInvalidValue;
-    const int bn = pick_bn(num_tiles, p.N, num_sms);
+    // fp8 pools: a head's 128 columns must sit in one N tile (its amax spans them) -> 256-column tiles only
+    const int bn = pg.kv_dtype == 1 ? 256 : pick_bn(num_tiles, p.N, num_sms);
+    if (pg.kv_dtype == 1 && (pg.head_dim_qk != 128 || pg.head_dim_v != 128)) return cudaErrorInvalidValue;
     GemmMaps maps;
     cudaError_t e = encode_maps(p, bn, &maps);
     if (e != cudaSuccess) return e;
@@ -292,12 +355,19 @@ cudaError_t launch_gemm_paged(const GemmProblem &p, const PoolGeom &pg, int laye
     g.K = p.K;
     g.num_m_tiles = num_tiles;
     g.row_tiles = tiles_dev;
-    const size_t kb = (size_t)kPage * pg.head_dim_qk * 2, vb = (size_t)kPage * pg.head_dim_v * 2;
+    const size_t kb = (size_t)kPage * pg.head_dim_qk * pg.elt_bytes(), vb = (size_t)kPage * pg.head_dim_v * pg.elt_bytes();
     g.k_layer = (char *)pg.k_arena + (size_t)layer * pg.num_pages * pg.num_kv_heads * kb;
     g.v_layer = (char *)pg.v_arena + (size_t)layer * pg.num_pages * pg.num_kv_heads * vb;
     g.hkv = pg.num_kv_heads;
     g.dqk = pg.head_dim_qk;
     g.dv = pg.head_dim_v;
+    if (pg.kv_dtype == 1) {
+        const size_t blocks = (size_t)pg.num_pages * pg.num_kv_heads;
+        g.k_scale = pg.k_scale + (size_t)layer * blocks;
+        g.v_scale = pg.v_scale + (size_t)layer * blocks;
+        g.num_n_tiles = (g.N + 255) / 256;
+        return launch_bn<kEpiPagedF8, 256>(g, maps, num_sms, stream);
+    }
     return launch_t<kEpiPaged>(g, maps, bn, num_sms, stream);
 }
 

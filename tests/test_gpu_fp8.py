@@ -185,15 +185,79 @@ def test_fp8_pool_rejects_what_is_not_built():
         with pytest.raises(comb.CombError) as e:
             comb.Pool(2, dq, dv, 16, kv_dtype=comb.KV_E4M3)
         assert e.value.status == comb.COMB_ERR_INVALID
-    w = cs.custom("rej8", k=8, num_q_heads=8, num_kv_heads=2, head_dim_qk=128, head_dim_v=128, chunk_len=[64],
-                  links=[[0]], lq=[4])
-    ld = H().load_workload(w, kv_dtype=comb.KV_E4M3)
-    hs = torch.zeros((64, 256), dtype=torch.bfloat16, device="cuda")
-    wkv = torch.zeros((2 * 256, 256), dtype=torch.bfloat16, device="cuda")
-    with pytest.raises(comb.CombError) as e:
-        ld.pool.project_store_chunks([5], np.array([0, 64], np.int32), hs, wkv)
-    assert e.value.status == comb.COMB_ERR_INVALID
-    ld.pool.close()
+
+
+@pytest.mark.parametrize("Hkv", [2, 8])
+def test_fp8_project_store_page_image_and_attention(Hkv):
+    """(f2) on an fp8 pool: K^cross = H^E W_K, V^cross = H^E W_V (Eq. 5-6) quantised by the GEMM's
+    epilogue.  Expected image: fp64 projection -> bf16 RNE (what a bf16 pool would hold) -> the fp8 rule of oracle/fp8.py.
+    The GPU accumulates in fp32, so a value within ~1e-6 relative of a bf16 (then e4m3) rounding boundary may land on
+    the neighbouring code: at least 99 % of the codes and of the scales identical, every dequantised element within
+    one e4m3 step (2^-3 relative, plus the subnormal spacing) of the expected one, tails byte 0, unowned pages
+    untouched; then decode over those pages against the oracle over the EXPECTED dequantised chunks."""
+    import paper_2602_01519_b200 as comb
+    from oracle import layer as ol
+    d_model = 320
+    lens = [128, 1, 16, 17, 250, 33, 512, 15, 129]
+    hs = [cs.hidden_states(3, c, int(t), d_model) for c, t in enumerate(lens)]
+    tok = np.zeros(len(lens) + 1, np.int32)
+    np.cumsum(lens, out=tok[1:])
+    w_kv = cs.projection_weight(3, 0, 0, Hkv * 256, d_model)
+    num_pages = int(sum((t + 15) // 16 for t in lens)) + 5
+    pool = comb.Pool(Hkv, 128, 128, num_pages, shuffle_seed=31, sentinel=BYTE_SENTINEL, kv_dtype=comb.KV_E4M3)
+    ids = list(range(len(lens)))
+    hd = H().bits_to_device(np.concatenate(hs, 0), "cuda")
+    wd = H().bits_to_device(w_kv, "cuda")
+    pool.project_store_chunks(ids[:1], tok[:2], hd[:tok[1]], wd)
+    pool.project_store_chunks(ids[1:], tok[1:] - tok[1], hd[tok[1]:], wd)
+    torch.cuda.synchronize()
+    model = oracle.PoolModel(num_pages, 31)
+    wk64 = ol.bf16_to_f64(w_kv)
+    chunks, pages = {}, {}
+    for c in ids:
+        pages[c] = model.store(c, lens[c])
+        K, V = ol.project_kv(ol.bf16_to_f64(hs[c]), wk64, Hkv, 128, 128)
+        chunks[c] = (ol.f64_to_bf16_bits(K), ol.f64_to_bf16_bits(V))
+        assert comb.comb_chunk_query(pool.handle, c)[1].tolist() == pages[c]
+    k_img, ks_img, v_img, vs_img = fp8.page_image(num_pages, (Hkv, 128, 128), chunks, pages, sentinel=BYTE_SENTINEL,
+                                                  scale_sentinel=-7.0)
+    owned = np.zeros(num_pages, bool)
+    for c in ids:
+        owned[pages[c]] = True
+    for name, arena, sc, img, simg in (("K", pool.k_arena, pool.k_scale, k_img, ks_img),
+                                       ("V", pool.v_arena, pool.v_scale, v_img, vs_img)):
+        got = arena.view(torch.uint8).cpu().numpy().reshape(img.shape)
+        gsc = sc.cpu().numpy().reshape(simg.shape)
+        assert np.all(got[~owned] == BYTE_SENTINEL) and np.all(gsc[~owned] == -7.0), name + ": an unowned page was touched"
+        assert (gsc[owned] == simg[owned]).mean() >= 0.99, name + ": scales"
+        assert (got[owned] == img[owned]).mean() >= 0.99, name + ": codes"
+        gv = fp8.e4m3_decode(got[owned]) * gsc[owned].astype(np.float64)[:, :, None, None]
+        wv = fp8.e4m3_decode(img[owned]) * simg[owned].astype(np.float64)[:, :, None, None]
+        step = np.maximum(np.abs(wv) * 2.0 ** -3, simg[owned].astype(np.float64)[:, :, None, None] * 2.0 ** -9)
+        assert np.all(np.abs(gv - wv) <= step * 1.001), name + ": not a neighbouring code of the expected value"
+        for c in ids:
+            n = lens[c] - 16 * (len(pages[c]) - 1)
+            assert np.all(got[pages[c][-1], :, n:, :] == 0), name + ": tail slots are not byte 0"
+    # attend over the projected pages
+    links = [[6, 0, 4], [8, 1], [2, 3, 5, 7]]
+    w = cs.custom("pj8", k=8, num_q_heads=4 * Hkv, num_kv_heads=Hkv, head_dim_qk=128, head_dim_v=128, chunk_len=lens,
+                  links=links, lq=[1, 1, 1])
+
+    class Projected:
+        def __getattr__(self, name):
+            return getattr(w, name)
+
+        def chunk_kv(self, c):
+            kb, vb = chunks[int(c)]
+            kc, ks, vc, vs = fp8.quantise_chunk(kb, vb)
+            return (cs.f32_to_bf16_bits(fp8.dequantise_chunk(kc, ks, kb.shape[0]).astype(np.float32)),
+                    cs.f32_to_bf16_bits(fp8.dequantise_chunk(vc, vs, vb.shape[0]).astype(np.float32)))
+    lb = pool.link(links)
+    out, lse = pool.decode(lb, H().bits_to_device(w.all_q(), "cuda"), w.scale)
+    torch.cuda.synchronize()
+    O, L = oracle.attention_for(Projected())
+    check(H().device_to_bits(out), lse.cpu().numpy().astype(np.float64), O, L, "decode over projected fp8 pages", 2e-3)
+    pool.close()
 
 
 @pytest.mark.parametrize("heads", [(32, 8), (16, 16), (8, 1)])
