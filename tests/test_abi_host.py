@@ -453,3 +453,42 @@ def test_directory_export_matches_oracle_model_and_rejects_bad_blobs():
     assert _lib.lib.comb_pool_export(pool, 2, None, aligned.ctypes.data, len(blob), C.byref(n)) == comb.COMB_ERR_INVALID
     assert _lib.lib.comb_pool_refresh(pool, aligned.ctypes.data, len(blob), None) == comb.COMB_ERR_INVALID  # not imported
     comb.comb_pool_destroy(pool)
+
+
+def test_fp8_pool_config_sizes_and_compact_page_table():
+    """(f4) fp8 pools on the host: one byte per element + fp32 scale tables; only 128/128 head dims; comb_link_plan
+    writes the compact page table (entry i of page_ids as an index into the batch's distinct-page list)."""
+    kb, vb, _ = comb.comb_pool_bytes(3, 8, 128, 128, 100, kv_dtype=comb.KV_E4M3)
+    kb16, vb16, _ = comb.comb_pool_bytes(3, 8, 128, 128, 100)
+    assert (kb, vb) == (kb16 // 2, vb16 // 2) == (3 * 100 * 8 * 16 * 128,) * 2
+    assert comb.comb_pool_scale_bytes(3, 8, 128, 128, 100) == 3 * 100 * 8 * 4
+    assert comb.comb_pool_scale_bytes(3, 8, 128, 128, 100, kv_dtype=comb.KV_BF16) == 0
+    for bad in (dict(Dqk=64, Dv=64), dict(Dqk=192, Dv=128), dict(Dqk=128, Dv=64)):
+        cfg = comb.PoolConfig(1, 2, bad["Dqk"], bad["Dv"], 16, 8, FAKE_K, FAKE_V, FAKE_S, 0, comb.KV_E4M3, 0, FAKE_S, FAKE_S)
+        out = C.c_void_p()
+        assert _lib.lib.comb_pool_create(C.byref(cfg), C.byref(out)) == comb.COMB_ERR_INVALID
+    for cfg in (comb.PoolConfig(1, 2, 128, 128, 16, 8, FAKE_K, FAKE_V, FAKE_S, 0, comb.KV_E4M3, 0, None, None),   # no scales
+                comb.PoolConfig(1, 2, 128, 128, 16, 8, FAKE_K, FAKE_V, FAKE_S, 0, 7, 0, FAKE_S, FAKE_S),           # dtype
+                comb.PoolConfig(1, 2, 128, 128, 16, 8, FAKE_K, FAKE_V, FAKE_S, 0, comb.KV_E4M3, 1, FAKE_S, FAKE_S)):
+        out = C.c_void_p()
+        assert _lib.lib.comb_pool_create(C.byref(cfg), C.byref(out)) == comb.COMB_ERR_INVALID
+    cfg = comb.PoolConfig(1, 2, 128, 128, 16, 64, FAKE_K, FAKE_V, FAKE_S, 5, comb.KV_E4M3, 0, FAKE_S, FAKE_S + 4096)
+    pool = comb.comb_pool_create(cfg)
+    for c, T in enumerate([40, 16, 100, 5]):
+        comb.comb_chunk_alloc(pool, c, T)
+    lists = [[2, 0], [], [3, 2, 2, 1]]
+    link, tabs = plan(pool, lists)
+    assert link.page_ids_compact
+    off = link.page_ids_compact - 0x10000
+    host = link._keepalive[0]
+    compact = host[off:off + 4 * int(link.total_pages)].view(np.int32)
+    assert np.array_equal(tabs["cas_page_ids"][compact], tabs["page_ids"])
+    assert compact.min() >= 0 and compact.max() < int(link.distinct_pages)
+    # a bf16 pool writes no such table
+    pool16 = make_pool(num_pages=64, Hkv=2, Dqk=128, Dv=128)
+    for c, T in enumerate([40, 16, 100, 5]):
+        comb.comb_chunk_alloc(pool16, c, T)
+    link16, _ = plan(pool16, lists)
+    assert not link16.page_ids_compact
+    comb.comb_pool_destroy(pool)
+    comb.comb_pool_destroy(pool16)
