@@ -249,8 +249,8 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                     m_used = m_new;
                 } else if (__any_sync(0xffffffffu, (m_new - m_used) * c > 8.f)) {
                     // rare: move the reference max and rescale this warp's rows of the accumulator
-                    ptx::mbar_wait(&o_done[t], (o_cnt + j - 1) & 1);  // P V_{j-1} has landed
-                    ptx::tc_fence_after();
+                    // P V_{j-1} has landed: the MMAs of the issuing thread complete in order and s_full was committed
+                    // after S_j, which it issued after P V_{j-1}
                     const float alpha = ptx::ex2((m_used - m_new) * c);
                     l_run *= alpha;
                     m_used = m_new;
@@ -287,8 +287,8 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                 l_run += (sA.x + sA.y) + (sB.x + sB.y);
             }
             // ---- epilogue: O / l -> bf16 (or an fp32 partial row) ----
-            ptx::mbar_wait(&o_done[t], (o_cnt + n_kv - 1) & 1);
-            o_cnt += n_kv;
+            ptx::mbar_wait(&o_done[t], o_cnt & 1);  // committed once per item, after its last P V
+            ++o_cnt;
             ptx::tc_fence_after();
             const float inv = 1.f / l_run;
             // partial: one KV range of several (compiled in only then)
@@ -439,7 +439,8 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                                                     (j > 0 || ks > 0) ? 1u : 0u);
                     }
                     ++pcnt[t];
-                    if (leader) ptx::mma_commit(&o_done[t]);
+                    if (t == nq - 1) if (leader) ptx::mma_commit(&kv_empty[vslot]);  // V_j is free once its last P V is done
+                    if (!more) if (leader) ptx::mma_commit(&o_done[t]);
                     if (more) {
                         if (t == 0) {
                             ptx::mbar_wait(&kv_full[kslot], kphase);
@@ -450,7 +451,6 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                         if (j + 2 == n_kv) if (leader) ptx::mma_commit(&q_empty[t]);
                     }
                 }
-                if (leader) ptx::mma_commit(&kv_empty[vslot]);
                 if (more) if (leader) ptx::mma_commit(&kv_empty[kslot]);
             }
         }
