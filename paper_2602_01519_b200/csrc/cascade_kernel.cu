@@ -1074,80 +1074,78 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
     if (warp == 5) ptx::tmem_dealloc(tmem, C::TMEM_COLS);
 }
 
-// One CTA of 4 warps per (request, q head): the request's entries are dealt round-robin to the warps, a lane owns
-// DV/32 consecutive output columns, and the four warps' weighted sums meet in shared memory.  Every warp first reads
-// ALL of the request's LSEs to agree on the maximum, then streams its share of the partial rows.  An entry's partials
-// (one per KV range of its chunk) are found through ent_info = (first index, stride, count).
+// One warp per (request, q head) row, 8 rows per CTA; a lane owns DV/32 consecutive output columns.  The row's
+// partials (one per (entry, KV range of the entry's chunk), found through ent_info = (first index, stride, count))
+// are merged ONLINE by identity P8 — running maximum m, weight sum and weighted row, rescaled when m grows — so the
+// LSE and the partial row of an entry are loaded together and four entries are in flight at once: the dependent
+// chain is entry_indptr -> ent_info -> (LSE, row), three round trips to L2 where the partials were just written.
+constexpr int kMergeRows = 8;
 template <int DV>
-__global__ void __launch_bounds__(128) cascade_merge_kernel(const float *__restrict__ part_o,
-                                                            const float *__restrict__ part_lse,
-                                                            const int4 *__restrict__ ent_info,
-                                                            const int32_t *__restrict__ entry_indptr,
-                                                            __nv_bfloat16 *__restrict__ out, float *__restrict__ lse,
-                                                            int Hq) {
+__global__ void __launch_bounds__(32 * kMergeRows) cascade_merge_kernel(const float *__restrict__ part_o,
+                                                                        const float *__restrict__ part_lse,
+                                                                        const int4 *__restrict__ ent_info,
+                                                                        const int32_t *__restrict__ entry_indptr,
+                                                                        __nv_bfloat16 *__restrict__ out,
+                                                                        float *__restrict__ lse, int Hq, int rows) {
     constexpr int CPL = DV / 32;
-    __shared__ float s_acc[4][DV];
-    __shared__ float s_w[4];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int row = blockIdx.x;  // (request, head)
+    const int row = blockIdx.x * kMergeRows + warp;  // (request, head)
+    if (row >= rows) return;
     const int r = row / Hq, h = row - r * Hq;
     const int e0 = entry_indptr[r], e1 = entry_indptr[r + 1];
-    __nv_bfloat16 *orow = out + (size_t)row * DV;
+    __nv_bfloat16 *orow = out + (size_t)row * DV + lane * CPL;
     if (e0 == e1) {  // no contexts linked (reading I13)
-        if (threadIdx.x < DV / 2) reinterpret_cast<uint32_t *>(orow)[threadIdx.x] = 0u;
-        if (threadIdx.x == 0 && lse) lse[row] = -INFINITY;
+        if constexpr (CPL == 4) *reinterpret_cast<uint2 *>(orow) = make_uint2(0u, 0u);
+        else *reinterpret_cast<uint32_t *>(orow) = 0u;
+        if (lane == 0 && lse) lse[row] = -INFINITY;
         return;
     }
-    float m = -INFINITY;
-    for (int e = e0 + lane; e < e1; e += 32) {
-        const int4 inf = ent_info[e];
-        for (int s = 0; s < inf.z; ++s) m = fmaxf(m, part_lse[(size_t)(inf.x + s * inf.y) * Hq + h]);
-    }
+    float m = -INFINITY, wsum = 0.f, acc[4] = {0.f, 0.f, 0.f, 0.f};
+    auto load_row = [&](size_t prow) {
+        const float *po = part_o + prow * DV + lane * CPL;
+        if constexpr (CPL == 4) return *reinterpret_cast<const float4 *>(po);
+        else { const float2 t = *reinterpret_cast<const float2 *>(po); return make_float4(t.x, t.y, 0.f, 0.f); }
+    };
+    auto fold = [&](float l2, const float4 v) {  // one partial into the running merge
+        if (l2 == -INFINITY) return;
+        const float mn = fmaxf(m, l2);
+        const float sa = ptx::ex2(m - mn), sb = ptx::ex2(l2 - mn);
+        m = mn;
+        wsum = wsum * sa + sb;
+        acc[0] = acc[0] * sa + sb * v.x;
+        acc[1] = acc[1] * sa + sb * v.y;
+        acc[2] = acc[2] * sa + sb * v.z;
+        acc[3] = acc[3] * sa + sb * v.w;
+    };
+    for (int e = e0; e < e1; e += 4) {
+        int4 inf[4];
 #pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, off));
-    float acc[CPL];
+        for (int u = 0; u < 4; ++u) inf[u] = e + u < e1 ? ent_info[e + u] : make_int4(0, 0, 0, 0);
+        float l2[4];
+        float4 v[4];
 #pragma unroll
-    for (int c = 0; c < CPL; ++c) acc[c] = 0.f;
-    float wsum = 0.f;
-    for (int e = e0 + warp; e < e1; e += 4) {
-        const int4 inf = ent_info[e];
-        for (int s0 = 0; s0 < inf.z; s0 += 4) {
-            float w[4];
-            float4 v[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const bool ok = s0 + u < inf.z;
-                const size_t prow = (size_t)(inf.x + (s0 + u) * inf.y) * Hq + h;
-                w[u] = ok ? ptx::ex2(part_lse[ok ? prow : 0] - m) : 0.f;
-                v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (ok) {
-                    const float *po = part_o + prow * DV + lane * CPL;
-                    if constexpr (CPL == 4) v[u] = *reinterpret_cast<const float4 *>(po);
-                    else { const float2 t = *reinterpret_cast<const float2 *>(po); v[u].x = t.x; v[u].y = t.y; }
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                wsum += w[u];
-                acc[0] += w[u] * v[u].x;
-                acc[1] += w[u] * v[u].y;
-                if constexpr (CPL == 4) { acc[2] += w[u] * v[u].z; acc[3] += w[u] * v[u].w; }
-            }
+        for (int u = 0; u < 4; ++u) {  // the first range of four entries, all loads independent
+            const bool ok = inf[u].z > 0;
+            const size_t prow = (size_t)inf[u].x * Hq + h;
+            l2[u] = ok ? part_lse[prow] : -INFINITY;
+            v[u] = ok ? load_row(prow) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
-    }
 #pragma unroll
-    for (int c = 0; c < CPL; ++c) s_acc[warp][lane * CPL + c] = acc[c];
-    if (lane == 0) s_w[warp] = wsum;
-    __syncthreads();
-    const float wtot = (s_w[0] + s_w[1]) + (s_w[2] + s_w[3]);
-    if (threadIdx.x < DV / 2) {
-        const int c = 2 * threadIdx.x;
-        const float inv = 1.f / wtot;
-        const float a0 = (s_acc[0][c] + s_acc[1][c]) + (s_acc[2][c] + s_acc[3][c]);
-        const float a1 = (s_acc[0][c + 1] + s_acc[1][c + 1]) + (s_acc[2][c + 1] + s_acc[3][c + 1]);
-        reinterpret_cast<uint32_t *>(orow)[threadIdx.x] = ptx::pack_bf16x2(a0 * inv, a1 * inv);
+        for (int u = 0; u < 4; ++u) fold(l2[u], v[u]);
+#pragma unroll
+        for (int u = 0; u < 4; ++u)  // further KV ranges of a long chunk
+            for (int s = 1; s < inf[u].z; ++s) {
+                const size_t prow = (size_t)(inf[u].x + s * inf[u].y) * Hq + h;
+                fold(part_lse[prow], load_row(prow));
+            }
     }
-    if (threadIdx.x == 0 && lse) lse[row] = (m + log2f(wtot)) * kLn2;
+    const float inv = 1.f / wsum;
+    if constexpr (CPL == 4)
+        *reinterpret_cast<uint2 *>(orow) = make_uint2(ptx::pack_bf16x2(acc[0] * inv, acc[1] * inv),
+                                                      ptx::pack_bf16x2(acc[2] * inv, acc[3] * inv));
+    else
+        *reinterpret_cast<uint32_t *>(orow) = ptx::pack_bf16x2(acc[0] * inv, acc[1] * inv);
+    if (lane == 0 && lse) lse[row] = (m + log2f(wsum)) * kLn2;
 }
 
 template <int DQK, int DV>
@@ -1241,13 +1239,14 @@ cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &
     if (e != cudaSuccess) return e;
     *launches += a.num_items > 0 ? 1 : 0;
     const int rows = num_requests * num_q_heads;
+    const int mgrid = (rows + kMergeRows - 1) / kMergeRows;
     if (hook) hook->begin(hook->ctx, kKernelCascadeMerge, stream);
     if (g.head_dim_v == 128)
-        cascade_merge_kernel<128><<<rows, 128, 0, stream>>>(a.part_o, a.part_lse, a.ent_info, lv.entry_indptr,
-                                                           (__nv_bfloat16 *)out, lse, num_q_heads);
+        cascade_merge_kernel<128><<<mgrid, 32 * kMergeRows, 0, stream>>>(a.part_o, a.part_lse, a.ent_info, lv.entry_indptr,
+                                                                        (__nv_bfloat16 *)out, lse, num_q_heads, rows);
     else
-        cascade_merge_kernel<64><<<rows, 128, 0, stream>>>(a.part_o, a.part_lse, a.ent_info, lv.entry_indptr,
-                                                          (__nv_bfloat16 *)out, lse, num_q_heads);
+        cascade_merge_kernel<64><<<mgrid, 32 * kMergeRows, 0, stream>>>(a.part_o, a.part_lse, a.ent_info, lv.entry_indptr,
+                                                                       (__nv_bfloat16 *)out, lse, num_q_heads, rows);
     if (hook) hook->end(hook->ctx, stream);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     *launches += 1;
