@@ -9,7 +9,8 @@ import ctypes as C
 import os
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libcomb.so")
+# COMB_LIBRARY names another build of the same sources (prefill_timeline.py points it at libcomb_trace.so)
+LIB_PATH = os.environ.get("COMB_LIBRARY") or os.path.join(HERE, "libcomb.so")
 
 COMB_OK = 0
 COMB_ERR_INVALID = -1

@@ -91,6 +91,37 @@ struct Maps {
     CUtensorMap q, k, v;
 };
 
+// Timeline of CTA 0 (profiling aid, compiled only into libcomb_trace*.so by `build.py --trace[=1]`, -DCOMB_TRACE=2 or
+// 1 = softmax stamps only; the product library has none of it): clock64() stamps of one softmax thread per warpgroup and of the issuing lane, per KV tile.
+//   softmax [tile slot][tile #][k]: 0 before / 1 after the s_full wait, 3 row maximum known, 4 / 5 first / second
+//                                   hand-over of P;   [1][127][0..3]: kernel entry, set-up done, loop end, exit
+//   issuer  [tile slot][tile #][k]: 0 before the wait for the first half of P, 1 / 2 first / second half seen,
+//                                   3 P V issued, 5 / 6 before / after the issue of the next S
+#ifdef COMB_TRACE
+__device__ unsigned long long g_trace_sm[2][128][8];
+__device__ unsigned long long g_trace_mma[2][128][8];
+#define COMB_TR_SM(t, seq, k)                                                                                   \
+    do {                                                                                                        \
+        if (blockIdx.x == 0 && lane == 0 && (warp & 3) == 0 && (seq) < 127u) g_trace_sm[t][seq][k] = clock64(); \
+    } while (0)
+#if COMB_TRACE >= 2  // the issuer's stamps lengthen the loop by ~10 % (it runs in step with the tensor pipe)
+#define COMB_TR_MMA(t, seq, k)                                                                \
+    do {                                                                                      \
+        if (blockIdx.x == 0 && leader && (seq) < 127u) g_trace_mma[t][seq][k] = clock64();    \
+    } while (0)
+#else
+#define COMB_TR_MMA(t, seq, k)
+#endif
+#define COMB_TR_CTA(k)                                                                \
+    do {                                                                              \
+        if (blockIdx.x == 0 && threadIdx.x == 0) g_trace_sm[1][127][k] = clock64();   \
+    } while (0)
+#else
+#define COMB_TR_SM(t, seq, k)
+#define COMB_TR_MMA(t, seq, k)
+#define COMB_TR_CTA(k)
+#endif
+
 // ============================================================================================
 // Persistent, warp-specialised, two Q tiles in ping-pong per CTA.
 //   warps 0-3 : softmax + epilogue of Q tile 0 (one thread per row)      warp 8 : TMA loader (Q tiles, K/V ring)
@@ -152,6 +183,7 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(bars + 12 + 2 * C::NSLOT);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    COMB_TR_CTA(0);
     if (tid == 0) {
         for (int t = 0; t < 2; ++t) {
             ptx::mbar_init(&q_full[t], 1);
@@ -178,6 +210,7 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
     __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    COMB_TR_CTA(1);
     const int G = a.group, Hq = a.num_q_heads;
     const int tok_per_tile = kTileM / G;
 
@@ -225,7 +258,9 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
             float m_used = -INFINITY, l_run = 0.f;
             for (int j = 0; j < n_kv; ++j) {
                 const uint64_t ntok8 = a.tile_ntok[tile0 + j];
+                COMB_TR_SM(t, s_cnt, 0);
                 ptx::mbar_wait(&s_full[t], s_cnt & 1);
+                COMB_TR_SM(t, s_cnt, 1);
                 ++s_cnt;
                 ptx::tc_fence_after();
                 uint32_t r[kTileN];
@@ -264,6 +299,7 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                         ptx::tmem_st32(tO + q * 32, o);
                     }
                 }
+                COMB_TR_SM(t, s_cnt - 1, 3);
                 const float neg = -m_used * c;
                 const float2 neg2 = make_float2(neg, neg);
                 float2 sum4[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
@@ -282,6 +318,7 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                     ptx::tmem_wait_st();
                     ptx::tc_fence_before();
                     ptx::mbar_arrive(&p_full[t * 2 + half]);
+                    COMB_TR_SM(t, s_cnt - 1, 4 + half);
                 }
                 const float2 sA = ptx::fadd2(sum4[0], sum4[1]), sB = ptx::fadd2(sum4[2], sum4[3]);
                 l_run += (sA.x + sA.y) + (sB.x + sB.y);
@@ -431,13 +468,16 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                 for (int t = 0; t < nq; ++t) {
 #pragma unroll
                     for (int half = 0; half < 2; ++half) {  // O_t += P_t V_j, one k-step of 16 keys per page
+                        if (half == 0) COMB_TR_MMA(t, pcnt[t], 0);
                         ptx::mbar_wait(&p_full[t * 2 + half], pcnt[t] & 1);
+                        COMB_TR_MMA(t, pcnt[t], 1 + half);
                         ptx::tc_fence_after();
                         for (int ks = half * 4; ks < min(pages_here, half * 4 + 4); ++ks)
                             if (leader) ptx::mma_ts(tmem + 128 * NT + t * DV, tmem + t * 128 + ks * 8,
                                                     dv0 + (uint64_t)((vslot * C::SLOT + ks * 2048) >> 4), idesc_o,
                                                     (j > 0 || ks > 0) ? 1u : 0u);
                     }
+                    COMB_TR_MMA(t, pcnt[t], 3);
                     ++pcnt[t];
                     if (t == nq - 1) if (leader) ptx::mma_commit(&kv_empty[vslot]);  // V_j is free once its last P V is done
                     if (!more) if (leader) ptx::mma_commit(&o_done[t]);
@@ -446,7 +486,9 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                             ptx::mbar_wait(&kv_full[kslot], kphase);
                             ptx::tc_fence_after();
                         }
+                        COMB_TR_MMA(t, pcnt[t] - 1, 5);
                         issue_s(t, kslot);
+                        COMB_TR_MMA(t, pcnt[t] - 1, 6);
                         if (leader) ptx::mma_commit(&s_full[t]);
                         if (j + 2 == n_kv) if (leader) ptx::mma_commit(&q_empty[t]);
                     }
@@ -456,10 +498,12 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
         }
     }
 
+    COMB_TR_CTA(2);
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
     if (warp == C::NSW) ptx::tmem_dealloc(tmem, C::TMEM_COLS);
+    COMB_TR_CTA(3);
 }
 
 }  // namespace

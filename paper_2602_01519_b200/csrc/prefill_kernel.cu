@@ -264,3 +264,16 @@ cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, con
 }
 
 }  // namespace comb
+
+#ifdef COMB_TRACE
+// libcomb_trace.so only (`build.py --trace`): copies the timeline of the most recent prefill launch to host arrays of
+// 2 x 128 x 8 uint64 each (attn_core.cuh says what the stamps are).  Synchronises the device.
+#pragma GCC visibility push(default)
+extern "C" int32_t comb_trace_prefill_read(void *softmax, void *issuer) {
+    if (cudaDeviceSynchronize() != cudaSuccess) return -6;
+    if (cudaMemcpyFromSymbol(softmax, comb::g_trace_sm, sizeof(comb::g_trace_sm)) != cudaSuccess) return -6;
+    if (cudaMemcpyFromSymbol(issuer, comb::g_trace_mma, sizeof(comb::g_trace_mma)) != cudaSuccess) return -6;
+    return 0;
+}
+#pragma GCC visibility pop
+#endif
