@@ -1074,50 +1074,48 @@ cascade_decode_f8_kernel(const CascadeArgs a, const __grid_constant__ KvMaps map
     if (warp == 5) ptx::tmem_dealloc(tmem, C::TMEM_COLS);
 }
 
-// One warp per (request, q head) row, 8 rows per CTA; a lane owns DV/32 consecutive output columns.  The row's
+// WPR warps per (request, q head) row, 8 warps per CTA; a lane owns DV/32 consecutive output columns.  The row's
 // partials (one per (entry, KV range of the entry's chunk), found through ent_info = (first index, stride, count))
 // are merged ONLINE by identity P8 — running maximum m, weight sum and weighted row, rescaled when m grows — so the
-// LSE and the partial row of an entry are loaded together and four entries are in flight at once: the dependent
+// LSE and the partial row of an entry are loaded together and four entries are in flight per warp: the dependent
 // chain is entry_indptr -> ent_info -> (LSE, row), three round trips to L2 where the partials were just written.
-constexpr int kMergeRows = 8;
-template <int DV>
-__global__ void __launch_bounds__(32 * kMergeRows) cascade_merge_kernel(const float *__restrict__ part_o,
-                                                                        const float *__restrict__ part_lse,
-                                                                        const int4 *__restrict__ ent_info,
-                                                                        const int32_t *__restrict__ entry_indptr,
-                                                                        __nv_bfloat16 *__restrict__ out,
-                                                                        float *__restrict__ lse, int Hq, int rows) {
-    constexpr int CPL = DV / 32;
+// WPR = 1 when a request links a handful of chunks (cfg 2: 8); requests with many entries (cfg 4: 64, each with
+// several KV ranges) deal them to 2, 4 or 8 warps whose (m, sum, row) triples meet in shared memory.
+constexpr int kMergeWarps = 8;
+template <int DV, int WPR>
+__global__ void __launch_bounds__(32 * kMergeWarps) cascade_merge_kernel(const float *__restrict__ part_o,
+                                                                         const float *__restrict__ part_lse,
+                                                                         const int4 *__restrict__ ent_info,
+                                                                         const int32_t *__restrict__ entry_indptr,
+                                                                         __nv_bfloat16 *__restrict__ out,
+                                                                         float *__restrict__ lse, int Hq, int rows) {
+    constexpr int CPL = DV / 32, RPC = kMergeWarps / WPR;  // columns per lane, rows per CTA
+    __shared__ float s_acc[WPR > 1 ? kMergeWarps : 1][WPR > 1 ? DV : 1];
+    __shared__ float2 s_mw[kMergeWarps];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int row = blockIdx.x * kMergeRows + warp;  // (request, head)
-    if (row >= rows) return;
-    const int r = row / Hq, h = row - r * Hq;
-    const int e0 = entry_indptr[r], e1 = entry_indptr[r + 1];
-    __nv_bfloat16 *orow = out + (size_t)row * DV + lane * CPL;
-    if (e0 == e1) {  // no contexts linked (reading I13)
-        if constexpr (CPL == 4) *reinterpret_cast<uint2 *>(orow) = make_uint2(0u, 0u);
-        else *reinterpret_cast<uint32_t *>(orow) = 0u;
-        if (lane == 0 && lse) lse[row] = -INFINITY;
-        return;
-    }
+    const int sub = warp % WPR;                               // this warp's share of the row's entries
+    const int row = blockIdx.x * RPC + warp / WPR;            // (request, head)
+    const bool live = row < rows;
+    const int r = live ? row / Hq : 0, h = live ? row - r * Hq : 0;
+    const int e0 = live ? entry_indptr[r] : 0, e1 = live ? entry_indptr[r + 1] : 0;
     float m = -INFINITY, wsum = 0.f, acc[4] = {0.f, 0.f, 0.f, 0.f};
     auto load_row = [&](size_t prow) {
         const float *po = part_o + prow * DV + lane * CPL;
         if constexpr (CPL == 4) return *reinterpret_cast<const float4 *>(po);
         else { const float2 t = *reinterpret_cast<const float2 *>(po); return make_float4(t.x, t.y, 0.f, 0.f); }
     };
-    auto fold = [&](float l2, const float4 v) {  // one partial into the running merge
+    auto fold = [&](float l2, float w, const float4 v) {  // a partial (weight sum w relative to 2^l2) into the merge
         if (l2 == -INFINITY) return;
         const float mn = fmaxf(m, l2);
         const float sa = ptx::ex2(m - mn), sb = ptx::ex2(l2 - mn);
         m = mn;
-        wsum = wsum * sa + sb;
+        wsum = wsum * sa + sb * w;
         acc[0] = acc[0] * sa + sb * v.x;
         acc[1] = acc[1] * sa + sb * v.y;
         acc[2] = acc[2] * sa + sb * v.z;
         acc[3] = acc[3] * sa + sb * v.w;
     };
-    for (int e = e0; e < e1; e += 4) {
+    for (int e = e0 + 4 * sub; e < e1; e += 4 * WPR) {
         int4 inf[4];
 #pragma unroll
         for (int u = 0; u < 4; ++u) inf[u] = e + u < e1 ? ent_info[e + u] : make_int4(0, 0, 0, 0);
@@ -1131,13 +1129,42 @@ __global__ void __launch_bounds__(32 * kMergeRows) cascade_merge_kernel(const fl
             v[u] = ok ? load_row(prow) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) fold(l2[u], v[u]);
+        for (int u = 0; u < 4; ++u) fold(l2[u], 1.f, v[u]);
 #pragma unroll
-        for (int u = 0; u < 4; ++u)  // further KV ranges of a long chunk
-            for (int s = 1; s < inf[u].z; ++s) {
-                const size_t prow = (size_t)(inf[u].x + s * inf[u].y) * Hq + h;
-                fold(part_lse[prow], load_row(prow));
+        for (int u = 0; u < 4; ++u)  // further KV ranges of a long chunk, two at a time
+            for (int s0 = 1; s0 < inf[u].z; s0 += 2) {
+                const bool two = s0 + 1 < inf[u].z;
+                const size_t pa = (size_t)(inf[u].x + s0 * inf[u].y) * Hq + h;
+                const size_t pb = two ? (size_t)(inf[u].x + (s0 + 1) * inf[u].y) * Hq + h : pa;
+                const float la = part_lse[pa], lb = two ? part_lse[pb] : -INFINITY;
+                const float4 va = load_row(pa), vb = load_row(pb);
+                fold(la, 1.f, va);
+                fold(lb, 1.f, vb);
             }
+    }
+    if constexpr (WPR > 1) {  // the row's warps meet: unnormalised rows, (m, sum) pairs
+#pragma unroll
+        for (int c = 0; c < CPL; ++c) s_acc[warp][lane * CPL + c] = acc[c];
+        if (lane == 0) s_mw[warp] = make_float2(m, wsum);
+        __syncthreads();
+        if (sub != 0) return;
+#pragma unroll
+        for (int o = 1; o < WPR; ++o) {
+            const float2 mw = s_mw[warp + o];
+            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            v.x = s_acc[warp + o][lane * CPL];
+            v.y = s_acc[warp + o][lane * CPL + 1];
+            if constexpr (CPL == 4) { v.z = s_acc[warp + o][lane * CPL + 2]; v.w = s_acc[warp + o][lane * CPL + 3]; }
+            fold(mw.x, mw.y, v);
+        }
+    }
+    if (!live) return;
+    __nv_bfloat16 *orow = out + (size_t)row * DV + lane * CPL;
+    if (e0 == e1) {  // no contexts linked (reading I13)
+        if constexpr (CPL == 4) *reinterpret_cast<uint2 *>(orow) = make_uint2(0u, 0u);
+        else *reinterpret_cast<uint32_t *>(orow) = 0u;
+        if (lane == 0 && lse) lse[row] = -INFINITY;
+        return;
     }
     const float inv = 1.f / wsum;
     if constexpr (CPL == 4)
@@ -1146,6 +1173,20 @@ __global__ void __launch_bounds__(32 * kMergeRows) cascade_merge_kernel(const fl
     else
         *reinterpret_cast<uint32_t *>(orow) = ptx::pack_bf16x2(acc[0] * inv, acc[1] * inv);
     if (lane == 0 && lse) lse[row] = (m + log2f(wsum)) * kLn2;
+}
+
+template <int DV>
+void launch_cascade_merge(const CascadeArgs &a, const int32_t *entry_indptr, void *out, float *lse, int Hq, int rows,
+                          int64_t num_partials, int num_requests, cudaStream_t stream) {
+    const int64_t per_row = num_requests > 0 ? num_partials / num_requests : 0;  // partials an output row merges
+#define COMB_MERGE_CASE(W)                                                                                         \
+    cascade_merge_kernel<DV, W><<<(rows + kMergeWarps / W - 1) / (kMergeWarps / W), 32 * kMergeWarps, 0, stream>>>( \
+        a.part_o, a.part_lse, a.ent_info, entry_indptr, (__nv_bfloat16 *)out, lse, Hq, rows)
+    if (per_row <= 16) COMB_MERGE_CASE(1);
+    else if (per_row <= 32) COMB_MERGE_CASE(2);
+    else if (per_row <= 64) COMB_MERGE_CASE(4);
+    else COMB_MERGE_CASE(8);
+#undef COMB_MERGE_CASE
 }
 
 template <int DQK, int DV>
@@ -1175,6 +1216,7 @@ CascadeLayout cascade_layout(size_t num_units, int64_t total_entries, int64_t nu
     L.off_part_o = up(L.off_ent + (size_t)(total_entries > 0 ? total_entries : 1) * sizeof(int4));
     L.off_part_lse = up(L.off_part_o + (size_t)num_partials * (size_t)num_q_heads * (size_t)dv * sizeof(float));
     L.bytes = up(L.off_part_lse + (size_t)num_partials * (size_t)num_q_heads * sizeof(float));
+    L.num_partials = num_partials;
     return L;
 }
 
@@ -1239,14 +1281,11 @@ cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &
     if (e != cudaSuccess) return e;
     *launches += a.num_items > 0 ? 1 : 0;
     const int rows = num_requests * num_q_heads;
-    const int mgrid = (rows + kMergeRows - 1) / kMergeRows;
     if (hook) hook->begin(hook->ctx, kKernelCascadeMerge, stream);
     if (g.head_dim_v == 128)
-        cascade_merge_kernel<128><<<mgrid, 32 * kMergeRows, 0, stream>>>(a.part_o, a.part_lse, a.ent_info, lv.entry_indptr,
-                                                                        (__nv_bfloat16 *)out, lse, num_q_heads, rows);
+        launch_cascade_merge<128>(a, lv.entry_indptr, out, lse, num_q_heads, rows, lay.num_partials, num_requests, stream);
     else
-        cascade_merge_kernel<64><<<mgrid, 32 * kMergeRows, 0, stream>>>(a.part_o, a.part_lse, a.ent_info, lv.entry_indptr,
-                                                                       (__nv_bfloat16 *)out, lse, num_q_heads, rows);
+        launch_cascade_merge<64>(a, lv.entry_indptr, out, lse, num_q_heads, rows, lay.num_partials, num_requests, stream);
     if (hook) hook->end(hook->ctx, stream);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     *launches += 1;

@@ -146,6 +146,7 @@ struct CascadeItem {
 constexpr size_t kCascadeHeaderBytes = 16;
 struct CascadeLayout {
     size_t off_items, off_ent, off_part_o, off_part_lse, bytes;
+    int64_t num_partials;  // (entry, KV range) partials of the call: the merge picks its warps per row from it
 };
 CascadeLayout cascade_layout(size_t num_units, int64_t total_entries, int64_t num_partials, int num_q_heads, int dv);
 bool cascade_supported(int group, int dqk, int dv);
