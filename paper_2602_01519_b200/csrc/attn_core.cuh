@@ -43,7 +43,9 @@ struct PrefillArgs {
     int layer_row0;      // first arena row of this layer = layer * num_pages * Hkv * 16
     float scale_log2;    // scale * log2(e)
     // KV ranges (items with split >= 0): normalised partial rows and their log2-domain LSE, merged by a second kernel
-    float *part_o;       // [partial rows][Dv]   (row of range s, tile slot t, tile row i of an item: PrefillItem::part_base)
+    float *part_o;       // partial rows in blocks of 128 (range s, tile slot t of an item: PrefillItem::part_base), a block
+                         // stored [Dv/4][128 rows][4]: the rows' k-th float4s are contiguous, so a warp (one row per
+                         // thread) writes 512 contiguous bytes per store instead of 32 separate lines
     float *part_lse;     // [partial rows]       log2(sum_j 2^(s_j * scale_log2)) over the item's range
     int64_t total_q;
     int nsplit;
@@ -248,10 +250,10 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                     for (int e = 0; e < DV / 8; ++e) reinterpret_cast<uint4 *>(orow)[e] = make_uint4(0, 0, 0, 0);
                     if (a.lse) a.lse[(size_t)tok * Hq + head] = -INFINITY;
                 } else if (MODE == kModeRanges && row_valid) {  // an empty KV range: weight zero in the merge
-                    const size_t prow = (size_t)it.part_base + (size_t)tv.split * (2 * kTileM) + t * kTileM + row;
+                    const size_t pblk = (size_t)it.part_base + (size_t)tv.split * (2 * kTileM) + t * kTileM;
                     for (int e = 0; e < DV / 4; ++e)
-                        reinterpret_cast<float4 *>(a.part_o + prow * DV)[e] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    a.part_lse[prow] = -INFINITY;
+                        reinterpret_cast<float4 *>(a.part_o + pblk * DV)[e * kTileM + row] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    a.part_lse[pblk + row] = -INFINITY;
                 }
                 continue;
             }
@@ -348,10 +350,10 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                         reinterpret_cast<uint4 *>(orow)[q * 4 + e] = w;
                     }
                 } else if (MODE != kModeFinal && row_valid) {  // fp32 partial row for the merge kernel
-                    float4 *prow_o = reinterpret_cast<float4 *>(a.part_o + prow * DV + q * 32);
+                    float4 *pblk_o = reinterpret_cast<float4 *>(a.part_o + (prow - row) * DV) + row;
 #pragma unroll
                     for (int e = 0; e < 8; ++e)
-                        prow_o[e] = make_float4(__uint_as_float(o[4 * e + 0]) * inv, __uint_as_float(o[4 * e + 1]) * inv,
+                        pblk_o[(q * 8 + e) * kTileM] = make_float4(__uint_as_float(o[4 * e + 0]) * inv, __uint_as_float(o[4 * e + 1]) * inv,
                                                 __uint_as_float(o[4 * e + 2]) * inv, __uint_as_float(o[4 * e + 3]) * inv);
                 }
             }

@@ -47,7 +47,9 @@ __global__ void __launch_bounds__(128) prefill_merge_kernel(const PrefillArgs a,
         for (int s = 0; s < nsp; ++s) {
             const float w = ptx::ex2(l2[s] - m);
             wsum += w;
-            const float *po = a.part_o + (p0 + s * stride) * DV + lane * CPL;
+            // block layout [Dv/4][128 rows][4] (attn_core.cuh): this lane's CPL columns of tile row `row % 128`
+            const float *po = a.part_o + (p0 - (size_t)(row % kTileM) + s * stride) * DV +
+                              ((size_t)((lane * CPL) / 4) * kTileM + (size_t)(row % kTileM)) * 4 + (lane * CPL) % 4;
             if constexpr (CPL == 4) {
                 const float4 v = *reinterpret_cast<const float4 *>(po);
                 acc[0] += w * v.x; acc[1] += w * v.y; acc[2] += w * v.z; acc[3] += w * v.w;
