@@ -23,11 +23,12 @@ constexpr int BM = 128, BK = 64;
 constexpr int A_BYTES = BM * BK * 2;
 constexpr int GEMM_THREADS = 192;
 // N tile: 256 columns (4 stages of 48 KB), or 64 columns with an 8-stage ring of 24 KB for problems whose 256-column
-// tiles would leave most SMs idle (a decode-phase projection: M <= 128 rows, so the weights are the traffic and every
-// SM should stream its share of them)
+// tiles would leave most SMs idle, or 32 columns with a 10-stage ring of 20 KB when 64-column tiles still would (a
+// decode-phase projection: M <= 128 rows and N = 4096 give 128 tiles of 32 columns; the weights are the traffic and
+// every SM should stream its share of them — a CTA's rate is set by the bytes its ring keeps in flight)
 template <int BN>
 struct GemmCfg {
-    static constexpr int STAGES = BN == 256 ? 4 : 8;
+    static constexpr int STAGES = BN == 256 ? 4 : BN == 64 ? 8 : 10;
     static constexpr int B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
     static constexpr int SMEM = 1024 + STAGES * STAGE_BYTES + 256;
 };
@@ -294,14 +295,17 @@ cudaError_t launch_bn(const GemmArgs &g, const GemmMaps &maps, int num_sms, cuda
     return cudaGetLastError();
 }
 
-// 64-column tiles when 256-column tiles would occupy fewer than half of the SMs
+// 64-column tiles when 256-column tiles would occupy fewer than half of the SMs, 32-column tiles when 64-column tiles
+// still would
 int pick_bn(int num_m_tiles, int N, int num_sms) {
+    if ((int64_t)num_m_tiles * ((N + 63) / 64) * 2 <= num_sms) return 32;
     return (int64_t)num_m_tiles * ((N + 255) / 256) * 2 <= num_sms ? 64 : 256;
 }
 
 template <int EPI>
 cudaError_t launch_t(GemmArgs &g, const GemmMaps &maps, int bn, int num_sms, cudaStream_t st) {
     g.num_n_tiles = (g.N + bn - 1) / bn;
+    if (bn == 32) return launch_bn<EPI, 32>(g, maps, num_sms, st);
     return bn == 64 ? launch_bn<EPI, 64>(g, maps, num_sms, st) : launch_bn<EPI, 256>(g, maps, num_sms, st);
 }
 
