@@ -336,6 +336,28 @@ int32_t comb_cross_attn_decode(comb_pool_t *pool, int32_t layer, const comb_link
                                const void *q, int32_t num_q_heads, float scale, void *out, float *lse,
                                void *workspace, size_t workspace_bytes, void *stream);
 
+/* (a5) decode for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): the SAME function as comb_cross_attn_decode (Eq. 7-8 at one query row per request)
+ * on its per-request path (split-KV kernel + LSE merge), with the split partials in a fixed device array that is part
+ * of the library image instead of a caller workspace.  The call allocates nothing — no cudaMalloc / cudaFree /
+ * cudaMallocHost, no host containers, no pinned staging (it copies nothing) — and takes no workspace argument; q, out
+ * and lse are the caller's as before and the link must already be resident (comb_link).
+ *   limit    the array is comb_noalloc_scratch_bytes() = 8 MiB, held by every GPU that loads the library until
+ *            the process exits.  A call whose partials need more — num_requests x num_q_heads x splits x (Dv + 2)
+ *            floats, splits chosen as in comb_cross_attn_decode (cfg 2: 4.3 MB, cfg 4 decode: 2.5 MB; the plan aims
+ *            at ~4 waves of CTAs, so on a 148-SM B200 no call needs more than ~5 MB) — returns COMB_ERR_CAPACITY
+ *            and launches nothing: use comb_cross_attn_decode with a workspace.
+ *   sharing  every call on a device uses the same array, whatever pool or stream: calls that overlap on the GPU
+ *            (different streams without an ordering between them) RACE on it.  The array keeps the previous call's
+ *            contents; nothing in it must start at zero (every partial the merge reads is written by the same call).
+ *   scope    bf16 pools only (an fp8 pool has no per-request kernel): INVALID.  COMB_OPT_DECODE_PATH is ignored.
+ *            comb_profile_* does not see these launches.
+ * Errors: INVALID, CAPACITY, CUDA. */
+int32_t comb_cross_attn_decode_noalloc(comb_pool_t *pool, int32_t layer, const comb_link_t *link,
+                                       int32_t num_requests, const void *q, int32_t num_q_heads, float scale,
+                                       void *out, float *lse, void *stream);
+size_t comb_noalloc_scratch_bytes(void);
+
 /* Workspace that suffices for either attention call on THIS link: num_q_heads heads, total_q query rows (decode:
  * total_q = num_requests). Holds the decode split partials or the chunk-major tiles and per-entry partials, or the
  * prefill work-item list plus the partial rows of its KV ranges. */

@@ -10,7 +10,7 @@ from .api import (KV_BF16, KV_E4M3, comb_pool_scale_bytes, DECODE_AUTO, DECODE_C
                   KERNEL_DECODE_MERGE, KERNEL_DECODE_SPLIT, KERNEL_GEMM, KERNEL_PREFILL, KERNEL_PREFILL_MERGE, KERNEL_STORE,
                   OPT_DECODE_PATH, OPT_EVICT_LRU, PAGE, LinkedBatch, Pool, comb_attn_workspace_bytes, comb_chunk_alloc,
                   comb_chunk_free, comb_chunk_pin, comb_chunk_query, comb_chunk_unpin, comb_pool_evicted,
-                  comb_pool_eviction_count, comb_pool_export, comb_pool_import, comb_pool_refresh, comb_cross_attn_decode, comb_cross_layer_forward, comb_gemm_bf16,
+                  comb_pool_eviction_count, comb_pool_export, comb_pool_import, comb_pool_refresh, comb_cross_attn_decode, comb_cross_attn_decode_noalloc, comb_noalloc_scratch_bytes, comb_cross_layer_forward, comb_gemm_bf16,
                   comb_layer_workspace_bytes, comb_project_store_chunks, comb_cross_attn_prefill, comb_link,
                   comb_link_bytes, comb_link_host_bytes, comb_link_plan, comb_pool_bytes, comb_pool_create,
                   comb_pool_destroy, comb_pool_launch_count, comb_pool_set_option, comb_profile_enable,

@@ -85,6 +85,9 @@ _SIGS = {
                                             _P, _P, _P, C.c_size_t, _P]),
     "comb_cross_attn_decode": (C.c_int32, [_P, C.c_int32, C.POINTER(Link), C.c_int32, _P, C.c_int32, C.c_float, _P,
                                            _P, _P, C.c_size_t, _P]),
+    "comb_cross_attn_decode_noalloc": (C.c_int32, [_P, C.c_int32, C.POINTER(Link), C.c_int32, _P, C.c_int32,
+                                                   C.c_float, _P, _P, _P]),
+    "comb_noalloc_scratch_bytes": (C.c_size_t, []),
     "comb_workspace_bytes": (C.c_size_t, [_P, C.c_int32, C.c_int32, C.c_int64, C.c_int32]),
     "comb_attn_workspace_bytes": (C.c_size_t, [_P, C.POINTER(Link), C.c_int32, C.c_int64]),
     "comb_pool_set_option": (C.c_int32, [_P, C.c_int32, C.c_int64]),

@@ -239,6 +239,17 @@ def comb_cross_attn_decode(pool: int, layer: int, link: Link, num_requests: int,
                                      _stream_ptr(stream)), "comb_cross_attn_decode")
 
 
+def comb_cross_attn_decode_noalloc(pool: int, layer: int, link: Link, num_requests: int, q, num_q_heads: int,
+                                   scale: float, out, lse=None, stream=None) -> None:
+    check(lib.comb_cross_attn_decode_noalloc(pool, layer, C.byref(link), num_requests, _ptr(q), num_q_heads,
+                                             float(scale), _ptr(out), _ptr(lse), _stream_ptr(stream)),
+          "comb_cross_attn_decode_noalloc")
+
+
+def comb_noalloc_scratch_bytes() -> int:
+    return int(lib.comb_noalloc_scratch_bytes())
+
+
 def comb_pool_launch_count(pool: int) -> int:
     return int(lib.comb_pool_launch_count(pool))
 
@@ -488,6 +499,13 @@ class Pool:
             lse = torch.empty((R, Hq), dtype=torch.float32, device=self.device)
         ws = self.workspace(lb, Hq, R)
         comb_cross_attn_decode(self.handle, layer, lb.link, R, q, Hq, scale, out, lse, ws, ws.numel(), stream)
+        return out, lse
+
+    def decode_noalloc(self, lb: LinkedBatch, q: torch.Tensor, scale: float, out: torch.Tensor,
+                       lse: Optional[torch.Tensor] = None, layer: int = 0, stream=None):
+        """comb_cross_attn_decode_noalloc: the caller passes q, out (and lse); nothing is allocated, here or in the library."""
+        comb_cross_attn_decode_noalloc(self.handle, layer, lb.link, int(q.shape[0]), q, int(q.shape[1]), scale, out,
+                                       lse, stream)
         return out, lse
 
     def set_decode_path(self, path: int) -> None:

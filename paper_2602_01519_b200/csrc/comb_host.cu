@@ -1708,3 +1708,76 @@ int32_t comb_pool_refresh(comb_pool_t *p, const void *blob, size_t bytes, void *
 
 }  // extern "C"
 #pragma GCC visibility pop
+
+// ============================================================================================
+// Decode without any allocation (comb_cross_attn_decode_noalloc, include/comb.h): the per-request split-KV path
+// with its split partials in a file-scope device array instead of a caller workspace.
+// ============================================================================================
+namespace comb {
+namespace {
+
+// 8 MiB, held by every GPU that loads the library. The decode plan aims at ~4 waves of 2 CTAs per SM, so on a
+// 148-SM B200 the partials never exceed ~5 MB (R x Hq x splits <= ~9.5 K rows of Dv + 2 floats); the bound below only
+// rejects calls on devices with more SMs (or a future plan that splits further).
+constexpr size_t kNoAllocScratchBytes = (size_t)8 << 20;
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocScratchBytes];
+
+// In host code `g_noalloc_scratch` is a host-side stand-in, not a device address: the address the kernels get comes
+// from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr int kNoAllocMaxDevices = 64;
+void *g_noalloc_ptr[kNoAllocMaxDevices];  // written once per device (a benign race writes the same value twice)
+
+int32_t noalloc_scratch(void **ptr) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return COMB_ERR_CUDA;
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return COMB_ERR_INVALID;
+    void *p = g_noalloc_ptr[dev];
+    if (!p) {
+        if (cudaGetSymbolAddress(&p, g_noalloc_scratch) != cudaSuccess || !p) return COMB_ERR_CUDA;
+        g_noalloc_ptr[dev] = p;
+    }
+    *ptr = p;
+    return COMB_OK;
+}
+
+}  // namespace
+}  // namespace comb
+
+#pragma GCC visibility push(default)
+extern "C" {
+
+size_t comb_noalloc_scratch_bytes(void) { return comb::kNoAllocScratchBytes; }
+
+int32_t comb_cross_attn_decode_noalloc(comb_pool_t *p, int32_t layer, const comb_link_t *link, int32_t R,
+                                       const void *q, int32_t Hq, float scale, void *out, float *lse, void *stream) {
+    using namespace comb;
+    if (!p || !link || R < 0 || Hq <= 0) return COMB_ERR_INVALID;
+    if (!(scale > 0.f) || scale > 3.0e38f) return COMB_ERR_INVALID;  // also rejects NaN
+    if (layer < 0 || layer >= p->cfg.num_layers) return COMB_ERR_INVALID;
+    if (Hq % p->cfg.num_kv_heads) return COMB_ERR_INVALID;
+    if (R != link->num_requests) return COMB_ERR_INVALID;
+    if (p->geom.kv_dtype == COMB_KV_E4M3) return COMB_ERR_INVALID;  // fp8 pools have no per-request kernel
+    if (R == 0) return COMB_OK;
+    if (!q || !out || !link->page_indptr) return COMB_ERR_INVALID;
+    const int G = Hq / p->cfg.num_kv_heads;
+    if (!decode_supported(G, p->cfg.head_dim_qk, p->cfg.head_dim_v)) return COMB_ERR_INVALID;
+    p->probe_device();
+    const DecodePlan plan = make_decode_plan(R, p->cfg.num_kv_heads * decode_head_subgroups(G),
+                                             link->max_pages_per_request, p->num_sms);
+    const size_t need = decode_workspace_bytes(R, Hq, p->cfg.head_dim_v, plan);
+    if (need > kNoAllocScratchBytes) return COMB_ERR_CAPACITY;  // beyond the fixed array: use comb_cross_attn_decode
+    void *scratch = nullptr;
+    const int32_t rc = noalloc_scratch(&scratch);
+    if (rc != COMB_OK) return rc;
+    // Nothing in the array must start at zero: the split kernel writes every (request, head, split) partial the
+    // merge kernel reads (the merge derives a request's split count from its page count), so the previous call's
+    // contents are never seen.
+    int launches = 0;
+    cudaError_t e = launch_decode(p->geom, layer, view_of(link), R, Hq, q, scale, out, lse, scratch, plan,
+                                  (cudaStream_t)stream, &launches, nullptr);
+    p->launches += launches;
+    return e == cudaSuccess ? COMB_OK : COMB_ERR_CUDA;
+}
+
+}  // extern "C"
+#pragma GCC visibility pop
