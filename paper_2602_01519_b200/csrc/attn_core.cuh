@@ -102,6 +102,7 @@ struct Maps {
 #ifdef COMB_TRACE
 __device__ unsigned long long g_trace_sm[2][128][8];
 __device__ unsigned long long g_trace_mma[2][128][8];
+__device__ unsigned long long g_trace_cta[1024][4];  // per CTA, %globaltimer (ns): entry, set-up done, loop end, exit
 #define COMB_TR_SM(t, seq, k)                                                                                   \
     do {                                                                                                        \
         if (blockIdx.x == 0 && lane == 0 && (warp & 3) == 0 && (seq) < 127u) g_trace_sm[t][seq][k] = clock64(); \
@@ -117,6 +118,11 @@ __device__ unsigned long long g_trace_mma[2][128][8];
 #define COMB_TR_CTA(k)                                                                \
     do {                                                                              \
         if (blockIdx.x == 0 && threadIdx.x == 0) g_trace_sm[1][127][k] = clock64();   \
+        if (threadIdx.x == 0 && blockIdx.x < 1024) {                                  \
+            unsigned long long gt;                                                    \
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));                    \
+            g_trace_cta[blockIdx.x][k] = gt;                                          \
+        }                                                                             \
     } while (0)
 #else
 #define COMB_TR_SM(t, seq, k)

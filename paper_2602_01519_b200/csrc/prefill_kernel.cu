@@ -277,5 +277,11 @@ extern "C" int32_t comb_trace_prefill_read(void *softmax, void *issuer) {
     if (cudaMemcpyFromSymbol(issuer, comb::g_trace_mma, sizeof(comb::g_trace_mma)) != cudaSuccess) return -6;
     return 0;
 }
+// per-CTA %globaltimer stamps of the most recent prefill launch: 1024 x 4 uint64 (entry, set-up done, loop end, exit)
+extern "C" int32_t comb_trace_prefill_read_ctas(void *ctas) {
+    if (cudaDeviceSynchronize() != cudaSuccess) return -6;
+    if (cudaMemcpyFromSymbol(ctas, comb::g_trace_cta, sizeof(comb::g_trace_cta)) != cudaSuccess) return -6;
+    return 0;
+}
 #pragma GCC visibility pop
 #endif

@@ -50,6 +50,15 @@ def main():
     rc = C.CDLL(_lib.LIB_PATH).comb_trace_prefill_read(C.c_void_p(sm.ctypes.data), C.c_void_p(mma.ctypes.data))
     if rc != 0:
         raise SystemExit("comb_trace_prefill_read: %d" % rc)
+    ctas = np.zeros((1024, 4), np.uint64)
+    if C.CDLL(_lib.LIB_PATH).comb_trace_prefill_read_ctas(C.c_void_p(ctas.ctypes.data)) == 0:
+        ctas = ctas.astype(np.int64)
+        live = ctas[ctas[:, 3] >= ctas[:, 0].max()]  # CTAs of the last launch (older launches' stamps are smaller)
+        t_first = live[:, 0].min()
+        rel = live - t_first
+        print("%d CTAs, %%globaltimer ns after the first CTA's entry (min / median / max): entry %d/%d/%d, set-up done "
+              "%d/%d/%d, loop end %d/%d/%d, exit %d/%d/%d" % ((len(live),) + tuple(
+                  int(f(rel[:, k])) for k in range(4) for f in (np.min, np.median, np.max))))
     sm = sm.astype(np.int64)
     mma = mma.astype(np.int64)
     t0 = int(sm[0, 0, 0])
