@@ -398,7 +398,12 @@ int32_t comb_gemm_bf16(comb_pool_t *pool, const void *a, const void *w, const vo
 /* Pool options. COMB_OPT_DECODE_PATH: 0 = automatic (chunk-major when total_entries >= 1.25 x distinct chunks,
  * i.e. the batch re-reads at least a fifth of its KV), 1 = always per-request, 2 = always chunk-major.
  * Errors: INVALID (unknown option or value). */
-enum { COMB_OPT_DECODE_PATH = 1, COMB_OPT_EVICT_LRU = 2 /* 0 (default) = never evict, 1 = LRU eviction, see (f4) */ };
+/* COMB_OPT_PREFILL_CLUSTERS: 1 (default) = a prefill call whose work items come in pairs that share their K/V stream
+ * (two Q-tile pairs of one (request, kv-head), whole KV each, at least one item per SM) runs on thread-block clusters
+ * of two CTAs that fetch each K/V tile once and TMA-multicast it to both; 0 = always one CTA per item. Same result
+ * bit for bit (same arithmetic in the same order); falls back by itself when the device cannot co-schedule the clusters. */
+enum { COMB_OPT_DECODE_PATH = 1, COMB_OPT_EVICT_LRU = 2 /* 0 (default) = never evict, 1 = LRU eviction, see (f4) */,
+       COMB_OPT_PREFILL_CLUSTERS = 3 };
 enum { COMB_DECODE_AUTO = 0, COMB_DECODE_PER_REQUEST = 1, COMB_DECODE_CHUNK_MAJOR = 2 };
 int32_t comb_pool_set_option(comb_pool_t *pool, int32_t option, int64_t value);
 

@@ -8,7 +8,7 @@ from ._lib import (COMB_ERR_BUSY, COMB_ERR_READ_ONLY, COMB_ERR_CAPACITY, COMB_ER
                    COMB_ERR_UNKNOWN_CHUNK, COMB_OK, CombError, Link, PoolConfig)
 from .api import (KV_BF16, KV_E4M3, comb_pool_scale_bytes, DECODE_AUTO, DECODE_CHUNK_MAJOR, DECODE_PER_REQUEST, KERNEL_CASCADE_MERGE, KERNEL_DECODE_CASCADE,
                   KERNEL_DECODE_MERGE, KERNEL_DECODE_SPLIT, KERNEL_GEMM, KERNEL_PREFILL, KERNEL_PREFILL_MERGE, KERNEL_STORE,
-                  OPT_DECODE_PATH, OPT_EVICT_LRU, PAGE, LinkedBatch, Pool, comb_attn_workspace_bytes, comb_chunk_alloc,
+                  OPT_DECODE_PATH, OPT_EVICT_LRU, OPT_PREFILL_CLUSTERS, PAGE, LinkedBatch, Pool, comb_attn_workspace_bytes, comb_chunk_alloc,
                   comb_chunk_free, comb_chunk_pin, comb_chunk_query, comb_chunk_unpin, comb_pool_evicted,
                   comb_pool_eviction_count, comb_pool_export, comb_pool_import, comb_pool_refresh, comb_cross_attn_decode, comb_cross_attn_decode_noalloc, comb_noalloc_scratch_bytes, comb_cross_layer_forward, comb_gemm_bf16,
                   comb_layer_workspace_bytes, comb_project_store_chunks, comb_cross_attn_prefill, comb_link,

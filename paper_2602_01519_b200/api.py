@@ -217,6 +217,7 @@ def comb_attn_workspace_bytes(pool: int, link: Link, num_q_heads: int, total_q: 
 
 OPT_DECODE_PATH = 1
 OPT_EVICT_LRU = 2
+OPT_PREFILL_CLUSTERS = 3
 DECODE_AUTO, DECODE_PER_REQUEST, DECODE_CHUNK_MAJOR = 0, 1, 2
 
 

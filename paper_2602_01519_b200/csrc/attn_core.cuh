@@ -175,7 +175,13 @@ __device__ __forceinline__ float fmax3(float a, float b, float c) {
     return d;
 }
 
-template <int DQK, int DV, int MODE, int NT>
+// CL = 2 (two-tile kernel, whole-KV items only): a thread-block CLUSTER of two CTAs works on two consecutive items that
+// share their K/V stream (two Q-tile pairs of one (request, kv-head)).  Each CTA's loader fetches every second page of
+// a tile and TMA-multicasts it into BOTH CTAs' ring slots, so a K/V tile crosses L2 -> SM once per cluster instead of
+// once per CTA; a ring slot is refilled when both CTAs' MMAs have released it (tcgen05.commit multicast on kv_empty,
+// which counts two arrivals).  The two CTAs run the same number of items with the same KV lengths, in lockstep by
+// construction of the ring.
+template <int DQK, int DV, int MODE, int NT, int CL = 1>
 __global__ void __launch_bounds__(V1Cfg<DQK, DV, NT>::THREADS, 3 - NT)  // registers: 168 (NT = 2) or 128 (NT = 1)
 attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const int num_items) {
     using C = V1Cfg<DQK, DV, NT>;
@@ -203,7 +209,7 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
         }
         for (int s = 0; s < C::NSLOT; ++s) {
             ptx::mbar_init(&kv_full[s], 1);
-            ptx::mbar_init(&kv_empty[s], 1);
+            ptx::mbar_init(&kv_empty[s], CL);  // one tcgen05.commit per CTA of the cluster
         }
         ptx::fence_barrier_init();
         ptx::tma_prefetch_desc(&maps.q);
@@ -216,8 +222,11 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
     }
     ptx::tc_fence_before();
     __syncthreads();
+    if (CL > 1) ptx::cluster_sync();  // the peer's barriers are initialised before anything is multicast into them
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    const uint32_t cta_rank = CL > 1 ? ptx::cluster_ctarank() : 0u;
+    constexpr uint16_t kClusterMask = (uint16_t)((1u << CL) - 1u);
     COMB_TR_CTA(1);
     const int G = a.group, Hq = a.num_q_heads;
     const int tok_per_tile = kTileM / G;
@@ -407,7 +416,14 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                 if (lane == 0)
                     ptx::mbar_expect_tx(&kv_full[slot], (uint32_t)pages_here * kPage * (is_v ? DV : DQK) * 2);
                 __syncwarp();
-                if (lane < pages_here) {
+                if (CL > 1) {  // this CTA's share of the pages, into both CTAs' slots
+                    if (lane < pages_here && (lane % CL) == (int)cta_rank) {
+                        const CUtensorMap *m = is_v ? &maps.v : &maps.k;
+                        for (int h = 0; h < (is_v ? C::VH : C::KH); ++h)
+                            ptx::tma_load_2d_multicast(dst + h * C::HALF + lane * 2048, m, h * 64, row0, &kv_full[slot],
+                                                       kClusterMask);
+                    }
+                } else if (lane < pages_here) {
                     if (!is_v) {
 #pragma unroll
                         for (int h = 0; h < C::KH; ++h)
@@ -437,6 +453,10 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
         const uint64_t dk0 = ptx::umma_desc_sw128(ptx::smem_u32(sKV), 16, 1024);
         const uint64_t dv0 = ptx::umma_desc_sw128(ptx::smem_u32(sKV), C::HALF, 1024);
         uint32_t slot = 0, phase = 0, qcnt[2] = {0, 0}, pcnt[2] = {0, 0};
+        auto release_slot = [&](uint32_t sl) {  // the slot is free when the MMAs issued so far have read it
+            if (CL > 1) ptx::mma_commit_multicast(&kv_empty[sl], kClusterMask);
+            else ptx::mma_commit(&kv_empty[sl]);
+        };
         auto issue_s = [&](int t, uint32_t kslot) {
             const uint64_t dq = dq0 + (uint64_t)((t * C::Q_BYTES) >> 4), dk = dk0 + (uint64_t)((kslot * C::SLOT) >> 4);
 #pragma unroll
@@ -463,7 +483,7 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                 if (leader) ptx::mma_commit(&s_full[t]);
                 if (n_kv == 1) if (leader) ptx::mma_commit(&q_empty[t]);
             }
-            if (leader) ptx::mma_commit(&kv_empty[kslot]);
+            if (leader) release_slot(kslot);
             for (int j = 0; j < n_kv; ++j) {
                 const int pages_here = min(kTilePages, npages - j * kTilePages);
                 const bool more = j + 1 < n_kv;
@@ -487,7 +507,7 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                     }
                     COMB_TR_MMA(t, pcnt[t], 3);
                     ++pcnt[t];
-                    if (t == nq - 1) if (leader) ptx::mma_commit(&kv_empty[vslot]);  // V_j is free once its last P V is done
+                    if (t == nq - 1) if (leader) release_slot(vslot);  // V_j is free once its last P V is done
                     if (!more) if (leader) ptx::mma_commit(&o_done[t]);
                     if (more) {
                         if (t == 0) {
@@ -501,7 +521,7 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
                         if (j + 2 == n_kv) if (leader) ptx::mma_commit(&q_empty[t]);
                     }
                 }
-                if (more) if (leader) ptx::mma_commit(&kv_empty[kslot]);
+                if (more) if (leader) release_slot(kslot);
             }
         }
     }
@@ -509,6 +529,7 @@ attn_core_kernel(const PrefillArgs a, const __grid_constant__ Maps maps, const i
     COMB_TR_CTA(2);
     ptx::tc_fence_before();
     __syncthreads();
+    if (CL > 1) ptx::cluster_sync();  // no CTA leaves while its peer may still write into its ring or barriers
     ptx::tc_fence_after();
     if (warp == C::NSW) ptx::tmem_dealloc(tmem, C::TMEM_COLS);
     COMB_TR_CTA(3);

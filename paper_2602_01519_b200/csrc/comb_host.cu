@@ -70,6 +70,7 @@ struct comb_pool {
     TensorMapBlob k_map, v_map;
     int64_t launches = 0;
     int64_t opt_decode_path = COMB_DECODE_AUTO;
+    bool opt_prefill_clusters = true;
     bool opt_evict_lru = false;
     uint64_t tick = 0, next_seq = 0;
     std::vector<uint64_t> last_evicted;
@@ -1201,6 +1202,11 @@ int32_t comb_pool_set_option(comb_pool_t *p, int32_t option, int64_t value) {
         p->opt_evict_lru = value == 1;
         return COMB_OK;
     }
+    if (option == COMB_OPT_PREFILL_CLUSTERS) {
+        if (value != 0 && value != 1) return COMB_ERR_INVALID;
+        p->opt_prefill_clusters = value == 1;
+        return COMB_OK;
+    }
     return COMB_ERR_INVALID;
 }
 
@@ -1376,9 +1382,15 @@ int32_t comb_cross_attn_prefill(comb_pool_t *p, int32_t layer, const comb_link_t
     if (cudaMemcpyAsync(ws, h, num_items * sizeof(PrefillItem), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return COMB_ERR_CUDA;
     int launches = 0;
+    // consecutive items that share their K/V stream (two Q-tile pairs of one (request, kv-head), whole KV each) may
+    // run on a cluster of two CTAs
+    bool paired = p->opt_prefill_clusters && plan.part_rows == 0 && num_items % 2 == 0;
+    for (size_t i = 0; paired && i < num_items; i += 2)
+        paired = plan.items[i].request == plan.items[i + 1].request && plan.items[i].kv_head == plan.items[i + 1].kv_head &&
+                 plan.items[i].split < 0 && plan.items[i + 1].split < 0;
     cudaError_t e = launch_prefill(geom, run_layer, lv, maps, (const PrefillItem *)ws, (int)num_items, Hq,
                                    scale, out, lse, total_q, (char *)ws + items_bytes, plan.part_rows,
-                                   plan.tiles_per_cta, p->num_sms, st, &launches, p->active_hook());
+                                   plan.tiles_per_cta, paired, p->num_sms, st, &launches, p->active_hook());
     if (e != cudaSuccess) return COMB_ERR_CUDA;
     p->launches += launches;
     if (!p->release(slot, st)) return COMB_ERR_CUDA;

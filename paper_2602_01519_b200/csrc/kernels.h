@@ -110,11 +110,12 @@ cudaError_t prefill_encode_kv_maps(const PoolGeom &g, TensorMapBlob *k_map, Tens
 cudaError_t prefill_encode_q_map(const void *q, int64_t total_q, int num_q_heads, int group, int dqk,
                                  TensorMapBlob *q_map);
 // part_rows > 0: some items are KV ranges; `partials` holds part_rows x (Dv + 1) floats and a second kernel merges
-// the ranges (*launches += 1).
+// the ranges (*launches += 1).  paired: items (2i, 2i + 1) have the same (request, kv-head) and see all of its KV, so a
+// cluster of two CTAs may share their K/V stream (TMA multicast).
 cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &maps,
                            const PrefillItem *items_dev, int num_items, int num_q_heads, float scale, void *out,
                            float *lse, int64_t total_q, void *partials, int64_t part_rows, int tiles_per_cta,
-                           int num_sms, cudaStream_t stream, int *launches, const LaunchHook *hook);
+                           bool paired, int num_sms, cudaStream_t stream, int *launches, const LaunchHook *hook);
 
 // Dense row-major bf16 matrix [outer][inner] -> 2-D TMA map with SWIZZLE_128B boxes {box_inner (<= 64), box_outer}.
 cudaError_t encode_tma_2d_bf16(const void *base, uint64_t inner, uint64_t outer, uint64_t row_pitch_bytes,

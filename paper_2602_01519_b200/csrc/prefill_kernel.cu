@@ -128,6 +128,45 @@ cudaError_t encode_arena_map(void *arena, int64_t rows, int d, bool fp8, TensorM
     return encode_tma_2d_bf16(arena, (uint64_t)d, (uint64_t)rows, (uint64_t)d * 2, 64, (uint32_t)kPage, out);
 }
 
+// Two-tile kernel on clusters of two CTAs (attn_core.cuh, CL = 2): consecutive items (2i, 2i + 1) share their K/V
+// stream.  cudaErrorNotSupported = the device cannot keep a cluster on every pair of SMs; the caller then takes the
+// plain launch.
+template <int DQK, int DV>
+cudaError_t launch_v1_clusters(const PrefillArgs &a, const Maps &maps, int num_items, int num_sms, cudaStream_t st) {
+    using C = V1Cfg<DQK, DV, 2>;
+    if constexpr (!C::FITS) {
+        return cudaErrorNotSupported;
+    } else {
+        auto kern = attn_core_kernel<DQK, DV, kModeFinal, 2, 2>;
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM);
+        if (e != cudaSuccess) return e;
+        const int pairs = num_items / 2, want = pairs < num_sms / 2 ? pairs : num_sms / 2;
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(2 * (unsigned)want, 1, 1);
+        cfg.blockDim = dim3(C::THREADS, 1, 1);
+        cfg.dynamicSmemBytes = C::SMEM;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        static int max_clusters = -1;  // per process; the library runs one device per process
+        if (max_clusters < 0) {
+            int n = 0;
+            if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) {
+                (void)cudaGetLastError();
+                n = 0;
+            }
+            max_clusters = n;
+        }
+        if (max_clusters < want) return cudaErrorNotSupported;  // a persistent grid must be co-resident
+        return cudaLaunchKernelEx(&cfg, kern, a, maps, num_items);
+    }
+}
+
 template <int DQK, int DV, int NT>
 cudaError_t launch_v1(const PrefillArgs &a, const Maps &maps, int num_items, int num_sms, cudaStream_t st) {
     using C = V1Cfg<DQK, DV, NT>;
@@ -213,7 +252,7 @@ int prefill_ctas_per_sm(int tiles_per_cta, int dqk, int dv) {
 cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, const PrefillMaps &pm,
                            const PrefillItem *items_dev, int num_items, int num_q_heads, float scale, void *out,
                            float *lse, int64_t total_q, void *partials, int64_t part_rows, int tiles_per_cta,
-                           int num_sms, cudaStream_t stream, int *launches, const LaunchHook *hook) {
+                           bool paired, int num_sms, cudaStream_t stream, int *launches, const LaunchHook *hook) {
     PrefillArgs a{};
     a.items = items_dev;
     a.page_indptr = lv.page_indptr;
@@ -239,10 +278,15 @@ cudaError_t launch_prefill(const PoolGeom &g, int layer, const LinkView &lv, con
     memcpy(&maps.v, &pm.v, sizeof(CUtensorMap));
     cudaError_t e = cudaErrorInvalidValue;
     if (hook) hook->begin(hook->ctx, kKernelPrefill, stream);
+    const bool clusters = paired && !ranges && tiles_per_cta == 2 && num_items % 2 == 0 && num_items >= num_sms;
 #define COMB_PREFILL_CASE(DQ, DVV)                                                              \
-    if (g.head_dim_qk == DQ && g.head_dim_v == DVV)                                             \
-        e = tiles_per_cta == 1 ? launch_v1<DQ, DVV, 1>(a, maps, num_items, num_sms, stream)     \
-                               : launch_v1<DQ, DVV, 2>(a, maps, num_items, num_sms, stream);
+    if (g.head_dim_qk == DQ && g.head_dim_v == DVV) {                                           \
+        e = cudaErrorNotSupported;                                                              \
+        if (clusters) e = launch_v1_clusters<DQ, DVV>(a, maps, num_items, num_sms, stream);     \
+        if (e == cudaErrorNotSupported)                                                         \
+            e = tiles_per_cta == 1 ? launch_v1<DQ, DVV, 1>(a, maps, num_items, num_sms, stream) \
+                                   : launch_v1<DQ, DVV, 2>(a, maps, num_items, num_sms, stream); \
+    }
     COMB_PREFILL_CASE(128, 128)
     COMB_PREFILL_CASE(64, 64)
     COMB_PREFILL_CASE(192, 128)
