@@ -153,16 +153,18 @@ cudaError_t launch_v1_clusters(const PrefillArgs &a, const Maps &maps, int num_i
         attr[0].val.clusterDim.z = 1;
         cfg.attrs = attr;
         cfg.numAttrs = 1;
-        static int max_clusters = -1;  // per process; the library runs one device per process
-        if (max_clusters < 0) {
+        static int max_clusters[64];  // per device: co-resident clusters of this kernel + 1 (0 = not asked yet)
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return cudaErrorNotSupported;
+        if (max_clusters[dev] == 0) {
             int n = 0;
             if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) {
                 (void)cudaGetLastError();
                 n = 0;
             }
-            max_clusters = n;
+            max_clusters[dev] = n + 1;
         }
-        if (max_clusters < want) return cudaErrorNotSupported;  // a persistent grid must be co-resident
+        if (max_clusters[dev] - 1 < want) return cudaErrorNotSupported;  // a persistent grid must be co-resident
         return cudaLaunchKernelEx(&cfg, kern, a, maps, num_items);
     }
 }

@@ -312,6 +312,22 @@ def test_options_and_decode_group_sizes():
         st = _lib.lib.comb_cross_attn_decode(pool, 0, C.byref(link), 1, 0x7400_0000_0000, Hq, C.c_float(0.1),
                                              0x7500_0000_0000, None, 0x7600_0000_0000, ws, None)
         assert (st != comb.COMB_ERR_INVALID) == ok, (Hq, st)
+    # the prefill cluster option takes 0 / 1 only
+    comb.comb_pool_set_option(pool, comb.OPT_PREFILL_CLUSTERS, 0)
+    comb.comb_pool_set_option(pool, comb.OPT_PREFILL_CLUSTERS, 1)
+    with pytest.raises(comb.CombError) as e:
+        comb.comb_pool_set_option(pool, comb.OPT_PREFILL_CLUSTERS, 2)
+    assert e.value.status == comb.COMB_ERR_INVALID
+    # comb_cross_attn_decode_noalloc: the same argument checks, no workspace argument, a fixed 8 MiB array
+    assert comb.comb_noalloc_scratch_bytes() == 8 << 20
+    na = _lib.lib.comb_cross_attn_decode_noalloc
+    q, o = 0x7400_0000_0000, 0x7500_0000_0000
+    assert na(None, 0, C.byref(link), 1, q, 4, C.c_float(0.1), o, None, None) == comb.COMB_ERR_INVALID
+    assert na(pool, 0, C.byref(link), 1, q, 3, C.c_float(0.1), o, None, None) == comb.COMB_ERR_INVALID      # Hq % Hkv, G
+    assert na(pool, 0, C.byref(link), 1, q, 4, C.c_float(-1.0), o, None, None) == comb.COMB_ERR_INVALID    # scale
+    assert na(pool, 1, C.byref(link), 1, q, 4, C.c_float(0.1), o, None, None) == comb.COMB_ERR_INVALID     # layer
+    assert na(pool, 0, C.byref(link), 2, q, 4, C.c_float(0.1), o, None, None) == comb.COMB_ERR_INVALID     # R != link's
+    assert na(pool, 0, C.byref(link), 1, None, 4, C.c_float(0.1), o, None, None) == comb.COMB_ERR_INVALID  # q
     comb.comb_pool_destroy(pool)
 
 
