@@ -614,20 +614,21 @@ def test_prefill_many_items_per_cta_all_elements():
     ld.pool.close()
 
 
-@pytest.mark.parametrize("peaked", [False, True])
-def test_prefill_cluster_pairs_all_elements(peaked):
+@pytest.mark.parametrize("lq,peaked", [(128, False), (128, True), (200, False)])
+def test_prefill_cluster_pairs_all_elements(lq, peaked):
     """37 requests x 128 tokens, 32/8 heads: 2 items per (request, kv-head) = 592 items = 4 waves of 148 CTAs, every
     pair of consecutive items sharing its K/V stream: the call runs on 74 clusters of two CTAs with TMA multicast
     (COMB_OPT_PREFILL_CLUSTERS, default on), each CTA 4 items back to back.  Checked on every element against the
     oracle, and bit for bit against the same call with clusters off (same arithmetic in the same order).  Ragged chunks:
     partial pages in the middle and at the end of a request, so tiles with an odd page count split unevenly between
-    the two loaders; the peaked variant takes the rescale path."""
+    the two loaders; the peaked variant takes the rescale path; lq = 200 gives 4 items per stream (8 waves) of which
+    the last has a single, partly filled Q tile while its cluster peer has two full ones."""
     import paper_2602_01519_b200 as comb
     rng = np.random.default_rng(43)
     lens = rng.integers(60, 260, size=12).astype(np.int32)
     links = [rng.choice(12, size=int(rng.integers(3, 8)), replace=False) for _ in range(37)]
     w = cs.custom("cluster_pairs", k=8, num_q_heads=32, num_kv_heads=8, head_dim_qk=128, head_dim_v=128,
-                  chunk_len=lens, links=links, lq=[128] * 37)
+                  chunk_len=lens, links=links, lq=[lq] * 37)
     if peaked:
         w = w.peaked()
     ld = H().load_workload(w, sentinel=SENTINEL, shuffle_seed=8)
@@ -642,7 +643,7 @@ def test_prefill_cluster_pairs_all_elements(peaked):
     assert torch.equal(out.view(torch.int16), out1.view(torch.int16)), "cluster path differs from the one-CTA path"
     assert torch.equal(lse, lse1)
     check_attention(H().device_to_bits(out), lse.cpu().numpy().astype(np.float64), *oracle.attention_for(w),
-                    tag="prefill cluster pairs peaked=%s" % peaked)
+                    tag="prefill cluster pairs lq=%d peaked=%s" % (lq, peaked))
     with pytest.raises(comb.CombError):
         comb.comb_pool_set_option(ld.pool.handle, comb.OPT_PREFILL_CLUSTERS, 2)
     ld.pool.close()
