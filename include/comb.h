@@ -222,7 +222,7 @@ int32_t comb_project_store_chunks(comb_pool_t *pool, int32_t layer, int32_t n, c
  * Request-major view (what prefill and the per-request decode read):
  *   page_indptr int32 [R+1]      page range of request r in page_ids / page_ntok
  *   page_ids    int32 [total]    pages(c_0) || ... || pages(c_{m-1}) in the caller's order
- *   page_ntok   int32 [total]    16, except the last page of each chunk = T - 16*(npages-1)
+ *   page_ntok   uint8 [total]    16, except the last page of each chunk = T - 16*(npages-1)
  *   kv_len      int32 [R]        sum of the linked chunks' lengths
  *   tile_indptr int32 [R+1]      tile range of request r in tile_ntok (a tile = 8 consecutive table
  *                                entries of the request, i.e. 128 slots, counted from its first page)
@@ -255,7 +255,7 @@ typedef struct {
     /* out: device pointers into device_buf */
     int32_t *page_indptr;
     int32_t *page_ids;
-    int32_t *page_ntok;
+    uint8_t *page_ntok;
     int32_t *kv_len;
     int32_t *tile_indptr;
     uint64_t *tile_ntok;

@@ -310,9 +310,10 @@ class LinkedBatch:
         R, n, t = L.num_requests, int(L.total_pages), int(L.total_tiles)
         U, E, pd = int(L.num_distinct_chunks), int(L.total_entries), int(L.distinct_pages)
         i32 = lambda ptr, cnt: self._view(ptr, cnt, torch.int32).cpu().numpy()  # noqa: E731
+        u8 = lambda ptr, cnt: self._view(ptr, cnt, torch.uint8).cpu().numpy()  # noqa: E731
         out = {
             "page_indptr": i32(L.page_indptr, R + 1), "page_ids": i32(L.page_ids, n),
-            "page_ntok": i32(L.page_ntok, n), "kv_len": i32(L.kv_len, R),
+            "page_ntok": u8(L.page_ntok, n), "kv_len": i32(L.kv_len, R),
             "tile_indptr": i32(L.tile_indptr, R + 1),
             "tile_ntok": self._view(L.tile_ntok, t, torch.int64).cpu().numpy().view(np.uint64),
             "entry_indptr": i32(L.entry_indptr, R + 1),

@@ -28,7 +28,8 @@ constexpr float kLn2 = 0.6931471805599453f;
 struct DecodeArgs {
     const char *k_layer;  // bf16 [num_pages][Hkv][16][Dqk]
     const char *v_layer;  // bf16 [num_pages][Hkv][16][Dv]
-    const int32_t *page_indptr, *page_ids, *page_ntok;
+    const int32_t *page_indptr, *page_ids;
+    const uint8_t *page_ntok;
     const uint16_t *q;  // bf16 [R][Hq][Dqk]
     __nv_bfloat16 *out;  // [R][Hq][Dv]
     float *lse;          // [R][Hq] or null

@@ -39,7 +39,8 @@ struct PoolGeom {
 
 // Device pointers of a link (see comb_link_t in include/comb.h).
 struct LinkView {
-    const int32_t *page_indptr, *page_ids, *page_ntok, *kv_len, *tile_indptr;
+    const int32_t *page_indptr, *page_ids, *kv_len, *tile_indptr;
+    const uint8_t *page_ntok;
     const uint64_t *tile_ntok;
     // chunk-major view (distinct chunks as slots) + the entries of every request
     const int32_t *entry_indptr, *cas_page_indptr, *cas_page_ids, *cas_tile_indptr;

@@ -43,7 +43,7 @@ def plan(pool, lists, host_mirror=True):
     tabs = {
         "page_indptr": view(link.page_indptr, R + 1, np.int32),
         "page_ids": view(link.page_ids, int(link.total_pages), np.int32),
-        "page_ntok": view(link.page_ntok, int(link.total_pages), np.int32),
+        "page_ntok": view(link.page_ntok, int(link.total_pages), np.uint8),
         "kv_len": view(link.kv_len, R, np.int32),
         "tile_indptr": view(link.tile_indptr, R + 1, np.int32),
         "tile_ntok": view(link.tile_ntok, int(link.total_tiles), np.uint64),

@@ -691,7 +691,7 @@ def test_prefill_through_a_caller_written_table():
         pn = t["page_ntok"][t["page_indptr"][r]:t["page_indptr"][r + 1]]
         for i in range(0, len(pn), 8):
             tile_ntok[tile_indptr[r] + i // 8] = sum(int(x) << (8 * j) for j, x in enumerate(pn[i:i + 8]))
-    parts = [t["page_indptr"], t["page_ids"], t["page_ntok"], t["kv_len"], tile_indptr]
+    parts = [t["page_indptr"], t["page_ids"], t["page_ntok"].astype(np.uint8), t["kv_len"], tile_indptr]
     offs, blob = [], b""
     for a in parts + [tile_ntok]:
         blob += b"\0" * ((-len(blob)) % 16)
