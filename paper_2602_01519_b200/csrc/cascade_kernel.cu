@@ -60,6 +60,20 @@ struct KvMaps {
     CUtensorMap k, v;
 };
 
+// Timeline of CTA 0 of the bf16 chunk-major kernel (profiling aid, compiled only with -DCOMB_TRACE; build.py --trace):
+// clock64() per KV tile t of the CTA.  softmax thread 0: [0] before / [1] after the s_full wait, [2] S read, [3] the
+// rescale vote done, [4] P buffer free, [5] P handed over.  issuer: [0] before the K / s_empty waits, [1] S issued,
+// [2] P seen, [3] P V issued (stamps of tile t - 1's P V are stored under t - 1).
+#ifdef COMB_TRACE
+__device__ unsigned long long g_trace_cas[2][256][8];
+#define COMB_TRC(w, t, k)                                                                              \
+    do {                                                                                               \
+        if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (t) < 256u) g_trace_cas[w][t][k] = clock64(); \
+    } while (0)
+#else
+#define COMB_TRC(w, t, k)
+#endif
+
 // what the scheduler hands to the other warps (shared memory)
 struct ItemEntry {
     int32_t valid, kvh, nrows, ncols;
@@ -188,7 +202,9 @@ __device__ __forceinline__ void softmax_item(const CascadeArgs &a, Misc *mi, uns
         const uint64_t ntok8 = a.cas_tile_ntok[it.tile0 + j];
         const bool key_valid = ks < (int)((ntok8 >> (8 * kp)) & 0xffu);
         const int sb = t & 1;
+        if (warp == 0) COMB_TRC(0, t, 0);
         ptx::mbar_wait(&mi->s_full[sb], (t >> 1) & 1);
+        if (warp == 0) COMB_TRC(0, t, 1);
         ptx::tc_fence_after();
         uint32_t r[NC];
 #pragma unroll
@@ -198,6 +214,7 @@ __device__ __forceinline__ void softmax_item(const CascadeArgs &a, Misc *mi, uns
         ptx::tc_fence_before();
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(&mi->s_empty[sb]);
+        if (warp == 0) COMB_TRC(0, t, 2);
         if (!key_valid) {  // slots past a chunk's length / pages the tile does not have
 #pragma unroll
             for (int n = 0; n < NC; ++n) r[n] = 0xff800000u;
@@ -213,6 +230,7 @@ __device__ __forceinline__ void softmax_item(const CascadeArgs &a, Misc *mi, uns
             }
             exact = named_bar_or(1, 128, over > 8.f);
         }
+        if (warp == 0) COMB_TRC(0, t, 3);
         if (exact) {  // the same decision in all 128 threads
             float wm[NC];
 #pragma unroll
@@ -265,6 +283,7 @@ __device__ __forceinline__ void softmax_item(const CascadeArgs &a, Misc *mi, uns
         } else {
             ptx::mbar_wait(&mi->p_empty, (t & 1) ^ 1);
         }
+        if (warp == 0) COMB_TRC(0, t, 4);
 #pragma unroll
         for (int n = 0; n < NC; ++n) {
             const float p = ptx::ex2(x[n]);
@@ -274,6 +293,7 @@ __device__ __forceinline__ void softmax_item(const CascadeArgs &a, Misc *mi, uns
         ptx::fence_proxy_async_smem();  // generic-proxy stores -> visible to the tensor core's shared-memory reads
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(&mi->p_full);
+        if (warp == 0) COMB_TRC(0, t, 5);
     }
     // ---- epilogue: row sums across the 128 keys, then O^T / l -> fp32 partial rows ----
     const float lsum = warp_row_sums<NC>(l_part, lane);
@@ -373,9 +393,6 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
                 const int e_pos = tid >> a.group_shift, head = tid & (G - 1);
                 const bool valid = e_pos < it.nrows;
                 mi->srow[k & 1][tid] = valid ? (it.part0 + e_pos) * Hq + it.kvh * G + head : -1;
-                if (valid && head == 0 && it.kvh == 0 && (it.range_nr & 0xff) == 0)
-                    a.ent_info[a.cas_row_entry[it.row0 + e_pos]] =
-                        make_int4(it.part0 + e_pos, it.stride, it.range_nr >> 8, 0);
             }
             // (srow is read after the barrier syncs of the tile loop below)
             if (it.ncols == 16) softmax_item<DQK, DV, 16>(a, mi, sP, tmem, it, k, t);
@@ -425,10 +442,12 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
                 prev_pages = pages_here;
                 have_prev = true;
             }
+            // the item's last V tile follows at once (the issuer runs the last P V before the next item's first S^T)
+            if (have_prev) issue(true, prev_row0, prev_pages);
+            have_prev = false;
         }
-        if (have_prev) issue(true, prev_row0, prev_pages);
     } else if (warp == 5) {
-        // ===================== MMA issuer: S^T_t is issued before P V_{t-1} =====================
+        // ===================== MMA issuer: inside an item S^T_t is issued before P V_{t-1} =====================
         const bool leader = ptx::elect_one();
         const uint64_t dq0 = ptx::umma_desc_sw128(ptx::smem_u32(sQ), 16, 1024);
         const uint64_t dp0 = ptx::umma_desc_sw128(ptx::smem_u32(sP), 16, 1024);
@@ -439,6 +458,7 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
         auto do_pv = [&]() {
             ptx::mbar_wait(&mi->kv_full[slot], phase);
             ptx::mbar_wait(&mi->p_full, pd.t & 1);
+            COMB_TRC(1, pd.t, 2);
             if (pd.first) ptx::mbar_wait(&mi->o_empty[pd.ip], ((pd.k >> 1) & 1) ^ 1);
             ptx::tc_fence_after();
             for (int ks = 0; ks < pd.pages; ++ks)  // one k-step of 16 keys per page the tile has
@@ -446,6 +466,7 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
                     ptx::mma_ss(tmem + 64 + pd.ip * kRowsMax, dv0 + (uint64_t)((slot * C::SLOT + ks * 2048) >> 4),
                                 dp0 + (uint64_t)(((ks >> 2) * C::QH + (ks & 3) * 32) >> 4), pd.idesc,
                                 (pd.first && ks == 0) ? 0u : 1u);
+            COMB_TRC(1, pd.t, 3);
             if (leader) {
                 ptx::mma_commit(&mi->p_empty);
                 ptx::mma_commit(&mi->kv_empty[slot]);
@@ -468,6 +489,7 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
             ptx::mbar_wait(&mi->q_full[ip], (k >> 1) & 1);
             for (int j = 0; j < n_kv; ++j, ++t) {
                 const int sb = t & 1;
+                COMB_TRC(1, t, 0);
                 ptx::mbar_wait(&mi->kv_full[slot], phase);
                 ptx::mbar_wait(&mi->s_empty[sb], ((t >> 1) & 1) ^ 1);
                 ptx::tc_fence_after();
@@ -477,6 +499,7 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
                     if (leader)
                         ptx::mma_ss(tmem + sb * kRowsMax, dk + (uint64_t)(((kk / 4) * C::HALF + (kk % 4) * 32) >> 4),
                                     dq + (uint64_t)(((kk / 4) * C::QH + (kk % 4) * 32) >> 4), idesc_s, kk > 0);
+                COMB_TRC(1, t, 1);
                 if (leader) {
                     ptx::mma_commit(&mi->s_full[sb]);
                     ptx::mma_commit(&mi->kv_empty[slot]);
@@ -486,8 +509,10 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
                 if (pd.on) do_pv();
                 pd = Pend{true, j == 0, j + 1 == n_kv, min(kTilePages, it.npages - j * kTilePages), ip, k, t, idesc_o};
             }
+            // the item's last P V is not deferred behind the next item's first S^T: the softmax threads wait for it
+            // (o_full) before their epilogue, and cannot start the next item earlier anyway
+            if (pd.on) do_pv();
         }
-        if (pd.on) do_pv();
     } else if (warp == 6) {
         // ===================== scheduler + Q gather =====================
         constexpr int UPR = DQK / 8;  // 16-byte units per Q row
@@ -527,6 +552,10 @@ cascade_decode_kernel(const CascadeArgs a, const __grid_constant__ KvMaps maps) 
                 mi->items[ir] = e;
                 ptx::mbar_arrive(&mi->item_full[ir]);
             }
+            // where the merge finds an entry's partials (once per entry: first kv-head, first range); written here so
+            // that the dependent load of the entry index is not on the softmax threads' path
+            if (lane < ci.nrows && kvh == 0 && (ci.range_nr & 0xff) == 0)
+                a.ent_info[a.cas_row_entry[ci.row0 + lane]] = make_int4(ci.part0 + lane, ci.part_stride, ci.range_nr >> 8, 0);
             // ---- Q rows of the item: entry e_pos of the tile, head hh of the kv-head -> row e_pos * G + hh, laid out
             // as the SWIZZLE_128B K-major tile TMA would have written (unit j of row r at unit j ^ (r & 7)); rows up
             // to ncols are zero-filled
@@ -1293,3 +1322,14 @@ cudaError_t launch_decode_cascade(const PoolGeom &g, int layer, const LinkView &
 }
 
 }  // namespace comb
+
+#ifdef COMB_TRACE
+// libcomb_trace*.so only: the timeline of the most recent bf16 chunk-major decode launch, 2 x 256 x 8 uint64.
+#pragma GCC visibility push(default)
+extern "C" int32_t comb_trace_cascade_read(void *out) {
+    if (cudaDeviceSynchronize() != cudaSuccess) return -6;
+    if (cudaMemcpyFromSymbol(out, comb::g_trace_cas, sizeof(comb::g_trace_cas)) != cudaSuccess) return -6;
+    return 0;
+}
+#pragma GCC visibility pop
+#endif
